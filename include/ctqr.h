@@ -1,0 +1,132 @@
+/* ctqr.h -- C-ABI of the B200-native dense Householder QR + batched solve for direct
+ * algebraic CT reconstruction (arXiv 2412.07631; PAPER.md in the reference mount).
+ *
+ * What the library computes (section 2):
+ *   Eq. 2   A = Q R          once per scanner geometry       -> ct_qr_factor
+ *   Eq. 3   X = R^{-1}(Q^T B) for a batch of S sinograms     -> ct_qr_solve
+ * Q is kept implicit as Householder reflectors in compact-WY blocks (V_k, T_k), R^{-1} is
+ * never formed (L48).  The in-core LAPACK analogues named by the paper are dgeqrf, dormqr
+ * (printed "dormar") and dtrsm (L52); the out-of-core tiling mirrors section 2.2 (L54-77).
+ *
+ * Conventions
+ *   - All matrices are column-major, leading dimensions in ELEMENTS.
+ *   - dtype applies to A, B, X, V, T, R alike (no mixed precision in the product path).
+ *   - Every pointer argument says whether it is a DEVICE pointer, a HOST pointer, or EITHER
+ *     (detected with cudaPointerGetAttributes; host memory may be pinned or pageable).
+ *   - Return value: 0 = success; negative -i = the i-th argument (1-based) is invalid;
+ *     positive = runtime failure (CTQR_ERR_*).  Nothing aborts, nothing throws across the
+ *     ABI.  ct_qr_last_error() returns a thread-local message for the last non-zero return.
+ *   - Calls are synchronous: on return all device work they enqueued has completed.
+ *   - A handle is not thread-safe; distinct handles may be used from distinct threads.
+ *   - There is NO CPU fallback: without a CUDA device every compute entry point returns
+ *     CTQR_ERR_CUDA.
+ *
+ * Householder convention (reading R4, LAPACK-like): H_j = I - tau_j v_j v_j^T,
+ * v_j[j] = 1, beta_j = -sign(alpha_j) ||x_j||_2 with sign(0) = +1, R_jj = beta_j; a column
+ * whose sub-diagonal part is exactly zero gets tau_j = 0.
+ */
+#ifndef CTQR_H
+#define CTQR_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ctqr_handle_s* ctqr_handle_t;   /* opaque; owns T, tau, diag(R) blocks, plan, and
+                                                  (unless in_place) the V\R storage */
+
+typedef enum { CTQR_F32 = 0, CTQR_F64 = 1 } ctqr_dtype_t;
+
+typedef enum {
+    CTQR_OK = 0,
+    CTQR_ERR_CUDA = 1,      /* a CUDA runtime call failed, or no device */
+    CTQR_ERR_NOMEM = 2,     /* device or host allocation failed / budget too small */
+    CTQR_ERR_IO = 3,        /* file tier read/write failed */
+    CTQR_ERR_SINGULAR = 4,  /* some R_jj == 0 at solve time (stats.singular_col = first j) */
+    CTQR_ERR_STATE = 5      /* handle is not in a state that allows the call */
+} ctqr_status_t;
+
+/* Options for ct_qr_factor.  Zero-initialise for defaults. */
+typedef struct {
+    int32_t nb;                 /* panel width; 0 = default (128). Must be a multiple of ib. */
+    int32_t ib;                 /* inner (register-resident) panel width: 8, 16 or 32; 0 = default */
+    int32_t lookahead;          /* 0 = off, 1 = factor panel k+1 while the rest of update k runs; -1 = default */
+    int32_t in_place;           /* 1: A (device) is overwritten and must outlive the handle.
+                                   0: A is read-only; the handle owns a copy. */
+    int64_t device_budget_bytes;/* 0 = unlimited (in-core if it fits). >0 caps the device bytes used
+                                   for matrix tiles: forces the out-of-core path when m*n*w exceeds it */
+    int32_t gemm_impl;          /* 0 = default (fp64: DMMA tensor cores, fp32: FFMA), 1 = SIMT reference kernels */
+    int32_t reserved0;
+    const char* file_path;      /* optional file-backed tier for the factor (NULL = none) */
+    void* stream;               /* cudaStream_t the caller's data is ordered on (NULL = legacy default) */
+} ctqr_options_t;
+
+/* Per-handle statistics (CUDA-event timed, milliseconds). */
+typedef struct {
+    int64_t m, n;
+    int32_t nb, ib, n_panels, n_superpanels;   /* n_superpanels == 1 when in-core */
+    int32_t out_of_core, singular_col;         /* singular_col = -1 when none */
+    double factor_ms;          /* whole ct_qr_factor device time */
+    double panel_ms;           /* sum of panel (a1) + T (a2) chains, as timed on their stream */
+    double update_ms;          /* sum of trailing updates (a3) */
+    double solve_ms;           /* last ct_qr_solve device time */
+    double apply_qt_ms;        /* last Q^T B part (a6) */
+    double trsm_ms;            /* last triangular solve part (a7) */
+    double h2d_bytes, d2h_bytes;   /* bytes moved over the host link by the last factor / solve */
+    double factor_flops;       /* 2 m n^2 - 2 n^3 / 3 */
+    int64_t kernel_launches;   /* kernels launched by the last factor or solve call */
+} ctqr_stats_t;
+
+/* Eq. 2: Householder QR of the m x n matrix A (m >= n >= 1, lda >= m).
+ *   A       EITHER. Device pointer: in-core factorisation (in place if opt->in_place, else
+ *           on a copy owned by the handle).  Host pointer (pinned preferred): the matrix is
+ *           staged through device memory; when m*n*w exceeds opt->device_budget_bytes (or
+ *           free device memory) the out-of-core path streams column super-panels from the
+ *           host buffer, which is then overwritten with the factor (always in place).
+ *   out     receives the handle on success; untouched on failure.
+ * On success the factor is: V (unit lower trapezoid, explicit 0/1 on and above the
+ * diagonal inside each diagonal block), tau[n], T_k (nb x nb upper) per panel, R
+ * (off-diagonal blocks inside the matrix storage, diagonal blocks owned by the handle). */
+int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dtype_t dtype,
+                 const ctqr_options_t* opt, ctqr_handle_t* out);
+
+/* Eq. 3: X = R^{-1} (Q^T B) for S right-hand sides.
+ *   B   EITHER, m x S, ldb >= m, read-only.   X   EITHER, n x S, ldx >= n, written.
+ * Returns CTQR_ERR_SINGULAR if some R_jj == 0. */
+int ct_qr_solve(ctqr_handle_t h, const void* B, int64_t ldb, int64_t S, void* X, int64_t ldx);
+
+/* First half of Eq. 3 alone: C <- Q^T C in place (C EITHER, m x S, ldc >= m). */
+int ct_qr_apply_qt(ctqr_handle_t h, void* C, int64_t ldc, int64_t S);
+
+/* Second half of Eq. 3 alone (blocked TRSM, task list PAPER.md:L62-73): X <- R^{-1} C[0:n,:].
+ * C EITHER (n x S used, ldc >= n, read-only), X EITHER (n x S, ldx >= n). */
+int ct_qr_trsm(ctqr_handle_t h, const void* C, int64_t ldc, int64_t S, void* X, int64_t ldx);
+
+/* Accessors (R, V, T, tau may be HOST or DEVICE pointers; output is dense column-major). */
+int ct_qr_get_R(ctqr_handle_t h, void* R, int64_t ldr);                  /* n x n upper; strictly lower part zeroed */
+int ct_qr_get_V(ctqr_handle_t h, int64_t j0, int64_t ncols, void* V, int64_t ldv); /* m x ncols, unit lower trapezoid */
+int ct_qr_get_T(ctqr_handle_t h, int64_t panel, void* T, int64_t ldt);   /* nb_k x nb_k upper (last panel may be narrower) */
+int ct_qr_get_tau(ctqr_handle_t h, void* tau);                           /* n values */
+int ct_qr_get_stats(ctqr_handle_t h, ctqr_stats_t* s);
+void ct_qr_destroy(ctqr_handle_t h);
+
+const char* ct_qr_strerror(int code);
+const char* ct_qr_last_error(void);
+int ct_qr_version(void);
+
+/* Kernel-level entry points used by the parity tests (SURVEY.md test rung T2) and by the
+ * micro-benchmarks of bench.py.  All pointers DEVICE.
+ *   ct_qr_gemm: C <- alpha*op(A)*B + beta*C with op(A) = A^T when trans_a (A is K x M) else A
+ *   (A is M x K); B is K x N; impl 0 = default kernel for the dtype, 1 = SIMT kernel.
+ *   ct_qr_peak_probe: runs a register-resident FMA/MMA loop and returns achieved TFLOP/s
+ *   (kind 0 = FFMA fp32, 1 = DFMA fp64, 2 = DMMA m8n8k4 fp64). */
+int ct_qr_gemm(int trans_a, int64_t M, int64_t N, int64_t K, double alpha, const void* A, int64_t lda,
+               const void* B, int64_t ldb, double beta, void* C, int64_t ldc, ctqr_dtype_t dtype, int impl);
+int ct_qr_peak_probe(int kind, int iters, double* tflops, double* ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CTQR_H */

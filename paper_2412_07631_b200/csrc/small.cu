@@ -1,0 +1,81 @@
+// small.cu -- launchers of the small kernels (larft, T^T W, diagonal-block TRSM, accessors).
+#include "small.cuh"
+#include "kernels.h"
+
+namespace ctqr {
+
+template <typename K>
+static cudaError_t ensure_smem(K kernel, size_t bytes, size_t& cur) {
+    if (bytes <= cur) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) cur = bytes;
+    return e;
+}
+
+template <typename T>
+cudaError_t larft_launch(const T* Gp, int nsplit, int64_t gstride, int ldg, const T* tau, int nbw, T* Tout, int ldt,
+                         cudaStream_t st) {
+    static size_t cur = 0;
+    const size_t smem = (size_t)nbw * (nbw + 1) * sizeof(T);
+    cudaError_t e = ensure_smem(larft_kernel<T>, smem, cur);
+    if (e != cudaSuccess) return e;
+    larft_kernel<T><<<1, 1024, smem, st>>>(Gp, nsplit, gstride, ldg, tau, nbw, Tout, ldt);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t ttw_launch(const T* Wp, int nsplit, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N,
+                       T* Wout, int64_t ldo, cudaStream_t st) {
+    constexpr int CW = 32;
+    static size_t cur = 0;
+    const size_t smem = ((size_t)kw * (kw + 1) + (size_t)CW * kw) * sizeof(T);
+    cudaError_t e = ensure_smem(ttw_kernel<T, CW>, smem, cur);
+    if (e != cudaSuccess) return e;
+    ttw_kernel<T, CW><<<(unsigned)ceil_div(N, CW), 256, smem, st>>>(Wp, nsplit, wstride, ldw, Tm, ldt, kw, N, Wout, ldo);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx,
+                             cudaStream_t st) {
+    static size_t cur = 0;
+    const size_t smem = (size_t)128 * 129 * sizeof(T);
+    cudaError_t e = ensure_smem(trsm_diag_kernel<T, 128>, smem, cur);
+    if (e != cudaSuccess) return e;
+    trsm_diag_kernel<T, 128><<<(unsigned)ceil_div(S, 16), 256, smem, st>>>(R, ldr, kw, C, ldc, S, X, ldx);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t copy2d_launch(const T* src, int64_t lds, T* dst, int64_t ldd, int64_t rows, int64_t cols, cudaStream_t st) {
+    if (rows <= 0 || cols <= 0) return cudaSuccess;
+    dim3 grid((unsigned)ceil_div(rows, 256), (unsigned)std::min<int64_t>(cols, 65535));
+    copy2d_kernel<T><<<grid, 256, 0, st>>>(src, lds, dst, ldd, rows, cols);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t gather_R_launch(const T* A, int64_t lda, const T* Rd, int nb, int64_t n, T* R, int64_t ldr, cudaStream_t st) {
+    dim3 grid((unsigned)ceil_div(n, 256), (unsigned)std::min<int64_t>(n, 65535));
+    gather_R_kernel<T><<<grid, 256, 0, st>>>(A, lda, Rd, nb, n, R, ldr);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, cudaStream_t st) {
+    find_zero_diag_kernel<T><<<(unsigned)ceil_div(n, 256), 256, 0, st>>>(Rd, nb, n, result);
+    return cudaGetLastError();
+}
+
+#define INST(T)                                                                                                        \
+    template cudaError_t larft_launch<T>(const T*, int, int64_t, int, const T*, int, T*, int, cudaStream_t);           \
+    template cudaError_t ttw_launch<T>(const T*, int, int64_t, int64_t, const T*, int, int, int64_t, T*, int64_t,      \
+                                       cudaStream_t);                                                                  \
+    template cudaError_t trsm_diag_launch<T>(const T*, int, int, const T*, int64_t, int64_t, T*, int64_t, cudaStream_t); \
+    template cudaError_t copy2d_launch<T>(const T*, int64_t, T*, int64_t, int64_t, int64_t, cudaStream_t);             \
+    template cudaError_t gather_R_launch<T>(const T*, int64_t, const T*, int, int64_t, T*, int64_t, cudaStream_t);     \
+    template cudaError_t find_zero_diag_launch<T>(const T*, int, int64_t, int*, cudaStream_t);
+INST(float)
+INST(double)
+
+}  // namespace ctqr

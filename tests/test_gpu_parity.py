@@ -1,0 +1,177 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle on the same
+seeded inputs (SURVEY.md 8c rungs T2-T3).  Tolerances are BASELINE.json north_star's:
+  fp64: ||A - QR||_F/||A||_F <= 1e-12, ||X - X_or||/||X_or|| <= 1e-9
+  fp32: <= 5e-5 and <= 1e-3 (against the fp32 oracle).
+R is unique up to row signs, X is unique (reading R4); both sides use the same
+Householder convention so V, tau, T are compared directly at rounding level as well.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2412_07631_b200 as ctqr
+from paper_2412_07631_b200 import workload as wl
+
+pytestmark = pytest.mark.gpu
+
+DT = [np.float64, np.float32]
+BACKWARD = {np.float64: 1e-12, np.float32: 5e-5}
+SOLUTION = {np.float64: 1e-9, np.float32: 1e-3}
+ROUND = {np.float64: 1e-11, np.float32: 5e-4}      # V / tau / T / R agreement (same convention)
+
+
+def relerr(a, b):
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    den = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / (den if den > 0 else 1.0)
+
+
+def backward_error(A, V, tau, R):
+    """||A - Q R||_F / ||A||_F with Q R evaluated in fp64 from the returned reflectors
+    (reading 17): apply H_{n-1} ... H_0 order reversed to [R; 0]."""
+    A = np.asarray(A, dtype=np.float64)
+    m, n = A.shape
+    QR = np.zeros((m, n))
+    QR[:n] = np.triu(np.asarray(R, dtype=np.float64))
+    V = np.asarray(V, dtype=np.float64); tau = np.asarray(tau, dtype=np.float64)
+    for j in range(n - 1, -1, -1):
+        v = V[:, j]
+        QR -= tau[j] * np.outer(v, v @ QR)
+    return np.linalg.norm(A - QR) / np.linalg.norm(A)
+
+
+def gpu_factor_solve(A, B, **opts):
+    m, n = A.shape
+    S = B.shape[1]
+    At = ctqr.colmajor_from_numpy(A)
+    Bt = ctqr.colmajor_from_numpy(B.astype(A.dtype))
+    f = ctqr.ct_qr_factor(At, m, n, **opts)
+    import torch
+    Xt = torch.zeros((S, n), dtype=At.dtype, device="cuda")
+    ctqr.ct_qr_solve(f, Bt, S, Xt)
+    out = dict(R=ctqr.ct_qr_get_R(f), V=ctqr.ct_qr_get_V(f), tau=ctqr.ct_qr_get_tau(f),
+               X=ctqr.numpy_from_colmajor(Xt), stats=f.stats(), f=f)
+    return out
+
+
+def check_against_oracle(A, B, dt, **opts):
+    A = np.asfortranarray(A.astype(dt)); B = np.asfortranarray(B.astype(dt))
+    g = gpu_factor_solve(A, B, **opts)
+    VR, tau = oracle.qr(A)
+    X_or = oracle.solve(VR, tau, B)
+    be = backward_error(A, g["V"], g["tau"], g["R"])
+    assert be <= BACKWARD[dt], f"backward error {be}"
+    se = relerr(g["X"], X_or)
+    assert se <= SOLUTION[dt], f"solution error {se}"
+    # same convention => same R (with signs), V, tau up to rounding
+    assert relerr(g["R"], oracle.R_of(VR)) <= ROUND[dt]
+    assert relerr(g["V"], oracle.V_of(VR)) <= ROUND[dt]
+    assert relerr(g["tau"], tau) <= ROUND[dt]
+    assert np.all(np.tril(g["R"], -1) == 0)
+    return g, VR, tau
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("shape", [(1, 1), (3, 2), (7, 4), (16, 16), (33, 17), (40, 40), (300, 130), (517, 259)])
+def test_random_small(shape, dt):
+    m, n = shape
+    rng = np.random.default_rng(100 * m + n)
+    A = rng.standard_normal((m, n)); B = rng.standard_normal((m, 5))
+    check_against_oracle(A, B, dt)
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("nb,ib", [(8, 8), (32, 16), (64, 16), (128, 16), (128, 32), (64, 8)])
+@pytest.mark.parametrize("la", [0, 1])
+def test_blocking_invariance(nb, ib, la, dt):
+    """Reading 6: results must not depend on nb / look-ahead beyond rounding; n not a multiple of
+    nb and m - n < nb are covered by the shape."""
+    rng = np.random.default_rng(7)
+    A = rng.standard_normal((700, 650)); B = rng.standard_normal((700, 9))
+    check_against_oracle(A, B, dt, nb=nb, ib=ib, lookahead=la)
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("cfg", ["c0", "c1"])
+def test_ct_config(cfg, dt):
+    c = wl.CONFIGS[cfg]
+    coo = wl.siddon_coo(c.N, c.n_ang, c.n_bins)
+    A, lam = wl.dense_augmented(c, np.float64, coo)
+    X0, B = wl.make_slices(c, coo=coo, lam=lam)
+    g, VR, tau = check_against_oracle(A, B, dt)
+    # T factor of the first and last panel against the oracle's larft recurrence
+    nb = g["stats"]["nb"]
+    for k in (0, g["stats"]["n_panels"] - 1):
+        Tg = ctqr.ct_qr_get_T(g["f"], k)
+        To = oracle.larft(VR, tau, k * nb, Tg.shape[0])
+        assert relerr(Tg, To) <= ROUND[dt]
+
+
+@pytest.mark.parametrize("dt", DT)
+def test_zero_column_and_triangular(dt):
+    rng = np.random.default_rng(3)
+    A = rng.standard_normal((90, 40))
+    A[:, 5] = 0.0                       # zero column: tau = 0, R_jj = 0 -> solve must refuse
+    At = ctqr.colmajor_from_numpy(np.asfortranarray(A.astype(dt)))
+    f = ctqr.ct_qr_factor(At, 90, 40)
+    tau = ctqr.ct_qr_get_tau(f)
+    VR, tau_o = oracle.qr(np.asfortranarray(A.astype(dt)))
+    assert relerr(tau, tau_o) <= ROUND[dt]
+    import torch
+    Bt = torch.ones((2, 90), dtype=At.dtype, device="cuda"); Xt = torch.zeros((2, 40), dtype=At.dtype, device="cuda")
+    # upper-triangular input: every sub-column is zero => tau = 0, R = A
+    U = np.triu(rng.standard_normal((30, 30))) + 3 * np.eye(30)
+    Ut = ctqr.colmajor_from_numpy(np.asfortranarray(U.astype(dt)))
+    f2 = ctqr.ct_qr_factor(Ut, 30, 30)
+    assert np.all(ctqr.ct_qr_get_tau(f2) == 0)
+    assert np.array_equal(ctqr.ct_qr_get_R(f2), U.astype(dt))
+
+
+def test_singular_solve_refused():
+    import torch
+    A = np.zeros((20, 4)); A[:4, :4] = np.eye(4); A[2, 2] = 0.0
+    At = ctqr.colmajor_from_numpy(np.asfortranarray(A))
+    f = ctqr.ct_qr_factor(At, 20, 4)
+    Bt = torch.ones((1, 20), dtype=torch.float64, device="cuda"); Xt = torch.zeros((1, 4), dtype=torch.float64, device="cuda")
+    with pytest.raises(ctqr.CtqrError) as ei:
+        ctqr.ct_qr_solve(f, Bt, 1, Xt)
+    assert ei.value.code == 4
+
+
+@pytest.mark.parametrize("dt", DT)
+def test_host_pointers_and_halves(dt):
+    """Host (numpy) A, B, X; apply_qt and trsm alone against the oracle's two halves."""
+    rng = np.random.default_rng(11)
+    A = np.asfortranarray(rng.standard_normal((400, 200)).astype(dt))
+    B = np.asfortranarray(rng.standard_normal((400, 17)).astype(dt))
+    f = ctqr.ct_qr_factor(A.copy(order="F"), 400, 200)
+    VR, tau = oracle.qr(A)
+    C = B.copy(order="F")
+    ctqr.ct_qr_apply_qt(f, C, 17)
+    C_or = oracle.apply_qt(VR, tau, B)
+    assert relerr(C, C_or) <= ROUND[dt]
+    X = np.zeros((200, 17), dtype=dt, order="F")
+    ctqr.ct_qr_trsm(f, np.asfortranarray(C_or[:200]), 17, X)
+    assert relerr(X, oracle.backsub(VR, C_or[:200])) <= SOLUTION[dt]
+    X2 = np.zeros((200, 17), dtype=dt, order="F")
+    ctqr.ct_qr_solve(f, B, 17, X2)
+    assert relerr(X2, oracle.solve(VR, tau, B)) <= SOLUTION[dt]
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("ta", [True, False])
+@pytest.mark.parametrize("impl", [0, 1])
+@pytest.mark.parametrize("mnk", [(128, 64, 256), (37, 150, 1001), (130, 9, 77), (5, 300, 4)])
+def test_gemm_kernel(mnk, impl, ta, dt):
+    """Kernel-level: C <- alpha op(A) B + beta C against the definition (numpy fp64)."""
+    import torch
+    M, N, K = mnk
+    rng = np.random.default_rng(M + N + K)
+    A = rng.standard_normal((K, M) if ta else (M, K)).astype(dt)
+    B = rng.standard_normal((K, N)).astype(dt)
+    C = rng.standard_normal((M, N)).astype(dt)
+    ref = -1.0 * (A.T.astype(np.float64) if ta else A.astype(np.float64)) @ B.astype(np.float64) + C.astype(np.float64)
+    At, Bt, Ct = (ctqr.colmajor_from_numpy(np.asfortranarray(x)) for x in (A, B, C))
+    ctqr.ct_qr_gemm(ta, M, N, K, -1.0, At, A.shape[0], Bt, K, 1.0, Ct, M, impl)
+    got = ctqr.numpy_from_colmajor(Ct)
+    assert relerr(got, ref) <= (1e-13 if dt == np.float64 else 2e-5)

@@ -1,0 +1,437 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of arXiv 2412.07631 (Eq. 2-3) on B200.
+
+One "step" = one pass of the whole hot path over one batch of synthetic input:
+    ct_qr_factor(A_aug)            a1-a4  (Householder QR of the Tikhonov-augmented CT matrix)
+  + ct_qr_solve(handle, B, S) -> X a6-a7  (X = R^-1 (Q^T B) for the config's S noisy sinograms)
+`value` is BASELINE.json's metric, "QR factor TFLOP/s" (flops = 2mn^2 - 2n^3/3), taken over the
+factorisation part of the K timed steps (CUDA events inside the library, inputs resident in
+HBM); the solve part of the same steps is reported as `solve.slices_per_s`; `ms_per_step` is
+the whole step.  `e2e` is the same metric through the same C-ABI calls with HOST (pinned)
+buffers, host<->device copies inside the timed region.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--dtype f64|f32]
+                    [--impl ours|reference] [--no-also]
+
+N > 1 (torchrun): the factorisation does not shard on one node without an exchange step
+(DESIGN.md "Multi-GPU"): every rank factors its own replica of A and solves its own S/N share
+of the slices; no data-path collective; value = N * flops / max-over-ranks time ("weak").
+--impl reference: the CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2412_07631_b200 import workload as wl  # noqa: E402
+
+METRIC = "qr_factor_tflops"
+UNIT = "TFLOP/s"
+
+
+# --------------------------------------------------------------------------------------------
+# clocks sampled DURING the timed region (B200_PROFILING.md "clocks line")
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int = 0):
+        self.lines, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._pump, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def load_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "_source": "fallback"}
+
+
+# Arithmetic peak of the path's own dtype: B200 has 148 SMs x 64 FP64
+# FMA lanes (DFMA and DMMA.8x8x4 share that rate) and 148 x 128 FP32 FMA lanes; x 2 flop x the
+# maximum SM clock.  MEASURED_PEAKS.json holds no fp64/fp32 figure, so the bench also runs the
+# library's register-resident probe (ct_qr_peak_probe) and reports it beside the nominal one.
+def nominal_peak_tflops(dtype: str, sm_max_mhz: float) -> float:
+    lanes = 64 if dtype == "f64" else 128
+    return 148 * lanes * 2 * sm_max_mhz * 1e6 / 1e12
+
+
+# --------------------------------------------------------------------------------------------
+# inputs (seeded, synthetic; recipe in DESIGN.md "Input recipe")
+# --------------------------------------------------------------------------------------------
+def build_inputs(cfg, dtype: str, S: int, s_lo: int = 0):
+    """A_aug resident in HBM (column-major m x n), B (m x S) as numpy fp64, phantoms X0."""
+    import torch
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
+    At, lam = wl.dense_augmented_device(cfg, tdt, coo)
+    X0, B = wl.make_slices(cfg, S=s_lo + S, coo=coo, lam=lam)
+    return At, X0[:, s_lo:], B[:, s_lo:], coo, lam
+
+
+def quality(cfg, X0: np.ndarray, X: np.ndarray) -> dict:
+    """PAPER.md Eq. 4-7 (L136-154): mean SNR / PSNR / SSIM of the reconstructions against the
+    generating phantoms (reported only)."""
+    N = cfg.N
+    ps, ss, sn = [], [], []
+    for s in range(X.shape[1]):
+        r, i = X0[:, s].reshape(N, N), X[:, s].astype(np.float64).reshape(N, N)
+        ps.append(wl.psnr(r, i)); ss.append(wl.ssim(r, i)); sn.append(wl.snr(r, i))
+    return {"psnr_db_mean": float(np.mean(ps)), "ssim_mean": float(np.mean(ss)), "snr_db_mean": float(np.mean(sn)),
+            "psnr_db_min": float(np.min(ps)), "slices": int(X.shape[1])}
+
+
+def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do_e2e: bool = True) -> dict:
+    import torch
+    import paper_2412_07631_b200 as ctqr
+    dist = torch.distributed if world > 1 else None
+    npdt = np.float64 if dtype == "f64" else np.float32
+    S_all = cfg.S
+    # slices are sharded over ranks (independent right-hand sides, no collective)
+    S = S_all // world + (1 if rank < S_all % world else 0)
+    s_lo = rank * (S_all // world) + min(rank, S_all % world)
+    At, X0, B, coo, lam = build_inputs(cfg, dtype, S, s_lo)
+    m, n = cfg.m, cfg.n
+    Bt = ctqr.colmajor_from_numpy(B.astype(npdt))
+    Xt = torch.zeros((S, n), dtype=At.dtype, device="cuda")
+    flops = cfg.factor_flops()
+
+    def one_step(profile: bool):
+        f = ctqr.ct_qr_factor(At, m, n, in_place=False, profile=profile)
+        factor_launches = f.stats()["kernel_launches"]      # the solve call restarts the counter
+        ctqr.ct_qr_solve(f, Bt, S, Xt)
+        st = f.stats()
+        st["launches_step"] = factor_launches + st["kernel_launches"]
+        f.destroy()
+        return st
+
+    for _ in range(max(warmup, 0)):
+        one_step(False)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    sampler = ClockSampler(torch.cuda.current_device())
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    stats = [one_step(True) for _ in range(steps)]
+    e1.record()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = e0.elapsed_time(e1)
+    factor_ms = sum(s["factor_ms"] for s in stats)
+    solve_ms = sum(s["solve_ms"] for s in stats)
+    launches = sum(s["launches_step"] for s in stats)
+    X = ctqr.numpy_from_colmajor(Xt)
+    t = torch.tensor([total_ms, factor_ms, solve_ms], dtype=torch.float64, device="cuda")
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, factor_ms, solve_ms = (float(x) for x in t.tolist())
+    out = {
+        "value": world * steps * flops / (factor_ms * 1e-3) / 1e12,
+        "ms_per_step": total_ms / steps,
+        "factor_ms_per_step": factor_ms / steps,
+        "solve": {"S": S_all, "ms_per_batch": solve_ms / steps, "slices_per_s": S_all * steps / (solve_ms * 1e-3),
+                  "apply_qt_ms": stats[-1]["apply_qt_ms"], "trsm_ms": stats[-1]["trsm_ms"]},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "quality_noisy": quality(cfg, X0, X),
+        "nb": stats[-1]["nb"], "ib": stats[-1]["ib"],
+    }
+    # roofline of the dominant kernel: the two contractions of the trailing update (a3)
+    vt = {"ms": sum(s["vtc_ms"] for s in stats), "flops": sum(s["vtc_flops"] for s in stats),
+          "launches": sum(s["vtc_launches"] for s in stats)}
+    up = {"ms": sum(s["upd_ms"] for s in stats), "flops": sum(s["upd_flops"] for s in stats),
+          "launches": sum(s["upd_launches"] for s in stats)}
+    out["_spans"] = {"vtc": vt, "upd": up}
+    if do_e2e and rank == 0:
+        out["e2e"] = run_e2e(cfg, dtype, At, B.astype(npdt), S, steps, flops)
+    elif do_e2e:
+        out["e2e"] = None
+    del At, Bt, Xt
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float) -> dict:
+    """Same metric through ct_qr_factor / ct_qr_solve with HOST buffers: every step copies A and
+    B host->device and X device->host inside the timed region (the library does the copies)."""
+    import torch
+    import paper_2412_07631_b200 as ctqr
+    m, n = cfg.m, cfg.n
+    Ah = At.cpu().pin_memory()
+    Bh = torch.from_numpy(np.ascontiguousarray(B.T)).pin_memory()
+    Xh = torch.zeros((S, n), dtype=Ah.dtype).pin_memory()
+    w = Ah.element_size()
+
+    def step():
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        f = ctqr.ct_qr_factor(Ah, m, n)
+        t1 = time.perf_counter()
+        ctqr.ct_qr_solve(f, Bh, S, Xh)
+        torch.cuda.synchronize()
+        t2 = time.perf_counter()
+        f.destroy()
+        return t1 - t0, t2 - t1
+
+    step()
+    ts = [step() for _ in range(max(1, min(steps, 3)))]
+    tf = sum(a for a, _ in ts) / len(ts)
+    tsol = sum(b for _, b in ts) / len(ts)
+    return {"value": flops / tf / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(m * n * w + m * S * w),
+            "d2h_bytes_per_step": int(n * S * w), "factor_s": tf, "solve_s": tsol,
+            "solve_slices_per_s": S / tsol, "steps": len(ts),
+            "note": "A, B, X in pinned host memory; wall clock around the synchronous C-ABI calls"}
+
+
+# --------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------
+def oracle_sample(cfg, dtype: str, k_cols: int, s_cols: int, reps: int = 1) -> dict:
+    """Time the oracle, as it stands, on a bounded sample of the same workload: the leading
+    k_cols columns of A_aug at full height m (an m x k Householder QR, 2mk^2 - 2k^3/3 flop) and
+    its solve of s_cols slices.  Inputs are built on the host; no GPU involved."""
+    import oracle
+    npdt = np.float64 if dtype == "f64" else np.float32
+    coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
+    rows, cols, vals = coo
+    lam = wl.tikhonov_lambda(vals, cfg.n)
+    k = min(k_cols, cfg.n)
+    A = np.zeros((cfg.m, k), dtype=np.float64, order="F")
+    sel = cols < k
+    np.add.at(A, (rows[sel], cols[sel]), vals[sel])
+    A[cfg.m0 + np.arange(k), np.arange(k)] = np.sqrt(lam)
+    A = np.asfortranarray(A.astype(npdt))
+    _, B = wl.make_slices(cfg, S=s_cols, coo=coo, lam=lam)
+    B = np.asfortranarray(B.astype(npdt))
+    fl = 2.0 * cfg.m * k * k - 2.0 * k ** 3 / 3.0
+    tq, ts = [], []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        VR, tau = oracle.qr(A)
+        t1 = time.perf_counter()
+        oracle.solve(VR, tau, B)
+        t2 = time.perf_counter()
+        tq.append(t1 - t0); ts.append(t2 - t1)
+    tqm, tsm = sum(tq) / reps, sum(ts) / reps
+    return {"value": fl / tqm / 1e12, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{cfg.name} {dtype}: oracle.qr on the leading {k} of {cfg.n} columns of A_aug at full m={cfg.m} "
+                      f"({fl:.3g} flop, {tqm:.2f} s) + oracle.solve of {s_cols} slices on that factor ({tsm:.2f} s)",
+            "factor_s": tqm, "solve_s": tsm, "solve_slices_per_s_on_sample": s_cols / tsm,
+            "sample_flops": fl}
+
+
+def sample_size(cfg) -> tuple[int, int]:
+    """Leading-column count giving roughly 10-20 s of oracle work at this config's m."""
+    target = 4e11                               # flop; the unblocked oracle runs at 15-35 GFLOP/s
+    k = int(min(cfg.n, max(64, (target / (2.0 * cfg.m)) ** 0.5)))
+    return (k // 64) * 64 if k >= 64 else k, min(cfg.S, 8)
+
+
+def run_reference(cfg, dtype: str, steps: int, warmup: int) -> dict:
+    k, s = sample_size(cfg)
+    for _ in range(min(warmup, 1)):
+        oracle_sample(cfg, dtype, max(64, k // 4), 1)
+    r = oracle_sample(cfg, dtype, k, s, reps=max(1, steps))
+    ms = (r["factor_s"] + r["solve_s"]) * 1e3
+    return {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": 0, "steps": steps,
+            "warmup": warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": dtype, "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "sample": r["sample"]},
+            "cpu_baseline": {k2: r[k2] for k2 in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def workload_name(cfg) -> str:
+    idx = cfg.cfg_id - 1
+    return (f"BASELINE.json configs[{idx}]: {cfg.N}x{cfg.N} image, parallel-beam Siddon, {cfg.n_ang} angles x "
+            f"{cfg.n_bins} bins + sqrt(lambda) I rows -> m={cfg.m}, n={cfg.n}; {cfg.S} noisy ellipse-phantom slices, "
+            f"I0={cfg.I0:g}")
+
+
+# per-launch DRAM traffic of the dominant kernel from the committed `ncu --set full` capture
+# (profiles/); filled in when a capture of the current kernel exists, else null.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+
+KERNEL_NAMES = {("f64", "upd"): "gemm_dmma_kernel<TA=false> (C <- C - V W, larfb)",
+                ("f64", "vtc"): "gemm_dmma_kernel<TA=true> (W = V^T C, larfb)",
+                ("f32", "upd"): "gemm_simt_kernel<float,TA=false> (C <- C - V W, larfb)",
+                ("f32", "vtc"): "gemm_simt_kernel<float,TA=true> (W = V^T C, larfb)"}
+
+
+def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:
+    dom = max(("upd", "vtc"), key=lambda k: spans[k]["ms"])
+    oth = "vtc" if dom == "upd" else "upd"
+    s, o = spans[dom], spans[oth]
+    ach = s["flops"] / (s["ms"] * 1e-3) / 1e12 if s["ms"] > 0 else 0.0
+    peak = nominal_peak_tflops(dtype, float(peaks.get("sm_max_mhz", 1965.0)))
+    return {"bound": "tensor" if dtype == "f64" else "alu", "kernel": KERNEL_NAMES[(dtype, dom)],
+            "achieved": ach, "peak": peak, "unit": UNIT, "frac": ach / peak,
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dtype, dom)),
+            "peak_source": ("derived: 148 SMs x %d %s FMA lanes x 2 x %.0f MHz max SM clock (MEASURED_PEAKS.json "
+                            "holds no %s figure; sm_max_mhz %s)" % (64 if dtype == "f64" else 128,
+                                                                   "FP64" if dtype == "f64" else "FP32",
+                                                                   float(peaks.get("sm_max_mhz", 1965.0)), dtype,
+                                                                   peaks.get("_source"))),
+            "peak_probe_tflops": probe_tflops,
+            "launches": int(s["launches"]), "avg_launch_ms": s["ms"] / max(1, s["launches"]),
+            "flops_per_launch_avg": s["flops"] / max(1, s["launches"]),
+            "other_contraction": {"kernel": KERNEL_NAMES[(dtype, oth)],
+                                  "achieved": o["flops"] / (o["ms"] * 1e-3) / 1e12 if o["ms"] > 0 else 0.0,
+                                  "launches": int(o["launches"]), "ms_total": o["ms"]},
+            "share_of_factor_time": None}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c3", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--no-also", action="store_true", help="skip the second precision")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    cfg = wl.CONFIGS[args.config]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(run_reference(cfg, args.dtype, args.steps, args.warmup)), flush=True)
+        return 0
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2412_07631_b200 import build as _build
+    if rank == 0:
+        _build.build()
+    if world > 1:
+        torch.distributed.barrier()
+    import paper_2412_07631_b200 as ctqr
+
+    warm = max(args.warmup, 3)
+    res = run_ours(cfg, args.dtype, args.steps, warm, rank, world, do_e2e=not args.no_e2e)
+    other = "f32" if args.dtype == "f64" else "f64"
+    res2 = None
+    if not args.no_also:
+        res2 = run_ours(cfg, other, args.steps, warm, rank, world, do_e2e=not args.no_e2e)
+    if rank != 0:
+        if world > 1:
+            torch.distributed.destroy_process_group()
+        return 0
+
+    peaks = load_peaks()
+    probe = {}
+    for kind, name in ((0, "ffma_f32"), (1, "dfma_f64"), (2, "dmma_f64")):
+        probe[name] = round(ctqr.ct_qr_peak_probe(kind, 8192)[0], 2)
+
+    def finish(r, dtype):
+        rf = roofline(r.pop("_spans"), dtype, peaks, probe["dmma_f64" if dtype == "f64" else "ffma_f32"])
+        rf["share_of_factor_time"] = (rf["launches"] * rf["avg_launch_ms"]) / (r["factor_ms_per_step"] * args.steps)
+        r["roofline"] = rf
+        r["frac_of_peak_whole_factor"] = r["value"] / (world * rf["peak"])
+        return r
+
+    res = finish(res, args.dtype)
+    line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": warm, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "m": cfg.m, "n": cfg.n, "S": cfg.S, "nb": res["nb"],
+                       "ib": res["ib"], "flops_per_factor": cfg.factor_flops(),
+                       "l2": "inputs larger than L2 (A is %.2f GB; every step re-reads it from HBM)"
+                             % (cfg.m * cfg.n * (8 if args.dtype == "f64" else 4) / 1e9),
+                       "parallelism": "1 GPU" if world == 1 else f"{world} replicas, slices sharded"},
+            "value_definition": "sum over timed steps of 2mn^2-2n^3/3 / device time of ct_qr_factor (A resident in HBM)",
+            "factor_ms_per_step": res["factor_ms_per_step"], "frac_of_peak_whole_factor": res["frac_of_peak_whole_factor"],
+            "solve": res["solve"], "quality_noisy": res["quality_noisy"], "clocks": res["clocks"],
+            "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
+            "peak_probe_tflops": probe}
+    if res2 is not None:
+        res2 = finish(res2, other)
+        line["also"] = {other: {k: res2[k] for k in ("value", "ms_per_step", "factor_ms_per_step",
+                                                     "frac_of_peak_whole_factor", "solve", "quality_noisy", "e2e",
+                                                     "gpu_launches", "roofline", "clocks")}}
+    if not args.no_cpu_baseline and world == 1:
+        k, s = sample_size(cfg)
+        line["cpu_baseline"] = {k2: v for k2, v in oracle_sample(cfg, args.dtype, k, s).items()
+                                if k2 in ("value", "unit", "cores", "kind", "sample", "solve_slices_per_s_on_sample")}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -58,7 +58,7 @@ typedef struct {
     int64_t device_budget_bytes;/* 0 = unlimited (in-core if it fits). >0 caps the device bytes used
                                    for matrix tiles: forces the out-of-core path when m*n*w exceeds it */
     int32_t gemm_impl;          /* 0 = default (fp64: DMMA tensor cores, fp32: FFMA), 1 = SIMT reference kernels */
-    int32_t reserved0;
+    int32_t profile;            /* 1: CUDA-event time every trailing-update contraction launch (stats.vtc_*, upd_*) */
     const char* file_path;      /* optional file-backed tier for the factor (NULL = none) */
     void* stream;               /* cudaStream_t the caller's data is ordered on (NULL = legacy default) */
 } ctqr_options_t;
@@ -77,6 +77,11 @@ typedef struct {
     double h2d_bytes, d2h_bytes;   /* bytes moved over the host link by the last factor / solve */
     double factor_flops;       /* 2 m n^2 - 2 n^3 / 3 */
     int64_t kernel_launches;   /* kernels launched by the last factor or solve call */
+    /* opt->profile only: the two contractions of every trailing update (a3) of the last factor,
+     * each launch bracketed by CUDA events on the stream it runs on.
+     *   vtc: W = V_k^T C  (K = m_k),   upd: C <- C - V_k W  (K = nb);  flops = 2*m_k*nb_k*n_c each. */
+    double vtc_ms, vtc_flops;  int64_t vtc_launches;
+    double upd_ms, upd_flops;  int64_t upd_launches;
 } ctqr_stats_t;
 
 /* Eq. 2: Householder QR of the m x n matrix A (m >= n >= 1, lda >= m).

@@ -92,6 +92,15 @@ struct ctqr_handle_s {
     std::vector<cudaEvent_t> ev;       // event pool
     ctqr_stats_t st;
     int64_t launches = 0;
+    // opt->profile: per-launch event spans of the trailing-update contractions
+    struct Span { cudaEvent_t a, b; double flops; int kind; };
+    int profile = 0;
+    std::vector<Span> spans;
+    std::vector<cudaEvent_t> tpool; size_t tpool_used = 0;
+    cudaEvent_t timing_event() {
+        if (tpool_used == tpool.size()) { cudaEvent_t e; cudaEventCreate(&e); tpool.push_back(e); }
+        return tpool[tpool_used++];
+    }
     bool factored = false;
     // out-of-core state
     bool ooc = false; void* hA = nullptr; int64_t hlda = 0; int n_super = 1;
@@ -101,6 +110,7 @@ struct ctqr_handle_s {
         for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); }
         cudaFree(dTin); cudaFree(dPart); cudaFree(dRow); cudaFree(dBar); cudaFree(dFlag);
         for (auto e : ev) cudaEventDestroy(e);
+        for (auto e : tpool) cudaEventDestroy(e);
         if (sU) cudaStreamDestroy(sU);
         if (sP) cudaStreamDestroy(sP);
     }
@@ -121,7 +131,7 @@ static bool is_device_ptr(const void* p) {
 // ------------------------------------------------------------------------------------------
 template <typename T>
 static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t mk, int kw, const T* Tm, int ldt,
-                 T* C, int64_t ldc, int64_t nc) {
+                 T* C, int64_t ldc, int64_t nc, bool prof = false) {
     if (nc <= 0 || mk <= 0 || kw <= 0) return 0;
     const int64_t ldw = round_up(kw, 4);
     // W = V^T C, split over K when the output grid cannot fill the machine
@@ -138,14 +148,32 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     GemmArgs<T> g1{};
     g1.M = kw; g1.N = nc; g1.K = mk; g1.A = V; g1.lda = ldv; g1.B = C; g1.ldb = ldc;
     g1.C = Wp; g1.ldc = ldw; g1.alpha = T(1); g1.beta = T(0); g1.split_stride = sstride;
+    prof = prof && h.profile;
+    const double fl = 2.0 * (double)mk * (double)kw * (double)nc;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
     CK(gemm_dispatch<T>(true, g1, splits, h.gemm_impl, st));
+    if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 0}); }
     CK(ttw_launch<T>(Wp, splits, sstride, ldw, Tm, ldt, kw, nc, W, ldw, st));
     GemmArgs<T> g2{};
     g2.M = mk; g2.N = nc; g2.K = kw; g2.A = V; g2.lda = ldv; g2.B = W; g2.ldb = ldw;
     g2.C = C; g2.ldc = ldc; g2.alpha = T(-1); g2.beta = T(1);
+    if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
     CK(gemm_dispatch<T>(false, g2, 1, h.gemm_impl, st));
+    if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 1}); }
     h.launches += 3;
     return 0;
+}
+
+// sum the profiled spans into the stats (after the streams have been synchronised)
+static void resolve_spans(H& h) {
+    h.st.vtc_ms = h.st.upd_ms = h.st.vtc_flops = h.st.upd_flops = 0; h.st.vtc_launches = h.st.upd_launches = 0;
+    for (auto& s : h.spans) {
+        float ms = 0; cudaEventElapsedTime(&ms, s.a, s.b);
+        if (s.kind == 0) { h.st.vtc_ms += ms; h.st.vtc_flops += s.flops; h.st.vtc_launches++; }
+        else             { h.st.upd_ms += ms; h.st.upd_flops += s.flops; h.st.upd_launches++; }
+    }
+    h.spans.clear(); h.tpool_used = 0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -256,7 +284,7 @@ static int factor_incore(H& h, T* A, int64_t lda) {
             CKI(panel_factor<T>(h, h.sU, A, lda, m, j0, nbw, k));
             const int64_t nc = n - (j0 + nbw);
             CKI(larfb<T>(h, 0, h.sU, A + j0 + j0 * lda, lda, m - j0, nbw,
-                         P_<T>(h.dT) + (size_t)k * nb * nb, nb, A + j0 + (j0 + nbw) * lda, lda, nc));
+                         P_<T>(h.dT) + (size_t)k * nb * nb, nb, A + j0 + (j0 + nbw) * lda, lda, nc, true));
         }
     } else {
         CKI(panel_factor<T>(h, h.sP, A, lda, m, 0, (int)std::min<int64_t>(nb, n), 0));
@@ -270,12 +298,12 @@ static int factor_incore(H& h, T* A, int64_t lda) {
             const T* V = A + j0 + j0 * lda;
             const T* Tk = P_<T>(h.dT) + (size_t)k * nb * nb;
             CK(cudaStreamWaitEvent(h.sU, evP, 0));             // V_k, T_k ready
-            CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + jn * lda, lda, nbn));
+            CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + jn * lda, lda, nbn, true));
             CK(cudaEventRecord(evL, h.sU));
             CK(cudaStreamWaitEvent(h.sP, evL, 0));
             CKI(panel_factor<T>(h, h.sP, A, lda, m, jn, nbn, k + 1));
             CK(cudaEventRecord(evP, h.sP));
-            CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + (jn + nbn) * lda, lda, n - jn - nbn));
+            CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + (jn + nbn) * lda, lda, n - jn - nbn, true));
         }
         CK(cudaStreamWaitEvent(h.sU, evP, 0));
     }
@@ -284,6 +312,7 @@ static int factor_incore(H& h, T* A, int64_t lda) {
     CK(cudaStreamSynchronize(h.sP));
     float ms = 0; CK(cudaEventElapsedTime(&ms, t0, t1));
     h.st.factor_ms = ms;
+    resolve_spans(h);
     return 0;
 }
 
@@ -397,6 +426,7 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
     if (h->nb > 128 || h->nb % h->ib != 0) { delete h; return set_err(-6, "nb must be a multiple of ib and <= 128"); }
     h->lookahead = o.lookahead < 0 ? 1 : (o.lookahead ? 1 : 0);
     h->gemm_impl = o.gemm_impl;
+    h->profile = o.profile ? 1 : 0;
     h->P = (int)ceil_div(n, h->nb);
     h->user = (cudaStream_t)o.stream;
     int dev = 0; cudaGetDevice(&dev);

@@ -29,7 +29,7 @@ from dataclasses import dataclass
 import numpy as np
 
 __all__ = [
-    "CTConfig", "CONFIGS", "siddon_coo", "tikhonov_lambda", "dense_augmented",
+    "CTConfig", "CONFIGS", "siddon_coo", "tikhonov_lambda", "dense_augmented", "dense_augmented_device",
     "ellipse_phantom", "make_slices", "chord_length", "psnr", "snr", "ssim",
 ]
 
@@ -169,6 +169,29 @@ def dense_augmented(cfg: CTConfig, dtype=np.float64, coo=None):
     np.add.at(A, (rows, cols), vals)
     A[cfg.m0 + np.arange(cfg.n), np.arange(cfg.n)] = math.sqrt(lam)
     return np.asfortranarray(A.astype(dtype)), lam
+
+
+def dense_augmented_device(cfg: CTConfig, torch_dtype, coo=None, device="cuda", lda: int | None = None):
+    """Same matrix as ``dense_augmented`` but scattered straight into device memory (the dense
+    matrix of the larger configs is too big to stage through numpy).  Returns (At, lam) where
+    ``At`` is a torch tensor of shape (n, lda) whose memory is the column-major m x n A_aug with
+    leading dimension lda (default m).  Duplicates are accumulated in fp64 before the single
+    rounding to ``torch_dtype``, like the host builder."""
+    import torch
+    rows, cols, vals = coo if coo is not None else siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
+    lam = tikhonov_lambda(vals, cfg.n)
+    lda = cfg.m if lda is None else lda
+    # accumulate duplicate (row, col) pairs on the host in fp64 (they are rare corner slivers)
+    key = cols * np.int64(lda) + rows
+    uk, inv = np.unique(key, return_inverse=True)
+    acc = np.zeros(uk.shape[0], dtype=np.float64)
+    np.add.at(acc, inv, vals)
+    At = torch.zeros((cfg.n, lda), dtype=torch_dtype, device=device)
+    flat = At.view(-1)
+    flat[torch.from_numpy(uk).to(device)] = torch.from_numpy(acc).to(device).to(torch_dtype)
+    d = torch.arange(cfg.n, device=device, dtype=torch.int64)
+    flat[d * lda + cfg.m0 + d] = torch.tensor(math.sqrt(lam), dtype=torch.float64).to(torch_dtype).item()
+    return At, lam
 
 
 def ellipse_phantom(N: int, rng: np.random.Generator) -> np.ndarray:

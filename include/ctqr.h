@@ -130,6 +130,9 @@ int ct_qr_version(void);
 int ct_qr_gemm(int trans_a, int64_t M, int64_t N, int64_t K, double alpha, const void* A, int64_t lda,
                const void* B, int64_t ldb, double beta, void* C, int64_t ldc, ctqr_dtype_t dtype, int impl);
 int ct_qr_peak_probe(int kind, int iters, double* tflops, double* ms);
+/* same loop with `threads` per CTA (multiple of 32, <= 256) and `ctas_per_sm` CTAs per SM: how many
+ * resident warps the pipe needs to reach its peak (ct_qr_peak_probe = 256 threads x 8 CTAs). */
+int ct_qr_peak_probe_cfg(int kind, int iters, int threads, int ctas_per_sm, double* tflops, double* ms);
 
 #ifdef __cplusplus
 }

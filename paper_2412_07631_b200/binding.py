@@ -72,6 +72,7 @@ EXPORTS = {
     "ct_qr_gemm": ([_I, _I64, _I64, _I64, ctypes.c_double, _P, _I64, _P, _I64, ctypes.c_double,
                     _P, _I64, _I, _I], _I),
     "ct_qr_peak_probe": ([_I, _I, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)], _I),
+    "ct_qr_peak_probe_cfg": ([_I, _I, _I, _I, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)], _I),
 }
 
 
@@ -124,7 +125,8 @@ def colmajor_from_numpy(a: np.ndarray, device="cuda", pin: bool = False):
     import torch
     t = torch.from_numpy(np.ascontiguousarray(np.asarray(a).T))
     if device == "cpu":
-        return t.pin_memory() if pin else t
+        # always a fresh buffer: an out-of-core ct_qr_factor overwrites its host matrix in place
+        return t.pin_memory() if pin else t.clone()
     return t.to(device)
 
 
@@ -234,8 +236,8 @@ def ct_qr_gemm(trans_a: bool, M: int, N: int, K: int, alpha: float, A, lda: int,
     return C
 
 
-def ct_qr_peak_probe(kind: int, iters: int = 4096):
+def ct_qr_peak_probe(kind: int, iters: int = 4096, threads: int = 256, ctas_per_sm: int = 8):
     """Measured register-resident peak: kind 0 FFMA, 1 DFMA, 2 DMMA.  Returns (TFLOP/s, ms)."""
     tf, ms = ctypes.c_double(), ctypes.c_double()
-    _check(lib().ct_qr_peak_probe(kind, iters, ctypes.byref(tf), ctypes.byref(ms)))
+    _check(lib().ct_qr_peak_probe_cfg(kind, iters, threads, ctas_per_sm, ctypes.byref(tf), ctypes.byref(ms)))
     return tf.value, ms.value

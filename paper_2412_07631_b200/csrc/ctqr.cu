@@ -88,7 +88,8 @@ struct ctqr_handle_s {
     void* dTin = nullptr; void* dPart = nullptr; void* dRow = nullptr;
     unsigned* dBar = nullptr; unsigned bar_count = 0;
     int* dFlag = nullptr;
-    cudaStream_t sU = nullptr, sP = nullptr, user = nullptr;
+    cudaStream_t sU = nullptr, sP = nullptr, sC = nullptr, sD = nullptr, user = nullptr;
+    cudaEvent_t evP = nullptr, evL = nullptr, evU = nullptr;
     std::vector<cudaEvent_t> ev;       // event pool
     ctqr_stats_t st;
     int64_t launches = 0;
@@ -104,6 +105,8 @@ struct ctqr_handle_s {
     bool factored = false;
     // out-of-core state
     bool ooc = false; void* hA = nullptr; int64_t hlda = 0; int n_super = 1;
+    void* dVb[2] = {nullptr, nullptr}; int64_t ldvb = 0;   // double buffer for streamed panels (m x nb each)
+    cudaEvent_t evVin[2] = {nullptr, nullptr}, evVfree[2] = {nullptr, nullptr};
     ~ctqr_handle_s() {
         if (own_A && dA) cudaFree(dA);
         cudaFree(dT); cudaFree(dRd); cudaFree(dTau);
@@ -113,6 +116,9 @@ struct ctqr_handle_s {
         for (auto e : tpool) cudaEventDestroy(e);
         if (sU) cudaStreamDestroy(sU);
         if (sP) cudaStreamDestroy(sP);
+        if (sC) cudaStreamDestroy(sC);
+        if (sD) cudaStreamDestroy(sD);
+        for (int i = 0; i < 2; ++i) cudaFree(dVb[i]);
     }
 };
 typedef ctqr_handle_s H;
@@ -265,54 +271,201 @@ static cudaEvent_t new_event(H& h, bool timing) {
 }
 
 // ------------------------------------------------------------------------------------------
-// a4: in-core right-looking blocked QR of columns [c_begin, n) given that panels before
-// c_begin are done; look-ahead overlaps panel k+1 with the bulk of update k.
+// a4: right-looking blocked QR of the columns [c0, c1) (c0 a multiple of nb) with look-ahead:
+// panel k+1 is factored on the high-priority stream sP while the bulk of update k runs on sU.
+// A is the VIRTUAL base of the buffer holding those columns: element (i, j) lives at
+// A[i + j * lda] and only c0 <= j < c1 is ever touched.  Earlier panels must already have been
+// applied.  Everything is enqueued; on return sU waits for the last panel.  No host sync.
 // ------------------------------------------------------------------------------------------
 template <typename T>
-static int factor_incore(H& h, T* A, int64_t lda) {
-    const int64_t m = h.m, n = h.n;
-    const int nb = h.nb, P = h.P;
-    cudaEvent_t evP = new_event(h, false), evL = new_event(h, false), evU = new_event(h, false);
-    cudaEvent_t t0 = new_event(h, true), t1 = new_event(h, true);
-    CK(cudaEventRecord(t0, h.sU));
+static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
+    const int64_t m = h.m;
+    const int nb = h.nb;
+    const int k0 = (int)(c0 / nb), k1 = (int)ceil_div(c1, nb);
+    if (!h.evP) { h.evP = new_event(h, false); h.evL = new_event(h, false); h.evU = new_event(h, false); }
+    cudaEvent_t evP = h.evP, evL = h.evL, evU = h.evU;
     CK(cudaEventRecord(evU, h.sU));
     CK(cudaStreamWaitEvent(h.sP, evU, 0));
     if (!h.lookahead) {
-        for (int k = 0; k < P; ++k) {
+        for (int k = k0; k < k1; ++k) {
             const int64_t j0 = (int64_t)k * nb;
-            const int nbw = (int)std::min<int64_t>(nb, n - j0);
+            const int nbw = (int)std::min<int64_t>(nb, c1 - j0);
             CKI(panel_factor<T>(h, h.sU, A, lda, m, j0, nbw, k));
-            const int64_t nc = n - (j0 + nbw);
+            const int64_t nc = c1 - (j0 + nbw);
             CKI(larfb<T>(h, 0, h.sU, A + j0 + j0 * lda, lda, m - j0, nbw,
                          P_<T>(h.dT) + (size_t)k * nb * nb, nb, A + j0 + (j0 + nbw) * lda, lda, nc, true));
         }
-    } else {
-        CKI(panel_factor<T>(h, h.sP, A, lda, m, 0, (int)std::min<int64_t>(nb, n), 0));
-        CK(cudaEventRecord(evP, h.sP));
-        for (int k = 0; k < P; ++k) {
-            const int64_t j0 = (int64_t)k * nb;
-            const int nbw = (int)std::min<int64_t>(nb, n - j0);
-            const int64_t jn = j0 + nbw;                       // first trailing column
-            if (jn >= n) break;
-            const int nbn = (int)std::min<int64_t>(nb, n - jn); // width of panel k+1
-            const T* V = A + j0 + j0 * lda;
-            const T* Tk = P_<T>(h.dT) + (size_t)k * nb * nb;
-            CK(cudaStreamWaitEvent(h.sU, evP, 0));             // V_k, T_k ready
-            CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + jn * lda, lda, nbn, true));
-            CK(cudaEventRecord(evL, h.sU));
-            CK(cudaStreamWaitEvent(h.sP, evL, 0));
-            CKI(panel_factor<T>(h, h.sP, A, lda, m, jn, nbn, k + 1));
-            CK(cudaEventRecord(evP, h.sP));
-            CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + (jn + nbn) * lda, lda, n - jn - nbn, true));
-        }
-        CK(cudaStreamWaitEvent(h.sU, evP, 0));
+        return 0;
     }
+    CKI(panel_factor<T>(h, h.sP, A, lda, m, c0, (int)std::min<int64_t>(nb, c1 - c0), k0));
+    CK(cudaEventRecord(evP, h.sP));
+    for (int k = k0; k < k1; ++k) {
+        const int64_t j0 = (int64_t)k * nb;
+        const int nbw = (int)std::min<int64_t>(nb, c1 - j0);
+        const int64_t jn = j0 + nbw;                        // first trailing column
+        if (jn >= c1) break;
+        const int nbn = (int)std::min<int64_t>(nb, c1 - jn); // width of panel k+1
+        const T* V = A + j0 + j0 * lda;
+        const T* Tk = P_<T>(h.dT) + (size_t)k * nb * nb;
+        CK(cudaStreamWaitEvent(h.sU, evP, 0));              // V_k, T_k ready
+        CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + jn * lda, lda, nbn, true));
+        CK(cudaEventRecord(evL, h.sU));
+        CK(cudaStreamWaitEvent(h.sP, evL, 0));
+        CKI(panel_factor<T>(h, h.sP, A, lda, m, jn, nbn, k + 1));
+        CK(cudaEventRecord(evP, h.sP));
+        CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + (jn + nbn) * lda, lda, c1 - jn - nbn, true));
+    }
+    CK(cudaStreamWaitEvent(h.sU, evP, 0));
+    return 0;
+}
+
+template <typename T>
+static int factor_incore(H& h, T* A, int64_t lda) {
+    cudaEvent_t t0 = new_event(h, true), t1 = new_event(h, true);
+    CK(cudaEventRecord(t0, h.sU));
+    CKI(factor_range<T>(h, A, lda, 0, h.n));
     CK(cudaEventRecord(t1, h.sU));
     CK(cudaStreamSynchronize(h.sU));
     CK(cudaStreamSynchronize(h.sP));
     float ms = 0; CK(cudaEventElapsedTime(&ms, t0, t1));
     h.st.factor_ms = ms;
     resolve_spans(h);
+    return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// a5: out-of-core tile scheduler (section 2.2: blocks, task list, prefetch of
+// the operands of the next tasks during the current one; here the slow tier is pinned host
+// memory and the overlap is copy streams + events instead of an I/O thread).
+//
+// Left-looking over column SUPER-PANELS of ns columns (ns a multiple of nb, two buffers):
+//   for s = 0 .. Ps-1:           (sC = H2D copy stream, sD = D2H copy stream, sU/sP compute)
+//     [sC] SP_s <- host A[:, c0:c1)                       (issued while SP_{s-1} is being factored)
+//     for every earlier panel k, in order:   SP_s[j0:m, :] <- (I - V_k T_k^T V_k^T) SP_s[j0:m, :]
+//          V_k comes from the other device buffer when k belongs to SP_{s-1} (still resident),
+//          else it is streamed host -> Vb[k & 1] on sC (double-buffered against the larfb on sU)
+//     [sU,sP] right-looking factorisation of SP_s with look-ahead (factor_range)
+//     [sD] host A[:, c0:c1) <- SP_s                       (in place; overlaps the work on SP_{s+1})
+// T_k, tau and the diagonal R blocks stay resident.  Host-link bytes: every super-panel in and
+// out once plus the earlier reflectors once per later super-panel = m n w (P_s + 3)/2.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+static int stream_panel_in(H& h, int slot, const T* hsrc, int64_t hld, int64_t rows, int cols) {
+    // [sC] wait until the larfb that last read Vb[slot] is done, copy, signal
+    CK(cudaStreamWaitEvent(h.sC, h.evVfree[slot], 0));
+    CK(cudaMemcpy2DAsync(h.dVb[slot], h.ldvb * sizeof(T), hsrc, hld * sizeof(T), rows * sizeof(T), cols,
+                         cudaMemcpyHostToDevice, h.sC));
+    CK(cudaEventRecord(h.evVin[slot], h.sC));
+    h.st.h2d_bytes += (double)rows * cols * sizeof(T);
+    return 0;
+}
+
+static int ensure_stream_bufs(H& h) {
+    if (h.dVb[0]) return 0;
+    h.ldvb = round_up(h.m, 16 / (int64_t)h.w);
+    for (int i = 0; i < 2; ++i) {
+        if (cudaMalloc(&h.dVb[i], (size_t)h.ldvb * h.nb * h.w) != cudaSuccess) {
+            cudaGetLastError();
+            return set_err(CTQR_ERR_NOMEM, "cannot allocate the panel stream buffers");
+        }
+        h.evVin[i] = new_event(h, false); h.evVfree[i] = new_event(h, false);
+        CK(cudaEventRecord(h.evVfree[i], h.sU));
+    }
+    if (!h.sC) CK(cudaStreamCreateWithFlags(&h.sC, cudaStreamNonBlocking));
+    if (!h.sD) CK(cudaStreamCreateWithFlags(&h.sD, cudaStreamNonBlocking));
+    return 0;
+}
+
+template <typename T>
+static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
+    const int64_t m = h.m, n = h.n;
+    const int nb = h.nb;
+    const int Ps = (int)ceil_div(n, ns);
+    const int64_t lds = round_up(m, 16 / (int64_t)sizeof(T));
+    CKI(ensure_stream_bufs(h));
+    T* sp[2] = {nullptr, nullptr};
+    for (int i = 0; i < 2; ++i)
+        if (cudaMalloc(&sp[i], (size_t)lds * std::min<int64_t>(ns, n) * sizeof(T)) != cudaSuccess) {
+            cudaGetLastError(); cudaFree(sp[0]);
+            return set_err(CTQR_ERR_NOMEM, "cannot allocate the super-panel buffers (%lld columns)", (long long)ns);
+        }
+    std::vector<cudaEvent_t> evIn(Ps), evOut(Ps), evDone(Ps), evFree(Ps);
+    for (int s = 0; s < Ps; ++s) {
+        evIn[s] = new_event(h, false); evOut[s] = new_event(h, false);
+        evDone[s] = new_event(h, false); evFree[s] = new_event(h, false);
+    }
+    cudaEvent_t t0 = new_event(h, true), t1 = new_event(h, true);
+    CK(cudaEventRecord(t0, h.sU));
+    CK(cudaStreamWaitEvent(h.sC, t0, 0));
+    auto load_sp = [&](int s) -> int {
+        const int64_t c0 = (int64_t)s * ns, c1 = std::min<int64_t>(n, c0 + ns);
+        if (s >= 2) {                                     // buffer reuse: SP_{s-2} written back and no longer read
+            CK(cudaStreamWaitEvent(h.sC, evOut[s - 2], 0));
+            CK(cudaStreamWaitEvent(h.sC, evFree[s - 2], 0));
+        }
+        CK(cudaMemcpy2DAsync(sp[s & 1], lds * sizeof(T), hA + c0 * hlda, hlda * sizeof(T), m * sizeof(T), c1 - c0,
+                             cudaMemcpyHostToDevice, h.sC));
+        CK(cudaEventRecord(evIn[s], h.sC));
+        h.st.h2d_bytes += (double)m * (c1 - c0) * sizeof(T);
+        return 0;
+    };
+    int rc = load_sp(0);
+    for (int s = 0; s < Ps && rc == 0; ++s) {
+        const int64_t c0 = (int64_t)s * ns, c1 = std::min<int64_t>(n, c0 + ns);
+        T* Cv = sp[s & 1] - c0 * lds;                     // virtual base of SP_s
+        CK(cudaStreamWaitEvent(h.sU, evIn[s], 0));
+        // ---- earlier reflectors, streamed from the host (super-panels 0 .. s-2) ----
+        const int kres = s >= 1 ? (int)(((int64_t)(s - 1) * ns) / nb) : 0;   // first panel of SP_{s-1}
+        const int kcur = (int)(c0 / nb);
+        for (int k = 0; k < kres && rc == 0; ++k) {
+            const int64_t j0 = (int64_t)k * nb;
+            const int slot = k & 1;
+            CK(cudaStreamWaitEvent(h.sC, evOut[(int)(j0 / ns)], 0));          // factor of that SP is on the host
+            rc = stream_panel_in<T>(h, slot, hA + j0 + j0 * hlda, hlda, m - j0, nb);
+            if (rc) break;
+            CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
+            rc = larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, m - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
+                          Cv + j0 + c0 * lds, lds, c1 - c0, true);
+            CK(cudaEventRecord(h.evVfree[slot], h.sU));
+        }
+        // ---- reflectors of SP_{s-1}, still resident in the other buffer ----
+        if (s >= 1 && rc == 0) {
+            const T* Pv = sp[(s - 1) & 1] - (int64_t)(s - 1) * ns * lds;
+            for (int k = kres; k < kcur && rc == 0; ++k) {
+                const int64_t j0 = (int64_t)k * nb;
+                rc = larfb<T>(h, 0, h.sU, Pv + j0 + j0 * lds, lds, m - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
+                              Cv + j0 + c0 * lds, lds, c1 - c0, true);
+            }
+            CK(cudaEventRecord(evFree[s - 1], h.sU));
+        }
+        if (rc) break;
+        // ---- prefetch the next super-panel while this one is factored ----
+        if (s + 1 < Ps) { rc = load_sp(s + 1); if (rc) break; }
+        rc = factor_range<T>(h, Cv, lds, c0, c1);
+        if (rc) break;
+        CK(cudaEventRecord(evDone[s], h.sU));
+        CK(cudaStreamWaitEvent(h.sD, evDone[s], 0));
+        CK(cudaMemcpy2DAsync(hA + c0 * hlda, hlda * sizeof(T), sp[s & 1], lds * sizeof(T), m * sizeof(T), c1 - c0,
+                             cudaMemcpyDeviceToHost, h.sD));
+        CK(cudaEventRecord(evOut[s], h.sD));
+        h.st.d2h_bytes += (double)m * (c1 - c0) * sizeof(T);
+    }
+    if (rc == 0) {
+        CK(cudaStreamWaitEvent(h.sU, evOut[Ps - 1], 0));
+        if (Ps >= 2) CK(cudaStreamWaitEvent(h.sU, evOut[Ps - 2], 0));
+        CK(cudaEventRecord(t1, h.sU));
+    }
+    cudaError_t e1 = cudaStreamSynchronize(h.sU), e2 = cudaStreamSynchronize(h.sP);
+    cudaError_t e3 = cudaStreamSynchronize(h.sC), e4 = cudaStreamSynchronize(h.sD);
+    cudaFree(sp[0]); cudaFree(sp[1]);
+    if (rc) return rc;
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess)
+        return set_err(CTQR_ERR_CUDA, "out-of-core factorisation failed: %s",
+                       cudaGetErrorString(e1 != cudaSuccess ? e1 : e2 != cudaSuccess ? e2 : e3 != cudaSuccess ? e3 : e4));
+    float ms = 0; CK(cudaEventElapsedTime(&ms, t0, t1));
+    h.st.factor_ms = ms;
+    resolve_spans(h);
+    h.ooc = true; h.hA = hA; h.hlda = hlda; h.n_super = Ps;
     return 0;
 }
 
@@ -369,13 +522,12 @@ static int ensure_solve_ws(H& h, int64_t S) {
 template <typename T>
 static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr_options_t& o) {
     const int64_t m = h.m, n = h.n;
-    CKI(alloc_state<T>(h, n));
     const size_t bytes = (size_t)m * n * sizeof(T);
     size_t freeb = 0, totb = 0;
     CK(cudaMemGetInfo(&freeb, &totb));
-    const bool fits = (o.device_budget_bytes > 0) ? (bytes <= (size_t)o.device_budget_bytes)
-                                                  : (bytes + ((size_t)1 << 30) <= freeb);
+    const size_t slack = (size_t)2 << 30;                 // workspaces, T, B/X of later solves
     if (a_on_device) {
+        CKI(alloc_state<T>(h, n));
         if (o.in_place) { h.dA = A; h.lda = lda; h.own_A = false; }
         else {
             h.lda = round_up(m, 16 / sizeof(T));
@@ -386,8 +538,11 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
         }
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
-    if (fits) {
+    const size_t budget = o.device_budget_bytes > 0 ? (size_t)o.device_budget_bytes
+                                                    : (freeb > slack ? freeb - slack : 0);
+    if (bytes <= budget) {
         // host matrix that fits: stage once, factor in core, keep the factor on the device
+        CKI(alloc_state<T>(h, n));
         h.lda = round_up(m, 16 / sizeof(T));
         CK(cudaMalloc(&h.dA, (size_t)h.lda * n * sizeof(T)));
         h.own_A = true;
@@ -396,7 +551,16 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
         h.st.h2d_bytes = (double)bytes;
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
-    return set_err(CTQR_ERR_NOMEM, "matrix of %zu bytes exceeds the device budget; out-of-core path not built in this library version", bytes);
+    // out of core: budget = 2 super-panel buffers + 2 panel stream buffers
+    const int64_t lds = round_up(m, 16 / (int64_t)sizeof(T));
+    const int64_t col_bytes = lds * (int64_t)sizeof(T);
+    int64_t ns = ((int64_t)budget / col_bytes - 2 * h.nb) / 2;
+    ns = (ns / h.nb) * h.nb;
+    if (ns < h.nb)
+        return set_err(CTQR_ERR_NOMEM, "device budget of %zu bytes cannot hold two %d-column super-panels and two "
+                       "panel buffers of %lld rows", budget, h.nb, (long long)m);
+    CKI(alloc_state<T>(h, std::min<int64_t>(ns, n)));
+    return factor_ooc<T>(h, (T*)A, lda, ns);
 }
 
 extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dtype_t dtype,
@@ -458,6 +622,21 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
 // ------------------------------------------------------------------------------------------
 template <typename T>
 static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
+    if (h.ooc) {
+        // factor on the host: stream V_k through the double buffer (sC) against the larfb on sU
+        const T* hA = P_<T>(h.hA);
+        for (int k = 0; k < h.P; ++k) {
+            const int64_t j0 = (int64_t)k * h.nb;
+            const int nbw = (int)std::min<int64_t>(h.nb, h.n - j0);
+            const int slot = k & 1;
+            CKI(stream_panel_in<T>(h, slot, hA + j0 + j0 * h.hlda, h.hlda, h.m - j0, nbw));
+            CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
+            CKI(larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, h.m - j0, nbw,
+                         P_<T>(h.dT) + (size_t)k * h.nb * h.nb, h.nb, C + j0, ldc, S));
+            CK(cudaEventRecord(h.evVfree[slot], h.sU));
+        }
+        return 0;
+    }
     const T* A = P_<T>(h.dA);
     for (int k = 0; k < h.P; ++k) {
         const int64_t j0 = (int64_t)k * h.nb;
@@ -472,7 +651,6 @@ template <typename T>
 static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
     // X holds C[0:n,:] on entry.  Bottom-up over diagonal blocks:
     //   R_ii X_i = C_i ;  C_j <- C_j - R_ji X_i  for all j < i (one GEMM over rows 0..i0)
-    const T* A = P_<T>(h.dA);
     CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
     CK(find_zero_diag_launch<T>(P_<T>(h.dRd), h.nb, h.n, h.dFlag, h.sU));
     int flag = 0;
@@ -482,14 +660,24 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
     for (int i = h.P - 1; i >= 0; --i) {
         const int64_t i0 = (int64_t)i * h.nb;
         const int nbw = (int)std::min<int64_t>(h.nb, h.n - i0);
+        const T* Rcol = nullptr; int64_t ldr = 0;        // R[0:i0, i0:i0+nbw]
+        const int slot = i & 1;
+        if (i0 > 0) {
+            if (h.ooc) {
+                CKI(stream_panel_in<T>(h, slot, P_<T>(h.hA) + i0 * h.hlda, h.hlda, i0, nbw));
+                Rcol = P_<T>(h.dVb[slot]); ldr = h.ldvb;
+            } else { Rcol = P_<T>(h.dA) + i0 * h.lda; ldr = h.lda; }
+        }
         CK(trsm_diag_launch<T>(P_<T>(h.dRd) + (size_t)i * h.nb * h.nb, h.nb, nbw, X + i0, ldx, S, X + i0, ldx, h.sU));
         h.launches += 1;
         if (i0 > 0) {
+            if (h.ooc) CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
             GemmArgs<T> g{};
-            g.M = i0; g.N = S; g.K = nbw; g.A = A + i0 * h.lda; g.lda = h.lda; g.B = X + i0; g.ldb = ldx;
+            g.M = i0; g.N = S; g.K = nbw; g.A = Rcol; g.lda = ldr; g.B = X + i0; g.ldb = ldx;
             g.C = X; g.ldc = ldx; g.alpha = T(-1); g.beta = T(1);
             CK(gemm_dispatch<T>(false, g, 1, h.gemm_impl, h.sU));
             h.launches += 1;
+            if (h.ooc) CK(cudaEventRecord(h.evVfree[slot], h.sU));
         }
     }
     return 0;
@@ -554,6 +742,7 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
         }
     }
     cudaError_t es = cudaStreamSynchronize(h.sU);
+    if (h.sC) { cudaError_t ec = cudaStreamSynchronize(h.sC); if (es == cudaSuccess) es = ec; }
     if (rc == 0 && es != cudaSuccess) rc = set_err(CTQR_ERR_CUDA, "solve failed: %s", cudaGetErrorString(es));
     if (rc == 0) {
         float a = 0, b = 0;
@@ -636,12 +825,29 @@ static int get_R_typed(H& h, void* R, int64_t ldr) {
     return rc;
 }
 
+// out-of-core factor: off-diagonal blocks of R sit in the host matrix, diagonal blocks in dRd
+template <typename T>
+static int get_R_ooc(H& h, void* R, int64_t ldr) {
+    const int64_t n = h.n; const int nb = h.nb;
+    std::vector<T> rd((size_t)h.P * nb * nb), tmp((size_t)n * n, T(0));
+    CK(cudaMemcpy(rd.data(), h.dRd, rd.size() * sizeof(T), cudaMemcpyDeviceToHost));
+    const T* hA = P_<T>(h.hA);
+    for (int64_t c = 0; c < n; ++c) {
+        const int64_t pc = c / nb, p0 = pc * nb;
+        for (int64_t r = 0; r < p0; ++r) tmp[r + c * n] = hA[r + c * h.hlda];
+        for (int64_t r = p0; r <= c; ++r) tmp[r + c * n] = rd[(size_t)pc * nb * nb + (r - p0) + (c - p0) * (int64_t)nb];
+    }
+    CK(cudaMemcpy2D(R, ldr * sizeof(T), tmp.data(), n * sizeof(T), n * sizeof(T), n,
+                    is_device_ptr(R) ? cudaMemcpyHostToDevice : cudaMemcpyHostToHost));
+    return 0;
+}
+
 extern "C" int ct_qr_get_R(ctqr_handle_t h, void* R, int64_t ldr) {
     g_err[0] = 0;
     CKI(check_handle(h));
     if (!R) return set_err(-2, "R is NULL");
     if (ldr < h->n) return set_err(-3, "ldr < n");
-    if (h->ooc) return set_err(CTQR_ERR_STATE, "get_R is not available for an out-of-core factor");
+    if (h->ooc) return h->dtype == CTQR_F64 ? get_R_ooc<double>(*h, R, ldr) : get_R_ooc<float>(*h, R, ldr);
     return h->dtype == CTQR_F64 ? get_R_typed<double>(*h, R, ldr) : get_R_typed<float>(*h, R, ldr);
 }
 
@@ -652,7 +858,6 @@ extern "C" int ct_qr_get_V(ctqr_handle_t h, int64_t j0, int64_t ncols, void* V, 
     if (ncols < 1 || j0 + ncols > h->n) return set_err(-3, "ncols out of range");
     if (!V) return set_err(-4, "V is NULL");
     if (ldv < h->m) return set_err(-5, "ldv < m");
-    if (h->ooc) return set_err(CTQR_ERR_STATE, "get_V is not available for an out-of-core factor");
     // In-matrix storage already holds explicit V inside each panel's row range; rows above the
     // panel (R entries of earlier block rows) must be reported as zero.
     const size_t w = h->w;
@@ -661,8 +866,12 @@ extern "C" int ct_qr_get_V(ctqr_handle_t h, int64_t j0, int64_t ncols, void* V, 
         const int64_t j = j0 + c, p0 = (j / h->nb) * h->nb;
         char* dst = (char*)V + (size_t)c * ldv * w;
         if (ddev) CK(cudaMemsetAsync(dst, 0, (size_t)p0 * w, h->sU)); else memset(dst, 0, (size_t)p0 * w);
-        CK(cudaMemcpyAsync(dst + (size_t)p0 * w, (char*)h->dA + ((size_t)j * h->lda + p0) * w, (size_t)(h->m - p0) * w,
-                           ddev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->sU));
+        if (h->ooc)
+            CK(cudaMemcpyAsync(dst + (size_t)p0 * w, (char*)h->hA + ((size_t)j * h->hlda + p0) * w, (size_t)(h->m - p0) * w,
+                               ddev ? cudaMemcpyHostToDevice : cudaMemcpyHostToHost, h->sU));
+        else
+            CK(cudaMemcpyAsync(dst + (size_t)p0 * w, (char*)h->dA + ((size_t)j * h->lda + p0) * w, (size_t)(h->m - p0) * w,
+                               ddev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->sU));
     }
     CK(cudaStreamSynchronize(h->sU));
     return 0;
@@ -764,22 +973,28 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, double* sink) {
     }
 }
 
+extern "C" int ct_qr_peak_probe_cfg(int kind, int iters, int threads, int ctas_per_sm, double* tflops, double* ms_out);
 extern "C" int ct_qr_peak_probe(int kind, int iters, double* tflops, double* ms_out) {
+    return ct_qr_peak_probe_cfg(kind, iters, 256, 8, tflops, ms_out);
+}
+extern "C" int ct_qr_peak_probe_cfg(int kind, int iters, int threads, int ctas_per_sm, double* tflops, double* ms_out) {
     g_err[0] = 0;
+    if (threads < 32 || threads > 256 || threads % 32) return set_err(-3, "threads must be a multiple of 32 in [32, 256]");
+    if (ctas_per_sm < 1 || ctas_per_sm > 16) return set_err(-4, "ctas_per_sm must be in [1, 16]");
     if (kind < 0 || kind > 2) return set_err(-1, "kind must be 0, 1 or 2");
     if (iters < 1) return set_err(-2, "iters < 1");
     if (!tflops) return set_err(-3, "tflops is NULL");
     int dev = 0; CK(cudaGetDevice(&dev));
     cudaDeviceProp prop; CK(cudaGetDeviceProperties(&prop, dev));
     double* sink = nullptr; CK(cudaMalloc(&sink, 8));
-    const int ctas = prop.multiProcessorCount * 8;   // 8 CTAs of 256 threads per SM
+    const int ctas = prop.multiProcessorCount * ctas_per_sm;
     cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     float best = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {
         CK(cudaEventRecord(e0, 0));
-        if (kind == 0) peak_kernel<0><<<ctas, 256>>>(iters, sink);
-        else if (kind == 1) peak_kernel<1><<<ctas, 256>>>(iters, sink);
-        else peak_kernel<2><<<ctas, 256>>>(iters, sink);
+        if (kind == 0) peak_kernel<0><<<ctas, threads>>>(iters, sink);
+        else if (kind == 1) peak_kernel<1><<<ctas, threads>>>(iters, sink);
+        else peak_kernel<2><<<ctas, threads>>>(iters, sink);
         CK(cudaEventRecord(e1, 0));
         CK(cudaEventSynchronize(e1));
         float ms = 0; CK(cudaEventElapsedTime(&ms, e0, e1));
@@ -788,7 +1003,7 @@ extern "C" int ct_qr_peak_probe(int kind, int iters, double* tflops, double* ms_
     CK(cudaGetLastError());
     // flops per thread-iteration: FMA kinds 16 * 2; DMMA 16 * 512 per warp = 16 * 16 per thread
     const double per_thread = (kind == 2) ? 16.0 * 16.0 : 16.0 * 2.0;
-    const double flops = per_thread * (double)iters * 256.0 * ctas;
+    const double flops = per_thread * (double)iters * (double)threads * ctas;
     *tflops = flops / (best * 1e-3) / 1e12;
     if (ms_out) *ms_out = best;
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);

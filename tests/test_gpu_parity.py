@@ -175,3 +175,69 @@ def test_gemm_kernel(mnk, impl, ta, dt):
     ctqr.ct_qr_gemm(ta, M, N, K, -1.0, At, A.shape[0], Bt, K, 1.0, Ct, M, impl)
     got = ctqr.numpy_from_colmajor(Ct)
     assert relerr(got, ref) <= (1e-13 if dt == np.float64 else 2e-5)
+
+
+# ---- a5: out-of-core scheduler (SURVEY.md 8c rung T4) ---------------------------------------
+def _ooc_budget(m, nb, ns, dt):
+    w = np.dtype(dt).itemsize
+    lds = -(-m // (16 // w)) * (16 // w)
+    return (2 * ns + 2 * nb) * lds * w + 64
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("nb,ns,pinned", [(32, 288, True), (32, 160, False), (32, 96, True), (64, 64, False)])
+def test_out_of_core_matches_oracle_and_in_core(nb, ns, pinned, dt):
+    """Host-resident A with a capped device budget (P_s = 3, 5, 7, 11 super-panels): the factor is
+    written back into the host buffer; results must meet the same gates as in core and agree
+    with the in-core path to rounding."""
+    import torch
+    m, n, S = 700, 650, 9
+    rng = np.random.default_rng(21)
+    A = np.asfortranarray(rng.standard_normal((m, n)).astype(dt))
+    B = np.asfortranarray(rng.standard_normal((m, S)).astype(dt))
+    Ah = ctqr.colmajor_from_numpy(A, device="cpu", pin=pinned)
+    f = ctqr.ct_qr_factor(Ah, m, n, nb=nb, ib=16, device_budget_bytes=_ooc_budget(m, nb, ns, dt))
+    st = f.stats()
+    assert st["out_of_core"] == 1 and st["n_superpanels"] == -(-n // ns)
+    w = np.dtype(dt).itemsize
+    Ps = st["n_superpanels"]
+    assert st["d2h_bytes"] == m * n * w and st["h2d_bytes"] >= m * n * w
+    X = np.zeros((n, S), dtype=dt, order="F")
+    ctqr.ct_qr_solve(f, B, S, X)
+    R, V, tau = ctqr.ct_qr_get_R(f), ctqr.ct_qr_get_V(f), ctqr.ct_qr_get_tau(f)
+    VR, tau_o = oracle.qr(A)
+    assert backward_error(A, V, tau, R) <= BACKWARD[dt]
+    assert relerr(X, oracle.solve(VR, tau_o, B)) <= SOLUTION[dt]
+    assert relerr(R, oracle.R_of(VR)) <= ROUND[dt]
+    assert relerr(V, oracle.V_of(VR)) <= ROUND[dt]
+    # in-core on the same input
+    g = gpu_factor_solve(A, B, nb=nb, ib=16)
+    assert relerr(R, g["R"]) <= ROUND[dt] and relerr(X, g["X"]) <= SOLUTION[dt]
+    # the two halves of the solve through the streamed path
+    C = B.copy(order="F"); ctqr.ct_qr_apply_qt(f, C, S)
+    assert relerr(C, oracle.apply_qt(VR, tau_o, B)) <= ROUND[dt]
+
+
+@pytest.mark.parametrize("dt", DT)
+def test_out_of_core_ct_config(dt):
+    """BASELINE.json configs[0] streamed through 4 super-panels of 256 columns."""
+    c = wl.CONFIGS["c1"]
+    coo = wl.siddon_coo(c.N, c.n_ang, c.n_bins)
+    A, lam = wl.dense_augmented(c, dt, coo)
+    X0, B = wl.make_slices(c, coo=coo, lam=lam)
+    B = np.asfortranarray(B.astype(dt))
+    Ah = ctqr.colmajor_from_numpy(A, device="cpu", pin=True)
+    f = ctqr.ct_qr_factor(Ah, c.m, c.n, device_budget_bytes=_ooc_budget(c.m, 128, 256, dt))
+    assert f.stats()["n_superpanels"] == 4
+    X = np.zeros((c.n, c.S), dtype=dt, order="F")
+    ctqr.ct_qr_solve(f, B, c.S, X)
+    VR, tau_o = oracle.qr(A)
+    assert relerr(X, oracle.solve(VR, tau_o, B)) <= SOLUTION[dt]
+    assert backward_error(A, ctqr.ct_qr_get_V(f), ctqr.ct_qr_get_tau(f), ctqr.ct_qr_get_R(f)) <= BACKWARD[dt]
+
+
+def test_out_of_core_budget_too_small():
+    A = np.asfortranarray(np.random.default_rng(0).standard_normal((300, 200)))
+    with pytest.raises(ctqr.CtqrError) as ei:
+        ctqr.ct_qr_factor(A.copy(order="F"), 300, 200, nb=32, device_budget_bytes=1000)
+    assert ei.value.code == 2

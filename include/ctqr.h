@@ -51,7 +51,7 @@ typedef enum {
 /* Options for ct_qr_factor.  Zero-initialise for defaults. */
 typedef struct {
     int32_t nb;                 /* panel width; 0 = default (128). Must be a multiple of ib. */
-    int32_t ib;                 /* inner (register-resident) panel width: 8, 16 or 32; 0 = default */
+    int32_t ib;                 /* inner (register-resident) panel width: 8, 16 or 32; 0 = default (32) */
     int32_t lookahead;          /* 0 = off, 1 = factor panel k+1 while the rest of update k runs; -1 = default */
     int32_t in_place;           /* 1: A (device) is overwritten and must outlive the handle.
                                    0: A is read-only; the handle owns a copy. */

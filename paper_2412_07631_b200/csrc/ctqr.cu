@@ -17,25 +17,22 @@
 
 using namespace ctqr;
 
-template <typename T> static cudaError_t gemm_dispatch(bool ta, const GemmArgs<T>& g, int splits, int impl, cudaStream_t st);
-template <> cudaError_t gemm_dispatch<double>(bool ta, const GemmArgs<double>& g, int splits, int impl, cudaStream_t st) { return gemm_f64(ta, g, splits, impl, st); }
-template <> cudaError_t gemm_dispatch<float>(bool ta, const GemmArgs<float>& g, int splits, int impl, cudaStream_t st) { return gemm_f32(ta, g, splits, impl, st); }
-template <typename T> static void gemm_tile(bool ta, int64_t M, int64_t N, int impl, int* bm, int* bn);
-template <> void gemm_tile<double>(bool ta, int64_t M, int64_t N, int impl, int* bm, int* bn) { gemm_tile_f64(ta, M, N, impl, bm, bn); }
-template <> void gemm_tile<float>(bool ta, int64_t M, int64_t N, int impl, int* bm, int* bn) { gemm_tile_f32(ta, M, N, impl, bm, bn); }
+template <typename T> static GemmLaunch gemm_plan(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned);
+template <> GemmLaunch gemm_plan<double>(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned) { return gemm_plan_f64(ta, M, N, K, impl, sms, partial, max_slots, aligned); }
+template <> GemmLaunch gemm_plan<float>(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned) { return gemm_plan_f32(ta, M, N, K, impl, sms, partial, max_slots, aligned); }
+template <typename T> static bool gemm_aligned(const GemmArgs<T>& g) {
+    return ((uintptr_t)g.A % 16 == 0) && ((uintptr_t)g.B % 16 == 0) && ((g.lda * (int64_t)sizeof(T)) % 16 == 0) &&
+           ((g.ldb * (int64_t)sizeof(T)) % 16 == 0);
+}
+template <typename T> static cudaError_t gemm_run(bool ta, const GemmArgs<T>& g, const GemmLaunch& L, int impl, cudaStream_t st);
+template <> cudaError_t gemm_run<double>(bool ta, const GemmArgs<double>& g, const GemmLaunch& L, int impl, cudaStream_t st) { return gemm_run_f64(ta, g, L, impl, st); }
+template <> cudaError_t gemm_run<float>(bool ta, const GemmArgs<float>& g, const GemmLaunch& L, int impl, cudaStream_t st) { return gemm_run_f32(ta, g, L, impl, st); }
+// direct product C <- alpha op(A) B + beta C
+template <typename T> static cudaError_t gemm_direct(bool ta, const GemmArgs<T>& g, int impl, int sms, cudaStream_t st) {
+    return gemm_run<T>(ta, g, gemm_plan<T>(ta, g.M, g.N, g.K, impl, sms, false, 1, gemm_aligned(g)), impl, st);
+}
 static cudaError_t panel_launch(int ib, int rpt, PanelArgs<double>& pa, int G, cudaStream_t st) { return panel_launch_f64(ib, rpt, pa, G, st); }
 static cudaError_t panel_launch(int ib, int rpt, PanelArgs<float>& pa, int G, cudaStream_t st) { return panel_launch_f32(ib, rpt, pa, G, st); }
-
-// split-K factor for a product whose output-tile grid cannot fill the machine
-static int pick_splits(int64_t tiles, int64_t K, int sms, int ctas_per_sm, int64_t min_chunk) {
-    int64_t slots = (int64_t)sms * ctas_per_sm;
-    if (tiles >= slots) return 1;
-    int64_t s = slots / tiles;
-    int64_t maxs = K / min_chunk; if (maxs < 1) maxs = 1;
-    if (s > maxs) s = maxs;
-    if (s < 1) s = 1;
-    return (int)s;
-}
 
 // ------------------------------------------------------------------------------------------
 // error plumbing
@@ -140,32 +137,29 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
                  T* C, int64_t ldc, int64_t nc, bool prof = false) {
     if (nc <= 0 || mk <= 0 || kw <= 0) return 0;
     const int64_t ldw = round_up(kw, 4);
-    // W = V^T C, split over K when the output grid cannot fill the machine
-    int bm = 128, bn = 128;
-    gemm_tile<T>(true, kw, nc, h.gemm_impl, &bm, &bn);
-    int64_t tiles = ceil_div(kw, bm) * ceil_div(nc, bn);
-    int splits = pick_splits(tiles, mk, h.sms, 2, kw <= 32 ? 256 : 512);
+    // W = V^T C as partial products over K (stream-K or split grid), summed by the T^T W kernel
     const int64_t sstride = ldw * nc;
-    while (splits > 1 && (size_t)splits * sstride > h.wp_elems[ws]) --splits;
-    if ((size_t)splits * sstride > h.wp_elems[ws] || (size_t)sstride > h.w_elems[ws])
+    if ((size_t)sstride > h.wp_elems[ws] || (size_t)sstride > h.w_elems[ws])
         return set_err(CTQR_ERR_NOMEM, "larfb workspace too small (kw=%d nc=%lld)", kw, (long long)nc);
     T* Wp = P_<T>(h.dWp[ws]);
     T* W = P_<T>(h.dW[ws]);
     GemmArgs<T> g1{};
     g1.M = kw; g1.N = nc; g1.K = mk; g1.A = V; g1.lda = ldv; g1.B = C; g1.ldb = ldc;
     g1.C = Wp; g1.ldc = ldw; g1.alpha = T(1); g1.beta = T(0); g1.split_stride = sstride;
+    const GemmLaunch L1 = gemm_plan<T>(true, kw, nc, mk, h.gemm_impl, h.sms, true,
+                                       (int64_t)(h.wp_elems[ws] / (size_t)sstride), gemm_aligned(g1));
     prof = prof && h.profile;
     const double fl = 2.0 * (double)mk * (double)kw * (double)nc;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
-    CK(gemm_dispatch<T>(true, g1, splits, h.gemm_impl, st));
+    CK(gemm_run<T>(true, g1, L1, h.gemm_impl, st));
     if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 0}); }
-    CK(ttw_launch<T>(Wp, splits, sstride, ldw, Tm, ldt, kw, nc, W, ldw, st));
+    CK(ttw_launch<T>(Wp, L1.seg, sstride, ldw, Tm, ldt, kw, nc, W, ldw, st));
     GemmArgs<T> g2{};
     g2.M = mk; g2.N = nc; g2.K = kw; g2.A = V; g2.lda = ldv; g2.B = W; g2.ldb = ldw;
     g2.C = C; g2.ldc = ldc; g2.alpha = T(-1); g2.beta = T(1);
     if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
-    CK(gemm_dispatch<T>(false, g2, 1, h.gemm_impl, st));
+    CK(gemm_direct<T>(false, g2, h.gemm_impl, h.sms, st));
     if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 1}); }
     h.launches += 3;
     return 0;
@@ -186,31 +180,42 @@ static void resolve_spans(H& h) {
 // panel factorisation (a1 + a2) of columns [j0, j0+nbw) of the device matrix A (rows j0..m)
 // ------------------------------------------------------------------------------------------
 template <typename T>
-static int launch_panel(H& h, cudaStream_t st, PanelArgs<T>& pa, int rpt, int G) {
+static int launch_panel(H& h, int ib, cudaStream_t st, PanelArgs<T>& pa, int rpt, int G) {
     pa.bar_base = h.bar_count;
-    cudaError_t e = panel_launch(h.ib, rpt, pa, G, st);
+    cudaError_t e = panel_launch(ib, rpt, pa, G, st);
     if (e != cudaSuccess)
-        return set_err(CTQR_ERR_CUDA, "panel kernel launch failed (ib=%d rpt=%d G=%d): %s", h.ib, rpt, G, cudaGetErrorString(e));
-    h.bar_count += (unsigned)G * (unsigned)pa.ibw;
+        return set_err(CTQR_ERR_CUDA, "panel kernel launch failed (ib=%d rpt=%d G=%d): %s", ib, rpt, G, cudaGetErrorString(e));
+    h.bar_count += (unsigned)pa.ibw;          // one step number per column, never reused by this handle
     h.launches += 1;
     return 0;
 }
 
+// rows-per-thread variants compiled for (dtype, ib), most rows first
 template <typename T>
-static int panel_inner(H& h, cudaStream_t st, T* A, int64_t lda, int64_t m, int64_t j0, int64_t jb, int ibw, T* Rd) {
+static const int* panel_rpts(int ib) {
+    static const int rpts_f64_16[] = {4, 2, 1, 0}, rpts_f32_16[] = {8, 4, 2, 1, 0};
+    static const int rpts_8[] = {8, 2, 0}, rpts_f64_32[] = {2, 1, 0}, rpts_f32_32[] = {4, 2, 1, 0};
+    return ib == 16 ? (sizeof(T) == 8 ? rpts_f64_16 : rpts_f32_16)
+         : ib == 8  ? rpts_8 : (sizeof(T) == 8 ? rpts_f64_32 : rpts_f32_32);
+}
+// widest inner block <= h.ib whose register-resident kernel can hold `rows` rows on this device
+template <typename T>
+static int panel_ib_for(const H& h, int64_t rows) {
+    for (int ib = h.ib; ib >= 8; ib /= 2)
+        if (ceil_div(rows, (int64_t)kPanelThreads * panel_rpts<T>(ib)[0]) <= h.sms) return ib;
+    return 0;
+}
+
+template <typename T>
+static int panel_inner(H& h, int ib, cudaStream_t st, T* A, int64_t lda, int64_t m, int64_t j0, int64_t jb, int ibw, T* Rd, T* Tin) {
     constexpr int NT = kPanelThreads;
     PanelArgs<T> pa{};
     pa.A = A; pa.lda = lda; pa.m = m; pa.j0 = j0; pa.jb = jb; pa.ibw = ibw;
-    pa.tau = P_<T>(h.dTau); pa.Rd = Rd; pa.ldrd = h.nb; pa.Tin = P_<T>(h.dTin);
+    pa.tau = P_<T>(h.dTau); pa.Rd = Rd; pa.ldrd = h.nb; pa.Tin = Tin; pa.ldtin = h.nb;
     pa.part = P_<T>(h.dPart); pa.rowbuf = P_<T>(h.dRow); pa.bar = h.dBar;
     const int64_t rows = m - jb;
     const int gmax = h.sms;
-    // rows-per-thread variants compiled for (dtype, ib); prefer the fewest CTAs that keep the
-    // register file un-spilled: the cross-CTA reduction costs grow with G
-    static const int rpts_f64_16[] = {4, 2, 1, 0}, rpts_f32_16[] = {8, 4, 2, 1, 0};
-    static const int rpts_8[] = {8, 2, 0}, rpts_f64_32[] = {2, 1, 0}, rpts_f32_32[] = {4, 2, 1, 0};
-    const int* list = h.ib == 16 ? (sizeof(T) == 8 ? rpts_f64_16 : rpts_f32_16)
-                    : h.ib == 8  ? rpts_8 : (sizeof(T) == 8 ? rpts_f64_32 : rpts_f32_32);
+    const int* list = panel_rpts<T>(ib);
     // largest rpt whose grid still has >= 8 CTAs (enough parallelism), else the smallest that fits
     int pick = 0;
     for (const int* r = list; *r; ++r) {
@@ -222,43 +227,41 @@ static int panel_inner(H& h, cudaStream_t st, T* A, int64_t lda, int64_t m, int6
             if (ceil_div(rows, (int64_t)NT * *r) <= gmax) { pick = *r; break; }
     if (!pick)
         return set_err(CTQR_ERR_NOMEM, "panel of %lld rows does not fit the register-resident kernel (ib=%d)",
-                       (long long)rows, h.ib);
-    return launch_panel<T>(h, st, pa, pick, (int)std::max<int64_t>(1, ceil_div(rows, (int64_t)NT * pick)));
+                       (long long)rows, ib);
+    return launch_panel<T>(h, ib, st, pa, pick, (int)std::max<int64_t>(1, ceil_div(rows, (int64_t)NT * pick)));
 }
 
 template <typename T>
 static int panel_factor(H& h, cudaStream_t st, T* A, int64_t lda, int64_t m, int64_t j0, int nbw, int k) {
     T* Rd = P_<T>(h.dRd) + (size_t)k * h.nb * h.nb;
     T* Tk = P_<T>(h.dT) + (size_t)k * h.nb * h.nb;
-    for (int64_t jb = j0; jb < j0 + nbw; jb += h.ib) {
-        const int ibw = (int)std::min<int64_t>(h.ib, j0 + nbw - jb);
-        CKI(panel_inner<T>(h, st, A, lda, m, j0, jb, ibw, Rd));
+    // inner width for this panel: h.ib unless the panel is too tall for that kernel's registers
+    const int ib = panel_ib_for<T>(h, m - j0);
+    if (!ib)
+        return set_err(CTQR_ERR_NOMEM, "panel of %lld rows does not fit the register-resident panel kernel",
+                       (long long)(m - j0));
+    for (int64_t jb = j0; jb < j0 + nbw; jb += ib) {
+        const int ibw = (int)std::min<int64_t>(ib, j0 + nbw - jb);
+        T* Tin = Tk + (jb - j0) + (jb - j0) * (int64_t)h.nb;      // diagonal block of T_k
+        CKI(panel_inner<T>(h, ib, st, A, lda, m, j0, jb, ibw, Rd, Tin));
         const int64_t ncp = j0 + nbw - (jb + ibw);
         if (ncp > 0)
-            CKI(larfb<T>(h, 1, st, A + jb + jb * lda, lda, m - jb, ibw, P_<T>(h.dTin), h.ib,
+            CKI(larfb<T>(h, 1, st, A + jb + jb * lda, lda, m - jb, ibw, Tin, h.nb,
                          A + jb + (jb + ibw) * lda, lda, ncp));
     }
-    if (nbw <= h.ib) {
-        // single inner block: its T is the panel's T
-        CK(copy2d_launch<T>(P_<T>(h.dTin), h.ib, Tk, h.nb, nbw, nbw, st));
-        h.launches += 1;
-        return 0;
-    }
+    if (nbw <= ib) return 0;            // single inner block: its T is the panel's T
     // T_k from the Gram matrix of the finished panel
     const T* V = A + j0 + j0 * lda;
     const int64_t mk = m - j0;
     const int64_t ldg = round_up(nbw, 4);
-    int bm = 128, bn = 128;
-    gemm_tile<T>(true, nbw, nbw, h.gemm_impl, &bm, &bn);
-    int64_t tiles = ceil_div(nbw, bm) * ceil_div(nbw, bn);
-    int splits = pick_splits(tiles, mk, h.sms, 1, 256);
     const int64_t gstride = ldg * nbw;
-    while (splits > 1 && (size_t)splits * gstride > h.wp_elems[1]) --splits;
     GemmArgs<T> g{};
     g.M = nbw; g.N = nbw; g.K = mk; g.A = V; g.lda = lda; g.B = V; g.ldb = lda;
     g.C = P_<T>(h.dWp[1]); g.ldc = ldg; g.alpha = T(1); g.beta = T(0); g.split_stride = gstride;
-    CK(gemm_dispatch<T>(true, g, splits, h.gemm_impl, st));
-    CK(larft_launch<T>(P_<T>(h.dWp[1]), splits, gstride, (int)ldg, P_<T>(h.dTau) + j0, nbw, Tk, h.nb, st));
+    const GemmLaunch LG = gemm_plan<T>(true, nbw, nbw, mk, h.gemm_impl, h.sms, true,
+                                       (int64_t)(h.wp_elems[1] / (size_t)gstride), gemm_aligned(g));
+    CK(gemm_run<T>(true, g, LG, h.gemm_impl, st));
+    CK(larft_launch<T>(P_<T>(h.dWp[1]), LG.seg, gstride, (int)ldg, nbw, ib, Tk, h.nb, st));
     h.launches += 2;
     return 0;
 }
@@ -492,7 +495,9 @@ static int alloc_state(H& h, int64_t max_nc) {
         CK(cudaMalloc(&h.dWp[i], h.wp_elems[i] * sizeof(T)));
     }
     CK(cudaMalloc(&h.dTin, 32 * 32 * sizeof(T)));
-    CK(cudaMalloc(&h.dPart, (size_t)2 * 256 * 32 * sizeof(T)));
+    // LL slots of the panel kernel: [2 parities][G + 1 <= 257][IB <= 32] x 16 bytes, step numbers start at 1
+    CK(cudaMalloc(&h.dPart, (size_t)2 * 257 * 32 * 16));
+    CK(cudaMemsetAsync(h.dPart, 0, (size_t)2 * 257 * 32 * 16, h.sU));
     CK(cudaMalloc(&h.dRow, 2 * 32 * sizeof(T)));
     CK(cudaMalloc(&h.dBar, sizeof(unsigned)));
     CK(cudaMemsetAsync(h.dBar, 0, sizeof(unsigned), h.sU));
@@ -585,7 +590,7 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
     h->dtype = dtype; h->w = dtype == CTQR_F64 ? 8 : 4;
     h->m = m; h->n = n;
     h->nb = o.nb > 0 ? o.nb : 128;
-    h->ib = o.ib > 0 ? o.ib : 16;
+    h->ib = o.ib > 0 ? o.ib : 32;
     if (h->ib != 8 && h->ib != 16 && h->ib != 32) { delete h; return set_err(-6, "ib must be 8, 16 or 32"); }
     if (h->nb > 128 || h->nb % h->ib != 0) { delete h; return set_err(-6, "nb must be a multiple of ib and <= 128"); }
     h->lookahead = o.lookahead < 0 ? 1 : (o.lookahead ? 1 : 0);
@@ -675,7 +680,7 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
             GemmArgs<T> g{};
             g.M = i0; g.N = S; g.K = nbw; g.A = Rcol; g.lda = ldr; g.B = X + i0; g.ldb = ldx;
             g.C = X; g.ldc = ldx; g.alpha = T(-1); g.beta = T(1);
-            CK(gemm_dispatch<T>(false, g, 1, h.gemm_impl, h.sU));
+            CK(gemm_direct<T>(false, g, h.gemm_impl, h.sms, h.sU));
             h.launches += 1;
             if (h.ooc) CK(cudaEventRecord(h.evVfree[slot], h.sU));
         }
@@ -922,7 +927,8 @@ static int gemm_typed(int ta, int64_t M, int64_t N, int64_t K, double alpha, con
     GemmArgs<T> g{};
     g.M = M; g.N = N; g.K = K; g.A = (const T*)A; g.lda = lda; g.B = (const T*)B; g.ldb = ldb;
     g.C = (T*)C; g.ldc = ldc; g.alpha = (T)alpha; g.beta = (T)beta; g.split_stride = 0;
-    CK(gemm_dispatch<T>(ta != 0, g, 1, impl, 0));
+    int dev = 0, sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    CK(gemm_direct<T>(ta != 0, g, impl, sms, 0));
     CK(cudaDeviceSynchronize());
     return 0;
 }
@@ -961,6 +967,51 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, double* sink) {
             for (int i = 0; i < 16; ++i) c[i] = fma(a, c[i], b);
         double s = 0; for (int i = 0; i < 16; ++i) s += c[i];
         if (s == 12345.678) sink[0] = s;
+    } else if (KIND == 4 || KIND == 5) {
+        // DMMA with a GEMM-like operand pattern: 4 x 4 outer product of fragments per k-step (16 DMMA);
+        // KIND 5 additionally reloads the 8 fragments from shared memory every k-step (no barrier).
+        __shared__ double sm[4 * 20 * 40];
+        for (int i = threadIdx.x; i < 4 * 20 * 40; i += blockDim.x) sm[i] = 1.0 + 1e-9 * i;
+        __syncthreads();
+        double a[4], b[4], c[4][4][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { a[i] = 1.0 + lane * 1e-9 + i; b[i] = 0.5 + i; }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { c[i][j][0] = i; c[i][j][1] = j; }
+        const int grp = lane >> 2, tig = lane & 3;
+        for (int it = 0; it < iters; ++it) {
+            if (KIND == 5) {
+                const double* As = sm + ((it & 3) * 4) ;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) { a[i] = As[(i * 8 + grp) * 20 + tig]; b[i] = As[(32 + i * 8 + grp) * 20 + tig]; }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+        }
+        double s = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) s += c[i][j][0] + c[i][j][1];
+        if (s == 12345.678) sink[0] = s;
+    } else if (KIND == 3) {
+        // legacy warp-level TF32 tensor path: mma.sync.m16n8k8 (SASS HMMA.1688.F32.TF32), 4096 flop per warp
+        unsigned a[4] = {0x3f800000u + lane, 0x3f800100u, 0x3f800200u, 0x3f800300u}, b[2] = {0x3f000000u, 0x3f000100u};
+        float c[16][4];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { c[i][0] = i; c[i][1] = -i; c[i][2] = 1; c[i][3] = 2; }
+        for (int it = 0; it < iters; ++it)
+#pragma unroll
+            for (int i = 0; i < 16; ++i)
+                asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+                             : "+f"(c[i][0]), "+f"(c[i][1]), "+f"(c[i][2]), "+f"(c[i][3])
+                             : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+        float s = 0; for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1] + c[i][2] + c[i][3];
+        if (s == 12345.678f) sink[0] = s;
     } else {
         double a = 1.0 + lane * 1e-9, b = 0.5, c[16][2];
 #pragma unroll
@@ -981,7 +1032,7 @@ extern "C" int ct_qr_peak_probe_cfg(int kind, int iters, int threads, int ctas_p
     g_err[0] = 0;
     if (threads < 32 || threads > 256 || threads % 32) return set_err(-3, "threads must be a multiple of 32 in [32, 256]");
     if (ctas_per_sm < 1 || ctas_per_sm > 16) return set_err(-4, "ctas_per_sm must be in [1, 16]");
-    if (kind < 0 || kind > 2) return set_err(-1, "kind must be 0, 1 or 2");
+    if (kind < 0 || kind > 5) return set_err(-1, "kind must be 0..5");
     if (iters < 1) return set_err(-2, "iters < 1");
     if (!tflops) return set_err(-3, "tflops is NULL");
     int dev = 0; CK(cudaGetDevice(&dev));
@@ -994,7 +1045,10 @@ extern "C" int ct_qr_peak_probe_cfg(int kind, int iters, int threads, int ctas_p
         CK(cudaEventRecord(e0, 0));
         if (kind == 0) peak_kernel<0><<<ctas, threads>>>(iters, sink);
         else if (kind == 1) peak_kernel<1><<<ctas, threads>>>(iters, sink);
-        else peak_kernel<2><<<ctas, threads>>>(iters, sink);
+        else if (kind == 2) peak_kernel<2><<<ctas, threads>>>(iters, sink);
+        else if (kind == 3) peak_kernel<3><<<ctas, threads>>>(iters, sink);
+        else if (kind == 4) peak_kernel<4><<<ctas, threads>>>(iters, sink);
+        else peak_kernel<5><<<ctas, threads>>>(iters, sink);
         CK(cudaEventRecord(e1, 0));
         CK(cudaEventSynchronize(e1));
         float ms = 0; CK(cudaEventElapsedTime(&ms, e0, e1));
@@ -1002,7 +1056,7 @@ extern "C" int ct_qr_peak_probe_cfg(int kind, int iters, int threads, int ctas_p
     }
     CK(cudaGetLastError());
     // flops per thread-iteration: FMA kinds 16 * 2; DMMA 16 * 512 per warp = 16 * 16 per thread
-    const double per_thread = (kind == 2) ? 16.0 * 16.0 : 16.0 * 2.0;
+    const double per_thread = (kind == 2 || kind >= 4) ? 16.0 * 16.0 : (kind == 3) ? 16.0 * 128.0 : 16.0 * 2.0;
     const double flops = per_thread * (double)iters * (double)threads * ctas;
     *tflops = flops / (best * 1e-3) / 1e12;
     if (ms_out) *ms_out = best;

@@ -1,28 +1,74 @@
-// gemm_f64.cu -- fp64 instantiations of the contraction kernels (DMMA tensor-core path + SIMT check).
+// gemm_f64.cu -- fp64 instantiations of the contraction kernels: persistent stream-K DMMA kernel
+// (gemm_mma.cuh) for the big products, the classic DMMA grid kernel for skinny in-panel shapes,
+// SIMT DFMA as cross-check (impl 1).
+#include <algorithm>
 #include "gemm.cuh"
+#include "gemm_mma.cuh"
 
 namespace ctqr {
 
-void gemm_tile_f64(bool ta, int64_t M, int64_t N, int impl, int* bm, int* bn) {
-    if (impl == 1) { *bm = 64; *bn = 64; return; }
-    if (ta) { if (M <= 32) { *bm = 32; *bn = 128; } else { *bm = 128; *bn = 64; } }
-    else    { if (N <= 32) { *bm = 128; *bn = 32; } else { *bm = 128; *bn = 64; } }
+static GemmLaunch classic_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, int sms, int64_t min_chunk,
+                               bool partial, int64_t max_slots, int cfg) {
+    GemmLaunch L{};
+    L.kind = 0; L.cfg = cfg; L.partial = partial ? 1 : 0;
+    int s = 1;
+    if (partial) {
+        s = pick_splits(ceil_div(M, bm) * ceil_div(N, bn), K, 16, sms, 2, min_chunk);
+        if (s > max_slots) s = (int)std::max<int64_t>(1, max_slots);
+    }
+    L.splits = s; L.slots = s;
+    L.seg = SegInfo{s, 0, 0, bn};
+    return L;
 }
 
-cudaError_t gemm_f64(bool ta, GemmArgs<double> g, int splits, int impl, cudaStream_t st) {
+static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, int bk, int sms, bool partial,
+                               int64_t max_slots, int cfg) {
+    int slots = sms * 2;
+    MmaPlan p = mma_plan(M, N, K, bm, bn, bk, slots, partial);
+    while (partial && p.maxseg > max_slots && slots > 1) { slots /= 2; p = mma_plan(M, N, K, bm, bn, bk, slots, partial); }
+    GemmLaunch L{};
+    L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
+    L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
+    L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
+    return L;
+}
+
+GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots,
+                         bool aligned) {
+    if (impl == 1) return classic_plan(M, N, K, 64, 64, sms, 256, partial, max_slots, 9);
+    if (ta) {
+        if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_slots, 0);
+        if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_slots, 6);
+        return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_slots, 1);
+    }
+    if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_slots, 2);
+    if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_slots, 7);
+    return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_slots, 3);
+}
+
+static MmaPlan to_plan(const GemmLaunch& L) {
+    MmaPlan p{};
+    p.sk.tilesM = L.tilesM; p.sk.tilesN = L.tilesN; p.sk.KT = L.KT; p.sk.U = L.U; p.sk.L = L.L; p.sk.partial = L.partial;
+    p.grid = L.grid; p.maxseg = L.slots;
+    return p;
+}
+
+cudaError_t gemm_run_f64(bool ta, GemmArgs<double> g, const GemmLaunch& L, int impl, cudaStream_t st) {
     if (g.M <= 0 || g.N <= 0) return cudaSuccess;
     g.a_vec_ok = aligned16(g.A, g.lda, 8);
     g.b_vec_ok = aligned16(g.B, g.ldb, 8);
-    if (impl == 1) {
-        return ta ? launch_simt<double, true, 64, 64, 8>(g, splits, st)
-                  : launch_simt<double, false, 64, 64, 8>(g, splits, st);
+    (void)impl;
+    switch (L.cfg) {
+        case 9: return ta ? launch_simt<double, true, 64, 64, 8>(g, L.splits, st)
+                          : launch_simt<double, false, 64, 64, 8>(g, L.splits, st);
+        case 0: return launch_dmma<true, 32, 128, 32, 32, 16, 4, 2>(g, L.splits, st);
+        case 1: return launch_mma<double, true, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
+        case 2: return launch_dmma<false, 128, 32, 32, 32, 16, 3, 2>(g, L.splits, st);
+        case 6: return launch_dmma<true, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);
+        case 7: return launch_dmma<false, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);
+        case 3: return launch_mma<double, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
     }
-    if (ta) {
-        if (g.M <= 32) return launch_dmma<true, 32, 128, 32, 32, 16, 4, 2>(g, splits, st);
-        return launch_dmma<true, 128, 64, 64, 32, 16, 3, 2>(g, splits, st);
-    }
-    if (g.N <= 32) return launch_dmma<false, 128, 32, 32, 32, 16, 3, 2>(g, splits, st);
-    return launch_dmma<false, 128, 64, 64, 32, 16, 3, 2>(g, splits, st);
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace ctqr

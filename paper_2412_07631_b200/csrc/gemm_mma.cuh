@@ -1,0 +1,386 @@
+// gemm_mma.cuh -- persistent, stream-K, warp-level tensor-core contraction (SURVEY.md 8a rows
+// a3 / a6 / a7: the larfb products W = V^T C and C <- C - V W, the Gram matrix of larft and the
+// GEMM tasks of the blocked TRSM).
+//
+//   C <- alpha * op(A) * B + beta * C,  column-major, op(A) = A^T (A is K x M) or A (M x K), B is K x N.
+//
+// Why this shape (ncu, profiles/r1a_launches_c3_f64.md): the first kernels were latency-bound by
+// occupancy (1-2 warps per SM sub-partition) and by wave quantisation (152 CTAs on 296 slots),
+// not by DRAM or by the tensor pipe.  So:
+//   * 8 warps per CTA with 32x32 warp tiles (<= 128 registers) -> 2 CTAs = 16 warps per SM;
+//   * the grid is one wave of co-resident CTAs (a multiple of the SM count); the flattened
+//     sequence of (output tile, k-tile) units is cut into equal contiguous ranges, one per CTA
+//     ("stream-K"), so every CTA does the same work whatever the tile count;
+//   * the cp.async pipeline runs over the FLAT unit sequence, i.e. it keeps prefetching across
+//     tile boundaries: no prologue bubble per tile (matters for C <- C - V W where K is only nb);
+//   * a tile whose k-range is cut writes per-segment partial tiles; the consumer kernel
+//     (T^T W, larft) sums them in a fixed order -> deterministic, no atomics.
+// Precision policies:
+//   double: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4) -- the only native FP64 tensor instruction
+//           of sm_100a (tcgen05 has no f64 kind).
+//   float : 3xTF32 split on mma.sync.m16n8k8.tf32 (SASS HMMA.1688.F32.TF32): x = hi + lo with
+//           hi = tf32(x), lo = tf32(x - hi); a*b ~= hi_a*hi_b + hi_a*lo_b + lo_a*hi_b accumulated
+//           in fp32.  Measured 557 TFLOP/s for the plain instruction on B200, i.e. ~185 TFLOP/s of
+//           fp32-equivalent work against 74 TFLOP/s of FFMA.  north_star allows it "only if it
+//           meets the fp32 tolerance": the parity tests run on this path.
+#pragma once
+#include <algorithm>
+#include "common.cuh"
+#include "kernels.h"
+
+namespace ctqr {
+
+// -------------------------------------------------------------------------------------------
+// precision policies: fragment loads + MMA for one k-step of a (WM x WN) warp tile
+// -------------------------------------------------------------------------------------------
+template <typename T> struct MmaPolicy;
+
+template <> struct MmaPolicy<double> {
+    static constexpr int BK = 16;        // k-tile: 16 doubles = 128 bytes per row
+    static constexpr int KSTEP = 4;      // k per MMA
+    static constexpr int MFRAG = 8;      // rows per A fragment
+    static constexpr int PAD_K = 4;      // K-contiguous tiles: ld = BK + 4  (== 4 mod 16 doubles)
+    static constexpr int PAD_M = 4;      // M-contiguous tiles: ld = BM + 4
+    static constexpr int ACC = 2;        // accumulator registers per (m-frag, n-frag)
+    template <bool TA, int MT, int NTL, int LDK, int LDM>
+    static __device__ __forceinline__ void kstep(const double* As, const double* Bs, int kk, int mrow0, int ncol0,
+                                                 int grp, int tig, double (&acc)[MT][NTL][2]) {
+        double a[MT], b[NTL];
+#pragma unroll
+        for (int i = 0; i < MT; ++i) {
+            const int mrow = mrow0 + i * 8 + grp;
+            a[i] = TA ? As[mrow * LDK + kk + tig] : As[(kk + tig) * LDM + mrow];
+        }
+#pragma unroll
+        for (int j = 0; j < NTL; ++j) b[j] = Bs[(ncol0 + j * 8 + grp) * LDK + kk + tig];
+#pragma unroll
+        for (int i = 0; i < MT; ++i)
+#pragma unroll
+            for (int j = 0; j < NTL; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+    }
+    // element (r, c) of accumulator register q inside an (8 x 8) fragment
+    static __device__ __forceinline__ int frag_row(int q, int grp) { (void)q; return grp; }
+    static __device__ __forceinline__ int frag_col(int q, int tig) { return 2 * tig + q; }
+};
+
+__device__ __forceinline__ unsigned tf32_of(float x) {
+    unsigned r;
+    asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ void mma_tf32(float (&c)[4], const unsigned (&a)[4], const unsigned (&b)[2]) {
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+
+template <> struct MmaPolicy<float> {
+    static constexpr int BK = 32;        // 32 floats = 128 bytes per row
+    static constexpr int KSTEP = 8;
+    static constexpr int MFRAG = 16;
+    static constexpr int PAD_K = 4;      // ld = 36 == 4 mod 32 words: rows grp*4 + tig hit 32 distinct banks
+    static constexpr int PAD_M = 8;      // ld = BM + 8 == 8 mod 32: tig*8 + grp distinct
+    static constexpr int ACC = 4;
+    template <bool TA, int MT, int NTL, int LDK, int LDM>
+    static __device__ __forceinline__ void kstep(const float* As, const float* Bs, int kk, int mrow0, int ncol0,
+                                                 int grp, int tig, float (&acc)[MT][NTL][4]) {
+        unsigned ah[MT][4], al[MT][4], bh[NTL][2], bl[NTL][2];
+#pragma unroll
+        for (int i = 0; i < MT; ++i) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int mrow = mrow0 + i * 16 + grp + (q & 1) * 8;
+                const int k = kk + tig + (q >> 1) * 4;
+                const float x = TA ? As[mrow * LDK + k] : As[k * LDM + mrow];
+                ah[i][q] = tf32_of(x);
+                al[i][q] = tf32_of(x - __uint_as_float(ah[i][q]));
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < NTL; ++j) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const float x = Bs[(ncol0 + j * 8 + grp) * LDK + kk + tig + q * 4];
+                bh[j][q] = tf32_of(x);
+                bl[j][q] = tf32_of(x - __uint_as_float(bh[j][q]));
+            }
+        }
+        // small terms first, the dominant hi*hi product last
+#pragma unroll
+        for (int i = 0; i < MT; ++i)
+#pragma unroll
+            for (int j = 0; j < NTL; ++j) {
+                mma_tf32(acc[i][j], al[i], bh[j]);
+                mma_tf32(acc[i][j], ah[i], bl[j]);
+                mma_tf32(acc[i][j], ah[i], bh[j]);
+            }
+    }
+    static __device__ __forceinline__ int frag_row(int q, int grp) { return grp + (q >> 1) * 8; }
+    static __device__ __forceinline__ int frag_col(int q, int tig) { return 2 * tig + (q & 1); }
+};
+
+// -------------------------------------------------------------------------------------------
+// stream-K partition of the flattened (tile, k-tile) unit sequence
+// -------------------------------------------------------------------------------------------
+struct StreamK {
+    int64_t tilesM, tilesN;   // output tiles; tile t = tn * tilesM + tm (m fastest)
+    int KT;                   // k-tiles per output tile
+    int64_t U;                // tilesM * tilesN * KT
+    int64_t L;                // units per CTA (a multiple of KT in direct mode)
+    int partial;              // 1: every segment writes alpha*acc to partial slot (g - g0(t)); 0: direct
+};
+// first CTA that touches tile t, and how many CTAs (= partial slots) it has
+__host__ __device__ inline int64_t sk_first_cta(int64_t t, int KT, int64_t L) { return (t * KT) / L; }
+__host__ __device__ inline int sk_nseg(int64_t t, int KT, int64_t L) {
+    return (int)((((t + 1) * KT - 1) / L) - ((t * KT) / L) + 1);
+}
+
+template <typename T, bool TA, int BM, int BN, int WM, int WN, int STAGES>
+struct MmaCfg {
+    using P = MmaPolicy<T>;
+    static constexpr int BK = P::BK;
+    static constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN;
+    static constexpr int NT = WARPS_M * WARPS_N * 32;
+    static constexpr int MT = WM / P::MFRAG, NTL = WN / 8;
+    static constexpr int LDK = BK + P::PAD_K;
+    static constexpr int LDM = BM + P::PAD_M;
+    static constexpr int A_ELEMS = TA ? BM * LDK : BK * LDM;
+    static constexpr int B_ELEMS = BN * LDK;
+    static constexpr int STAGE_ELEMS = A_ELEMS + B_ELEMS;
+    static constexpr size_t SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(T);
+    static constexpr int VEC = 16 / (int)sizeof(T);
+};
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
+
+// Requires 16-byte aligned operands (a_vec_ok && b_vec_ok); the host falls back to the classic
+// kernels of gemm.cuh otherwise.
+template <typename T, bool TA, int BM, int BN, int WM, int WN, int STAGES, int MINB>
+__global__ void __launch_bounds__(MmaCfg<T, TA, BM, BN, WM, WN, STAGES>::NT, MINB)
+gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
+    using Cfg = MmaCfg<T, TA, BM, BN, WM, WN, STAGES>;
+    using P = MmaPolicy<T>;
+    constexpr int NT = Cfg::NT, MT = Cfg::MT, NTL = Cfg::NTL, LDK = Cfg::LDK, LDM = Cfg::LDM, BK = Cfg::BK;
+    constexpr int VEC = Cfg::VEC, ACC = P::ACC, W = (int)sizeof(T);
+    constexpr int CPR = BK / VEC;                         // 16-byte chunks per K-contiguous row
+    constexpr int CPM = BM / VEC;                         // chunks per M-contiguous row (!TA)
+    constexpr int PA = (TA ? BM * CPR : BK * CPM) / NT;   // chunks per thread per k-tile
+    constexpr int PB = BN * CPR / NT;
+    static_assert((TA ? BM * CPR : BK * CPM) % NT == 0 && (BN * CPR) % NT == 0, "tile/thread mismatch");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* smem = reinterpret_cast<T*>(smem_raw);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp % Cfg::WARPS_M, wn = warp / Cfg::WARPS_M;
+    const int grp = lane >> 2, tig = lane & 3;
+    const int64_t u0 = (int64_t)blockIdx.x * sk.L;
+    const int64_t u1 = min(sk.U, u0 + sk.L);
+    if (u0 >= u1) return;
+
+    // L2 residency: the reflector block V (operand A) is re-read by every CTA -> keep it; the big
+    // matrix C streams through once per launch -> let it go first.  In W = V^T C the streamed
+    // matrix is operand B; in C <- C - V W operand B is the small W (keep) and C itself is
+    // read/written by the accumulator path with streaming loads/stores.
+    const uint64_t pol_a = l2_policy_evict_last();
+    const uint64_t pol_b = TA ? l2_policy_evict_first() : l2_policy_evict_last();
+
+    // ---- producer state: runs STAGES-1 units ahead of the consumer, advanced incrementally ----
+    const T* pa[PA]; const T* pb[PB];
+    unsigned abytes = 0, bbytes = 0;      // 5 bits per chunk: valid bytes of the chunk's row/vector (0..16)
+    int64_t ltile = u0 / sk.KT;
+    int lkt = (int)(u0 - ltile * sk.KT);
+    int64_t ltn = ltile / sk.tilesM, ltm = ltile - ltn * sk.tilesM;
+    auto set_tile = [&]() {
+        const int64_t m0 = ltm * BM, n0 = ltn * BN;
+        abytes = 0; bbytes = 0;
+#pragma unroll
+        for (int p = 0; p < PA; ++p) {
+            const int c = tid + p * NT;
+            if (TA) {
+                const int r = c / CPR, ck = (c % CPR) * VEC;
+                const int64_t gr = m0 + r;
+                const bool ok = gr < g.M;
+                pa[p] = g.A + (ok ? gr : 0) * g.lda + ck;
+                abytes |= (ok ? 16u : 0u) << (5 * p);
+            } else {
+                const int kk = c / CPM, cm = (c % CPM) * VEC;
+                const int64_t gm = m0 + cm;
+                const int nv = (int)max((int64_t)0, min((int64_t)VEC, g.M - gm));
+                pa[p] = g.A + (nv ? gm : 0) + (int64_t)kk * g.lda;
+                abytes |= (unsigned)(nv * W) << (5 * p);
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < PB; ++p) {
+            const int c = tid + p * NT;
+            const int r = c / CPR, ck = (c % CPR) * VEC;
+            const int64_t gr = n0 + r;
+            const bool ok = gr < g.N;
+            pb[p] = g.B + (ok ? gr : 0) * g.ldb + ck;
+            bbytes |= (ok ? 16u : 0u) << (5 * p);
+        }
+    };
+    auto issue = [&](int stage) {
+        T* As = smem + (size_t)stage * Cfg::STAGE_ELEMS;
+        T* Bs = As + Cfg::A_ELEMS;
+        const int64_t k0 = (int64_t)lkt * BK;
+        const bool tail = k0 + BK > g.K;
+        const int64_t aoff = TA ? k0 : k0 * g.lda;
+#pragma unroll
+        for (int p = 0; p < PA; ++p) {
+            const int c = tid + p * NT;
+            int bytes = (int)((abytes >> (5 * p)) & 31u);
+            if (TA) {
+                const int r = c / CPR, ck = (c % CPR) * VEC;
+                if (tail) bytes = min(bytes, max(0, (int)(g.K - k0 - ck) * W));
+                cp_async16_hint(As + r * LDK + ck, pa[p] + aoff, bytes, pol_a);
+            } else {
+                const int kk = c / CPM, cm = (c % CPM) * VEC;
+                if (tail && k0 + kk >= g.K) bytes = 0;
+                cp_async16_hint(As + kk * LDM + cm, pa[p] + aoff, bytes, pol_a);
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < PB; ++p) {
+            const int c = tid + p * NT;
+            const int r = c / CPR, ck = (c % CPR) * VEC;
+            int bytes = (int)((bbytes >> (5 * p)) & 31u);
+            if (tail) bytes = min(bytes, max(0, (int)(g.K - k0 - ck) * W));
+            cp_async16_hint(Bs + r * LDK + ck, pb[p] + k0, bytes, pol_b);
+        }
+        // advance to the next unit
+        if (++lkt == sk.KT) {
+            lkt = 0;
+            if (++ltm == sk.tilesM) { ltm = 0; ++ltn; }
+            set_tile();
+        }
+    };
+
+    set_tile();
+    int64_t lu = u0;                      // next unit the producer will issue
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (lu < u1) { issue(s); ++lu; }
+        cp_async_commit();
+    }
+
+    const T cscale = (sk.partial || g.beta == T(0)) ? T(0) : g.beta / g.alpha;
+    int64_t t = u0 / sk.KT;
+    int64_t tn = t / sk.tilesM, tm = t - tn * sk.tilesM;
+    int64_t u = u0;
+    int cstage = 0, pstage = STAGES - 1;  // consumer / producer ring positions
+    while (u < u1) {
+        const int64_t seg_end = min(u1, (t + 1) * sk.KT);
+        const int64_t m0 = tm * BM, n0 = tn * BN;
+        const bool interior = (m0 + BM <= g.M) && (n0 + BN <= g.N);
+        T acc[MT][NTL][ACC];
+        if (cscale != T(0)) {
+            // all loads of the C tile are issued before the first use (one memory round trip per tile)
+            const T* Cb = g.C + (m0 + wm * WM) + (n0 + wn * WN) * g.ldc;
+#pragma unroll
+            for (int i = 0; i < MT; ++i)
+#pragma unroll
+                for (int j = 0; j < NTL; ++j)
+#pragma unroll
+                    for (int q = 0; q < ACC; ++q) {
+                        const int r = i * P::MFRAG + P::frag_row(q, grp), c = j * 8 + P::frag_col(q, tig);
+                        const bool ok = interior || (m0 + wm * WM + r < g.M && n0 + wn * WN + c < g.N);
+                        acc[i][j][q] = ok ? __ldcs(Cb + r + c * g.ldc) : T(0);
+                    }
+#pragma unroll
+            for (int i = 0; i < MT; ++i)
+#pragma unroll
+                for (int j = 0; j < NTL; ++j)
+#pragma unroll
+                    for (int q = 0; q < ACC; ++q) acc[i][j][q] *= cscale;
+        } else {
+#pragma unroll
+            for (int i = 0; i < MT; ++i)
+#pragma unroll
+                for (int j = 0; j < NTL; ++j)
+#pragma unroll
+                    for (int q = 0; q < ACC; ++q) acc[i][j][q] = T(0);
+        }
+        for (; u < seg_end; ++u) {
+            cp_async_wait<STAGES - 2>();
+            __syncthreads();
+            if (lu < u1) { issue(pstage); ++lu; }
+            cp_async_commit();
+            pstage = (pstage + 1 == STAGES) ? 0 : pstage + 1;
+            const T* As = smem + (size_t)cstage * Cfg::STAGE_ELEMS;
+            const T* Bs = As + Cfg::A_ELEMS;
+            cstage = (cstage + 1 == STAGES) ? 0 : cstage + 1;
+#pragma unroll
+            for (int kk = 0; kk < BK; kk += P::KSTEP)
+                P::template kstep<TA, MT, NTL, LDK, LDM>(As, Bs, kk, wm * WM, wn * WN, grp, tig, acc);
+        }
+        // ---- epilogue of this segment ----
+        T* Cout = g.C;
+        if (sk.partial) Cout += ((int64_t)blockIdx.x - sk_first_cta(t, sk.KT, sk.L)) * g.split_stride;
+#pragma unroll
+        for (int i = 0; i < MT; ++i)
+#pragma unroll
+            for (int j = 0; j < NTL; ++j)
+#pragma unroll
+                for (int q = 0; q < ACC; ++q) {
+                    const int64_t m = m0 + wm * WM + i * P::MFRAG + P::frag_row(q, grp);
+                    const int64_t n = n0 + wn * WN + j * 8 + P::frag_col(q, tig);
+                    if (interior || (m < g.M && n < g.N)) {
+                        if (sk.partial) Cout[m + n * g.ldc] = g.alpha * acc[i][j][q];
+                        else __stcs(&Cout[m + n * g.ldc], g.alpha * acc[i][j][q]);
+                    }
+                }
+        ++t;
+        if (++tm == sk.tilesM) { tm = 0; ++tn; }
+    }
+    cp_async_wait<0>();
+}
+
+// -------------------------------------------------------------------------------------------
+// host side: plan + launch
+// -------------------------------------------------------------------------------------------
+struct MmaPlan {
+    StreamK sk;
+    int grid;        // CTAs
+    int maxseg;      // partial slots needed (partial mode)
+};
+
+// slots = co-resident CTAs (SMs * CTAs per SM).  Direct mode keeps whole tiles per CTA.
+inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK, int slots, bool partial) {
+    MmaPlan p{};
+    p.sk.tilesM = ceil_div(M, BM); p.sk.tilesN = ceil_div(N, BN);
+    p.sk.KT = (int)std::max<int64_t>(1, ceil_div(K, BK));
+    const int64_t tiles = p.sk.tilesM * p.sk.tilesN;
+    p.sk.U = tiles * p.sk.KT;
+    p.sk.partial = partial ? 1 : 0;
+    if (partial) {
+        // no CTA shorter than 8 k-tiles: the pipeline prologue would dominate
+        int64_t G = std::min<int64_t>(slots, std::max<int64_t>(1, p.sk.U / 8));
+        p.sk.L = ceil_div(p.sk.U, G);
+        p.grid = (int)ceil_div(p.sk.U, p.sk.L);
+        p.maxseg = (int)std::min<int64_t>(ceil_div(p.sk.KT, p.sk.L) + 1, p.grid);
+        if (p.sk.L >= p.sk.KT && p.sk.L % p.sk.KT == 0) p.maxseg = 1;
+    } else {
+        const int64_t tpc = ceil_div(tiles, (int64_t)slots);
+        p.sk.L = tpc * p.sk.KT;
+        p.grid = (int)ceil_div(tiles, tpc);
+        p.maxseg = 1;
+    }
+    return p;
+}
+
+template <typename T, bool TA, int BM, int BN, int WM, int WN, int STAGES, int MINB>
+inline cudaError_t launch_mma(GemmArgs<T> g, const MmaPlan& p, cudaStream_t st) {
+    using Cfg = MmaCfg<T, TA, BM, BN, WM, WN, STAGES>;
+    auto kern = gemm_mma_kernel<T, TA, BM, BN, WM, WN, STAGES, MINB>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    kern<<<p.grid, Cfg::NT, Cfg::SMEM, st>>>(g, p.sk);
+    return cudaGetLastError();
+}
+
+}  // namespace ctqr

@@ -26,27 +26,48 @@ struct PanelArgs {
     int ibw;           // actual width of this inner block (<= IB)
     T* tau;            // tau + jb written
     T* Rd; int ldrd;   // diagonal block of R for the enclosing panel (ldrd x ldrd, zero-initialised)
-    T* Tin;            // IB x IB (ld = IB) inner T factor, written by CTA 0
+    T* Tin; int ldtin; // ibw x ibw inner T factor (ld = ldtin), written by CTA 0 into the diagonal block of T_k
     T* part;           // [2][G][IB] per-CTA partial sums
     T* rowbuf;         // [2][IB] the pivot row broadcast
     unsigned* bar;     // grid barrier counter (monotone)
     unsigned bar_base; // counter value when this launch starts
 };
 
-// C <- alpha*op(A)*B + beta*C (see gemm.cuh).  impl: 0 = default for the dtype, 1 = SIMT.
-cudaError_t gemm_f64(bool ta, GemmArgs<double> g, int splits, int impl, cudaStream_t st);
-cudaError_t gemm_f32(bool ta, GemmArgs<float> g, int splits, int impl, cudaStream_t st);
-// output tile (bm, bn) the default kernel will use for an M x N product (for split-K planning)
-void gemm_tile_f64(bool ta, int64_t M, int64_t N, int impl, int* bm, int* bn);
-void gemm_tile_f32(bool ta, int64_t M, int64_t N, int impl, int* bm, int* bn);
+// How the K range of a product was cut, for the kernels that sum the partial outputs.
+//   L == 0: classic split grid, every output tile has `nsplit` partials (slot z = blockIdx.z).
+//   L  > 0: stream-K (gemm_mma.cuh): the output tile of BN columns with index t has
+//           sk_nseg(t, KT, L) partials in slots 0 .. nseg-1 (tilesM == 1 in partial mode).
+struct SegInfo { int nsplit; int KT; int64_t L; int BN; };
+
+// A planned product C <- alpha*op(A)*B + beta*C.
+struct GemmLaunch {
+    int kind;          // 0 = classic kernels (gemm.cuh) with `splits` K slices; 1 = persistent stream-K (gemm_mma.cuh)
+    int splits;        // kind 0
+    int grid;          // kind 1: CTAs
+    int64_t tilesM, tilesN, U, L; int KT; int partial;   // kind 1: StreamK fields
+    int slots;         // partial output buffers needed (each g.split_stride elements apart)
+    int cfg;           // kernel configuration index inside the dtype's dispatcher
+    SegInfo seg;       // for the consumer of the partials
+};
+
+// impl: 0 = default for the dtype (fp64: DMMA tensor cores, fp32: 3xTF32 tensor cores),
+//       1 = SIMT kernels (DFMA / FFMA).  partial: the product goes to partial buffers that a
+//       consumer kernel sums (at most max_slots of them); otherwise beta*C is added and C written.
+// aligned: both operands have 16-byte aligned base pointers and leading dimensions (the stream-K kernel needs it)
+GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned);
+GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned);
+cudaError_t gemm_run_f64(bool ta, GemmArgs<double> g, const GemmLaunch& L, int impl, cudaStream_t st);
+cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int impl, cudaStream_t st);
 
 // cooperative register-resident panel kernel; returns cudaErrorInvalidValue for an unsupported (ib, rpt)
 cudaError_t panel_launch_f64(int ib, int rpt, PanelArgs<double>& pa, int G, cudaStream_t st);
 cudaError_t panel_launch_f32(int ib, int rpt, PanelArgs<float>& pa, int G, cudaStream_t st);
 constexpr int kPanelThreads = 256;
 
-template <typename T> cudaError_t larft_launch(const T* Gp, int nsplit, int64_t gstride, int ldg, const T* tau, int nbw, T* Tout, int ldt, cudaStream_t st);
-template <typename T> cudaError_t ttw_launch(const T* Wp, int nsplit, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st);
+// panel T from the Gram partials; the ib x ib diagonal blocks of Tk must already hold the inner T factors
+template <typename T> cudaError_t larft_launch(const T* Gp, SegInfo seg, int64_t gstride, int ldg, int nbw, int ib, T* Tk, int ldt, cudaStream_t st);
+// W <- T^T (sum of partials): scalar kernel for kw <= 32, tensor-core kernel otherwise
+template <typename T> cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st);
 template <typename T> cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx, cudaStream_t st);
 template <typename T> cudaError_t copy2d_launch(const T* src, int64_t lds, T* dst, int64_t ldd, int64_t rows, int64_t cols, cudaStream_t st);
 template <typename T> cudaError_t gather_R_launch(const T* A, int64_t lda, const T* Rd, int nb, int64_t n, T* R, int64_t ldr, cudaStream_t st);

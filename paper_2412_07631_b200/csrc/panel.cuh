@@ -7,9 +7,12 @@
 // w_c = v^T a_c; both follow from s_c = sum_{i>j} x_i a_c[i] (c = 0..IB-1, one pass, before
 // beta is known):  sigma^2 = s_j,  w_c = a_c[j] + s_c/(alpha-beta).  The same pass also yields
 // V[:,0:j]^T v_j, so the inner T factor comes for free.  Hence ONE grid-wide reduction per
-// column: warp-shuffle transpose-reduce -> shared memory -> per-CTA partial in global ->
-// software grid barrier (release/acquire counter) -> every CTA sums the G partials in the
-// same fixed order (bit-identical scalars everywhere, deterministic run to run).
+// column: warp-shuffle transpose-reduce -> shared memory -> per-CTA partial published in global
+// memory with the "LL" flag-in-data protocol (every 8-byte store carries 4 bytes of payload and
+// the 4-byte step number, so a reader that sees the right step number in both halves has the
+// value: data exchange and grid barrier are ONE L2 round trip, no fence, no counter) -> every
+// CTA sums the G partials in the same fixed order (bit-identical scalars everywhere,
+// deterministic run to run).
 // The update by reflector j and the dot products for column j+1 are fused into one register pass.
 #pragma once
 #include "common.cuh"
@@ -41,6 +44,33 @@ __device__ __forceinline__ void warp_transpose_reduce(T (&v)[IB], int lane) {
     }
 }
 
+// ---- LL slots: one 16-byte slot per value: {lo, seq, hi, seq} (fp32 uses lo only) -------------
+__device__ __forceinline__ void ll_store(uint4* slot, double v, unsigned seq) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %2};\n" ::"l"(slot), "r"((unsigned)b), "r"(seq),
+                 "r"((unsigned)(b >> 32)) : "memory");
+}
+__device__ __forceinline__ void ll_store(uint4* slot, float v, unsigned seq) {
+    asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %1, %2};\n" ::"l"(slot), "r"(__float_as_uint(v)), "r"(seq) : "memory");
+}
+__device__ __forceinline__ uint4 ll_load(const uint4* slot) {
+    uint4 r;
+    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];\n" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(slot) : "memory");
+    return r;
+}
+template <typename T> __device__ __forceinline__ T ll_value(uint4 r);
+template <> __device__ __forceinline__ double ll_value<double>(uint4 r) {
+    return __longlong_as_double((long long)(((unsigned long long)r.z << 32) | r.x));
+}
+template <> __device__ __forceinline__ float ll_value<float>(uint4 r) { return __uint_as_float(r.x); }
+// spin until the slot carries step `seq`, return its value
+template <typename T>
+__device__ __forceinline__ T ll_wait(const uint4* slot, unsigned seq) {
+    uint4 r = ll_load(slot);
+    while (r.y != seq || r.w != seq) r = ll_load(slot);
+    return ll_value<T>(r);
+}
+
 template <typename T, int IB, int RPT, int NT>
 __global__ void __launch_bounds__(NT, 1) panel_geqr2_kernel(PanelArgs<T> p) {
     static_assert(IB == 8 || IB == 16 || IB == 32, "IB");
@@ -70,11 +100,16 @@ __global__ void __launch_bounds__(NT, 1) panel_geqr2_kernel(PanelArgs<T> p) {
     if (cta == 0)
         for (int i = tid; i < IB * (IB + 1); i += NT) (&sh_T[0][0])[i] = T(0);
 
-    unsigned bar_target = p.bar_base;
+    // slots: [parity][G + 1][IB]; record G of a parity is the pivot row published by CTA 0
+    uint4* slots = reinterpret_cast<uint4*>(p.part);
 
     // Reduce acc[] over the whole grid; afterwards warp 0 lane c (< IB) holds s_c and rj_c.
-    auto grid_reduce = [&](T (&acc)[IB], int step, T& s_out, T& rj_out) {
+    // `pivot` (CTA 0 only): thread tid < IB passes its pivot-row entry to publish.
+    auto grid_reduce = [&](T (&acc)[IB], int step, T pivot_val, bool has_pivot, T& s_out, T& rj_out) {
         const int par = step & 1;
+        const unsigned seq = p.bar_base + (unsigned)step + 1u;
+        uint4* base = slots + (size_t)par * (G + 1) * IB;
+        if (has_pivot) ll_store(base + (size_t)G * IB + (tid % IB), pivot_val, seq);
         warp_transpose_reduce<T, IB>(acc, lane);
         if ((lane % LPC) == 0) sh_warp[warp][lane / LPC] = acc[0];
         __syncthreads();
@@ -82,28 +117,30 @@ __global__ void __launch_bounds__(NT, 1) panel_geqr2_kernel(PanelArgs<T> p) {
             T t = sh_warp[0][tid];
 #pragma unroll
             for (int w = 1; w < NW; ++w) t += sh_warp[w][tid];
-            __stcg(&p.part[((size_t)par * G + cta) * IB + tid], t);
+            ll_store(base + (size_t)cta * IB + tid, t, seq);
         }
-        __syncthreads();
-        bar_target += (unsigned)G;
-        if (tid == 0) {
-            __threadfence();
-            red_release_add_u32(p.bar, 1u);
-            while ((int)(ld_acquire_u32(p.bar) - bar_target) < 0) { }
-            __threadfence();
-        }
-        __syncthreads();
         {
-            // fixed summation order (same in every CTA); loads batched 4 deep to overlap L2 latency
+            // fixed summation order (same in every CTA); each thread waits for its own slots
+            // the loads of a batch are issued before the first flag is examined; a slot that is
+            // not there yet is re-polled individually
             const int c = tid % IB, grp = tid / IB;
-            const T* pp = p.part + (size_t)par * G * IB + c;
+            constexpr int MAXB = 4;
             T t = T(0);
-            for (int b = grp; b < G; b += 4 * NG) {
-                T v0 = __ldcg(pp + (size_t)b * IB);
-                T v1 = (b + NG < G) ? __ldcg(pp + (size_t)(b + NG) * IB) : T(0);
-                T v2 = (b + 2 * NG < G) ? __ldcg(pp + (size_t)(b + 2 * NG) * IB) : T(0);
-                T v3 = (b + 3 * NG < G) ? __ldcg(pp + (size_t)(b + 3 * NG) * IB) : T(0);
-                t += v0; t += v1; t += v2; t += v3;
+            for (int b0 = grp; b0 < G; b0 += NG * MAXB) {
+                uint4 r[MAXB];
+#pragma unroll
+                for (int i = 0; i < MAXB; ++i) {
+                    const int b = b0 + i * NG;
+                    if (b < G) r[i] = ll_load(base + (size_t)b * IB + c);
+                }
+#pragma unroll
+                for (int i = 0; i < MAXB; ++i) {
+                    const int b = b0 + i * NG;
+                    if (b < G) {
+                        while (r[i].y != seq || r[i].w != seq) r[i] = ll_load(base + (size_t)b * IB + c);
+                        t += ll_value<T>(r[i]);
+                    }
+                }
             }
             sh_red[grp][c] = t;
         }
@@ -113,40 +150,46 @@ __global__ void __launch_bounds__(NT, 1) panel_geqr2_kernel(PanelArgs<T> p) {
 #pragma unroll
             for (int gI = 1; gI < NG; ++gI) t += sh_red[gI][tid];
             s_out = t;
-            rj_out = __ldcg(&p.rowbuf[par * IB + tid]);
+            rj_out = ll_wait<T>(base + (size_t)G * IB + tid, seq);
         }
     };
 
-    // dots for column jn: acc[c] = sum over own rows strictly below the pivot row jb+jn
-    // (jn is a compile-time constant at every call site after unrolling)
+    // The column loop is NOT unrolled (a fully unrolled IB = 32 body is ~350 KB of SASS and the
+    // kernel was instruction-fetch bound: ncu "no_instruction" stall 11.6 of 17 cycles per issue).
+    // To keep every register index a compile-time constant anyway, the register tile is ROTATED by
+    // one column per iteration: at the top of iteration j, position c of a[q][.] holds panel column
+    // (j + c) mod IB, i.e. position 0 is always the current column, positions 1 .. ibw-1-j the
+    // columns still to be updated, and the finished reflectors sit at the high positions (they are
+    // still needed: the same dot-product pass yields V[:,0:j]^T v_j for the inner T factor).
     T s_c = T(0), rj_c = T(0);
-
+    {
+        // dots for column 0: acc[c] = sum over own rows strictly below the pivot row jb
+        T acc[IB];
 #pragma unroll
-    for (int j = 0; j < IB; ++j) {
-        if (j >= ibw) break;
-        // ---- (1) dots for column j (fused with the previous update at the end of the loop body
-        //          for j > 0; computed here for j == 0) ----
-        if (j == 0) {
-            T acc[IB];
+        for (int c = 0; c < IB; ++c) acc[c] = T(0);
 #pragma unroll
-            for (int c = 0; c < IB; ++c) acc[c] = T(0);
+        for (int q = 0; q < RPT; ++q) {
+            const bool below = row[q] > p.jb;
+            const T x = below ? a[q][0] : T(0);
 #pragma unroll
-            for (int q = 0; q < RPT; ++q) {
-                const bool below = row[q] > p.jb;
-                const T x = below ? a[q][0] : T(0);
-#pragma unroll
-                for (int c = 0; c < IB; ++c) acc[c] = fma(x, a[q][c], acc[c]);
-            }
-            if (cta == 0 && tid == 0) {
-#pragma unroll
-                for (int c = 0; c < IB; ++c) __stcg(&p.rowbuf[0 * IB + c], a[0][c]);
-            }
-            grid_reduce(acc, 0, s_c, rj_c);
+            for (int c = 0; c < IB; ++c) acc[c] = fma(x, a[q][c], acc[c]);
         }
-        // ---- (2) scalars of reflector j (warp 0, lanes < IB; identical in every CTA) ----
+        // pivot row of column 0 = row jb, held by CTA 0 / thread 0 / q = 0
+        if (cta == 0 && tid == 0) {
+            const unsigned seq0 = p.bar_base + 1u;
+#pragma unroll
+            for (int c = 0; c < IB; ++c) ll_store(slots + (size_t)G * IB + c, a[0][c], seq0);
+        }
+        grid_reduce(acc, 0, T(0), false, s_c, rj_c);
+    }
+
+#pragma unroll 1
+    for (int j = 0; j < ibw; ++j) {
+        const int nact = ibw - 1 - j;          // positions 1 .. nact are columns still to be updated
+        // ---- (2) scalars of reflector j (warp 0, lane = position; identical in every CTA) ----
         if (warp == 0) {
-            const T alpha = __shfl_sync(0xffffffffu, rj_c, j);
-            const T sigma2 = __shfl_sync(0xffffffffu, s_c, j);
+            const T alpha = __shfl_sync(0xffffffffu, rj_c, 0);
+            const T sigma2 = __shfl_sync(0xffffffffu, s_c, 0);
             T beta = alpha, tauj = T(0), denom = T(1);
             const bool nz = sigma2 != T(0);
             if (nz) {
@@ -155,15 +198,16 @@ __global__ void __launch_bounds__(NT, 1) panel_geqr2_kernel(PanelArgs<T> p) {
                 tauj = Num<T>::div(beta - alpha, beta);
                 denom = alpha - beta;
             }
-            // g_c = row-j entry + s_c/denom : c > j gives w_c, c < j gives (V^T v_j)_c
+            // g = pivot-row entry + s/denom: active positions give w_c, finished ones (V^T v_j)_c
             const T gc = nz ? rj_c + Num<T>::div(s_c, denom) : T(0);
-            if (lane < IB) sh_tw[lane] = tauj * gc;
+            if (lane < IB) sh_tw[lane] = (lane >= 1 && lane <= nact) ? tauj * gc : T(0);
             if (lane == 0) { sh_scal[0] = denom; sh_scal[1] = beta; sh_scal[2] = tauj; sh_scal[3] = nz ? T(1) : T(0); }
             if (cta == 0) {
                 // inner T: T[0:j, j] = -tau_j * T[0:j,0:j] * g[0:j],  T[j][j] = tau_j
+                // (panel column b < j sits at position b - j + IB)
                 T sum = T(0);
                 for (int b = 0; b < j; ++b) {
-                    const T gb = __shfl_sync(0xffffffffu, gc, b);
+                    const T gb = __shfl_sync(0xffffffffu, gc, (b - j + IB) & 31);
                     if (lane < j && b >= lane) sum = fma(sh_T[lane][b], gb, sum);
                 }
                 __syncwarp();
@@ -175,41 +219,57 @@ __global__ void __launch_bounds__(NT, 1) panel_geqr2_kernel(PanelArgs<T> p) {
         __syncthreads();
         const T denom = sh_scal[0], beta = sh_scal[1];
         const bool nz = sh_scal[3] != T(0);
-        T tw[IB];
-#pragma unroll
-        for (int c = 0; c < IB; ++c) tw[c] = (c > j) ? sh_tw[c] : T(0);
-        // ---- (3) apply reflector j to own rows, fused with the dots for column j+1 ----
+        const volatile T* tw = sh_tw;      // re-read per use: keeps IB values out of the register file
+        // ---- (3) apply reflector j to own rows, rotate, dots for column j+1 ----
         T acc[IB];
 #pragma unroll
         for (int c = 0; c < IB; ++c) acc[c] = T(0);
+        const int64_t piv = p.jb + j;
 #pragma unroll
         for (int q = 0; q < RPT; ++q) {
-            const int64_t piv = p.jb + j;
             if (nz) {
                 if (row[q] > piv) {
-                    const T v = Num<T>::div(a[q][j], denom);
-                    a[q][j] = v;
+                    const T v = Num<T>::div(a[q][0], denom);
+                    a[q][0] = v;
 #pragma unroll
-                    for (int c = j + 1; c < IB; ++c) a[q][c] = fma(-tw[c], v, a[q][c]);
+                    for (int c = 1; c < IB; ++c) a[q][c] = fma(-tw[c], v, a[q][c]);
                 } else if (row[q] == piv) {
-                    a[q][j] = beta;
+                    a[q][0] = beta;
 #pragma unroll
-                    for (int c = j + 1; c < IB; ++c) a[q][c] -= tw[c];
+                    for (int c = 1; c < IB; ++c) a[q][c] -= tw[c];
                 }
             }
-            if (j + 1 < IB) {
-                const bool below = row[q] > piv + 1;
-                const T x = below ? a[q][(j + 1) % IB] : T(0);
+            {
+                const T t0 = a[q][0];
 #pragma unroll
-                for (int c = 0; c < IB; ++c) acc[c] = fma(x, a[q][c], acc[c]);
+                for (int c = 0; c + 1 < IB; ++c) a[q][c] = a[q][c + 1];
+                a[q][IB - 1] = t0;
             }
+            const bool below = row[q] > piv + 1;
+            const T x = below ? a[q][0] : T(0);
+#pragma unroll
+            for (int c = 0; c < IB; ++c) acc[c] = fma(x, a[q][c], acc[c]);
         }
         if (j + 1 < ibw) {
+            // pivot row of column j+1 = row jb+j+1, held by CTA 0 / thread j+1 / q = 0
             if (cta == 0 && tid == j + 1) {
+                const unsigned seqn = p.bar_base + (unsigned)(j + 1) + 1u;
+                uint4* rb = slots + ((size_t)((j + 1) & 1) * (G + 1) + G) * IB;
 #pragma unroll
-                for (int c = 0; c < IB; ++c) __stcg(&p.rowbuf[((j + 1) & 1) * IB + c], a[0][c]);
+                for (int c = 0; c < IB; ++c) ll_store(rb + c, a[0][c], seqn);
             }
-            grid_reduce(acc, j + 1, s_c, rj_c);
+            grid_reduce(acc, j + 1, T(0), false, s_c, rj_c);
+        }
+    }
+    // undo the rotation (ibw rotations done; IB - ibw more bring every column back to its index)
+#pragma unroll 1
+    for (int r = ibw; r < IB; ++r) {
+#pragma unroll
+        for (int q = 0; q < RPT; ++q) {
+            const T t0 = a[q][0];
+#pragma unroll
+            for (int c = 0; c + 1 < IB; ++c) a[q][c] = a[q][c + 1];
+            a[q][IB - 1] = t0;
         }
     }
 
@@ -242,7 +302,10 @@ __global__ void __launch_bounds__(NT, 1) panel_geqr2_kernel(PanelArgs<T> p) {
     }
     if (cta == 0) {
         __syncthreads();
-        for (int i = tid; i < IB * IB; i += NT) p.Tin[i] = sh_T[i % IB][i / IB];
+        for (int i = tid; i < IB * IB; i += NT) {
+            const int r = i % IB, c = i / IB;
+            if (r < ibw && c < ibw) p.Tin[r + (size_t)c * p.ldtin] = sh_T[r][c];
+        }
     }
 }
 

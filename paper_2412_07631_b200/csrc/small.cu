@@ -13,25 +13,32 @@ static cudaError_t ensure_smem(K kernel, size_t bytes, size_t& cur) {
 }
 
 template <typename T>
-cudaError_t larft_launch(const T* Gp, int nsplit, int64_t gstride, int ldg, const T* tau, int nbw, T* Tout, int ldt,
+cudaError_t larft_launch(const T* Gp, SegInfo seg, int64_t gstride, int ldg, int nbw, int ib, T* Tk, int ldt,
                          cudaStream_t st) {
     static size_t cur = 0;
-    const size_t smem = (size_t)nbw * (nbw + 1) * sizeof(T);
+    const size_t smem = ((size_t)nbw * (nbw + 1) + (size_t)2 * nbw * (ib + 1)) * sizeof(T);
     cudaError_t e = ensure_smem(larft_kernel<T>, smem, cur);
     if (e != cudaSuccess) return e;
-    larft_kernel<T><<<1, 1024, smem, st>>>(Gp, nsplit, gstride, ldg, tau, nbw, Tout, ldt);
+    larft_kernel<T><<<1, 1024, smem, st>>>(Gp, seg, gstride, ldg, nbw, ib, Tk, ldt);
     return cudaGetLastError();
 }
 
 template <typename T>
-cudaError_t ttw_launch(const T* Wp, int nsplit, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N,
+cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N,
                        T* Wout, int64_t ldo, cudaStream_t st) {
-    constexpr int CW = 32;
-    static size_t cur = 0;
-    const size_t smem = ((size_t)kw * (kw + 1) + (size_t)CW * kw) * sizeof(T);
-    cudaError_t e = ensure_smem(ttw_kernel<T, CW>, smem, cur);
-    if (e != cudaSuccess) return e;
-    ttw_kernel<T, CW><<<(unsigned)ceil_div(N, CW), 256, smem, st>>>(Wp, nsplit, wstride, ldw, Tm, ldt, kw, N, Wout, ldo);
+    if (kw > 32 && kw <= 128 && (seg.L == 0 || seg.BN == 64)) {
+        static size_t cur2 = 0;
+        const size_t smem2 = (size_t)(128 + 64) * 132 * sizeof(T);
+        cudaError_t e2 = ensure_smem(ttw_mma_kernel<T>, smem2, cur2);
+        if (e2 != cudaSuccess) return e2;
+        ttw_mma_kernel<T><<<(unsigned)ceil_div(N, 64), 256, smem2, st>>>(Wp, seg, wstride, ldw, Tm, ldt, kw, N, Wout, ldo);
+        return cudaGetLastError();
+    }
+    if (seg.L != 0 || kw > 32) return cudaErrorInvalidValue;   // the scalar kernel only sums uniform splits
+    const int cw = std::max(1, 64 / kw);
+    int tpe = 1;
+    while (tpe * 2 * kw * cw <= 256 && tpe < 32) tpe *= 2;
+    ttw_kernel<T><<<(unsigned)ceil_div(N, cw), 256, 0, st>>>(Wp, seg.nsplit, wstride, ldw, Tm, ldt, kw, N, Wout, ldo, cw, tpe);
     return cudaGetLastError();
 }
 
@@ -68,8 +75,8 @@ cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, c
 }
 
 #define INST(T)                                                                                                        \
-    template cudaError_t larft_launch<T>(const T*, int, int64_t, int, const T*, int, T*, int, cudaStream_t);           \
-    template cudaError_t ttw_launch<T>(const T*, int, int64_t, int64_t, const T*, int, int, int64_t, T*, int64_t,      \
+    template cudaError_t larft_launch<T>(const T*, SegInfo, int64_t, int, int, int, T*, int, cudaStream_t);           \
+    template cudaError_t ttw_launch<T>(const T*, SegInfo, int64_t, int64_t, const T*, int, int, int64_t, T*, int64_t,  \
                                        cudaStream_t);                                                                  \
     template cudaError_t trsm_diag_launch<T>(const T*, int, int, const T*, int64_t, int64_t, T*, int64_t, cudaStream_t); \
     template cudaError_t copy2d_launch<T>(const T*, int64_t, T*, int64_t, int64_t, int64_t, cudaStream_t);             \

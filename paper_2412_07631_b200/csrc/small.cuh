@@ -6,85 +6,162 @@
 //                    "R22 X2 = C2" task of PAPER.md:L62-73)
 #pragma once
 #include "common.cuh"
+#include "kernels.h"
+#include "gemm_mma.cuh"
 #include <algorithm>
 
 namespace ctqr {
 
-// ---- larft from Gram partials ------------------------------------------------------------
-// G partials: nsplit buffers of nbw x nbw (ld = ldg, stride gstride) holding alpha*V^T V slices.
-// One CTA of 1024 threads: 8 threads per row of T cooperate on each dot product.
+// ---- larft from Gram partials, block by block ------------------------------------------------
+// The panel kernel has already written the ib x ib inner T factors into the diagonal blocks of
+// T_k.  For two reflector blocks H1 = I - V1 T1 V1^T, H2 = I - V2 T2 V2^T:
+//   H1 H2 = I - [V1 V2] [[T1, -T1 (V1^T V2) T2], [0, T2]] [V1 V2]^T,
+// so block column b of T_k is  T[0:ob, blk] = -T[0:ob,0:ob] * G[0:ob, blk] * T_bb  with G = V^T V
+// (same values as the column recurrence T[0:j,j] = -tau_j T[0:j,0:j] V[:,0:j]^T v_j, two small
+// matrix products per inner block instead of one dependent step per column).
+// G partials: nseg buffers of nbw x nbw (ld = ldg, stride gstride), see SegInfo.  One CTA.
 template <typename T>
 __global__ void __launch_bounds__(1024, 1)
-larft_kernel(const T* __restrict__ Gp, int nsplit, int64_t gstride, int ldg, const T* __restrict__ tau,
-             int nbw, T* __restrict__ Tout, int ldt) {
+larft_kernel(const T* __restrict__ Gp, SegInfo seg, int64_t gstride, int ldg, int nbw, int ib,
+             T* __restrict__ Tk, int ldt) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // One (nbw x (nbw+1)) array: column j holds G[:,j] until step j, then T[:,j] (in place).
-    T* Ms = reinterpret_cast<T*>(smem_raw);
-    const int tid = threadIdx.x;
+    T* Ts = reinterpret_cast<T*>(smem_raw);          // [nbw][nbw+1]  Ts[r*ld + c] = T[r][c]
     const int ld = nbw + 1;
+    T* Zs = Ts + (size_t)nbw * ld;                   // [nbw][ib+1]
+    const int ldz = ib + 1;
+    T* Gs = Zs + (size_t)nbw * ldz;                  // [nbw][ib+1]
+    const int tid = threadIdx.x;
     for (int i = tid; i < nbw * nbw; i += blockDim.x) {
-        int a = i % nbw, j = i / nbw;
-        T s = T(0);
-        for (int sp = 0; sp < nsplit; ++sp) s += Gp[(size_t)sp * gstride + a + (size_t)j * ldg];
-        Ms[a * ld + j] = s;
+        const int r = i % nbw, c = i / nbw;
+        Ts[r * ld + c] = (r <= c && r / ib == c / ib) ? Tk[r + (size_t)c * ldt] : T(0);
     }
     __syncthreads();
-    const int a = tid >> 3, sub = tid & 7;           // row a (< 128), 8 threads per row
-    for (int j = 0; j < nbw; ++j) {
-        const T tj = tau[j];
-        T sum = T(0);
-        if (a < j) {
-            for (int b = a + sub; b < j; b += 8) sum = fma(Ms[a * ld + b], Ms[b * ld + j], sum);
+    for (int ob = ib; ob < nbw; ob += ib) {
+        const int ibw = min(ib, nbw - ob);
+        // stage G[0:ob, blk] = sum of its partials (independent, coalesced loads)
+        for (int e = tid; e < ob * ibw; e += blockDim.x) {
+            const int a = e % ob, k = e / ob, col = ob + k;
+            const int nseg = seg.L > 0 ? sk_nseg(col / seg.BN, seg.KT, seg.L) : seg.nsplit;
+            T gv = T(0);
+            for (int sp = 0; sp < nseg; ++sp) gv += Gp[(size_t)sp * gstride + a + (size_t)col * ldg];
+            Gs[a * ldz + k] = gv;
         }
-        sum += shfl_xor(sum, 4);
-        sum += shfl_xor(sum, 2);
-        sum += shfl_xor(sum, 1);
         __syncthreads();
-        if (sub == 0 && a < nbw) {
-            if (a < j) Ms[a * ld + j] = -tj * sum;
-            else if (a == j) Ms[a * ld + j] = tj;
+        // Z = G[0:ob, blk] * T_bb   (T_bb upper triangular: k <= c)
+        for (int e = tid; e < ob * ibw; e += blockDim.x) {
+            const int a = e % ob, c = e / ob;
+            T z = T(0);
+            for (int k = 0; k <= c; ++k) z = fma(Gs[a * ldz + k], Ts[(ob + k) * ld + ob + c], z);
+            Zs[a * ldz + c] = z;
+        }
+        __syncthreads();
+        // T[0:ob, blk] = -T[0:ob,0:ob] * Z   (upper triangular: k >= a)
+        for (int e = tid; e < ob * ibw; e += blockDim.x) {
+            const int a = e % ob, c = e / ob;
+            T t = T(0);
+            for (int k = a; k < ob; ++k) t = fma(Ts[a * ld + k], Zs[k * ldz + c], t);
+            Ts[a * ld + ob + c] = -t;
         }
         __syncthreads();
     }
     for (int i = tid; i < nbw * nbw; i += blockDim.x) {
-        int r = i % nbw, c = i / nbw;
-        Tout[r + (size_t)c * ldt] = (r <= c) ? Ms[r * ld + c] : T(0);
+        const int r = i % nbw, c = i / nbw;
+        Tk[r + (size_t)c * ldt] = (r <= c) ? Ts[r * ld + c] : T(0);
     }
 }
 
-// ---- W <- T^T * sum_s Wp[s] ---------------------------------------------------------------
+// ---- W <- T^T * sum_s Wp[s] ---- (scalar kernel for the narrow in-panel blocks, kw <= 32) ------
 // Wp: nsplit partial buffers (kw x N, ld = ldw, stride wstride).  T: kw x kw upper (ld = ldt).
-// Output W (kw x N, ld = ldo).  Each CTA handles CW columns.
-template <typename T, int CW>
+// Each CTA handles cw columns with kw * cw <= 64 outputs; the (many) split-K partials of an
+// output are summed by a group of tpe threads in a fixed order, then combined by shuffles.
+template <typename T>
 __global__ void __launch_bounds__(256)
 ttw_kernel(const T* __restrict__ Wp, int nsplit, int64_t wstride, int64_t ldw, const T* __restrict__ Tm, int ldt,
-           int kw, int64_t N, T* __restrict__ Wout, int64_t ldo) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* Tt = reinterpret_cast<T*>(smem_raw);          // [kw][kw+1]  Tt[i][k] = T[k][i]
-    T* Ws = Tt + (size_t)kw * (kw + 1);              // [CW][kw]
+           int kw, int64_t N, T* __restrict__ Wout, int64_t ldo, int cw, int tpe) {
+    __shared__ T Tt[32][33];                         // Tt[i][k] = T[k][i]
+    __shared__ T Ws[64];                             // [cw][kw]
     const int tid = threadIdx.x;
-    const int64_t c0 = (int64_t)blockIdx.x * CW;
+    const int64_t c0 = (int64_t)blockIdx.x * cw;
     for (int i = tid; i < kw * kw; i += 256) {
-        int k = i % kw, col = i / kw;                // T[k][col], contiguous in k
-        Tt[col * (kw + 1) + k] = Tm[k + (size_t)col * ldt];
+        const int k = i % kw, col = i / kw;
+        Tt[col][k] = Tm[k + (size_t)col * ldt];
     }
-    for (int i = tid; i < kw * CW; i += 256) {
-        int k = i % kw, c = i / kw;
+    const int ne = kw * cw;
+    {
+        const int e = tid / tpe, sub = tid % tpe;
         T s = T(0);
-        if (c0 + c < N)
-            for (int sp = 0; sp < nsplit; ++sp) s += Wp[(size_t)sp * wstride + k + (c0 + c) * ldw];
-        Ws[c * kw + k] = s;
+        if (e < ne) {
+            const int k = e % kw, c = e / kw;
+            if (c0 + c < N)
+                for (int sp = sub; sp < nsplit; sp += tpe) s += Wp[(size_t)sp * wstride + k + (c0 + c) * ldw];
+        }
+        for (int off = tpe >> 1; off >= 1; off >>= 1) s += shfl_xor(s, off);
+        if (e < ne && sub == 0) Ws[e] = s;
     }
     __syncthreads();
-    for (int i = tid; i < kw * CW; i += 256) {
-        int r = i % kw, c = i / kw;
-        if (c0 + c >= N) continue;
-        T acc = T(0);
-        const T* tr = Tt + r * (kw + 1);
-        const T* wc = Ws + c * kw;
-        for (int k = 0; k <= r; ++k) acc = fma(tr[k], wc[k], acc);
-        Wout[r + (c0 + c) * ldo] = acc;
+    if (tid < ne) {
+        const int r = tid % kw, c = tid / kw;
+        if (c0 + c < N) {
+            T acc = T(0);
+            for (int k = 0; k <= r; ++k) acc = fma(Tt[r][k], Ws[c * kw + k], acc);
+            Wout[r + (c0 + c) * ldo] = acc;
+        }
     }
+}
+
+// ---- W <- T^T * sum_s Wp[s] on the tensor cores (kw up to 128) -------------------------------
+// One CTA per 64-column tile (the tile of the stream-K product that wrote the partials), 8 warps of
+// 32 x 32.  T (upper triangular, explicit zeros below) sits in shared memory K-contiguous:
+// Ts[m][k] = T[k][m]; the summed partial tile Ws[n][k] likewise.  Rows of T^T below the warp's
+// m-range are zero, so the k-loop stops at the warp's last row.
+template <typename T>
+__global__ void __launch_bounds__(256, 1)
+ttw_mma_kernel(const T* __restrict__ Wp, SegInfo seg, int64_t wstride, int64_t ldw, const T* __restrict__ Tm, int ldt,
+               int kw, int64_t N, T* __restrict__ Wout, int64_t ldo) {
+    using P = MmaPolicy<T>;
+    constexpr int BN = 64, KMAX = 128, LD = KMAX + 4, MT = 32 / P::MFRAG, NTL = 4;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* Ts = reinterpret_cast<T*>(smem_raw);          // [KMAX][LD]
+    T* Ws = Ts + KMAX * LD;                          // [BN][LD]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp & 3, wn = warp >> 2;
+    const int grp = lane >> 2, tig = lane & 3;
+    const int64_t c0 = (int64_t)blockIdx.x * BN;
+    const int kpad = (kw + P::KSTEP - 1) / P::KSTEP * P::KSTEP;
+    const int nseg = seg.L > 0 ? sk_nseg(blockIdx.x, seg.KT, seg.L) : seg.nsplit;
+    for (int i = tid; i < KMAX * kpad; i += 256) {
+        const int k = i % kpad, mm = i / kpad;
+        Ts[mm * LD + k] = (k < kw && mm < kw) ? Tm[k + (size_t)mm * ldt] : T(0);
+    }
+    for (int i = tid; i < BN * kpad; i += 256) {
+        const int k = i % kpad, c = i / kpad;
+        T s = T(0);
+        if (k < kw && c0 + c < N)
+            for (int sp = 0; sp < nseg; ++sp) s += Wp[(size_t)sp * wstride + k + (c0 + c) * ldw];
+        Ws[c * LD + k] = s;
+    }
+    __syncthreads();
+    if (wm * 32 >= kw) return;
+    T acc[MT][NTL][P::ACC];
+#pragma unroll
+    for (int i = 0; i < MT; ++i)
+#pragma unroll
+        for (int j = 0; j < NTL; ++j)
+#pragma unroll
+            for (int q = 0; q < P::ACC; ++q) acc[i][j][q] = T(0);
+    const int kend = min(kpad, wm * 32 + 32);
+    for (int kk = 0; kk < kend; kk += P::KSTEP)
+        P::template kstep<true, MT, NTL, LD, LD>(Ts, Ws, kk, wm * 32, wn * 32, grp, tig, acc);
+#pragma unroll
+    for (int i = 0; i < MT; ++i)
+#pragma unroll
+        for (int j = 0; j < NTL; ++j)
+#pragma unroll
+            for (int q = 0; q < P::ACC; ++q) {
+                const int r = wm * 32 + i * P::MFRAG + P::frag_row(q, grp);
+                const int64_t c = c0 + wn * 32 + j * 8 + P::frag_col(q, tig);
+                if (r < kw && c < N) Wout[r + c * ldo] = acc[i][j][q];
+            }
 }
 
 // ---- diagonal-block triangular solve -------------------------------------------------------

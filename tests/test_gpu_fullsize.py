@@ -1,0 +1,132 @@
+"""Full-size parity (rung T5): the configuration bench.py times (BASELINE.json
+configs[2], m = 32764, n = 16384, 256 noisy slices; default options, A resident in HBM), checked
+where the O(mn^2) oracle cannot run in seconds:
+
+  (i)   leading-columns property: the QR of A[:, 0:k] is the first k columns of the full QR, so the
+        oracle factors the leading k columns at full height and V, tau, R, T_0 are compared directly;
+  (ii)  R^T R = A^T A on sampled entries, with A^T A from the sparse Siddon rows in fp64 on the CPU
+        (independent of every GPU kernel) -- covers the late columns the oracle cannot reach;
+  (iii) certified solution error: g = A^T (b - A x) from the sparse rows in fp64; exactly
+        x* - x = (A^T A)^{-1} g and sigma_min(A_aug)^2 >= lambda, so ||x - x*|| <= ||g|| / lambda;
+  (iv)  fp32 against fp64 solution.
+
+Set CTQR_FULLSIZE=c4 to run the same checks on configs[3] (57 GB fp64 in core; minutes).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import scipy.sparse as sp
+
+import oracle
+import paper_2412_07631_b200 as ctqr
+from paper_2412_07631_b200 import workload as wl
+
+pytestmark = pytest.mark.gpu
+
+CFG = os.environ.get("CTQR_FULLSIZE", "c3")
+K_LEAD = 96
+
+
+@pytest.fixture(scope="module")
+def problem():
+    c = wl.CONFIGS[CFG]
+    coo = wl.siddon_coo(c.N, c.n_ang, c.n_bins)
+    rows, cols, vals = coo
+    lam = wl.tikhonov_lambda(vals, c.n)
+    S = min(c.S, 64)
+    X0, B = wl.make_slices(c, S=S, coo=coo, lam=lam)
+    A0 = sp.coo_matrix((vals, (rows, cols)), shape=(c.m0, c.n)).tocsr()
+    return dict(c=c, coo=coo, lam=lam, B=B, X0=X0, A0=A0, S=S)
+
+
+def sparse_aug(P, dt):
+    """A_aug as the working precision sees it (entries rounded once to dt), promoted to fp64."""
+    c = P["c"]
+    A0 = P["A0"].astype(dt).astype(np.float64)
+    sl = float(np.asarray(math.sqrt(P["lam"]), dtype=dt))
+    return sp.vstack([A0, sl * sp.identity(c.n, format="csr")]).tocsr(), sl
+
+
+def run(P, dt):
+    import torch
+    c = P["c"]
+    tdt = torch.float64 if dt == np.float64 else torch.float32
+    At, lam = wl.dense_augmented_device(c, tdt, P["coo"])
+    f = ctqr.ct_qr_factor(At, c.m, c.n, in_place=False)
+    del At
+    torch.cuda.empty_cache()
+    Bt = ctqr.colmajor_from_numpy(P["B"].astype(dt))
+    Xt = torch.zeros((P["S"], c.n), dtype=tdt, device="cuda")
+    ctqr.ct_qr_solve(f, Bt, P["S"], Xt)
+    return f, ctqr.numpy_from_colmajor(Xt)
+
+
+def relerr(a, b):
+    a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+RESULTS = {}
+
+
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_fullsize_factor_and_solve(problem, dt):
+    P = problem
+    c = P["c"]
+    f, X = run(P, dt)
+    RESULTS[dt] = X
+    tol_round = 1e-11 if dt == np.float64 else 5e-4
+    # (i) leading columns against the oracle
+    k = K_LEAD
+    rows, cols, vals = P["coo"]
+    sel = cols < k
+    Ak = np.zeros((c.m, k), order="F")
+    np.add.at(Ak, (rows[sel], cols[sel]), vals[sel])
+    Ak[c.m0 + np.arange(k), np.arange(k)] = math.sqrt(P["lam"])
+    Ak = np.asfortranarray(Ak.astype(dt))
+    VR, tau_o = oracle.qr(Ak)
+    V = ctqr.ct_qr_get_V(f, 0, k)
+    tau = ctqr.ct_qr_get_tau(f)
+    assert relerr(V, oracle.V_of(VR)) <= tol_round
+    assert relerr(tau[:k], tau_o) <= tol_round
+    R = ctqr.ct_qr_get_R(f)
+    assert relerr(R[:k, :k], oracle.R_of(VR)) <= tol_round
+    T0 = ctqr.ct_qr_get_T(f, 0)
+    kt = min(k, T0.shape[0])
+    assert relerr(T0[:kt, :kt], oracle.larft(VR, tau_o, 0, kt)) <= tol_round
+    assert np.all(np.tril(R, -1) == 0)
+    # (ii) R^T R = A^T A on sampled columns (late ones included)
+    Aaug, _ = sparse_aug(P, dt)
+    rng = np.random.default_rng(5)
+    js = np.unique(np.concatenate([rng.integers(0, c.n, 24), [0, c.n - 1, c.n // 2]]))
+    G_cols = (Aaug.T @ Aaug[:, js]).toarray()                     # n x len(js), fp64
+    R64 = R.astype(np.float64)
+    RtR_cols = R64.T @ R64[:, js]
+    scale = np.linalg.norm(G_cols)
+    gram_err = np.linalg.norm(RtR_cols - G_cols) / scale
+    assert gram_err <= (1e-12 if dt == np.float64 else 5e-5), gram_err
+    del R, R64
+    # (iii) certified solution error from the normal-equations residual
+    B = P["B"].astype(dt).astype(np.float64)
+    X64 = X.astype(np.float64)
+    g = Aaug.T @ (B - Aaug @ X64)
+    lam_eff = sparse_aug(P, dt)[1] ** 2
+    bound = np.linalg.norm(g) / lam_eff / np.linalg.norm(X64)
+    opt = np.linalg.norm(g) / (np.linalg.norm(Aaug.data) * np.linalg.norm(B))
+    print(f"\n[{CFG} {np.dtype(dt).name}] R^T R vs A^T A {gram_err:.2e}; optimality residual {opt:.2e}; "
+          f"certified ||x - x*||/||x|| <= {bound:.2e}; factor {f.stats()['factor_ms']:.1f} ms")
+    if dt == np.float64:
+        assert bound <= 1e-9, bound            # the north_star fp64 solution gate, certified
+    else:
+        assert opt <= 1e-5, opt                # rigorous bound is ~100x pessimistic in fp32
+    f.destroy()
+
+
+def test_fullsize_fp32_vs_fp64(problem):
+    if np.float64 not in RESULTS or np.float32 not in RESULTS:
+        pytest.skip("needs both precisions from the previous test")
+    d = relerr(RESULTS[np.float32], RESULTS[np.float64])
+    print(f"\n[{CFG}] ||X32 - X64|| / ||X64|| = {d:.2e}")
+    assert d <= 1e-3

@@ -241,3 +241,22 @@ def test_out_of_core_budget_too_small():
     with pytest.raises(ctqr.CtqrError) as ei:
         ctqr.ct_qr_factor(A.copy(order="F"), 300, 200, nb=32, device_budget_bytes=1000)
     assert ei.value.code == 2
+
+
+@pytest.mark.parametrize("ta", [True, False])
+def test_gemm_fp32_long_k_accumulation(ta):
+    """The fp32 contraction runs as a 3xTF32 split on the tensor cores; the tensor core's own
+    accumulator truncates, so the kernel must not let the error grow with K.
+    Same-sign data makes a biased accumulation visible: at K = 32768 the result must be as good as
+    an FFMA sum (a few 1e-6), two orders below what in-MMA accumulation gives (3e-4)."""
+    import torch
+    M, N, K = 128, 192, 32768
+    rng = np.random.default_rng(1)
+    A = np.abs(rng.standard_normal((K, M) if ta else (M, K))).astype(np.float32)
+    B = np.abs(rng.standard_normal((K, N))).astype(np.float32)
+    ref = (A.T.astype(np.float64) if ta else A.astype(np.float64)) @ B.astype(np.float64)
+    At, Bt = (ctqr.colmajor_from_numpy(np.asfortranarray(x)) for x in (A, B))
+    Ct = torch.zeros((N, M), dtype=torch.float32, device="cuda")
+    ctqr.ct_qr_gemm(ta, M, N, K, 1.0, At, A.shape[0], Bt, K, 0.0, Ct, M, 0)
+    err = np.max(np.abs(ctqr.numpy_from_colmajor(Ct) - ref) / np.abs(ref))
+    assert err <= 1e-5, err

@@ -146,8 +146,7 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     npdt = np.float64 if dtype == "f64" else np.float32
     S_all = cfg.S
     # slices are sharded over ranks (independent right-hand sides, no collective)
-    S = S_all // world + (1 if rank < S_all % world else 0)
-    s_lo = rank * (S_all // world) + min(rank, S_all % world)
+    s_lo, S = wl.shard_slices(S_all, rank, world)
     At, X0, B, coo, lam = build_inputs(cfg, dtype, S, s_lo)
     m, n = cfg.m, cfg.n
     Bt = ctqr.colmajor_from_numpy(B.astype(npdt))
@@ -317,10 +316,10 @@ def workload_name(cfg) -> str:
 # (profiles/); filled in when a capture of the current kernel exists, else null.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
 
-KERNEL_NAMES = {("f64", "upd"): "gemm_dmma_kernel<TA=false> (C <- C - V W, larfb)",
-                ("f64", "vtc"): "gemm_dmma_kernel<TA=true> (W = V^T C, larfb)",
-                ("f32", "upd"): "gemm_simt_kernel<float,TA=false> (C <- C - V W, larfb)",
-                ("f32", "vtc"): "gemm_simt_kernel<float,TA=true> (W = V^T C, larfb)"}
+KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; DMMA.8x8x4)",
+                ("f64", "vtc"): "gemm_mma_kernel<double,TA=true,128,64,32,32,3,2> (W = V^T C, larfb; DMMA.8x8x4)",
+                ("f32", "upd"): "gemm_mma_kernel<float,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; 3xTF32 HMMA.1688)",
+                ("f32", "vtc"): "gemm_mma_kernel<float,TA=true,128,64,32,32,3,2> (W = V^T C, larfb; 3xTF32 HMMA.1688)"}
 
 
 def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:
@@ -329,6 +328,10 @@ def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:
     s, o = spans[dom], spans[oth]
     ach = s["flops"] / (s["ms"] * 1e-3) / 1e12 if s["ms"] > 0 else 0.0
     peak = nominal_peak_tflops(dtype, float(peaks.get("sm_max_mhz", 1965.0)))
+    # fp64 runs on the FP64 tensor pipe (DMMA), whose peak equals the DFMA peak.  fp32 runs as a 3xTF32
+    # split on the tensor cores, but the work it replaces is fp32 FMA work and north_star asks for the
+    # fraction of the FP32 peak, so the denominator stays the FFMA peak ("alu"): a fraction above 1
+    # would mean the tensor-core path beats what FFMA could ever do.
     return {"bound": "tensor" if dtype == "f64" else "alu", "kernel": KERNEL_NAMES[(dtype, dom)],
             "achieved": ach, "peak": peak, "unit": UNIT, "frac": ach / peak,
             "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dtype, dom)),

@@ -30,7 +30,7 @@ import numpy as np
 
 __all__ = [
     "CTConfig", "CONFIGS", "siddon_coo", "tikhonov_lambda", "dense_augmented", "dense_augmented_device",
-    "ellipse_phantom", "make_slices", "chord_length", "psnr", "snr", "ssim",
+    "ellipse_phantom", "make_slices", "chord_length", "psnr", "snr", "ssim", "shard_slices",
 ]
 
 
@@ -248,6 +248,14 @@ def make_slices(cfg: CTConfig, S: int | None = None, coo=None, noise: bool = Tru
         else:
             B[: cfg.m0, sl] = p
     return X0, B
+
+
+def shard_slices(S: int, rank: int, world: int):
+    """Contiguous, balanced share of S independent slices for `rank` of `world` (first S % world
+    ranks get one more).  Returns (first slice, count).  The solve shards over right-hand sides with
+    no exchange step."""
+    base, extra = divmod(S, world)
+    return rank * base + min(rank, extra), base + (1 if rank < extra else 0)
 
 
 # ----------------------------------------------------------------------------------------

@@ -1,0 +1,76 @@
+"""Host-side checks that need no GPU: libctqr.so builds for sm_100a, loads, and exports every
+symbol include/ctqr.h declares; the ctypes mirrors of the two ABI structs have the C layout;
+argument errors are reported LAPACK-style without touching a device."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2412_07631_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    build.build()
+    return binding.lib()
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "ctqr.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(ct_qr_\w+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported_and_bound(L):
+    syms = declared_symbols()
+    assert {"ct_qr_factor", "ct_qr_solve", "ct_qr_apply_qt", "ct_qr_trsm", "ct_qr_get_R", "ct_qr_get_V",
+            "ct_qr_get_T", "ct_qr_get_tau", "ct_qr_get_stats", "ct_qr_destroy"} <= set(syms)
+    raw = ctypes.CDLL(binding.LIB_PATH)
+    for s in syms:
+        assert hasattr(raw, s), f"{s} declared in ctqr.h but not exported"
+        assert s in binding.EXPORTS, f"{s} has no ctypes prototype in binding.py"
+    assert set(binding.EXPORTS) <= set(syms)
+
+
+def test_struct_layouts_match_the_header():
+    # ctqr_options_t: 4 x int32, int64, 2 x int32, 2 pointers; ctqr_stats_t as declared
+    assert ctypes.sizeof(binding.Options) == 4 * 4 + 8 + 2 * 4 + 2 * 8
+    assert binding.Options.device_budget_bytes.offset == 16 and binding.Options.file_path.offset == 32
+    assert ctypes.sizeof(binding.Stats) == 2 * 8 + 6 * 4 + 9 * 8 + 8 + 2 * (8 + 8 + 8)
+    assert binding.Stats.factor_ms.offset == 40 and binding.Stats.vtc_ms.offset == 120
+
+
+def test_version_and_error_strings(L):
+    assert L.ct_qr_version() >= 100
+    assert b"success" in L.ct_qr_strerror(0)
+    assert b"argument" in L.ct_qr_strerror(-3)
+    assert b"zero" in L.ct_qr_strerror(4)
+
+
+def test_argument_errors_need_no_device(L):
+    h = ctypes.c_void_p()
+    A = np.zeros((4, 2), order="F")
+    P = A.ctypes.data
+    assert L.ct_qr_factor(None, 4, 2, 4, 1, None, ctypes.byref(h)) == -1
+    assert L.ct_qr_factor(P, 0, 2, 4, 1, None, ctypes.byref(h)) == -2
+    assert L.ct_qr_factor(P, 4, 5, 4, 1, None, ctypes.byref(h)) == -3
+    assert L.ct_qr_factor(P, 4, 2, 3, 1, None, ctypes.byref(h)) == -4
+    assert L.ct_qr_factor(P, 4, 2, 4, 7, None, ctypes.byref(h)) == -5
+    assert L.ct_qr_factor(P, 4, 2, 4, 1, None, None) == -7
+    assert L.ct_qr_solve(None, P, 4, 1, P, 2) == -1
+    assert L.ct_qr_get_stats(None, None) == -1
+    assert b"" != L.ct_qr_last_error()
+
+
+def test_no_cpu_fallback(L):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    h = ctypes.c_void_p()
+    A = np.eye(4, 2).copy(order="F")
+    rc = L.ct_qr_factor(A.ctypes.data, 4, 2, 4, 1, None, ctypes.byref(h))
+    assert rc == 1 and b"no CPU fallback" in L.ct_qr_last_error()

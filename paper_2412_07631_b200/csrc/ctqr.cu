@@ -17,9 +17,9 @@
 
 using namespace ctqr;
 
-template <typename T> static GemmLaunch gemm_plan(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned);
-template <> GemmLaunch gemm_plan<double>(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned) { return gemm_plan_f64(ta, M, N, K, impl, sms, partial, max_slots, aligned); }
-template <> GemmLaunch gemm_plan<float>(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned) { return gemm_plan_f32(ta, M, N, K, impl, sms, partial, max_slots, aligned); }
+template <typename T> static GemmLaunch gemm_plan(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems, int64_t sstride, bool aligned);
+template <> GemmLaunch gemm_plan<double>(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems, int64_t sstride, bool aligned) { return gemm_plan_f64(ta, M, N, K, impl, sms, partial, max_elems, sstride, aligned); }
+template <> GemmLaunch gemm_plan<float>(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems, int64_t sstride, bool aligned) { return gemm_plan_f32(ta, M, N, K, impl, sms, partial, max_elems, sstride, aligned); }
 template <typename T> static bool gemm_aligned(const GemmArgs<T>& g) {
     return ((uintptr_t)g.A % 16 == 0) && ((uintptr_t)g.B % 16 == 0) && ((g.lda * (int64_t)sizeof(T)) % 16 == 0) &&
            ((g.ldb * (int64_t)sizeof(T)) % 16 == 0);
@@ -29,7 +29,7 @@ template <> cudaError_t gemm_run<double>(bool ta, const GemmArgs<double>& g, con
 template <> cudaError_t gemm_run<float>(bool ta, const GemmArgs<float>& g, const GemmLaunch& L, int impl, cudaStream_t st) { return gemm_run_f32(ta, g, L, impl, st); }
 // direct product C <- alpha op(A) B + beta C
 template <typename T> static cudaError_t gemm_direct(bool ta, const GemmArgs<T>& g, int impl, int sms, cudaStream_t st) {
-    return gemm_run<T>(ta, g, gemm_plan<T>(ta, g.M, g.N, g.K, impl, sms, false, 1, gemm_aligned(g)), impl, st);
+    return gemm_run<T>(ta, g, gemm_plan<T>(ta, g.M, g.N, g.K, impl, sms, false, 0, 0, gemm_aligned(g)), impl, st);
 }
 static cudaError_t panel_launch(int ib, int rpt, PanelArgs<double>& pa, int G, cudaStream_t st) { return panel_launch_f64(ib, rpt, pa, G, st); }
 static cudaError_t panel_launch(int ib, int rpt, PanelArgs<float>& pa, int G, cudaStream_t st) { return panel_launch_f32(ib, rpt, pa, G, st); }
@@ -147,7 +147,7 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     g1.M = kw; g1.N = nc; g1.K = mk; g1.A = V; g1.lda = ldv; g1.B = C; g1.ldb = ldc;
     g1.C = Wp; g1.ldc = ldw; g1.alpha = T(1); g1.beta = T(0); g1.split_stride = sstride;
     const GemmLaunch L1 = gemm_plan<T>(true, kw, nc, mk, h.gemm_impl, h.sms, true,
-                                       (int64_t)(h.wp_elems[ws] / (size_t)sstride), gemm_aligned(g1));
+                                       (int64_t)h.wp_elems[ws], sstride, gemm_aligned(g1));
     prof = prof && h.profile;
     const double fl = 2.0 * (double)mk * (double)kw * (double)nc;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -259,7 +259,7 @@ static int panel_factor(H& h, cudaStream_t st, T* A, int64_t lda, int64_t m, int
     g.M = nbw; g.N = nbw; g.K = mk; g.A = V; g.lda = lda; g.B = V; g.ldb = lda;
     g.C = P_<T>(h.dWp[1]); g.ldc = ldg; g.alpha = T(1); g.beta = T(0); g.split_stride = gstride;
     const GemmLaunch LG = gemm_plan<T>(true, nbw, nbw, mk, h.gemm_impl, h.sms, true,
-                                       (int64_t)(h.wp_elems[1] / (size_t)gstride), gemm_aligned(g));
+                                       (int64_t)h.wp_elems[1], gstride, gemm_aligned(g));
     CK(gemm_run<T>(true, g, LG, h.gemm_impl, st));
     CK(larft_launch<T>(P_<T>(h.dWp[1]), LG.seg, gstride, (int)ldg, nbw, ib, Tk, h.nb, st));
     h.launches += 2;

@@ -8,7 +8,8 @@
 namespace ctqr {
 
 static GemmLaunch classic_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, int sms, int64_t min_chunk,
-                               bool partial, int64_t max_slots, int cfg) {
+                               bool partial, int64_t max_elems, int64_t sstride, int cfg) {
+    const int64_t max_slots = sstride > 0 ? max_elems / sstride : 1;
     GemmLaunch L{};
     L.kind = 0; L.cfg = cfg; L.partial = partial ? 1 : 0;
     int s = 1;
@@ -22,37 +23,39 @@ static GemmLaunch classic_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
 }
 
 static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, int bk, int sms, bool partial,
-                               int64_t max_slots, int cfg) {
+                               int64_t max_elems, int64_t sstride, int cfg) {
+    (void)sstride;
     int slots = sms * 2;
     MmaPlan p = mma_plan(M, N, K, bm, bn, bk, slots, partial);
-    while (partial && p.maxseg > max_slots && slots > 1) { slots /= 2; p = mma_plan(M, N, K, bm, bn, bk, slots, partial); }
+    while (partial && p.partial_elems > max_elems && slots > 1) { slots /= 2; p = mma_plan(M, N, K, bm, bn, bk, slots, partial); }
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
+    L.G = p.sk.G; L.Gm = p.sk.Gm;
     L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
 }
 
-GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots,
-                         bool aligned) {
+GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems,
+                         int64_t sstride, bool aligned) {
     if (impl == 1 || !aligned) {
-        if (ta) return M <= 32 ? classic_plan(M, N, K, 32, 128, sms, 256, partial, max_slots, 0)
-                               : classic_plan(M, N, K, 128, 128, sms, 512, partial, max_slots, 4);
-        return N <= 32 ? classic_plan(M, N, K, 128, 32, sms, 256, partial, max_slots, 2)
-                       : classic_plan(M, N, K, 128, 128, sms, 512, partial, max_slots, 5);
+        if (ta) return M <= 32 ? classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0)
+                               : classic_plan(M, N, K, 128, 128, sms, 512, partial, max_elems, sstride, 4);
+        return N <= 32 ? classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2)
+                       : classic_plan(M, N, K, 128, 128, sms, 512, partial, max_elems, sstride, 5);
     }
     if (ta) {
-        if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_slots, 0);
-        return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_slots, 1);
+        if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0);
+        return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_elems, sstride, 1);
     }
-    if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_slots, 2);
-    return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_slots, 3);
+    if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
+    return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_elems, sstride, 3);
 }
 
 static MmaPlan to_plan(const GemmLaunch& L) {
     MmaPlan p{};
     p.sk.tilesM = L.tilesM; p.sk.tilesN = L.tilesN; p.sk.KT = L.KT; p.sk.U = L.U; p.sk.L = L.L; p.sk.partial = L.partial;
-    p.grid = L.grid; p.maxseg = L.slots;
+    p.grid = L.grid; p.maxseg = L.slots; p.sk.G = L.G; p.sk.Gm = L.Gm;
     return p;
 }
 

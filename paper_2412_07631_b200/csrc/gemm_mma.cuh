@@ -63,10 +63,14 @@ template <> struct MmaPolicy<double> {
     static __device__ __forceinline__ int frag_col(int q, int tig) { return 2 * tig + q; }
 };
 
-__device__ __forceinline__ unsigned tf32_of(float x) {
-    unsigned r;
-    asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(r) : "f"(x));
-    return r;
+// x = hi + lo with hi, lo on the TF32 grid (10-bit mantissa).  cvt.rna.tf32.f32 is not a single
+// instruction on sm_100a (it expands to ~8 integer ops per value and made the ALU pipe the
+// co-bottleneck), so round to nearest on the bit pattern instead: add half a TF32 ulp, and mask
+// where the exact value is needed.  The tensor core ignores the low 13 mantissa bits of a .tf32
+// operand, so lo needs no mask.  (Values within 2^-11 of FLT_MAX would round to inf; not handled.)
+__device__ __forceinline__ void split_tf32(float x, unsigned& hi, unsigned& lo) {
+    hi = (__float_as_uint(x) + 0x1000u) & 0xffffe000u;
+    lo = __float_as_uint(x - __uint_as_float(hi)) + 0x1000u;
 }
 __device__ __forceinline__ void mma_tf32(float (&c)[4], const unsigned (&a)[4], const unsigned (&b)[2]) {
     asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
@@ -104,8 +108,7 @@ template <> struct MmaPolicy<float> {
                 const int mrow = mrow0 + i * 16 + grp + (q & 1) * 8;
                 const int k = kk + tig + (q >> 1) * 4;
                 const float x = TA ? As[mrow * LDK + k] : As[k * LDM + mrow];
-                ah[i][q] = tf32_of(x);
-                al[i][q] = tf32_of(x - __uint_as_float(ah[i][q]));
+                split_tf32(x, ah[i][q], al[i][q]);
             }
         }
 #pragma unroll
@@ -114,8 +117,7 @@ template <> struct MmaPolicy<float> {
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
                 const float x = Bs[(ncol0 + j * 8 + grp) * LDK + kk + tig + q * 4];
-                bh[q] = tf32_of(x);
-                bl[q] = tf32_of(x - __uint_as_float(bh[q]));
+                split_tf32(x, bh[q], bl[q]);
             }
 #pragma unroll
             for (int i = 0; i < MT; ++i) {
@@ -140,7 +142,12 @@ struct StreamK {
     int KT;                   // k-tiles per output tile
     int64_t U;                // tilesM * tilesN * KT
     int64_t L;                // units per CTA (a multiple of KT in direct mode)
-    int partial;              // 1: every segment writes alpha*acc to partial slot (g - g0(t)); 0: direct
+    int partial;              // 1: every segment writes alpha*acc to its compact partial slot; 0: direct
+    // direct mode only: tiles are dealt round-robin (CTA g's i-th tile has rank i * G + g), and ranks
+    // walk the tile grid in bands of Gm tile rows, n outer / m inner inside a band: the CTAs that
+    // run at the same time then share Gm V tiles and ~G/Gm W tiles (L2-resident) instead of
+    // cycling through all of V (which no longer fits the L2 at m = 1e5)
+    int G, Gm;
 };
 // first CTA that touches tile t, and how many CTAs (= partial slots) it has
 __host__ __device__ inline int64_t sk_first_cta(int64_t t, int KT, int64_t L) { return (t * KT) / L; }
@@ -187,8 +194,20 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
     const int wm = warp % Cfg::WARPS_M, wn = warp / Cfg::WARPS_M;
     const int grp = lane >> 2, tig = lane & 3;
     const int64_t u0 = (int64_t)blockIdx.x * sk.L;
-    const int64_t u1 = min(sk.U, u0 + sk.L);
+    const int64_t ntiles = sk.tilesM * sk.tilesN;
+    const bool rr = !sk.partial && sk.G > 0;
+    const int64_t u1 = !rr ? min(sk.U, u0 + sk.L)
+                                  : u0 + ((ntiles - (int64_t)blockIdx.x + sk.G - 1) / sk.G) * sk.KT;
     if (u0 >= u1) return;
+    // flat tile index (contiguous per CTA) -> tile coordinates
+    auto decode = [&](int64_t t, int64_t& tm, int64_t& tn) {
+        if (!rr) { tn = t / sk.tilesM; tm = t - tn * sk.tilesM; return; }
+        const int64_t rank = (t - u0 / sk.KT) * sk.G + (int64_t)blockIdx.x;
+        const int64_t per_band = (int64_t)sk.Gm * sk.tilesN;
+        const int64_t band = rank / per_band, r = rank - band * per_band;
+        const int64_t hb = min((int64_t)sk.Gm, sk.tilesM - band * sk.Gm);
+        tn = r / hb; tm = band * sk.Gm + (r - tn * hb);
+    };
 
     // L2 residency: the reflector block V (operand A) is re-read by every CTA -> keep it; the big
     // matrix C streams through once per launch -> let it go first.  In W = V^T C the streamed
@@ -202,7 +221,8 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
     unsigned abytes = 0, bbytes = 0;      // 5 bits per chunk: valid bytes of the chunk's row/vector (0..16)
     int64_t ltile = u0 / sk.KT;
     int lkt = (int)(u0 - ltile * sk.KT);
-    int64_t ltn = ltile / sk.tilesM, ltm = ltile - ltn * sk.tilesM;
+    int64_t ltn, ltm;
+    decode(ltile, ltm, ltn);
     auto set_tile = [&]() {
         const int64_t m0 = ltm * BM, n0 = ltn * BN;
         abytes = 0; bbytes = 0;
@@ -264,7 +284,8 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
         // advance to the next unit
         if (++lkt == sk.KT) {
             lkt = 0;
-            if (++ltm == sk.tilesM) { ltm = 0; ++ltn; }
+            ++ltile;
+            decode(ltile, ltm, ltn);
             set_tile();
         }
     };
@@ -279,7 +300,8 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
 
     const T cscale = (sk.partial || g.beta == T(0)) ? T(0) : g.beta / g.alpha;
     int64_t t = u0 / sk.KT;
-    int64_t tn = t / sk.tilesM, tm = t - tn * sk.tilesM;
+    int64_t tn, tm;
+    decode(t, tm, tn);
     int64_t u = u0;
     int cstage = 0, pstage = STAGES - 1;  // consumer / producer ring positions
     while (u < u1) {
@@ -328,23 +350,34 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
                 P::template kstep<TA, MT, NTL, LDK, LDM>(As, Bs, kk, wm * WM, wn * WN, grp, tig, acc);
         }
         // ---- epilogue of this segment ----
-        T* Cout = g.C;
-        if (sk.partial) Cout += ((int64_t)blockIdx.x - sk_first_cta(t, sk.KT, sk.L)) * g.split_stride;
+        if (sk.partial) {
+            // compact partial tiles: the (CTA, tile) pairs of a stream-K schedule form a staircase
+            // on which tile + CTA is strictly increasing, so that sum indexes a dense BM x BN slot
+            T* Pt = g.C + (t + (int64_t)blockIdx.x) * (int64_t)(BM * BN);
 #pragma unroll
-        for (int i = 0; i < MT; ++i)
+            for (int i = 0; i < MT; ++i)
 #pragma unroll
-            for (int j = 0; j < NTL; ++j)
+                for (int j = 0; j < NTL; ++j)
 #pragma unroll
-                for (int q = 0; q < ACC; ++q) {
-                    const int64_t m = m0 + wm * WM + i * P::MFRAG + P::frag_row(q, grp);
-                    const int64_t n = n0 + wn * WN + j * 8 + P::frag_col(q, tig);
-                    if (interior || (m < g.M && n < g.N)) {
-                        if (sk.partial) Cout[m + n * g.ldc] = g.alpha * acc[i][j][q];
-                        else __stcs(&Cout[m + n * g.ldc], g.alpha * acc[i][j][q]);
+                    for (int q = 0; q < ACC; ++q) {
+                        const int r = wm * WM + i * P::MFRAG + P::frag_row(q, grp);
+                        const int c = wn * WN + j * 8 + P::frag_col(q, tig);
+                        Pt[r + c * BM] = g.alpha * acc[i][j][q];
                     }
-                }
+        } else {
+#pragma unroll
+            for (int i = 0; i < MT; ++i)
+#pragma unroll
+                for (int j = 0; j < NTL; ++j)
+#pragma unroll
+                    for (int q = 0; q < ACC; ++q) {
+                        const int64_t m = m0 + wm * WM + i * P::MFRAG + P::frag_row(q, grp);
+                        const int64_t n = n0 + wn * WN + j * 8 + P::frag_col(q, tig);
+                        if (interior || (m < g.M && n < g.N)) __stcs(&g.C[m + n * g.ldc], g.alpha * acc[i][j][q]);
+                    }
+        }
         ++t;
-        if (++tm == sk.tilesM) { tm = 0; ++tn; }
+        decode(t, tm, tn);
     }
     cp_async_wait<0>();
 }
@@ -355,7 +388,8 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
 struct MmaPlan {
     StreamK sk;
     int grid;        // CTAs
-    int maxseg;      // partial slots needed (partial mode)
+    int maxseg;      // most segments any tile has (partial mode)
+    int64_t partial_elems;   // elements of the compact partial buffer: (tiles + grid) * BM * BN
 };
 
 // slots = co-resident CTAs (SMs * CTAs per SM).  Direct mode keeps whole tiles per CTA.
@@ -373,11 +407,17 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
         p.grid = (int)ceil_div(p.sk.U, p.sk.L);
         p.maxseg = (int)std::min<int64_t>(ceil_div(p.sk.KT, p.sk.L) + 1, p.grid);
         if (p.sk.L >= p.sk.KT && p.sk.L % p.sk.KT == 0) p.maxseg = 1;
+        p.partial_elems = (tiles + p.grid) * (int64_t)BM * BN;
     } else {
         const int64_t tpc = ceil_div(tiles, (int64_t)slots);
         p.sk.L = tpc * p.sk.KT;
         p.grid = (int)ceil_div(tiles, tpc);
         p.maxseg = 1;
+        // G > 0 would deal the tiles round-robin in bands of Gm tile rows (see StreamK); measured
+        // neutral to slightly slower than contiguous ranges at m = 3e4 and 1e5 (the L2 hints already
+        // keep V resident), so the contiguous order stays the default
+        p.sk.G = 0;
+        p.sk.Gm = (int)std::max<int64_t>(1, std::min<int64_t>(p.sk.tilesM, slots / 4));
     }
     return p;
 }

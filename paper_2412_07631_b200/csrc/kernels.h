@@ -44,7 +44,7 @@ struct GemmLaunch {
     int kind;          // 0 = classic kernels (gemm.cuh) with `splits` K slices; 1 = persistent stream-K (gemm_mma.cuh)
     int splits;        // kind 0
     int grid;          // kind 1: CTAs
-    int64_t tilesM, tilesN, U, L; int KT; int partial;   // kind 1: StreamK fields
+    int64_t tilesM, tilesN, U, L; int KT; int partial; int G, Gm;   // kind 1: StreamK fields
     int slots;         // partial output buffers needed (each g.split_stride elements apart)
     int cfg;           // kernel configuration index inside the dtype's dispatcher
     SegInfo seg;       // for the consumer of the partials
@@ -52,10 +52,12 @@ struct GemmLaunch {
 
 // impl: 0 = default for the dtype (fp64: DMMA tensor cores, fp32: 3xTF32 tensor cores),
 //       1 = SIMT kernels (DFMA / FFMA).  partial: the product goes to partial buffers that a
-//       consumer kernel sums (at most max_slots of them); otherwise beta*C is added and C written.
+//       consumer kernel sums (the partial buffer holds max_elems elements; the classic kernels put
+//       slice z at z * sstride, the stream-K kernel uses compact 128 x 64 tiles); otherwise beta*C
+//       is added and C written.
 // aligned: both operands have 16-byte aligned base pointers and leading dimensions (the stream-K kernel needs it)
-GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned);
-GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_slots, bool aligned);
+GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems, int64_t sstride, bool aligned);
+GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems, int64_t sstride, bool aligned);
 cudaError_t gemm_run_f64(bool ta, GemmArgs<double> g, const GemmLaunch& L, int impl, cudaStream_t st);
 cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int impl, cudaStream_t st);
 

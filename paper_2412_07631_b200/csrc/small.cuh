@@ -41,9 +41,15 @@ larft_kernel(const T* __restrict__ Gp, SegInfo seg, int64_t gstride, int ldg, in
         // stage G[0:ob, blk] = sum of its partials (independent, coalesced loads)
         for (int e = tid; e < ob * ibw; e += blockDim.x) {
             const int a = e % ob, k = e / ob, col = ob + k;
-            const int nseg = seg.L > 0 ? sk_nseg(col / seg.BN, seg.KT, seg.L) : seg.nsplit;
             T gv = T(0);
-            for (int sp = 0; sp < nseg; ++sp) gv += Gp[(size_t)sp * gstride + a + (size_t)col * ldg];
+            if (seg.L > 0) {            // compact stream-K partial tiles (128 x 64 slots), see gemm_mma.cuh
+                const int64_t t = col / 64;
+                const int nseg = sk_nseg(t, seg.KT, seg.L);
+                const T* base = Gp + (t + sk_first_cta(t, seg.KT, seg.L)) * (int64_t)(128 * 64) + a + (col % 64) * 128;
+                for (int sp = 0; sp < nseg; ++sp) gv += base[(int64_t)sp * (128 * 64)];
+            } else {
+                for (int sp = 0; sp < seg.nsplit; ++sp) gv += Gp[(size_t)sp * gstride + a + (size_t)col * ldg];
+            }
             Gs[a * ldz + k] = gv;
         }
         __syncthreads();
@@ -136,8 +142,14 @@ ttw_mma_kernel(const T* __restrict__ Wp, SegInfo seg, int64_t wstride, int64_t l
     for (int i = tid; i < BN * kpad; i += 256) {
         const int k = i % kpad, c = i / kpad;
         T s = T(0);
-        if (k < kw && c0 + c < N)
-            for (int sp = 0; sp < nseg; ++sp) s += Wp[(size_t)sp * wstride + k + (c0 + c) * ldw];
+        if (k < kw && c0 + c < N) {
+            if (seg.L > 0) {            // compact stream-K partial tiles (128 x 64 slots)
+                const T* base = Wp + ((int64_t)blockIdx.x + sk_first_cta(blockIdx.x, seg.KT, seg.L)) * (int64_t)(128 * 64) + k + c * 128;
+                for (int sp = 0; sp < nseg; ++sp) s += base[(int64_t)sp * (128 * 64)];
+            } else {
+                for (int sp = 0; sp < nseg; ++sp) s += Wp[(size_t)sp * wstride + k + (c0 + c) * ldw];
+            }
+        }
         Ws[c * LD + k] = s;
     }
     __syncthreads();

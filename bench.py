@@ -246,6 +246,70 @@ def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float
             "note": "A, B, X in pinned host memory; wall clock around the synchronous C-ABI calls"}
 
 
+def run_extras(cfg, dtype: str) -> dict:
+    """The other rooflines north_star asks evidence for, on the same workload (rank 0, N = 1):
+    solve S-sweep (Fig. 1: throughput rises with the number of slices solved at
+    once; small S is bound by reading the factor from HBM, m*n*w bytes per batch) and the
+    out-of-core path from pinned host memory with the device budget capped at a quarter of the
+    matrix (achieved host-link GB/s, time against the in-core factorisation)."""
+    import torch
+    import paper_2412_07631_b200 as ctqr
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    npdt = np.float64 if dtype == "f64" else np.float32
+    w = 8 if dtype == "f64" else 4
+    m, n = cfg.m, cfg.n
+    coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
+    At, lam = wl.dense_augmented_device(cfg, tdt, coo)
+    _, B = wl.make_slices(cfg, S=min(cfg.S, 256), coo=coo, lam=lam)
+    out = {}
+    f = ctqr.ct_qr_factor(At, m, n, in_place=False)
+    incore_ms = f.stats()["factor_ms"]
+    sweep = []
+    for S in (1, 8, 64, min(cfg.S, 256)):
+        Bt = ctqr.colmajor_from_numpy(B[:, :S].astype(npdt))
+        Xt = torch.zeros((S, n), dtype=tdt, device="cuda")
+        ctqr.ct_qr_solve(f, Bt, S, Xt)
+        ms = []
+        for _ in range(3):
+            ctqr.ct_qr_solve(f, Bt, S, Xt)
+            ms.append(f.stats()["solve_ms"])
+        t = min(ms)
+        sweep.append({"S": S, "ms": t, "slices_per_s": S / (t * 1e-3),
+                      "factor_read_gbs": m * n * w / (t * 1e-3) / 1e9,
+                      "tflops": (4.0 * m * n - n * n) * S / (t * 1e-3) / 1e12,
+                      "launches": f.stats()["kernel_launches"]})
+    out["solve_sweep"] = sweep
+    f.destroy()
+    # out of core
+    Ah = At.cpu().pin_memory()
+    del At
+    torch.cuda.empty_cache()
+    budget = int(m * n * w // 4)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    f = ctqr.ct_qr_factor(Ah, m, n, device_budget_bytes=budget)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    st = f.stats()
+    S = min(cfg.S, 64)
+    Bh = torch.from_numpy(np.ascontiguousarray(B[:, :S].astype(npdt).T)).pin_memory()
+    Xh = torch.zeros((S, n), dtype=tdt).pin_memory()
+    ctqr.ct_qr_solve(f, Bh, S, Xh)
+    st2 = f.stats()
+    out["out_of_core"] = {
+        "device_budget_bytes": budget, "n_superpanels": st["n_superpanels"], "factor_ms": st["factor_ms"],
+        "wall_s": wall, "tflops": cfg.factor_flops() / (st["factor_ms"] * 1e-3) / 1e12,
+        "vs_in_core_time": st["factor_ms"] / incore_ms,
+        "h2d_bytes": st["h2d_bytes"], "d2h_bytes": st["d2h_bytes"],
+        "host_link_gbs_avg": (st["h2d_bytes"] + st["d2h_bytes"]) / (st["factor_ms"] * 1e-3) / 1e9,
+        "algorithmic_link_bytes": m * n * w * (st["n_superpanels"] + 3) / 2.0,
+        "solve_streamed": {"S": S, "ms": st2["solve_ms"], "slices_per_s": S / (st2["solve_ms"] * 1e-3),
+                           "h2d_gbs": st2["h2d_bytes"] / (st2["solve_ms"] * 1e-3) / 1e9},
+        "note": "matrix in pinned host memory, factor written back in place; the link is shared by H2D and D2H streams"}
+    f.destroy()
+    return out
+
+
 # --------------------------------------------------------------------------------------------
 # CPU oracle arm (cpu_baseline leg and --impl reference)
 # --------------------------------------------------------------------------------------------
@@ -360,6 +424,8 @@ def main():
     ap.add_argument("--no-also", action="store_true", help="skip the second precision")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--short-warmup", action="store_true", help="honour --warmup < 3 (profiling runs under ncu only; not a valid bench number)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the solve S-sweep and the out-of-core run")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     rank = int(os.environ.get("RANK", "0"))
@@ -384,7 +450,7 @@ def main():
         torch.distributed.barrier()
     import paper_2412_07631_b200 as ctqr
 
-    warm = max(args.warmup, 3)
+    warm = args.warmup if args.short_warmup else max(args.warmup, 3)
     res = run_ours(cfg, args.dtype, args.steps, warm, rank, world, do_e2e=not args.no_e2e)
     other = "f32" if args.dtype == "f64" else "f64"
     res2 = None
@@ -426,6 +492,8 @@ def main():
         line["also"] = {other: {k: res2[k] for k in ("value", "ms_per_step", "factor_ms_per_step",
                                                      "frac_of_peak_whole_factor", "solve", "quality_noisy", "e2e",
                                                      "gpu_launches", "roofline", "clocks")}}
+    if not args.no_extras and world == 1:
+        line["extras"] = run_extras(cfg, args.dtype)
     if not args.no_cpu_baseline and world == 1:
         k, s = sample_size(cfg)
         line["cpu_baseline"] = {k2: v for k2, v in oracle_sample(cfg, args.dtype, k, s).items()

@@ -4,6 +4,8 @@
 #include <algorithm>
 #include "gemm.cuh"
 #include "gemm_mma.cuh"
+#include "gemm_umma.cuh"
+#include <cstdlib>
 
 namespace ctqr {
 
@@ -36,6 +38,23 @@ static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
     return L;
 }
 
+// tcgen05 (UMMA) plan: 128 x 128 tiles, one CTA per SM
+static GemmLaunch umma_plan_f32(int64_t M, int64_t N, int64_t K, int sms, bool partial, int64_t max_elems, int cfg) {
+    int slots = sms;
+    MmaPlan p = umma::umma_plan(M, N, K, slots, partial);
+    while (partial && p.partial_elems > max_elems && slots > 1) { slots /= 2; p = umma::umma_plan(M, N, K, slots, partial); }
+    GemmLaunch L{};
+    L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
+    L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
+    L.G = 0; L.Gm = 1;
+    L.seg = SegInfo{1, p.sk.KT, p.sk.L, umma::BN};
+    return L;
+}
+static bool umma_enabled() {
+    static const bool on = [] { const char* e = getenv("CTQR_NO_UMMA"); return !(e && e[0] == '1'); }();
+    return on;
+}
+
 GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems,
                          int64_t sstride, bool aligned) {
     if (impl == 1 || !aligned) {
@@ -44,11 +63,15 @@ GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
         return N <= 32 ? classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2)
                        : classic_plan(M, N, K, 128, 128, sms, 512, partial, max_elems, sstride, 5);
     }
+    // the big products go to the tcgen05 kernel (float4 chunks: K, and M when A is m-contiguous, multiples of 4)
+    const bool umma_ok = umma_enabled() && N >= 128 && K % 4 == 0;
     if (ta) {
         if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0);
+        if (umma_ok && M <= 128) return umma_plan_f32(M, N, K, sms, partial, max_elems, 21);
         return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_elems, sstride, 1);
     }
     if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
+    if (umma_ok && M % 4 == 0) return umma_plan_f32(M, N, K, sms, partial, max_elems, 23);
     return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_elems, sstride, 3);
 }
 
@@ -71,6 +94,8 @@ cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int im
         case 5: return launch_simt<float, false, 128, 128, 8>(g, L.splits, st);
         case 1: return launch_mma<float, true, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
         case 3: return launch_mma<float, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
+        case 21: return umma::launch_umma<true>(g, to_plan(L), st);
+        case 23: return umma::launch_umma<false>(g, to_plan(L), st);
     }
     return cudaErrorInvalidValue;
 }

@@ -26,7 +26,7 @@ cudaError_t larft_launch(const T* Gp, SegInfo seg, int64_t gstride, int ldg, int
 template <typename T>
 cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N,
                        T* Wout, int64_t ldo, cudaStream_t st) {
-    if (kw > 32 && kw <= 128 && (seg.L == 0 || seg.BN == 64)) {
+    if (kw > 32 && kw <= 128 && (seg.L == 0 || seg.BN == 64 || seg.BN == 128)) {
         static size_t cur2 = 0;
         const size_t smem2 = (size_t)(128 + 64) * 132 * sizeof(T);
         cudaError_t e2 = ensure_smem(ttw_mma_kernel<T>, smem2, cur2);

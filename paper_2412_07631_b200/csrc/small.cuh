@@ -42,11 +42,11 @@ larft_kernel(const T* __restrict__ Gp, SegInfo seg, int64_t gstride, int ldg, in
         for (int e = tid; e < ob * ibw; e += blockDim.x) {
             const int a = e % ob, k = e / ob, col = ob + k;
             T gv = T(0);
-            if (seg.L > 0) {            // compact stream-K partial tiles (128 x 64 slots), see gemm_mma.cuh
-                const int64_t t = col / 64;
+            if (seg.L > 0) {            // compact stream-K partial tiles (128 x BN slots), see gemm_mma.cuh
+                const int64_t t = col / seg.BN, slot = (int64_t)128 * seg.BN;
                 const int nseg = sk_nseg(t, seg.KT, seg.L);
-                const T* base = Gp + (t + sk_first_cta(t, seg.KT, seg.L)) * (int64_t)(128 * 64) + a + (col % 64) * 128;
-                for (int sp = 0; sp < nseg; ++sp) gv += base[(int64_t)sp * (128 * 64)];
+                const T* base = Gp + (t + sk_first_cta(t, seg.KT, seg.L)) * slot + a + (col % seg.BN) * 128;
+                for (int sp = 0; sp < nseg; ++sp) gv += base[(int64_t)sp * slot];
             } else {
                 for (int sp = 0; sp < seg.nsplit; ++sp) gv += Gp[(size_t)sp * gstride + a + (size_t)col * ldg];
             }
@@ -134,7 +134,7 @@ ttw_mma_kernel(const T* __restrict__ Wp, SegInfo seg, int64_t wstride, int64_t l
     const int grp = lane >> 2, tig = lane & 3;
     const int64_t c0 = (int64_t)blockIdx.x * BN;
     const int kpad = (kw + P::KSTEP - 1) / P::KSTEP * P::KSTEP;
-    const int nseg = seg.L > 0 ? sk_nseg(blockIdx.x, seg.KT, seg.L) : seg.nsplit;
+    const int nseg = seg.L > 0 ? sk_nseg(((int64_t)blockIdx.x * BN) / seg.BN, seg.KT, seg.L) : seg.nsplit;
     for (int i = tid; i < KMAX * kpad; i += 256) {
         const int k = i % kpad, mm = i / kpad;
         Ts[mm * LD + k] = (k < kw && mm < kw) ? Tm[k + (size_t)mm * ldt] : T(0);
@@ -144,8 +144,9 @@ ttw_mma_kernel(const T* __restrict__ Wp, SegInfo seg, int64_t wstride, int64_t l
         T s = T(0);
         if (k < kw && c0 + c < N) {
             if (seg.L > 0) {            // compact stream-K partial tiles (128 x 64 slots)
-                const T* base = Wp + ((int64_t)blockIdx.x + sk_first_cta(blockIdx.x, seg.KT, seg.L)) * (int64_t)(128 * 64) + k + c * 128;
-                for (int sp = 0; sp < nseg; ++sp) s += base[(int64_t)sp * (128 * 64)];
+                const int64_t t = c0 / seg.BN, slot = (int64_t)128 * seg.BN;
+                const T* base = Wp + (t + sk_first_cta(t, seg.KT, seg.L)) * slot + k + (int64_t)(c0 % seg.BN + c) * 128;
+                for (int sp = 0; sp < nseg; ++sp) s += base[(int64_t)sp * slot];
             } else {
                 for (int sp = 0; sp < nseg; ++sp) s += Wp[(size_t)sp * wstride + k + (c0 + c) * ldw];
             }

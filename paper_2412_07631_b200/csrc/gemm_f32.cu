@@ -39,15 +39,15 @@ static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
 }
 
 // tcgen05 (UMMA) plan: 128 x 128 tiles, one CTA per SM
-static GemmLaunch umma_plan_f32(int64_t M, int64_t N, int64_t K, int sms, bool partial, int64_t max_elems, int cfg) {
+static GemmLaunch umma_plan_f32(int64_t M, int64_t N, int64_t K, int bn, int sms, bool partial, int64_t max_elems, int cfg) {
     int slots = sms;
-    MmaPlan p = umma::umma_plan(M, N, K, slots, partial);
-    while (partial && p.partial_elems > max_elems && slots > 1) { slots /= 2; p = umma::umma_plan(M, N, K, slots, partial); }
+    MmaPlan p = umma::umma_plan(M, N, K, bn, slots, partial);
+    while (partial && p.partial_elems > max_elems && slots > 1) { slots /= 2; p = umma::umma_plan(M, N, K, bn, slots, partial); }
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
     L.G = 0; L.Gm = 1;
-    L.seg = SegInfo{1, p.sk.KT, p.sk.L, umma::BN};
+    L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
 }
 static bool umma_enabled() {
@@ -67,11 +67,11 @@ GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
     const bool umma_ok = umma_enabled() && N >= 128 && K % 4 == 0;
     if (ta) {
         if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0);
-        if (umma_ok && M <= 128) return umma_plan_f32(M, N, K, sms, partial, max_elems, 21);
+        if (umma_ok && M <= 128) return umma_plan_f32(M, N, K, 128, sms, partial, max_elems, 21);
         return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_elems, sstride, 1);
     }
     if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
-    if (umma_ok && M % 4 == 0) return umma_plan_f32(M, N, K, sms, partial, max_elems, 23);
+    if (umma_ok && M % 4 == 0) return umma_plan_f32(M, N, K, partial ? 128 : 64, sms, partial, max_elems, partial ? 24 : 23);
     return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_elems, sstride, 3);
 }
 
@@ -94,8 +94,9 @@ cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int im
         case 5: return launch_simt<float, false, 128, 128, 8>(g, L.splits, st);
         case 1: return launch_mma<float, true, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
         case 3: return launch_mma<float, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
-        case 21: return umma::launch_umma<true>(g, to_plan(L), st);
-        case 23: return umma::launch_umma<false>(g, to_plan(L), st);
+        case 21: return umma::launch_umma<true, 128>(g, to_plan(L), st);
+        case 23: return umma::launch_umma<false, 64>(g, to_plan(L), st);
+        case 24: return umma::launch_umma<false, 128>(g, to_plan(L), st);
     }
     return cudaErrorInvalidValue;
 }

@@ -29,10 +29,10 @@
 namespace ctqr {
 namespace umma {
 
-constexpr int BM = 128, BN = 128, BK = 32, STAGES = 3;
+constexpr int BM = 128, BK = 32, STAGES = 3;   // BN: 128 for W = V^T C, 64 for C <- C - V W (template)
 constexpr int WORKERS = 256, NT = WORKERS + 32;
 constexpr int TILE_BYTES = 128 * BK * 4;                 // one operand tile: 16 KB
-constexpr int STAGE_BYTES = 4 * TILE_BYTES;              // A_hi, A_lo, B_hi, B_lo
+constexpr int STAGE_BYTES = 4 * TILE_BYTES;              // A_hi, A_lo, B_hi, B_lo (B tiles sized for BN = 128)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -96,8 +96,11 @@ __device__ __forceinline__ void split4(const float4& x, uint4& hi, uint4& lo) {
     split_tf32(x.z, hi.z, lo.z); split_tf32(x.w, hi.w, lo.w);
 }
 
-template <bool TA>
+template <bool TA, int BN>
 __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, StreamK sk) {
+    constexpr int NC = BN / 2;                 // output columns per worker thread
+    constexpr int PBN = BN * 8 / WORKERS;      // B chunks per thread per k-block
+    constexpr bool DEFER = (BN == 64);         // registers allow holding the C tile until the epilogue
     extern __shared__ unsigned char smem_raw[];
     const unsigned sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;          // SWIZZLE_128B atoms need 1 KB alignment
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
@@ -163,9 +166,9 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
     } else {
         // ================= workers: producer + accumulator drain + epilogue =================
         const int rowq = (warp & 3) * 32 + lane;         // TMEM lane = output row inside the tile
-        const int colh = (warp >> 2) * 64;               // this thread's 64 output columns
-        float acc[64];
-        float4 ra[4], rb[4];                             // one k-block of operand chunks, in flight
+        const int colh = (warp >> 2) * NC;               // this thread's NC output columns
+        float acc[NC], cin[DEFER ? NC : 1];
+        float4 ra[4], rb[PBN];                             // one k-block of operand chunks, in flight
         // ---- producer state ----
         int64_t pt = u0 / sk.KT; int pkt = (int)(u0 - pt * sk.KT);
         auto load_regs = [&]() {
@@ -174,7 +177,7 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
 #pragma unroll
             for (int p = 0; p < 4; ++p) {
                 const int c = tid + p * WORKERS;
-                ra[p] = make_float4(0.f, 0.f, 0.f, 0.f); rb[p] = make_float4(0.f, 0.f, 0.f, 0.f);
+                ra[p] = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (TA) {
                     const int r = c >> 3, kc = (c & 7) * 4;
                     if (m0 + r < g.M && k0 + kc < g.K)
@@ -184,10 +187,11 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
                     if (k0 + kk < g.K && m0 + mc < g.M)
                         ra[p] = __ldg(reinterpret_cast<const float4*>(g.A + (m0 + mc) + (k0 + kk) * g.lda));
                 }
-                {
+                if (p < PBN) {
                     const int r = c >> 3, kc = (c & 7) * 4;
+                    rb[p < PBN ? p : 0] = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (n0 + r < g.N && k0 + kc < g.K)
-                        rb[p] = __ldg(reinterpret_cast<const float4*>(g.B + (n0 + r) * g.ldb + k0 + kc));
+                        rb[p < PBN ? p : 0] = __ldg(reinterpret_cast<const float4*>(g.B + (n0 + r) * g.ldb + k0 + kc));
                 }
             }
             if (++pkt == sk.KT) { pkt = 0; ++pt; }
@@ -205,16 +209,19 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
                 split4(ra[p], hi, lo);
                 *reinterpret_cast<uint4*>(st + off) = hi;
                 *reinterpret_cast<uint4*>(st + TILE_BYTES + off) = lo;
-                { const int r = c >> 3, kc = c & 7; off = (r >> 3) * 1024 + (r & 7) * 128 + ((kc ^ (r & 7)) << 4); }
-                split4(rb[p], hi, lo);
-                *reinterpret_cast<uint4*>(st + 2 * TILE_BYTES + off) = hi;
-                *reinterpret_cast<uint4*>(st + 3 * TILE_BYTES + off) = lo;
+                if (p < PBN) {
+                    const int r = c >> 3, kc = c & 7;
+                    off = (r >> 3) * 1024 + (r & 7) * 128 + ((kc ^ (r & 7)) << 4);
+                    split4(rb[p < PBN ? p : 0], hi, lo);
+                    *reinterpret_cast<uint4*>(st + 2 * TILE_BYTES + off) = hi;
+                    *reinterpret_cast<uint4*>(st + 3 * TILE_BYTES + off) = lo;
+                }
             }
         };
         // ---- consumer state ----
         int64_t ct = u0 / sk.KT; int ckt = (int)(u0 - ct * sk.KT);
         bool fresh = true;                                // next drain starts a tile segment
-        const float cscale = (sk.partial || g.beta == 0.f) ? 0.f : g.beta / g.alpha;
+        const float cscale = (sk.partial || g.beta == 0.f) ? 0.f : (DEFER ? 1.f : g.beta / g.alpha);
 
         int64_t pi = 0, ci = 0;
         load_regs();
@@ -233,30 +240,27 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
                 const int64_t tn = ct / sk.tilesM, tm = ct - tn * sk.tilesM;
                 const int64_t m0 = tm * BM, n0 = tn * BN;
                 if (fresh) {
-                    // running sum starts at (beta/alpha) * C (direct mode) or 0
-                    if (cscale != 0.f) {
+                    // direct mode: DEFER requests the C tile now and uses it only in the epilogue, so
+                    // its memory latency hides behind this tile's drains (C <- C - V W has just 4
+                    // k-blocks per tile); otherwise the running sum starts at (beta/alpha) * C
 #pragma unroll
-                        for (int c = 0; c < 64; ++c) {
-                            const int64_t m = m0 + rowq, n = n0 + colh + c;
-                            acc[c] = (m < g.M && n < g.N) ? cscale * __ldcs(&g.C[m + n * g.ldc]) : 0.f;
-                        }
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 64; ++c) acc[c] = 0.f;
+                    for (int c = 0; c < NC; ++c) {
+                        const int64_t m = m0 + rowq, n = n0 + colh + c;
+                        float cv = 0.f;
+                        if (cscale != 0.f && m < g.M && n < g.N) cv = __ldcs(&g.C[m + n * g.ldc]);
+                        if (DEFER) { cin[c] = cv; acc[c] = 0.f; } else acc[c] = cscale * cv;
                     }
                     fresh = false;
                 }
                 mbar_wait(tfull(b), (unsigned)((ci >> 1) & 1));
                 tc_fence_after();
                 const unsigned taddr = tmem + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(b * BN + colh);
-                {
+#pragma unroll
+                for (int c0 = 0; c0 < NC; c0 += 32) {
                     float v[32];
-                    tmem_ld32(taddr, v);
+                    tmem_ld32(taddr + c0, v);
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) acc[c] += v[c];
-                    tmem_ld32(taddr + 32, v);
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) acc[32 + c] += v[c];
+                    for (int c = 0; c < 32; ++c) acc[c0 + c] += v[c];
                 }
                 tc_fence_before();
                 mbar_arrive(tempty(b));
@@ -266,12 +270,13 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
                     if (sk.partial) {
                         float* Pt = g.C + (ct + (int64_t)blockIdx.x) * (int64_t)(BM * BN) + rowq + (int64_t)colh * BM;
 #pragma unroll
-                        for (int c = 0; c < 64; ++c) Pt[c * BM] = g.alpha * acc[c];
+                        for (int c = 0; c < NC; ++c) Pt[c * BM] = g.alpha * acc[c];
                     } else {
 #pragma unroll
-                        for (int c = 0; c < 64; ++c) {
+                        for (int c = 0; c < NC; ++c) {
                             const int64_t m = m0 + rowq, n = n0 + colh + c;
-                            if (m < g.M && n < g.N) __stcs(&g.C[m + n * g.ldc], g.alpha * acc[c]);
+                            if (m < g.M && n < g.N)
+                                __stcs(&g.C[m + n * g.ldc], DEFER ? fmaf(g.alpha, acc[c], g.beta * cin[c < (DEFER ? NC : 1) ? c : 0]) : g.alpha * acc[c]);
                         }
                     }
                     ckt = 0; ++ct; fresh = true;
@@ -286,13 +291,13 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
 }
 
 // plan: same stream-K partition as gemm_mma.cuh with 128 x 128 tiles, one CTA per SM
-inline MmaPlan umma_plan(int64_t M, int64_t N, int64_t K, int sms, bool partial) {
-    return mma_plan(M, N, K, BM, BN, BK, sms, partial);
+inline MmaPlan umma_plan(int64_t M, int64_t N, int64_t K, int bn, int sms, bool partial) {
+    return mma_plan(M, N, K, BM, bn, BK, sms, partial);
 }
 
-template <bool TA>
+template <bool TA, int BN>
 inline cudaError_t launch_umma(GemmArgs<float> g, const MmaPlan& p, cudaStream_t st) {
-    auto kern = gemm_umma_kernel<TA>;
+    auto kern = gemm_umma_kernel<TA, BN>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);

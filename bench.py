@@ -382,8 +382,8 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
 
 KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; DMMA.8x8x4)",
                 ("f64", "vtc"): "gemm_mma_kernel<double,TA=true,128,64,32,32,3,2> (W = V^T C, larfb; DMMA.8x8x4)",
-                ("f32", "upd"): "gemm_mma_kernel<float,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; 3xTF32 HMMA.1688)",
-                ("f32", "vtc"): "gemm_mma_kernel<float,TA=true,128,64,32,32,3,2> (W = V^T C, larfb; 3xTF32 HMMA.1688)"}
+                ("f32", "upd"): "umma::gemm_umma_kernel<TA=false,BN=64> (C <- C - V W, larfb; 3xTF32 on tcgen05.mma kind::tf32 / TMEM)",
+                ("f32", "vtc"): "umma::gemm_umma_kernel<TA=true,BN=128> (W = V^T C, larfb; 3xTF32 on tcgen05.mma kind::tf32 / TMEM)"}
 
 
 def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:

@@ -20,9 +20,10 @@
 //           of sm_100a (tcgen05 has no f64 kind).
 //   float : 3xTF32 split on mma.sync.m16n8k8.tf32 (SASS HMMA.1688.F32.TF32): x = hi + lo with
 //           hi = tf32(x), lo = tf32(x - hi); a*b ~= hi_a*hi_b + hi_a*lo_b + lo_a*hi_b accumulated
-//           in fp32.  Measured 557 TFLOP/s for the plain instruction on B200, i.e. ~185 TFLOP/s of
+//           in fp32.  Measured 278 TFLOP/s for the plain instruction on B200, i.e. <= 93 TFLOP/s of
 //           fp32-equivalent work against 74 TFLOP/s of FFMA.  north_star allows it "only if it
-//           meets the fp32 tolerance": the parity tests run on this path.
+//           meets the fp32 tolerance": the parity tests run on it.  The big products go to the
+//           tcgen05 kernel of gemm_umma.cuh instead (4x the MMA rate); this one serves the rest.
 #pragma once
 #include <algorithm>
 #include "common.cuh"
@@ -401,8 +402,10 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
     p.sk.U = tiles * p.sk.KT;
     p.sk.partial = partial ? 1 : 0;
     if (partial) {
-        // no CTA shorter than 8 k-tiles: the pipeline prologue would dominate
-        int64_t G = std::min<int64_t>(slots, std::max<int64_t>(1, p.sk.U / 8));
+        // no CTA shorter than ~1024 rows of K: a small product split over every SM costs more in the
+        // consumer (which sums one partial tile per segment) than it gains in the contraction
+        const int64_t min_units = std::max<int64_t>(8, 1024 / BK);
+        int64_t G = std::min<int64_t>(slots, std::max<int64_t>(1, p.sk.U / min_units));
         p.sk.L = ceil_div(p.sk.U, G);
         p.grid = (int)ceil_div(p.sk.U, p.sk.L);
         p.maxseg = (int)std::min<int64_t>(ceil_div(p.sk.KT, p.sk.L) + 1, p.grid);

@@ -4,13 +4,14 @@
 //
 //   C <- alpha * op(A) * B + beta * C,  column-major fp32, op(A) = A^T (A is K x M, "TA") or A (M x K).
 //
-// Structure (one CTA per SM, 128 x 128 output tile, k-blocks of 32):
+// Structure (one CTA per SM, 128 x BN output tile -- BN = 128 for W = V^T C, 64 for C <- C - V W so
+// that the C tile fits in registers until the epilogue -- k-blocks of 32):
 //   * warps 0-7 ("workers", 256 threads) load fp32 operand chunks global -> registers (one k-block
 //     ahead), split every value into hi + lo on the TF32 grid and store the four tiles A_hi, A_lo,
 //     B_hi, B_lo into shared memory in the UMMA canonical 128-byte-swizzled layouts (K-major for
 //     k-contiguous operands, MN-major for the m-contiguous V of C <- C - V W: no transposes);
 //   * warp 8 issues, per k-block, 4 k-steps x 3 products (lo*hi, hi*lo, hi*hi) of
-//     tcgen05.mma.cta_group::1.kind::tf32 (M = N = 128, K = 8) into one of two 128-column TMEM
+//     tcgen05.mma.cta_group::1.kind::tf32 (M = 128, N = BN, K = 8) into one of two BN-column TMEM
 //     accumulators, the first with accumulate = 0, and commits to mbarriers;
 //   * the workers drain that TMEM accumulator (tcgen05.ld 32x32b, thread = row) and add it to the
 //     running sum in registers with round-to-nearest FADDs.  The tensor core's own accumulation

@@ -95,7 +95,7 @@ cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int im
         case 1: return launch_mma<float, true, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
         case 3: return launch_mma<float, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
         case 21: return umma::launch_umma<true, 128>(g, to_plan(L), st);
-        case 23: return umma::launch_umma<false, 64>(g, to_plan(L), st);
+        case 23: return umma::launch_umma_ws<false, 64>(g, to_plan(L), st);
         case 24: return umma::launch_umma<false, 128>(g, to_plan(L), st);
     }
     return cudaErrorInvalidValue;

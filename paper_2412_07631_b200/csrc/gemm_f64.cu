@@ -2,6 +2,7 @@
 // (gemm_mma.cuh) for the big products, the classic DMMA grid kernel for skinny in-panel shapes,
 // SIMT DFMA as cross-check (impl 1).
 #include <algorithm>
+#include <cstdlib>
 #include "gemm.cuh"
 #include "gemm_mma.cuh"
 
@@ -23,9 +24,9 @@ static GemmLaunch classic_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
 }
 
 static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, int bk, int sms, bool partial,
-                               int64_t max_elems, int64_t sstride, int cfg) {
+                               int64_t max_elems, int64_t sstride, int cfg, int ctas_per_sm = 2) {
     (void)sstride;
-    int slots = sms * 2;
+    int slots = sms * ctas_per_sm;
     MmaPlan p = mma_plan(M, N, K, bm, bn, bk, slots, partial);
     while (partial && p.partial_elems > max_elems && slots > 1) { slots /= 2; p = mma_plan(M, N, K, bm, bn, bk, slots, partial); }
     GemmLaunch L{};
@@ -46,6 +47,8 @@ GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
     }
     if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
     if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_elems, sstride, 7);
+    static const bool defer = [] { const char* e = getenv("CTQR_F64_DEFER"); return e && e[0] == '1'; }();
+    if (defer && !partial) return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_elems, sstride, 13, 1);
     return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_elems, sstride, 3);
 }
 
@@ -70,6 +73,7 @@ cudaError_t gemm_run_f64(bool ta, GemmArgs<double> g, const GemmLaunch& L, int i
         case 6: return launch_dmma<true, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);
         case 7: return launch_dmma<false, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);
         case 3: return launch_mma<double, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
+        case 13: return launch_mma<double, false, 128, 64, 32, 32, 6, 1>(g, to_plan(L), st);
     }
     return cudaErrorInvalidValue;
 }

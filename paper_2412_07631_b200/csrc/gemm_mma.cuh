@@ -299,7 +299,10 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
         cp_async_commit();
     }
 
-    const T cscale = (sk.partial || g.beta == T(0)) ? T(0) : g.beta / g.alpha;
+    // MINB == 1 (one CTA per SM, 255 registers): the C tile is held separately from the accumulators,
+    // so its loads are issued at the start of a tile and consumed only in the epilogue
+    constexpr bool DEFER = (MINB == 1);
+    const T cscale = (sk.partial || g.beta == T(0)) ? T(0) : (DEFER ? T(1) : g.beta / g.alpha);
     int64_t t = u0 / sk.KT;
     int64_t tn, tm;
     decode(t, tm, tn);
@@ -310,6 +313,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
         const int64_t m0 = tm * BM, n0 = tn * BN;
         const bool interior = (m0 + BM <= g.M) && (n0 + BN <= g.N);
         T acc[MT][NTL][ACC];
+        T cin[DEFER ? MT : 1][DEFER ? NTL : 1][ACC];     // DEFER: C tile requested now, used in the epilogue
         if (cscale != T(0)) {
             // all loads of the C tile are issued before the first use (one memory round trip per tile)
             const T* Cb = g.C + (m0 + wm * WM) + (n0 + wn * WN) * g.ldc;
@@ -321,14 +325,18 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
                     for (int q = 0; q < ACC; ++q) {
                         const int r = i * P::MFRAG + P::frag_row(q, grp), c = j * 8 + P::frag_col(q, tig);
                         const bool ok = interior || (m0 + wm * WM + r < g.M && n0 + wn * WN + c < g.N);
-                        acc[i][j][q] = ok ? __ldcs(Cb + r + c * g.ldc) : T(0);
+                        const T cv = ok ? __ldcs(Cb + r + c * g.ldc) : T(0);
+                        if (DEFER) { cin[DEFER ? i : 0][DEFER ? j : 0][q] = cv; acc[i][j][q] = T(0); }
+                        else acc[i][j][q] = cv;
                     }
+            if (!DEFER) {
 #pragma unroll
-            for (int i = 0; i < MT; ++i)
+                for (int i = 0; i < MT; ++i)
 #pragma unroll
-                for (int j = 0; j < NTL; ++j)
+                    for (int j = 0; j < NTL; ++j)
 #pragma unroll
-                    for (int q = 0; q < ACC; ++q) acc[i][j][q] *= cscale;
+                        for (int q = 0; q < ACC; ++q) acc[i][j][q] *= cscale;
+            }
         } else {
 #pragma unroll
             for (int i = 0; i < MT; ++i)
@@ -374,7 +382,11 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
                     for (int q = 0; q < ACC; ++q) {
                         const int64_t m = m0 + wm * WM + i * P::MFRAG + P::frag_row(q, grp);
                         const int64_t n = n0 + wn * WN + j * 8 + P::frag_col(q, tig);
-                        if (interior || (m < g.M && n < g.N)) __stcs(&g.C[m + n * g.ldc], g.alpha * acc[i][j][q]);
+                        if (interior || (m < g.M && n < g.N)) {
+                            T o = g.alpha * acc[i][j][q];
+                            if (DEFER && cscale != T(0)) o = fma(g.beta, cin[DEFER ? i : 0][DEFER ? j : 0][q], o);
+                            __stcs(&g.C[m + n * g.ldc], o);
+                        }
                     }
         }
         ++t;

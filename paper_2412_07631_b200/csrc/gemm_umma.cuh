@@ -291,6 +291,252 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem), "r"(256u) : "memory");
 }
 
+// -------------------------------------------------------------------------------------------
+// Fully warp-specialised variant (used for C <- C - V W, BN = 64): the combined worker of the
+// kernel above stalls once per k-block on its own global loads (prefetch distance = one drain),
+// which with only 4 k-blocks per tile left the tensor core idle most of the time.  Here
+//   warps 0-3   producers: global -> registers TWO k-blocks ahead, split, store UMMA tiles
+//   warps 4-11  drainers:  TMEM -> registers, running sum, C tile requested at tile start and
+//                          consumed in the epilogue
+//   warp 12     MMA issuer
+// so global-load latency, tensor-core latency and C latency overlap instead of adding up.
+// -------------------------------------------------------------------------------------------
+constexpr int WS_PROD = 128, WS_DRAIN = 256, WS_NT = WS_PROD + WS_DRAIN + 32;
+// memory-level parallelism: the operands of a k-block are fetched with cp.async into a staging ring
+// WS_DEPTH k-blocks ahead (registers held only 2 k-blocks = 48 KB per SM in flight, which at ~1.5 us
+// of loaded memory latency capped a tile at ~3 us; the tensor core needs < 1 us)
+constexpr int WS_USTAGES = 2, WS_NSTG = 5, WS_DEPTH = WS_NSTG - 1;
+template <int BN> struct WsSmem {
+    static constexpr int B_TILE = BN * BK * 4;
+    static constexpr int USTAGE = 2 * TILE_BYTES + 2 * B_TILE;                 // A_hi, A_lo, B_hi, B_lo
+    static constexpr int CHUNKS = (1024 + BN * 8) / WS_PROD;                   // 16-byte chunks per producer thread per k-block
+    static constexpr int STG = CHUNKS * WS_PROD * 16;                          // one staging stage
+    static constexpr int BAR_OFF = WS_USTAGES * USTAGE + WS_NSTG * STG;
+    static constexpr int BYTES = BAR_OFF + 256 + 1024;
+};
+
+template <bool TA, int BN>
+__global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> g, StreamK sk) {
+    constexpr int NC = BN / 2;                 // output columns per drainer thread
+    constexpr int PA = 1024 / WS_PROD;         // A chunks (float4) per producer thread per k-block
+    constexpr int PB = BN * 8 / WS_PROD;       // B chunks
+    extern __shared__ unsigned char smem_raw[];
+    const unsigned sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
+    using SM = WsSmem<BN>;
+    constexpr int STAGES = WS_USTAGES;
+    constexpr int STAGE_BYTES = SM::USTAGE;
+    constexpr int B_TILE = SM::B_TILE;
+    const unsigned bars = sbase + SM::BAR_OFF;
+    auto full = [&](int s) { return bars + 8u * s; };
+    auto empty = [&](int s) { return bars + 8u * (STAGES + s); };
+    auto tfull = [&](int b) { return bars + 8u * (2 * STAGES + b); };
+    auto tempty = [&](int b) { return bars + 8u * (2 * STAGES + 2 + b); };
+    unsigned* tmem_slot = reinterpret_cast<unsigned*>(sgen + SM::BAR_OFF + 8 * (2 * STAGES + 4));
+    unsigned char* stg = sgen + WS_USTAGES * SM::USTAGE;                       // staging ring
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int MMA_WARP = (WS_PROD + WS_DRAIN) / 32;
+    const int64_t u0 = (int64_t)blockIdx.x * sk.L;
+    const int64_t u1 = min(sk.U, u0 + sk.L);
+    const int64_t nunits = u1 - u0;
+
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), WS_PROD); mbar_init(empty(s), 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tfull(b), 1); mbar_init(tempty(b), WS_DRAIN); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    if (warp == MMA_WARP) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(tmem_slot)), "r"(256u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const unsigned tmem = *tmem_slot;
+
+    if (warp == MMA_WARP) {
+        const unsigned idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((TA ? 0u : 1u) << 15) | ((unsigned)(BN >> 3) << 17) |
+                               ((unsigned)(BM >> 4) << 24);
+        for (int64_t j = 0; j < nunits; ++j) {
+            const int s = (int)(j % STAGES), b = (int)(j & 1);
+            mbar_wait(tempty(b), (unsigned)(((j >> 1) & 1) ^ 1));
+            mbar_wait(full(s), (unsigned)((j / STAGES) & 1));
+            tc_fence_after();
+            if (lane == 0) {
+                const unsigned a_hi = sbase + s * STAGE_BYTES, a_lo = a_hi + TILE_BYTES;
+                const unsigned b_hi = a_hi + 2 * TILE_BYTES, b_lo = b_hi + B_TILE;
+                const unsigned d = tmem + (unsigned)b * BN;
+#pragma unroll
+                for (int ks = 0; ks < BK / 8; ++ks) {
+                    const unsigned aoff = TA ? ks * 32 : ks * 4096;
+                    const uint64_t dah = TA ? make_desc(a_hi + aoff, 16, 1024) : make_desc(a_hi + aoff, 512, 2048, 1);
+                    const uint64_t dal = TA ? make_desc(a_lo + aoff, 16, 1024) : make_desc(a_lo + aoff, 512, 2048, 1);
+                    const uint64_t dbh = make_desc(b_hi + ks * 32, 16, 1024);
+                    const uint64_t dbl = make_desc(b_lo + ks * 32, 16, 1024);
+                    tc_mma_tf32(d, dal, dbh, idesc, ks > 0 ? 1u : 0u);
+                    tc_mma_tf32(d, dah, dbl, idesc, 1u);
+                    tc_mma_tf32(d, dah, dbh, idesc, 1u);
+                }
+                tc_commit(empty(s));
+                tc_commit(tfull(b));
+            }
+            __syncwarp();
+        }
+    } else if (warp < WS_PROD / 32) {
+        // ================= producers =================
+        int64_t pt = u0 / sk.KT; int pkt = (int)(u0 - pt * sk.KT);
+        // cp.async of k-block (pt, pkt) into staging stage q: chunk p of this thread sits at
+        // (p * WS_PROD + tid) * 16 -- every thread later reads back exactly the chunks it copied, so
+        // cp.async.wait_group is the only synchronisation the staging ring needs
+        auto issue_copy = [&](int q) {
+            const int64_t tn = pt / sk.tilesM, tm = pt - tn * sk.tilesM;
+            const int64_t m0 = tm * BM, n0 = tn * BN, k0 = (int64_t)pkt * BK;
+            unsigned char* dst = stg + (size_t)q * SM::STG + tid * 16;
+#pragma unroll
+            for (int p = 0; p < PA; ++p) {
+                const int c = tid + p * WS_PROD;
+                const float* src = g.A; int bytes = 0;
+                if (TA) {
+                    const int r = c >> 3, kc = (c & 7) * 4;
+                    if (m0 + r < g.M && k0 + kc < g.K) { src = g.A + (m0 + r) * g.lda + k0 + kc; bytes = 16; }
+                } else {
+                    const int kk = c >> 5, mc = (c & 31) * 4;
+                    if (k0 + kk < g.K && m0 + mc < g.M) { src = g.A + (m0 + mc) + (k0 + kk) * g.lda; bytes = 16; }
+                }
+                cp_async16(dst + p * WS_PROD * 16, src, bytes);
+            }
+#pragma unroll
+            for (int p = 0; p < PB; ++p) {
+                const int c = tid + p * WS_PROD;
+                const int r = c >> 3, kc = (c & 7) * 4;
+                const float* src = g.B; int bytes = 0;
+                if (n0 + r < g.N && k0 + kc < g.K) { src = g.B + (n0 + r) * g.ldb + k0 + kc; bytes = 16; }
+                cp_async16(dst + (PA + p) * WS_PROD * 16, src, bytes);
+            }
+            if (++pkt == sk.KT) { pkt = 0; ++pt; }
+        };
+        auto read_stage = [&](int q, float4 (&ra)[PA], float4 (&rb)[PB]) {
+            const unsigned char* srcp = stg + (size_t)q * SM::STG + tid * 16;
+#pragma unroll
+            for (int p = 0; p < PA; ++p) ra[p] = *reinterpret_cast<const float4*>(srcp + p * WS_PROD * 16);
+#pragma unroll
+            for (int p = 0; p < PB; ++p) rb[p] = *reinterpret_cast<const float4*>(srcp + (PA + p) * WS_PROD * 16);
+        };
+        auto store_stage = [&](int s, const float4 (&ra)[PA], const float4 (&rb)[PB]) {
+            unsigned char* st = sgen + (size_t)s * STAGE_BYTES;
+            uint4 hi, lo;
+#pragma unroll
+            for (int p = 0; p < PA; ++p) {
+                const int c = tid + p * WS_PROD;
+                unsigned off;
+                if (TA) { const int r = c >> 3, kc = c & 7; off = (r >> 3) * 1024 + (r & 7) * 128 + ((kc ^ (r & 7)) << 4); }
+                else    { const int kk = c >> 5, mc = c & 31, x = mc & 7;
+                          off = (kk >> 2) * 2048 + (mc >> 3) * 512 + (kk & 3) * 128 + ((((x >> 1) ^ (kk & 3)) << 5) | ((x & 1) << 4)); }
+                split4(ra[p], hi, lo);
+                *reinterpret_cast<uint4*>(st + off) = hi;
+                *reinterpret_cast<uint4*>(st + TILE_BYTES + off) = lo;
+            }
+#pragma unroll
+            for (int p = 0; p < PB; ++p) {
+                const int c = tid + p * WS_PROD;
+                const int r = c >> 3, kc = c & 7;
+                const unsigned off = (r >> 3) * 1024 + (r & 7) * 128 + ((kc ^ (r & 7)) << 4);
+                split4(rb[p], hi, lo);
+                *reinterpret_cast<uint4*>(st + 2 * TILE_BYTES + off) = hi;
+                *reinterpret_cast<uint4*>(st + 2 * TILE_BYTES + B_TILE + off) = lo;
+            }
+        };
+        auto publish = [&](int64_t pi, const float4 (&ra)[PA], const float4 (&rb)[PB]) {
+            const int s = (int)(pi % STAGES);
+            mbar_wait(empty(s), (unsigned)(((pi / STAGES) & 1) ^ 1));
+            store_stage(s, ra, rb);
+            fence_proxy_async();
+            mbar_arrive(full(s));
+        };
+        float4 ra[PA], rb[PB];
+        int64_t issued = 0;
+        for (int i = 0; i < WS_DEPTH; ++i) {
+            if (issued < nunits) { issue_copy((int)(issued % WS_NSTG)); ++issued; }
+            cp_async_commit();
+        }
+        for (int64_t pi = 0; pi < nunits; ++pi) {
+            cp_async_wait<WS_DEPTH - 1>();                 // this thread's copies of k-block pi have landed
+            read_stage((int)(pi % WS_NSTG), ra, rb);
+            if (issued < nunits) { issue_copy((int)(issued % WS_NSTG)); ++issued; }
+            cp_async_commit();
+            publish(pi, ra, rb);
+        }
+        cp_async_wait<0>();
+    } else {
+        // ================= drainers + epilogue =================
+        const int dw = warp - WS_PROD / 32;              // 0..7
+        const int rowq = (dw & 3) * 32 + lane;           // TMEM lane = output row (warp % 4 selects the lane quarter)
+        const int colh = (dw >> 2) * NC;
+        float acc[NC], cin[NC];
+        int64_t ct = u0 / sk.KT; int ckt = (int)(u0 - ct * sk.KT);
+        bool fresh = true;
+        const bool use_c = !sk.partial && g.beta != 0.f;
+        for (int64_t ci = 0; ci < nunits; ++ci) {
+            const int b = (int)(ci & 1);
+            const int64_t tn = ct / sk.tilesM, tm = ct - tn * sk.tilesM;
+            const int64_t m0 = tm * BM, n0 = tn * BN;
+            if (fresh) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const int64_t m = m0 + rowq, n = n0 + colh + c;
+                    cin[c] = (use_c && m < g.M && n < g.N) ? __ldcs(&g.C[m + n * g.ldc]) : 0.f;
+                    acc[c] = 0.f;
+                }
+                fresh = false;
+            }
+            mbar_wait(tfull(b), (unsigned)((ci >> 1) & 1));
+            tc_fence_after();
+            const unsigned taddr = tmem + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(b * BN + colh);
+#pragma unroll
+            for (int c0 = 0; c0 < NC; c0 += 32) {
+                float v[32];
+                tmem_ld32(taddr + c0, v);
+#pragma unroll
+                for (int c = 0; c < 32; ++c) acc[c0 + c] += v[c];
+            }
+            tc_fence_before();
+            mbar_arrive(tempty(b));
+            if (++ckt == sk.KT || ci + 1 == nunits) {
+                if (sk.partial) {
+                    float* Pt = g.C + (ct + (int64_t)blockIdx.x) * (int64_t)(BM * BN) + rowq + (int64_t)colh * BM;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) Pt[c * BM] = g.alpha * acc[c];
+                } else {
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) {
+                        const int64_t m = m0 + rowq, n = n0 + colh + c;
+                        if (m < g.M && n < g.N) __stcs(&g.C[m + n * g.ldc], fmaf(g.alpha, acc[c], g.beta * cin[c]));
+                    }
+                }
+                ckt = 0; ++ct; fresh = true;
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == MMA_WARP)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem), "r"(256u) : "memory");
+}
+
+template <bool TA, int BN>
+inline cudaError_t launch_umma_ws(GemmArgs<float> g, const MmaPlan& p, cudaStream_t st) {
+    auto kern = gemm_umma_ws_kernel<TA, BN>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<BN>::BYTES);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    kern<<<p.grid, WS_NT, WsSmem<BN>::BYTES, st>>>(g, p.sk);
+    return cudaGetLastError();
+}
+
 // plan: same stream-K partition as gemm_mma.cuh with 128 x 128 tiles, one CTA per SM
 inline MmaPlan umma_plan(int64_t M, int64_t N, int64_t K, int bn, int sms, bool partial) {
     return mma_plan(M, N, K, BM, bn, BK, sms, partial);

@@ -136,10 +136,11 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
         // instruction descriptor (cute::UMMA::InstrDescriptor): D = F32, A = B = TF32, A major, N >> 3, M >> 4
         const unsigned idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((TA ? 0u : 1u) << 15) | ((unsigned)(BN >> 3) << 17) |
                                ((unsigned)(BM >> 4) << 24);
+        int s = 0; unsigned fph = 0;
         for (int64_t j = 0; j < nunits; ++j) {
-            const int s = (int)(j % STAGES), b = (int)(j & 1);
+            const int b = (int)(j & 1);
             mbar_wait(tempty(b), (unsigned)(((j >> 1) & 1) ^ 1));
-            mbar_wait(full(s), (unsigned)((j / STAGES) & 1));
+            mbar_wait(full(s), fph);
             tc_fence_after();
             if (lane == 0) {
                 const unsigned a_hi = sbase + s * STAGE_BYTES, a_lo = a_hi + TILE_BYTES;
@@ -163,6 +164,7 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
                 tc_commit(tfull(b));       // accumulator b is complete
             }
             __syncwarp();
+            if (++s == STAGES) { s = 0; fph ^= 1u; }
         }
     } else {
         // ================= workers: producer + accumulator drain + epilogue =================
@@ -172,9 +174,9 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
         float4 ra[4], rb[PBN];                             // one k-block of operand chunks, in flight
         // ---- producer state ----
         int64_t pt = u0 / sk.KT; int pkt = (int)(u0 - pt * sk.KT);
+        int64_t ptn = pt / sk.tilesM, ptm = pt - ptn * sk.tilesM;     // advanced incrementally (no division per k-block)
         auto load_regs = [&]() {
-            const int64_t tn = pt / sk.tilesM, tm = pt - tn * sk.tilesM;
-            const int64_t m0 = tm * BM, n0 = tn * BN, k0 = (int64_t)pkt * BK;
+            const int64_t m0 = ptm * BM, n0 = ptn * BN, k0 = (int64_t)pkt * BK;
 #pragma unroll
             for (int p = 0; p < 4; ++p) {
                 const int c = tid + p * WORKERS;
@@ -195,7 +197,7 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
                         rb[p < PBN ? p : 0] = __ldg(reinterpret_cast<const float4*>(g.B + (n0 + r) * g.ldb + k0 + kc));
                 }
             }
-            if (++pkt == sk.KT) { pkt = 0; ++pt; }
+            if (++pkt == sk.KT) { pkt = 0; if (++ptm == sk.tilesM) { ptm = 0; ++ptn; } }
         };
         auto store_stage = [&](int s) {
             unsigned char* st = sgen + (size_t)s * STAGE_BYTES;
@@ -221,25 +223,26 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
         };
         // ---- consumer state ----
         int64_t ct = u0 / sk.KT; int ckt = (int)(u0 - ct * sk.KT);
+        int64_t ctn = ct / sk.tilesM, ctm = ct - ctn * sk.tilesM;
         bool fresh = true;                                // next drain starts a tile segment
         const float cscale = (sk.partial || g.beta == 0.f) ? 0.f : (DEFER ? 1.f : g.beta / g.alpha);
 
         int64_t pi = 0, ci = 0;
+        int ps = 0; unsigned pph = 1;
         load_regs();
         while (ci < nunits) {
             if (pi < nunits) {
-                const int s = (int)(pi % STAGES);
-                mbar_wait(empty(s), (unsigned)(((pi / STAGES) & 1) ^ 1));
-                store_stage(s);
+                mbar_wait(empty(ps), pph);
+                store_stage(ps);
                 fence_proxy_async();
-                mbar_arrive(full(s));
+                mbar_arrive(full(ps));
+                if (++ps == STAGES) { ps = 0; pph ^= 1u; }
                 ++pi;
                 if (pi < nunits) load_regs();
             }
             if (pi - ci >= STAGES - 1 || pi == nunits) {
                 const int b = (int)(ci & 1);
-                const int64_t tn = ct / sk.tilesM, tm = ct - tn * sk.tilesM;
-                const int64_t m0 = tm * BM, n0 = tn * BN;
+                const int64_t m0 = ctm * BM, n0 = ctn * BN;
                 if (fresh) {
                     // direct mode: DEFER requests the C tile now and uses it only in the epilogue, so
                     // its memory latency hides behind this tile's drains (C <- C - V W has just 4
@@ -281,6 +284,7 @@ __global__ void __launch_bounds__(NT, 1) gemm_umma_kernel(GemmArgs<float> g, Str
                         }
                     }
                     ckt = 0; ++ct; fresh = true;
+                    if (++ctm == sk.tilesM) { ctm = 0; ++ctn; }
                 }
             }
         }
@@ -358,10 +362,11 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
     if (warp == MMA_WARP) {
         const unsigned idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((TA ? 0u : 1u) << 15) | ((unsigned)(BN >> 3) << 17) |
                                ((unsigned)(BM >> 4) << 24);
+        int s = 0; unsigned fph = 0;
         for (int64_t j = 0; j < nunits; ++j) {
-            const int s = (int)(j % STAGES), b = (int)(j & 1);
+            const int b = (int)(j & 1);
             mbar_wait(tempty(b), (unsigned)(((j >> 1) & 1) ^ 1));
-            mbar_wait(full(s), (unsigned)((j / STAGES) & 1));
+            mbar_wait(full(s), fph);
             tc_fence_after();
             if (lane == 0) {
                 const unsigned a_hi = sbase + s * STAGE_BYTES, a_lo = a_hi + TILE_BYTES;
@@ -382,16 +387,18 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
                 tc_commit(tfull(b));
             }
             __syncwarp();
+            if (++s == STAGES) { s = 0; fph ^= 1u; }
         }
     } else if (warp < WS_PROD / 32) {
         // ================= producers =================
+        // tile coordinates advance incrementally: no 64-bit division on the per-k-block path
         int64_t pt = u0 / sk.KT; int pkt = (int)(u0 - pt * sk.KT);
+        int64_t ptn = pt / sk.tilesM, ptm = pt - ptn * sk.tilesM;
         // cp.async of k-block (pt, pkt) into staging stage q: chunk p of this thread sits at
         // (p * WS_PROD + tid) * 16 -- every thread later reads back exactly the chunks it copied, so
         // cp.async.wait_group is the only synchronisation the staging ring needs
         auto issue_copy = [&](int q) {
-            const int64_t tn = pt / sk.tilesM, tm = pt - tn * sk.tilesM;
-            const int64_t m0 = tm * BM, n0 = tn * BN, k0 = (int64_t)pkt * BK;
+            const int64_t m0 = ptm * BM, n0 = ptn * BN, k0 = (int64_t)pkt * BK;
             unsigned char* dst = stg + (size_t)q * SM::STG + tid * 16;
 #pragma unroll
             for (int p = 0; p < PA; ++p) {
@@ -414,7 +421,7 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
                 if (n0 + r < g.N && k0 + kc < g.K) { src = g.B + (n0 + r) * g.ldb + k0 + kc; bytes = 16; }
                 cp_async16(dst + (PA + p) * WS_PROD * 16, src, bytes);
             }
-            if (++pkt == sk.KT) { pkt = 0; ++pt; }
+            if (++pkt == sk.KT) { pkt = 0; if (++ptm == sk.tilesM) { ptm = 0; ++ptn; } }
         };
         auto read_stage = [&](int q, float4 (&ra)[PA], float4 (&rb)[PB]) {
             const unsigned char* srcp = stg + (size_t)q * SM::STG + tid * 16;
@@ -447,25 +454,28 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
                 *reinterpret_cast<uint4*>(st + 2 * TILE_BYTES + B_TILE + off) = lo;
             }
         };
-        auto publish = [&](int64_t pi, const float4 (&ra)[PA], const float4 (&rb)[PB]) {
-            const int s = (int)(pi % STAGES);
-            mbar_wait(empty(s), (unsigned)(((pi / STAGES) & 1) ^ 1));
-            store_stage(s, ra, rb);
+        int ps = 0; unsigned pph = 1;                       // UMMA stage ring position / empty-barrier parity
+        auto publish = [&](const float4 (&ra)[PA], const float4 (&rb)[PB]) {
+            mbar_wait(empty(ps), pph);
+            store_stage(ps, ra, rb);
             fence_proxy_async();
-            mbar_arrive(full(s));
+            mbar_arrive(full(ps));
+            if (++ps == STAGES) { ps = 0; pph ^= 1u; }
         };
         float4 ra[PA], rb[PB];
         int64_t issued = 0;
+        int qi = 0, qr = 0;                                 // staging ring: next stage to fill / to read
         for (int i = 0; i < WS_DEPTH; ++i) {
-            if (issued < nunits) { issue_copy((int)(issued % WS_NSTG)); ++issued; }
+            if (issued < nunits) { issue_copy(qi); ++issued; if (++qi == WS_NSTG) qi = 0; }
             cp_async_commit();
         }
         for (int64_t pi = 0; pi < nunits; ++pi) {
             cp_async_wait<WS_DEPTH - 1>();                 // this thread's copies of k-block pi have landed
-            read_stage((int)(pi % WS_NSTG), ra, rb);
-            if (issued < nunits) { issue_copy((int)(issued % WS_NSTG)); ++issued; }
+            read_stage(qr, ra, rb);
+            if (++qr == WS_NSTG) qr = 0;
+            if (issued < nunits) { issue_copy(qi); ++issued; if (++qi == WS_NSTG) qi = 0; }
             cp_async_commit();
-            publish(pi, ra, rb);
+            publish(ra, rb);
         }
         cp_async_wait<0>();
     } else {
@@ -475,13 +485,14 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
         const int colh = (dw >> 2) * NC;
         float acc[NC], cin[NC];
         int64_t ct = u0 / sk.KT; int ckt = (int)(u0 - ct * sk.KT);
+        int64_t ctn = ct / sk.tilesM, ctm = ct - ctn * sk.tilesM;
+        int64_t m0 = 0, n0 = 0;
         bool fresh = true;
         const bool use_c = !sk.partial && g.beta != 0.f;
         for (int64_t ci = 0; ci < nunits; ++ci) {
             const int b = (int)(ci & 1);
-            const int64_t tn = ct / sk.tilesM, tm = ct - tn * sk.tilesM;
-            const int64_t m0 = tm * BM, n0 = tn * BN;
             if (fresh) {
+                m0 = ctm * BM; n0 = ctn * BN;
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
                     const int64_t m = m0 + rowq, n = n0 + colh + c;
@@ -515,6 +526,7 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
                     }
                 }
                 ckt = 0; ++ct; fresh = true;
+                if (++ctm == sk.tilesM) { ctm = 0; ++ctn; }
             }
         }
     }

@@ -93,6 +93,7 @@ struct ctqr_handle_s {
     // opt->profile: per-launch event spans of the trailing-update contractions
     struct Span { cudaEvent_t a, b; double flops; int kind; };
     int profile = 0;
+    int reserve_sms = -1;  // SMs left to the look-ahead panel chain during the bulk update (fp32 tcgen05 path): -1 auto, 0 off
     std::vector<Span> spans;
     std::vector<cudaEvent_t> tpool; size_t tpool_used = 0;
     cudaEvent_t timing_event() {
@@ -134,8 +135,11 @@ static bool is_device_ptr(const void* p) {
 // ------------------------------------------------------------------------------------------
 template <typename T>
 static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t mk, int kw, const T* Tm, int ldt,
-                 T* C, int64_t ldc, int64_t nc, bool prof = false) {
+                 T* C, int64_t ldc, int64_t nc, bool prof = false, int reserve_sms = 0) {
     if (nc <= 0 || mk <= 0 || kw <= 0) return 0;
+    // reserve_sms: leave that many SMs to the look-ahead panel chain running on the other stream (only
+    // meaningful for one-CTA-per-SM kernels: a smaller persistent grid then leaves whole SMs empty)
+    const int sms = std::max(8, h.sms - reserve_sms);
     const int64_t ldw = round_up(kw, 4);
     // W = V^T C as partial products over K (stream-K or split grid), summed by the T^T W kernel
     const int64_t sstride = ldw * nc;
@@ -146,7 +150,7 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     GemmArgs<T> g1{};
     g1.M = kw; g1.N = nc; g1.K = mk; g1.A = V; g1.lda = ldv; g1.B = C; g1.ldb = ldc;
     g1.C = Wp; g1.ldc = ldw; g1.alpha = T(1); g1.beta = T(0); g1.split_stride = sstride;
-    const GemmLaunch L1 = gemm_plan<T>(true, kw, nc, mk, h.gemm_impl, h.sms, true,
+    const GemmLaunch L1 = gemm_plan<T>(true, kw, nc, mk, h.gemm_impl, sms, true,
                                        (int64_t)h.wp_elems[ws], sstride, gemm_aligned(g1));
     prof = prof && h.profile;
     const double fl = 2.0 * (double)mk * (double)kw * (double)nc;
@@ -159,7 +163,7 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     g2.M = mk; g2.N = nc; g2.K = kw; g2.A = V; g2.lda = ldv; g2.B = W; g2.ldb = ldw;
     g2.C = C; g2.ldc = ldc; g2.alpha = T(-1); g2.beta = T(1);
     if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
-    CK(gemm_direct<T>(false, g2, h.gemm_impl, h.sms, st));
+    CK(gemm_direct<T>(false, g2, h.gemm_impl, sms, st));
     if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 1}); }
     h.launches += 3;
     return 0;
@@ -316,7 +320,31 @@ static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
         CK(cudaStreamWaitEvent(h.sP, evL, 0));
         CKI(panel_factor<T>(h, h.sP, A, lda, m, jn, nbn, k + 1));
         CK(cudaEventRecord(evP, h.sP));
-        CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + (jn + nbn) * lda, lda, c1 - jn - nbn, true));
+        // Bulk update.  The fp32 contractions are one-CTA-per-SM persistent kernels, so a smaller grid
+        // leaves whole SMs empty: the first part of the bulk runs on (SMs - R) while the look-ahead
+        // panel chain (R co-resident CTAs of the cooperative panel kernel + its small kernels, on the
+        // high-priority stream) uses the rest; the remainder of the bulk then takes every SM.
+        // (The fp64 kernels run two CTAs per SM and cannot be confined this way; measured: a
+        // one-CTA fp64 variant loses more than the overlap gains.)
+        const int64_t ncb = c1 - jn - nbn;
+        int R = 0; int64_t nA = ncb;
+        if (sizeof(T) == 4 && h.gemm_impl == 0 && h.reserve_sms != 0 && ncb > 0) {
+            const int64_t mk1 = m - jn;
+            const int ibn = panel_ib_for<T>(h, mk1);
+            const int Gp = ibn ? (int)ceil_div(mk1, (int64_t)kPanelThreads * panel_rpts<T>(ibn)[0]) : h.sms;
+            R = h.reserve_sms > 0 ? h.reserve_sms : Gp + 2;
+            if (R > h.sms / 3) R = 0;                       // tall panels: the chain is negligible against the update
+            if (R > 0) {
+                const double t_panel = 0.25e-3 + 1.5e-8 * (double)mk1;                   // s, calibrated at c3
+                const double rate = 69e12 * (double)(h.sms - R) / (double)h.sms;          // flop/s of the pair of products
+                nA = (int64_t)(t_panel * rate / (4.0 * (double)(m - j0) * nbw));
+                nA = std::min<int64_t>(ncb, round_up(std::max<int64_t>(nA, 128), 128));
+                if (ncb - nA < 256) nA = ncb;
+            }
+        }
+        T* Cb = A + j0 + (jn + nbn) * lda;
+        CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, Cb, lda, nA, true, R));
+        if (nA < ncb) CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, Cb + nA * lda, lda, ncb - nA, true, 0));
     }
     CK(cudaStreamWaitEvent(h.sU, evP, 0));
     return 0;
@@ -596,6 +624,7 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
     h->lookahead = o.lookahead < 0 ? 1 : (o.lookahead ? 1 : 0);
     h->gemm_impl = o.gemm_impl;
     h->profile = o.profile ? 1 : 0;
+    { const char* e = getenv("CTQR_RESERVE_SMS"); h->reserve_sms = e ? atoi(e) : -1; }   // -1 = automatic, 0 = off
     h->P = (int)ceil_div(n, h->nb);
     h->user = (cudaStream_t)o.stream;
     int dev = 0; cudaGetDevice(&dev);

@@ -301,7 +301,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
 
     // MINB == 1 (one CTA per SM, 255 registers): the C tile is held separately from the accumulators,
     // so its loads are issued at the start of a tile and consumed only in the epilogue
-    constexpr bool DEFER = (MINB == 1);
+    constexpr bool DEFER = (MINB == 1) && (NT <= 256);
     const T cscale = (sk.partial || g.beta == T(0)) ? T(0) : (DEFER ? T(1) : g.beta / g.alpha);
     int64_t t = u0 / sk.KT;
     int64_t tn, tm;

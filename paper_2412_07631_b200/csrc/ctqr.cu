@@ -158,9 +158,22 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
     CK(gemm_run<T>(true, g1, L1, h.gemm_impl, st));
     if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 0}); }
-    CK(ttw_launch<T>(Wp, L1.seg, sstride, ldw, Tm, ldt, kw, nc, W, ldw, st));
+    const T* W2 = W;
+    if (L1.kind == 1 && kw == 128 && nc >= 128 && ldt % (16 / (int)sizeof(T)) == 0 && (uintptr_t)Tm % 16 == 0) {
+        // full-width panel: W <- sum of the partial tiles, then T^T W as one more tensor-core
+        // contraction (T is stored with explicit zeros below the diagonal), written over the partials
+        CK(partial_sum_launch<T>(Wp, L1.seg, kw, nc, W, ldw, st));
+        GemmArgs<T> gt{};
+        gt.M = kw; gt.N = nc; gt.K = kw; gt.A = Tm; gt.lda = ldt; gt.B = W; gt.ldb = ldw;
+        gt.C = Wp; gt.ldc = ldw; gt.alpha = T(1); gt.beta = T(0);
+        CK(gemm_direct<T>(true, gt, h.gemm_impl, sms, st));
+        W2 = Wp;
+        h.launches += 1;
+    } else {
+        CK(ttw_launch<T>(Wp, L1.seg, sstride, ldw, Tm, ldt, kw, nc, W, ldw, st));
+    }
     GemmArgs<T> g2{};
-    g2.M = mk; g2.N = nc; g2.K = kw; g2.A = V; g2.lda = ldv; g2.B = W; g2.ldb = ldw;
+    g2.M = mk; g2.N = nc; g2.K = kw; g2.A = V; g2.lda = ldv; g2.B = W2; g2.ldb = ldw;
     g2.C = C; g2.ldc = ldc; g2.alpha = T(-1); g2.beta = T(1);
     if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
     CK(gemm_direct<T>(false, g2, h.gemm_impl, sms, st));

@@ -70,6 +70,8 @@ constexpr int kPanelThreads = 256;
 template <typename T> cudaError_t larft_launch(const T* Gp, SegInfo seg, int64_t gstride, int ldg, int nbw, int ib, T* Tk, int ldt, cudaStream_t st);
 // W <- T^T (sum of partials): scalar kernel for kw <= 32, tensor-core kernel otherwise
 template <typename T> cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st);
+// dense (kw x N, ld = ldo) sum of the compact stream-K partial tiles (seg.L > 0)
+template <typename T> cudaError_t partial_sum_launch(const T* Wp, SegInfo seg, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st);
 template <typename T> cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx, cudaStream_t st);
 template <typename T> cudaError_t copy2d_launch(const T* src, int64_t lds, T* dst, int64_t ldd, int64_t rows, int64_t cols, cudaStream_t st);
 template <typename T> cudaError_t gather_R_launch(const T* A, int64_t lda, const T* Rd, int nb, int64_t n, T* R, int64_t ldr, cudaStream_t st);

@@ -43,6 +43,12 @@ cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t wstride, int64_t ldw, c
 }
 
 template <typename T>
+cudaError_t partial_sum_launch(const T* Wp, SegInfo seg, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st) {
+    partial_sum_kernel<T><<<(unsigned)ceil_div(N, 2), 256, 0, st>>>(Wp, seg, kw, N, Wout, ldo);
+    return cudaGetLastError();
+}
+
+template <typename T>
 cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx,
                              cudaStream_t st) {
     static size_t cur = 0;
@@ -75,6 +81,7 @@ cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, c
 }
 
 #define INST(T)                                                                                                        \
+    template cudaError_t partial_sum_launch<T>(const T*, SegInfo, int, int64_t, T*, int64_t, cudaStream_t);            \
     template cudaError_t larft_launch<T>(const T*, SegInfo, int64_t, int, int, int, T*, int, cudaStream_t);           \
     template cudaError_t ttw_launch<T>(const T*, SegInfo, int64_t, int64_t, const T*, int, int, int64_t, T*, int64_t,  \
                                        cudaStream_t);                                                                  \

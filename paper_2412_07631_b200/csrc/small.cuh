@@ -177,6 +177,21 @@ ttw_mma_kernel(const T* __restrict__ Wp, SegInfo seg, int64_t wstride, int64_t l
             }
 }
 
+// ---- sum of the compact stream-K partial tiles of a (kw <= 128) x N product -> dense W (ld = ldo) ----
+template <typename T>
+__global__ void __launch_bounds__(256)
+partial_sum_kernel(const T* __restrict__ Wp, SegInfo seg, int kw, int64_t N, T* __restrict__ Wout, int64_t ldo) {
+    const int64_t c = (int64_t)blockIdx.x * 2 + (threadIdx.x >> 7);
+    const int k = threadIdx.x & 127;
+    if (c >= N || k >= kw) return;
+    const int64_t t = c / seg.BN, slot = (int64_t)128 * seg.BN;
+    const int nseg = sk_nseg(t, seg.KT, seg.L);
+    const T* base = Wp + (t + sk_first_cta(t, seg.KT, seg.L)) * slot + k + (c % seg.BN) * 128;
+    T s = T(0);
+    for (int sp = 0; sp < nseg; ++sp) s += base[(int64_t)sp * slot];
+    Wout[k + c * ldo] = s;
+}
+
 // ---- diagonal-block triangular solve -------------------------------------------------------
 // R: kw x kw upper triangular (ld = ldr, explicit storage); C: kw x S in (ld = ldc); X out (ld = ldx).
 // Thread layout: 16 threads per right-hand side (a half-warp), each owning rows r = sub + 16 q in

@@ -26,6 +26,7 @@
 //           tcgen05 kernel of gemm_umma.cuh instead (4x the MMA rate); this one serves the rest.
 #pragma once
 #include <algorithm>
+#include <cstdlib>
 #include "common.cuh"
 #include "kernels.h"
 
@@ -149,6 +150,7 @@ struct StreamK {
     // run at the same time then share Gm V tiles and ~G/Gm W tiles (L2-resident) instead of
     // cycling through all of V (which no longer fits the L2 at m = 1e5)
     int G, Gm;
+    int l2_prefetch;          // direct mode: prefetch the next tile's C into L2 (set by the launcher)
 };
 // first CTA that touches tile t, and how many CTAs (= partial slots) it has
 __host__ __device__ inline int64_t sk_first_cta(int64_t t, int KT, int64_t L) { return (t * KT) / L; }
@@ -312,6 +314,17 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
         const int64_t seg_end = min(u1, (t + 1) * sk.KT);
         const int64_t m0 = tm * BM, n0 = tn * BN;
         const bool interior = (m0 + BM <= g.M) && (n0 + BN <= g.N);
+        if (sk.l2_prefetch && cscale != T(0) && seg_end < u1) {
+            // pull the NEXT tile's C into L2 while this tile is computed: its accumulator-init loads
+            // then cost an L2 hit instead of a DRAM round trip (the tile has only K/BK k-tiles to hide it)
+            int64_t ntm, ntn;
+            decode(t + 1, ntm, ntn);
+            constexpr int LPC = BM * (int)sizeof(T) / 128;          // 128-byte lines per tile column
+            for (int i = tid; i < BN * LPC; i += NT) {
+                const int64_t n = ntn * BN + i / LPC, m = ntm * BM + (int64_t)(i % LPC) * (128 / (int)sizeof(T));
+                if (m < g.M && n < g.N) prefetch_l2(&g.C[m + n * g.ldc]);
+            }
+        }
         T acc[MT][NTL][ACC];
         T cin[DEFER ? MT : 1][DEFER ? NTL : 1][ACC];     // DEFER: C tile requested now, used in the epilogue
         if (cscale != T(0)) {
@@ -447,7 +460,10 @@ inline cudaError_t launch_mma(GemmArgs<T> g, const MmaPlan& p, cudaStream_t st) 
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    kern<<<p.grid, Cfg::NT, Cfg::SMEM, st>>>(g, p.sk);
+    StreamK sk = p.sk;
+    static const int pf = [] { const char* e = getenv("CTQR_L2_PREFETCH"); return e ? atoi(e) : 0; }();
+    sk.l2_prefetch = pf;
+    kern<<<p.grid, Cfg::NT, Cfg::SMEM, st>>>(g, sk);
     return cudaGetLastError();
 }
 

@@ -10,7 +10,10 @@ where the O(mn^2) oracle cannot run in seconds:
         x* - x = (A^T A)^{-1} g and sigma_min(A_aug)^2 >= lambda, so ||x - x*|| <= ||g|| / lambda;
   (iv)  fp32 against fp64 solution.
 
-Set CTQR_FULLSIZE=c4 to run the same checks on configs[3] (57 GB fp64 in core; minutes).
+Set CTQR_FULLSIZE=c4 to run the same checks on configs[3] (57 GB fp64 in core; minutes), or
+CTQR_FULLSIZE=c5 for configs[4] in fp32 (145 GB, factored in place; the n x n accessor copy of R does
+not fit beside it, so (ii) is skipped there and fp64 -- 290 GB, out of core -- needs more host RAM
+than this box has).
 """
 import math
 import os
@@ -54,9 +57,11 @@ def run(P, dt):
     c = P["c"]
     tdt = torch.float64 if dt == np.float64 else torch.float32
     At, lam = wl.dense_augmented_device(c, tdt, P["coo"])
-    f = ctqr.ct_qr_factor(At, c.m, c.n, in_place=False)
-    del At
-    torch.cuda.empty_cache()
+    big = c.m * c.n * At.element_size() > 60e9            # no room for a second copy: factor in place
+    f = ctqr.ct_qr_factor(At, c.m, c.n, in_place=big)
+    if not big:
+        del At
+        torch.cuda.empty_cache()
     Bt = ctqr.colmajor_from_numpy(P["B"].astype(dt))
     Xt = torch.zeros((P["S"], c.n), dtype=tdt, device="cuda")
     ctqr.ct_qr_solve(f, Bt, P["S"], Xt)
@@ -75,6 +80,8 @@ RESULTS = {}
 def test_fullsize_factor_and_solve(problem, dt):
     P = problem
     c = P["c"]
+    if c.m * c.n * np.dtype(dt).itemsize > 170e9:
+        pytest.skip("does not fit the 180 GB of HBM in core; the out-of-core run needs the matrix in host RAM")
     f, X = run(P, dt)
     RESULTS[dt] = X
     tol_round = 1e-11 if dt == np.float64 else 5e-4
@@ -91,23 +98,25 @@ def test_fullsize_factor_and_solve(problem, dt):
     tau = ctqr.ct_qr_get_tau(f)
     assert relerr(V, oracle.V_of(VR)) <= tol_round
     assert relerr(tau[:k], tau_o) <= tol_round
-    R = ctqr.ct_qr_get_R(f)
-    assert relerr(R[:k, :k], oracle.R_of(VR)) <= tol_round
     T0 = ctqr.ct_qr_get_T(f, 0)
     kt = min(k, T0.shape[0])
     assert relerr(T0[:kt, :kt], oracle.larft(VR, tau_o, 0, kt)) <= tol_round
-    assert np.all(np.tril(R, -1) == 0)
-    # (ii) R^T R = A^T A on sampled columns (late ones included)
     Aaug, _ = sparse_aug(P, dt)
-    rng = np.random.default_rng(5)
-    js = np.unique(np.concatenate([rng.integers(0, c.n, 24), [0, c.n - 1, c.n // 2]]))
-    G_cols = (Aaug.T @ Aaug[:, js]).toarray()                     # n x len(js), fp64
-    R64 = R.astype(np.float64)
-    RtR_cols = R64.T @ R64[:, js]
-    scale = np.linalg.norm(G_cols)
-    gram_err = np.linalg.norm(RtR_cols - G_cols) / scale
-    assert gram_err <= (1e-12 if dt == np.float64 else 5e-5), gram_err
-    del R, R64
+    gram_err = float("nan")
+    if c.n <= 70000:
+        R = ctqr.ct_qr_get_R(f)
+        assert relerr(R[:k, :k], oracle.R_of(VR)) <= tol_round
+        assert np.all(np.tril(R, -1) == 0)
+        # (ii) R^T R = A^T A on sampled columns (late ones included)
+        rng = np.random.default_rng(5)
+        js = np.unique(np.concatenate([rng.integers(0, c.n, 24), [0, c.n - 1, c.n // 2]]))
+        G_cols = (Aaug.T @ Aaug[:, js]).toarray()                     # n x len(js), fp64
+        R64 = R.astype(np.float64)
+        RtR_cols = R64.T @ R64[:, js]
+        scale = np.linalg.norm(G_cols)
+        gram_err = np.linalg.norm(RtR_cols - G_cols) / scale
+        assert gram_err <= (1e-12 if dt == np.float64 else 5e-5), gram_err
+        del R, R64
     # (iii) certified solution error from the normal-equations residual
     B = P["B"].astype(dt).astype(np.float64)
     X64 = X.astype(np.float64)

@@ -59,7 +59,10 @@ typedef struct {
                                    for matrix tiles: forces the out-of-core path when m*n*w exceeds it */
     int32_t gemm_impl;          /* 0 = default (fp64: DMMA tensor cores, fp32: FFMA), 1 = SIMT reference kernels */
     int32_t profile;            /* 1: CUDA-event time every trailing-update contraction launch (stats.vtc_*, upd_*) */
-    const char* file_path;      /* optional file-backed tier for the factor (NULL = none) */
+    const char* file_path;      /* optional file-backed tier: path of a file holding the column-major m x n matrix
+                                   (leading dimension lda, offset 0).  The A argument is then ignored (may be NULL);
+                                   the file is mapped read-write, factored out of core through the page cache and
+                                   overwritten with the factor, which ct_qr_solve streams from it.  NULL = none */
     void* stream;               /* cudaStream_t the caller's data is ordered on (NULL = legacy default) */
 } ctqr_options_t;
 
@@ -69,8 +72,8 @@ typedef struct {
     int32_t nb, ib, n_panels, n_superpanels;   /* n_superpanels == 1 when in-core */
     int32_t out_of_core, singular_col;         /* singular_col = -1 when none */
     double factor_ms;          /* whole ct_qr_factor device time */
-    double panel_ms;           /* sum of panel (a1) + T (a2) chains, as timed on their stream */
-    double update_ms;          /* sum of trailing updates (a3) */
+    double panel_ms;           /* opt->profile: factor_ms minus update_ms (panel chains a1 + a2, narrow updates, T^T W) */
+    double update_ms;          /* opt->profile: time inside the two contractions of the trailing updates (a3) */
     double solve_ms;           /* last ct_qr_solve device time */
     double apply_qt_ms;        /* last Q^T B part (a6) */
     double trsm_ms;            /* last triangular solve part (a7) */

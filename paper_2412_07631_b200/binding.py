@@ -172,16 +172,17 @@ class Factor:
 
 def ct_qr_factor(A, m: int, n: int, lda: int | None = None, *, nb: int = 0, ib: int = 0,
                  lookahead: int = -1, in_place: bool = False, device_budget_bytes: int = 0,
-                 gemm_impl: int = 0, profile: bool = False, stream=None) -> Factor:
+                 gemm_impl: int = 0, profile: bool = False, stream=None, file_path: str | None = None,
+                 dtype=None) -> Factor:
     """Eq. 2.  ``A``: torch tensor (device or pinned/pageable host) or numpy array whose MEMORY
     is the column-major m x n matrix with leading dimension ``lda`` (default m)."""
-    code = _code_of(A)
+    code = _code_of(A) if A is not None else (F64 if np.dtype(dtype) == np.float64 else F32)
     lda = m if lda is None else lda
     o = Options(nb=nb, ib=ib, lookahead=lookahead, in_place=int(in_place),
                 device_budget_bytes=device_budget_bytes, gemm_impl=gemm_impl, profile=int(profile),
-                file_path=None, stream=stream)
+                file_path=file_path.encode() if file_path else None, stream=stream)
     h = _P()
-    _check(lib().ct_qr_factor(_ptr(A), m, n, lda, code, ctypes.byref(o), ctypes.byref(h)))
+    _check(lib().ct_qr_factor(_ptr(A) if A is not None else None, m, n, lda, code, ctypes.byref(o), ctypes.byref(h)))
     return Factor(h, m, n, code, keep=A if in_place else None)
 
 

@@ -6,6 +6,10 @@
 #include <cooperative_groups.h>
 #include <stdarg.h>
 #include <stdlib.h>
+#include <fcntl.h>
+#include <sys/mman.h>
+#include <sys/stat.h>
+#include <unistd.h>
 #include <string.h>
 #include <algorithm>
 #include <new>
@@ -103,10 +107,15 @@ struct ctqr_handle_s {
     bool factored = false;
     // out-of-core state
     bool ooc = false; void* hA = nullptr; int64_t hlda = 0; int n_super = 1;
+    // file-backed tier: the matrix / factor lives in a file mapped MAP_SHARED (the OS page cache is the
+    // host-RAM block cache over the disk of PAPER.md L58)
+    void* fmap = nullptr; size_t fmap_len = 0; int ffd = -1;
     void* dVb[2] = {nullptr, nullptr}; int64_t ldvb = 0;   // double buffer for streamed panels (m x nb each)
     cudaEvent_t evVin[2] = {nullptr, nullptr}, evVfree[2] = {nullptr, nullptr};
     ~ctqr_handle_s() {
         if (own_A && dA) cudaFree(dA);
+        if (fmap) { msync(fmap, fmap_len, MS_SYNC); munmap(fmap, fmap_len); }
+        if (ffd >= 0) close(ffd);
         cudaFree(dT); cudaFree(dRd); cudaFree(dTau);
         for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); }
         cudaFree(dTin); cudaFree(dPart); cudaFree(dRow); cudaFree(dBar); cudaFree(dFlag);
@@ -586,7 +595,7 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
     }
     const size_t budget = o.device_budget_bytes > 0 ? (size_t)o.device_budget_bytes
                                                     : (freeb > slack ? freeb - slack : 0);
-    if (bytes <= budget) {
+    if (bytes <= budget && !h.fmap) {
         // host matrix that fits: stage once, factor in core, keep the factor on the device
         CKI(alloc_state<T>(h, n));
         h.lda = round_up(m, 16 / sizeof(T));
@@ -602,6 +611,7 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
     const int64_t col_bytes = lds * (int64_t)sizeof(T);
     int64_t ns = ((int64_t)budget / col_bytes - 2 * h.nb) / 2;
     ns = (ns / h.nb) * h.nb;
+    if (ns > round_up(n, h.nb)) ns = round_up(n, h.nb);
     if (ns < h.nb)
         return set_err(CTQR_ERR_NOMEM, "device budget of %zu bytes cannot hold two %d-column super-panels and two "
                        "panel buffers of %lld rows", budget, h.nb, (long long)m);
@@ -612,7 +622,8 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
 extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dtype_t dtype,
                             const ctqr_options_t* opt, ctqr_handle_t* out) {
     g_err[0] = 0;
-    if (!A) return set_err(-1, "A is NULL");
+    const bool use_file = opt && opt->file_path && opt->file_path[0];
+    if (!A && !use_file) return set_err(-1, "A is NULL");
     if (m < 1) return set_err(-2, "m < 1");
     if (n < 1 || n > m) return set_err(-3, "need 1 <= n <= m");
     if (lda < m) return set_err(-4, "lda < m");
@@ -651,10 +662,27 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
     }
     // order after the caller's stream
     if (cudaStreamSynchronize(h->user) != cudaSuccess) { delete h; return set_err(CTQR_ERR_CUDA, "user stream sync failed"); }
-    const bool on_dev = is_device_ptr(A);
+    if (use_file) {
+        // file tier: column-major m x n matrix with leading dimension lda at offset 0 of the file
+        const size_t need = (size_t)lda * (size_t)n * h->w;
+        h->ffd = open(o.file_path, O_RDWR);
+        struct stat sb;
+        if (h->ffd < 0 || fstat(h->ffd, &sb) != 0 || (size_t)sb.st_size < need) {
+            delete h;
+            return set_err(CTQR_ERR_IO, "cannot open %s read-write with at least %zu bytes", o.file_path, need);
+        }
+        void* mp = mmap(nullptr, need, PROT_READ | PROT_WRITE, MAP_SHARED, h->ffd, 0);
+        if (mp == MAP_FAILED) { delete h; return set_err(CTQR_ERR_IO, "mmap of %s failed", o.file_path); }
+        h->fmap = mp; h->fmap_len = need;
+        A = mp;
+    }
+    const bool on_dev = !use_file && is_device_ptr(A);
     int rc = (dtype == CTQR_F64) ? factor_typed<double>(*h, A, lda, on_dev, o)
                                  : factor_typed<float>(*h, A, lda, on_dev, o);
     if (rc != 0) { cudaDeviceSynchronize(); delete h; return rc; }
+    if (h->fmap) msync(h->fmap, h->fmap_len, MS_ASYNC);
+    h->st.update_ms = h->st.vtc_ms + h->st.upd_ms;              // opt->profile only
+    h->st.panel_ms = h->profile ? h->st.factor_ms - h->st.update_ms : 0.0;   // time not inside the two bulk contractions
     h->st.m = m; h->st.n = n; h->st.nb = h->nb; h->st.ib = h->ib; h->st.n_panels = h->P;
     h->st.n_superpanels = h->n_super; h->st.out_of_core = h->ooc ? 1 : 0; h->st.singular_col = -1;
     h->st.factor_flops = 2.0 * (double)m * (double)n * (double)n - 2.0 * (double)n * (double)n * (double)n / 3.0;

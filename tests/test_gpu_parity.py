@@ -260,3 +260,42 @@ def test_gemm_fp32_long_k_accumulation(ta):
     ctqr.ct_qr_gemm(ta, M, N, K, 1.0, At, A.shape[0], Bt, K, 0.0, Ct, M, 0)
     err = np.max(np.abs(ctqr.numpy_from_colmajor(Ct) - ref) / np.abs(ref))
     assert err <= 1e-5, err
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("budget_cols", [0, 96])
+def test_file_backed_tier(tmp_path, dt, budget_cols):
+    """Optional file tier (the matrix lives on secondary storage behind a host-RAM
+    cache): the matrix is read from a file through the page cache, the factor is written back into
+    the same file, the solve streams it from there.  budget 0 = one super-panel if it fits."""
+    m, n, S, nb = 600, 500, 7, 32
+    rng = np.random.default_rng(33)
+    A = np.asfortranarray(rng.standard_normal((m, n)).astype(dt))
+    B = np.asfortranarray(rng.standard_normal((m, S)).astype(dt))
+    path = str(tmp_path / "A.bin")
+    A.T.tofile(path)                                  # column-major bytes, lda = m
+    budget = _ooc_budget(m, nb, budget_cols, dt) if budget_cols else 0
+    f = ctqr.ct_qr_factor(None, m, n, nb=nb, file_path=path, dtype=dt, device_budget_bytes=budget)
+    st = f.stats()
+    assert st["out_of_core"] == 1 and st["n_superpanels"] == (-(-n // budget_cols) if budget_cols else 1)
+    X = np.zeros((n, S), dtype=dt, order="F")
+    ctqr.ct_qr_solve(f, B, S, X)
+    R, V, tau = ctqr.ct_qr_get_R(f), ctqr.ct_qr_get_V(f), ctqr.ct_qr_get_tau(f)
+    VR, tau_o = oracle.qr(A)
+    assert backward_error(A, V, tau, R) <= BACKWARD[dt]
+    assert relerr(X, oracle.solve(VR, tau_o, B)) <= SOLUTION[dt]
+    f.destroy()
+    # the file now holds the factor: V below the diagonal blocks (and R above them)
+    F = np.fromfile(path, dtype=dt).reshape(n, m).T
+    assert relerr(np.tril(F, -nb)[:, :n], np.tril(oracle.V_of(VR), -nb)) <= ROUND[dt]
+
+
+def test_file_tier_errors(tmp_path):
+    with pytest.raises(ctqr.CtqrError) as ei:
+        ctqr.ct_qr_factor(None, 100, 50, file_path=str(tmp_path / "missing.bin"), dtype=np.float64)
+    assert ei.value.code == 3
+    p = tmp_path / "short.bin"
+    p.write_bytes(b"\0" * 64)
+    with pytest.raises(ctqr.CtqrError) as ei:
+        ctqr.ct_qr_factor(None, 100, 50, file_path=str(p), dtype=np.float64)
+    assert ei.value.code == 3

@@ -1,7 +1,7 @@
 // ctqr.cu -- C-ABI (include/ctqr.h) and the host-side drivers of the hot path:
 //   a4 in-core blocked Householder QR with look-ahead, a6 batched Q^T B, a7 blocked TRSM
 //   (Eq. 2-3; TRSM task list L62-73).
-// The out-of-core scheduler (a5) lives in ooc.cuh.
+// and a5, the out-of-core scheduler (factor_ooc, streamed solve, optional file tier).
 #include <cuda_runtime.h>
 #include <cooperative_groups.h>
 #include <stdarg.h>
@@ -86,8 +86,8 @@ struct ctqr_handle_s {
     // workspaces: [0] update stream, [1] panel stream
     void* dWp[2] = {nullptr, nullptr}; size_t wp_elems[2] = {0, 0};
     void* dW[2] = {nullptr, nullptr};  size_t w_elems[2] = {0, 0};
-    void* dTin = nullptr; void* dPart = nullptr; void* dRow = nullptr;
-    unsigned* dBar = nullptr; unsigned bar_count = 0;
+    void* dPart = nullptr;             // LL slots of the panel kernel
+    unsigned bar_count = 0;            // step numbers handed to the panel kernel (never reused)
     int* dFlag = nullptr;
     cudaStream_t sU = nullptr, sP = nullptr, sC = nullptr, sD = nullptr, user = nullptr;
     cudaEvent_t evP = nullptr, evL = nullptr, evU = nullptr;
@@ -110,6 +110,7 @@ struct ctqr_handle_s {
     // file-backed tier: the matrix / factor lives in a file mapped MAP_SHARED (the OS page cache is the
     // host-RAM block cache over the disk of PAPER.md L58)
     void* fmap = nullptr; size_t fmap_len = 0; int ffd = -1;
+    void* spbuf[2] = {nullptr, nullptr};   // super-panel buffers, alive only during factor_ooc
     void* dVb[2] = {nullptr, nullptr}; int64_t ldvb = 0;   // double buffer for streamed panels (m x nb each)
     cudaEvent_t evVin[2] = {nullptr, nullptr}, evVfree[2] = {nullptr, nullptr};
     ~ctqr_handle_s() {
@@ -118,7 +119,8 @@ struct ctqr_handle_s {
         if (ffd >= 0) close(ffd);
         cudaFree(dT); cudaFree(dRd); cudaFree(dTau);
         for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); }
-        cudaFree(dTin); cudaFree(dPart); cudaFree(dRow); cudaFree(dBar); cudaFree(dFlag);
+        cudaFree(dPart); cudaFree(dFlag);
+        for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
         for (auto e : tpool) cudaEventDestroy(e);
         if (sU) cudaStreamDestroy(sU);
@@ -238,7 +240,7 @@ static int panel_inner(H& h, int ib, cudaStream_t st, T* A, int64_t lda, int64_t
     PanelArgs<T> pa{};
     pa.A = A; pa.lda = lda; pa.m = m; pa.j0 = j0; pa.jb = jb; pa.ibw = ibw;
     pa.tau = P_<T>(h.dTau); pa.Rd = Rd; pa.ldrd = h.nb; pa.Tin = Tin; pa.ldtin = h.nb;
-    pa.part = P_<T>(h.dPart); pa.rowbuf = P_<T>(h.dRow); pa.bar = h.dBar;
+    pa.part = P_<T>(h.dPart);
     const int64_t rows = m - jb;
     const int gmax = h.sms;
     const int* list = panel_rpts<T>(ib);
@@ -437,11 +439,13 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
     const int64_t lds = round_up(m, 16 / (int64_t)sizeof(T));
     CKI(ensure_stream_bufs(h));
     T* sp[2] = {nullptr, nullptr};
-    for (int i = 0; i < 2; ++i)
-        if (cudaMalloc(&sp[i], (size_t)lds * std::min<int64_t>(ns, n) * sizeof(T)) != cudaSuccess) {
-            cudaGetLastError(); cudaFree(sp[0]);
+    for (int i = 0; i < 2; ++i) {
+        if (cudaMalloc(&h.spbuf[i], (size_t)lds * std::min<int64_t>(ns, n) * sizeof(T)) != cudaSuccess) {
+            cudaGetLastError();
             return set_err(CTQR_ERR_NOMEM, "cannot allocate the super-panel buffers (%lld columns)", (long long)ns);
         }
+        sp[i] = P_<T>(h.spbuf[i]);         // owned by the handle: freed below, or by the destructor on an error path
+    }
     std::vector<cudaEvent_t> evIn(Ps), evOut(Ps), evDone(Ps), evFree(Ps);
     for (int s = 0; s < Ps; ++s) {
         evIn[s] = new_event(h, false); evOut[s] = new_event(h, false);
@@ -510,7 +514,7 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
     }
     cudaError_t e1 = cudaStreamSynchronize(h.sU), e2 = cudaStreamSynchronize(h.sP);
     cudaError_t e3 = cudaStreamSynchronize(h.sC), e4 = cudaStreamSynchronize(h.sD);
-    cudaFree(sp[0]); cudaFree(sp[1]);
+    for (int i = 0; i < 2; ++i) { cudaFree(h.spbuf[i]); h.spbuf[i] = nullptr; }
     if (rc) return rc;
     if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess)
         return set_err(CTQR_ERR_CUDA, "out-of-core factorisation failed: %s",
@@ -544,13 +548,9 @@ static int alloc_state(H& h, int64_t max_nc) {
         CK(cudaMalloc(&h.dW[i], h.w_elems[i] * sizeof(T)));
         CK(cudaMalloc(&h.dWp[i], h.wp_elems[i] * sizeof(T)));
     }
-    CK(cudaMalloc(&h.dTin, 32 * 32 * sizeof(T)));
     // LL slots of the panel kernel: [2 parities][G + 1 <= 257][IB <= 32] x 16 bytes, step numbers start at 1
     CK(cudaMalloc(&h.dPart, (size_t)2 * 257 * 32 * 16));
     CK(cudaMemsetAsync(h.dPart, 0, (size_t)2 * 257 * 32 * 16, h.sU));
-    CK(cudaMalloc(&h.dRow, 2 * 32 * sizeof(T)));
-    CK(cudaMalloc(&h.dBar, sizeof(unsigned)));
-    CK(cudaMemsetAsync(h.dBar, 0, sizeof(unsigned), h.sU));
     CK(cudaMalloc(&h.dFlag, sizeof(int)));
     h.bar_count = 0;
     return 0;

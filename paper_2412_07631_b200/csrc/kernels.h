@@ -27,10 +27,8 @@ struct PanelArgs {
     T* tau;            // tau + jb written
     T* Rd; int ldrd;   // diagonal block of R for the enclosing panel (ldrd x ldrd, zero-initialised)
     T* Tin; int ldtin; // ibw x ibw inner T factor (ld = ldtin), written by CTA 0 into the diagonal block of T_k
-    T* part;           // [2][G][IB] per-CTA partial sums
-    T* rowbuf;         // [2][IB] the pivot row broadcast
-    unsigned* bar;     // grid barrier counter (monotone)
-    unsigned bar_base; // counter value when this launch starts
+    T* part;           // LL slots: [2 parities][G + 1][IB] x 16 bytes (record G = pivot row published by CTA 0)
+    unsigned bar_base; // step number before this launch; column j of the launch uses bar_base + j + 1
 };
 
 // How the K range of a product was cut, for the kernels that sum the partial outputs.

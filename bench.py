@@ -427,7 +427,13 @@ def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:
             "other_contraction": {"kernel": KERNEL_NAMES[(dtype, oth)],
                                   "achieved": o["flops"] / (o["ms"] * 1e-3) / 1e12 if o["ms"] > 0 else 0.0,
                                   "launches": int(o["launches"]), "ms_total": o["ms"]},
-            "share_of_factor_time": None}
+            "share_of_factor_time": None,
+            # fp32 only: the same work against the tensor roofline of the 3xTF32 split it actually runs as
+            # (measured bf16 peak x nominal tf32/bf16 ratio 1.1/2.25, three MMAs per product)
+            "tensor_roofline_3xtf32": (None if dtype == "f64" else {
+                "peak": float(peaks.get("bf16_tflops", 1590.0)) * (1.1 / 2.25) / 3.0, "unit": UNIT,
+                "frac": ach / (float(peaks.get("bf16_tflops", 1590.0)) * (1.1 / 2.25) / 3.0),
+                "peak_source": "MEASURED_PEAKS.json bf16_tflops (%s) x 1.1/2.25 / 3" % peaks.get("_source")})}
 
 
 def main():

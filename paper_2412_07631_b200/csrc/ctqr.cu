@@ -246,6 +246,11 @@ static int panel_inner(H& h, int ib, cudaStream_t st, T* A, int64_t lda, int64_t
     const int* list = panel_rpts<T>(ib);
     // largest rpt whose grid still has >= 8 CTAs (enough parallelism), else the smallest that fits
     int pick = 0;
+    static const int force_rpt = [] { const char* e = getenv("CTQR_PANEL_RPT"); return e ? atoi(e) : 0; }();
+    if (force_rpt > 0)
+        for (const int* r = list; *r; ++r)
+            if (*r == force_rpt && ceil_div(rows, (int64_t)NT * *r) <= gmax) { pick = *r; break; }
+    if (!pick)
     for (const int* r = list; *r; ++r) {
         int64_t g = ceil_div(rows, (int64_t)NT * *r);
         if (g <= gmax && (g >= 8 || r[1] == 0)) { pick = *r; break; }

@@ -161,7 +161,9 @@ def test_host_pointers_and_halves(dt):
 @pytest.mark.parametrize("dt", DT)
 @pytest.mark.parametrize("ta", [True, False])
 @pytest.mark.parametrize("impl", [0, 1])
-@pytest.mark.parametrize("mnk", [(128, 64, 256), (37, 150, 1001), (130, 9, 77), (5, 300, 4)])
+@pytest.mark.parametrize("mnk", [(128, 64, 256), (37, 150, 1001), (130, 9, 77), (5, 300, 4),
+                                 # shapes that reach the stream-K / tcgen05 kernels with ragged tiles and K tails
+                                 (100, 300, 1000), (1000, 300, 100), (256, 128, 4096), (128, 1000, 36)])
 def test_gemm_kernel(mnk, impl, ta, dt):
     """Kernel-level: C <- alpha op(A) B + beta C against the definition (numpy fp64)."""
     import torch

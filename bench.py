@@ -512,7 +512,7 @@ def main():
             "peak_probe_tflops": probe}
     if res2 is not None:
         res2 = finish(res2, other)
-        line["also"] = {other: {k: res2[k] for k in ("value", "ms_per_step", "factor_ms_per_step",
+        line["also"] = {other: {k: res2.get(k) for k in ("value", "ms_per_step", "factor_ms_per_step",
                                                      "frac_of_peak_whole_factor", "solve", "quality_noisy", "quality_consistent", "e2e",
                                                      "gpu_launches", "roofline", "clocks")}}
     if not args.no_extras and world == 1:

@@ -82,6 +82,8 @@ struct ctqr_handle_s {
     void* dA = nullptr; bool own_A = false;   // factored matrix (device, in-core path)
     void* dT = nullptr;                // P blocks of nb x nb (ld nb)
     void* dRd = nullptr;               // P blocks of nb x nb (ld nb): diagonal blocks of R
+    void* dRinv = nullptr;             // their inverses (nb == 128 only), filled at the first solve
+    bool rinv_ready = false;
     void* dTau = nullptr;              // n
     // workspaces: [0] update stream, [1] panel stream
     void* dWp[2] = {nullptr, nullptr}; size_t wp_elems[2] = {0, 0};
@@ -117,7 +119,7 @@ struct ctqr_handle_s {
         if (own_A && dA) cudaFree(dA);
         if (fmap) { msync(fmap, fmap_len, MS_SYNC); munmap(fmap, fmap_len); }
         if (ffd >= 0) close(ffd);
-        cudaFree(dT); cudaFree(dRd); cudaFree(dTau);
+        cudaFree(dT); cudaFree(dRd); cudaFree(dRinv); cudaFree(dTau);
         for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); }
         cudaFree(dPart); cudaFree(dFlag);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
@@ -543,6 +545,7 @@ static int alloc_state(H& h, int64_t max_nc) {
     CK(cudaMemsetAsync(h.dT, 0, blk * h.P * sizeof(T), h.sU));
     CK(cudaMemsetAsync(h.dRd, 0, blk * h.P * sizeof(T), h.sU));
     CK(cudaMalloc(&h.dTau, (size_t)h.n * sizeof(T)));
+    if (nb == 128) CK(cudaMalloc(&h.dRinv, blk * h.P * sizeof(T)));
     const int64_t slots = (int64_t)h.sms * 2;
     // [0]: trailing update / solve; [1]: in-panel work
     h.w_elems[0] = (size_t)nb * (size_t)max_nc;
@@ -737,6 +740,15 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
     CK(cudaMemcpyAsync(&flag, h.dFlag, sizeof(int), cudaMemcpyDeviceToHost, h.sU));
     CK(cudaStreamSynchronize(h.sU));
     if (flag < h.n) { h.st.singular_col = flag; return set_err(CTQR_ERR_SINGULAR, "R[%d,%d] == 0", flag, flag); }
+    // diagonal tasks through the inverses of the diagonal blocks (built once per handle) unless
+    // CTQR_TRSM_EXACT=1 asks for the back-substitution kernel
+    static const bool exact = [] { const char* e = getenv("CTQR_TRSM_EXACT"); return e && e[0] == '1'; }();
+    const bool use_inv = !exact && h.dRinv && ldx % (16 / (int64_t)sizeof(T)) == 0;
+    if (use_inv && !h.rinv_ready) {
+        CK(trinv_launch<T>(P_<T>(h.dRd), h.nb, h.n, h.P, P_<T>(h.dRinv), h.sU));
+        h.rinv_ready = true;
+        h.launches += 1;
+    }
     for (int i = h.P - 1; i >= 0; --i) {
         const int64_t i0 = (int64_t)i * h.nb;
         const int nbw = (int)std::min<int64_t>(h.nb, h.n - i0);
@@ -748,12 +760,25 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
                 Rcol = P_<T>(h.dVb[slot]); ldr = h.ldvb;
             } else { Rcol = P_<T>(h.dA) + i0 * h.lda; ldr = h.lda; }
         }
-        CK(trsm_diag_launch<T>(P_<T>(h.dRd) + (size_t)i * h.nb * h.nb, h.nb, nbw, X + i0, ldx, S, X + i0, ldx, h.sU));
-        h.launches += 1;
+        const T* Xi = X + i0; int64_t ldxi = ldx;         // where the update below reads X_i
+        if (use_inv) {
+            // X_i = R_ii^{-1} C_i as a contraction (out of place into W, copied back over C_i)
+            T* W = P_<T>(h.dW[0]);
+            GemmArgs<T> gi{};
+            gi.M = nbw; gi.N = S; gi.K = nbw; gi.A = P_<T>(h.dRinv) + (size_t)i * h.nb * h.nb; gi.lda = h.nb;
+            gi.B = X + i0; gi.ldb = ldx; gi.C = W; gi.ldc = h.nb; gi.alpha = T(1); gi.beta = T(0);
+            CK(gemm_direct<T>(false, gi, h.gemm_impl, h.sms, h.sU));
+            CK(copy2d_launch<T>(W, h.nb, X + i0, ldx, nbw, S, h.sU));
+            Xi = W; ldxi = h.nb;
+            h.launches += 2;
+        } else {
+            CK(trsm_diag_launch<T>(P_<T>(h.dRd) + (size_t)i * h.nb * h.nb, h.nb, nbw, X + i0, ldx, S, X + i0, ldx, h.sU));
+            h.launches += 1;
+        }
         if (i0 > 0) {
             if (h.ooc) CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
             GemmArgs<T> g{};
-            g.M = i0; g.N = S; g.K = nbw; g.A = Rcol; g.lda = ldr; g.B = X + i0; g.ldb = ldx;
+            g.M = i0; g.N = S; g.K = nbw; g.A = Rcol; g.lda = ldr; g.B = Xi; g.ldb = ldxi;
             g.C = X; g.ldc = ldx; g.alpha = T(-1); g.beta = T(1);
             CK(gemm_direct<T>(false, g, h.gemm_impl, h.sms, h.sU));
             h.launches += 1;

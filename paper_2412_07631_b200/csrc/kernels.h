@@ -71,6 +71,8 @@ template <typename T> cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t w
 // dense (kw x N, ld = ldo) sum of the compact stream-K partial tiles (seg.L > 0)
 template <typename T> cudaError_t partial_sum_launch(const T* Wp, SegInfo seg, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st);
 template <typename T> cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx, cudaStream_t st);
+// inverses of the P diagonal blocks of R (nb x nb each, ld = nb; a narrower last block is padded with zeros)
+template <typename T> cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, cudaStream_t st);
 template <typename T> cudaError_t copy2d_launch(const T* src, int64_t lds, T* dst, int64_t ldd, int64_t rows, int64_t cols, cudaStream_t st);
 template <typename T> cudaError_t gather_R_launch(const T* A, int64_t lda, const T* Rd, int nb, int64_t n, T* R, int64_t ldr, cudaStream_t st);
 template <typename T> cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, cudaStream_t st);

@@ -60,6 +60,16 @@ cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ld
 }
 
 template <typename T>
+cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, cudaStream_t st) {
+    static size_t cur = 0;
+    const size_t smem = (size_t)nb * (nb + 1) * sizeof(T);
+    cudaError_t e = ensure_smem(trinv_kernel<T>, smem, cur);
+    if (e != cudaSuccess) return e;
+    trinv_kernel<T><<<P, 128, smem, st>>>(Rd, nb, n, Rinv);
+    return cudaGetLastError();
+}
+
+template <typename T>
 cudaError_t copy2d_launch(const T* src, int64_t lds, T* dst, int64_t ldd, int64_t rows, int64_t cols, cudaStream_t st) {
     if (rows <= 0 || cols <= 0) return cudaSuccess;
     dim3 grid((unsigned)ceil_div(rows, 256), (unsigned)std::min<int64_t>(cols, 65535));
@@ -81,6 +91,7 @@ cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, c
 }
 
 #define INST(T)                                                                                                        \
+    template cudaError_t trinv_launch<T>(const T*, int, int64_t, int, T*, cudaStream_t);                               \
     template cudaError_t partial_sum_launch<T>(const T*, SegInfo, int, int64_t, T*, int64_t, cudaStream_t);            \
     template cudaError_t larft_launch<T>(const T*, SegInfo, int64_t, int, int, int, T*, int, cudaStream_t);           \
     template cudaError_t ttw_launch<T>(const T*, SegInfo, int64_t, int64_t, const T*, int, int, int64_t, T*, int64_t,  \

@@ -240,6 +240,43 @@ trsm_diag_kernel(const T* __restrict__ R, int ldr, int kw, const T* __restrict__
     }
 }
 
+// ---- inverse of the diagonal blocks of R (one CTA per block, thread j computes column j) ----------
+// X = R_ii^{-1} by back-substitution on the identity, in the working precision.  Used by the blocked
+// TRSM so that the diagonal task "R_ii X_i = C_i" becomes a tensor-core product
+// X_i = R_ii^{-1} C_i instead of 128 dependent steps per right-hand side.
+template <typename T>
+__global__ void __launch_bounds__(128)
+trinv_kernel(const T* __restrict__ Rd, int nb, int64_t n, T* __restrict__ Rinv) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* Ms = reinterpret_cast<T*>(smem_raw);          // [nb][nb+1]: R on entry, R^{-1} on exit (in place, column by column)
+    const int ld = nb + 1;
+    const int64_t i0 = (int64_t)blockIdx.x * nb;
+    const int kw = (int)min((int64_t)nb, n - i0);
+    const T* R = Rd + (size_t)blockIdx.x * nb * nb;
+    for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) {
+        const int i = e % nb, k = e / nb;
+        Ms[i * ld + k] = (i < kw && k < kw && i <= k) ? R[i + (size_t)k * nb] : T(0);
+    }
+    __syncthreads();
+    const int i = threadIdx.x;
+    for (int j = 0; j < kw; ++j) {
+        // X[0:j, j] = -X[0:j,0:j] * R[0:j, j] / R[j][j]   (the leading block is already inverted)
+        const T xjj = Num<T>::div(T(1), Ms[j * ld + j]);
+        T t = T(0);
+        if (i < j)
+            for (int k = i; k < j; ++k) t = fma(Ms[i * ld + k], Ms[k * ld + j], t);
+        __syncthreads();
+        if (i < j) Ms[i * ld + j] = -t * xjj;
+        else if (i == j) Ms[j * ld + j] = xjj;
+        __syncthreads();
+    }
+    T* out = Rinv + (size_t)blockIdx.x * nb * nb;
+    for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) {
+        const int r = e % nb, c = e / nb;
+        out[r + (size_t)c * nb] = Ms[r * ld + c];
+    }
+}
+
 // ---- utility kernels -----------------------------------------------------------------------
 template <typename T>
 __global__ void copy2d_kernel(const T* __restrict__ src, int64_t lds, T* __restrict__ dst, int64_t ldd,

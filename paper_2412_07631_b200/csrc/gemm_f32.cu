@@ -94,7 +94,10 @@ cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int im
         case 5: return launch_simt<float, false, 128, 128, 8>(g, L.splits, st);
         case 1: return launch_mma<float, true, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
         case 3: return launch_mma<float, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
-        case 21: return umma::launch_umma<true, 128>(g, to_plan(L), st);
+        case 21: {
+            static const bool ws = [] { const char* e = getenv("CTQR_TN_WS"); return e && e[0] == '1'; }();
+            return ws ? umma::launch_umma_ws<true, 128>(g, to_plan(L), st) : umma::launch_umma<true, 128>(g, to_plan(L), st);
+        }
         case 23: return umma::launch_umma_ws<false, 64>(g, to_plan(L), st);
         case 24: return umma::launch_umma<false, 128>(g, to_plan(L), st);
     }

@@ -309,13 +309,15 @@ constexpr int WS_PROD = 128, WS_DRAIN = 256, WS_NT = WS_PROD + WS_DRAIN + 32;
 // memory-level parallelism: the operands of a k-block are fetched with cp.async into a staging ring
 // WS_DEPTH k-blocks ahead (registers held only 2 k-blocks = 48 KB per SM in flight, which at ~1.5 us
 // of loaded memory latency capped a tile at ~3 us; the tensor core needs < 1 us)
-constexpr int WS_USTAGES = 2, WS_NSTG = 5, WS_DEPTH = WS_NSTG - 1;
+constexpr int WS_USTAGES = 2;
+__host__ __device__ constexpr int ws_nstg(int bn) { return bn == 64 ? 5 : 3; }   // staging stages that fit beside the two UMMA stages
 template <int BN> struct WsSmem {
     static constexpr int B_TILE = BN * BK * 4;
     static constexpr int USTAGE = 2 * TILE_BYTES + 2 * B_TILE;                 // A_hi, A_lo, B_hi, B_lo
     static constexpr int CHUNKS = (1024 + BN * 8) / WS_PROD;                   // 16-byte chunks per producer thread per k-block
     static constexpr int STG = CHUNKS * WS_PROD * 16;                          // one staging stage
-    static constexpr int BAR_OFF = WS_USTAGES * USTAGE + WS_NSTG * STG;
+    static constexpr int NSTG = ws_nstg(BN);
+    static constexpr int BAR_OFF = WS_USTAGES * USTAGE + NSTG * STG;
     static constexpr int BYTES = BAR_OFF + 256 + 1024;
 };
 
@@ -324,6 +326,8 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
     constexpr int NC = BN / 2;                 // output columns per drainer thread
     constexpr int PA = 1024 / WS_PROD;         // A chunks (float4) per producer thread per k-block
     constexpr int PB = BN * 8 / WS_PROD;       // B chunks
+    constexpr int WS_NSTG = WsSmem<BN>::NSTG, WS_DEPTH = WS_NSTG - 1;
+    constexpr bool DEFER = (BN == 64);         // drainer registers allow holding the C tile until the epilogue
     extern __shared__ unsigned char smem_raw[];
     const unsigned sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
@@ -483,7 +487,7 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
         const int dw = warp - WS_PROD / 32;              // 0..7
         const int rowq = (dw & 3) * 32 + lane;           // TMEM lane = output row (warp % 4 selects the lane quarter)
         const int colh = (dw >> 2) * NC;
-        float acc[NC], cin[NC];
+        float acc[NC], cin[DEFER ? NC : 1];
         int64_t ct = u0 / sk.KT; int ckt = (int)(u0 - ct * sk.KT);
         int64_t ctn = ct / sk.tilesM, ctm = ct - ctn * sk.tilesM;
         int64_t m0 = 0, n0 = 0;
@@ -496,8 +500,8 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
                     const int64_t m = m0 + rowq, n = n0 + colh + c;
-                    cin[c] = (use_c && m < g.M && n < g.N) ? __ldcs(&g.C[m + n * g.ldc]) : 0.f;
-                    acc[c] = 0.f;
+                    const float cv = (use_c && m < g.M && n < g.N) ? __ldcs(&g.C[m + n * g.ldc]) : 0.f;
+                    if (DEFER) { cin[c] = cv; acc[c] = 0.f; } else acc[c] = cv * (g.beta / g.alpha);
                 }
                 fresh = false;
             }
@@ -522,7 +526,8 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
 #pragma unroll
                     for (int c = 0; c < NC; ++c) {
                         const int64_t m = m0 + rowq, n = n0 + colh + c;
-                        if (m < g.M && n < g.N) __stcs(&g.C[m + n * g.ldc], fmaf(g.alpha, acc[c], g.beta * cin[c]));
+                        if (m < g.M && n < g.N)
+                            __stcs(&g.C[m + n * g.ldc], DEFER ? fmaf(g.alpha, acc[c], g.beta * cin[DEFER ? c : 0]) : g.alpha * acc[c]);
                     }
                 }
                 ckt = 0; ++ct; fresh = true;

@@ -18,6 +18,7 @@
 #include "../../include/ctqr.h"
 #include "common.cuh"
 #include "kernels.h"
+#include "solve_small.cuh"
 
 using namespace ctqr;
 
@@ -89,6 +90,7 @@ struct ctqr_handle_s {
     void* dWp[2] = {nullptr, nullptr}; size_t wp_elems[2] = {0, 0};
     void* dW[2] = {nullptr, nullptr};  size_t w_elems[2] = {0, 0};
     void* dPart = nullptr;             // LL slots of the panel kernel
+    void* dLLs = nullptr; unsigned ll_seq = 0;   // LL slots / step numbers of the fused small-S solve kernels
     unsigned bar_count = 0;            // step numbers handed to the panel kernel (never reused)
     int* dFlag = nullptr;
     cudaStream_t sU = nullptr, sP = nullptr, sC = nullptr, sD = nullptr, user = nullptr;
@@ -121,7 +123,7 @@ struct ctqr_handle_s {
         if (ffd >= 0) close(ffd);
         cudaFree(dT); cudaFree(dRd); cudaFree(dRinv); cudaFree(dTau);
         for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); }
-        cudaFree(dPart); cudaFree(dFlag);
+        cudaFree(dPart); cudaFree(dLLs); cudaFree(dFlag);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
         for (auto e : tpool) cudaEventDestroy(e);
@@ -560,6 +562,12 @@ static int alloc_state(H& h, int64_t max_nc) {
     CK(cudaMalloc(&h.dPart, (size_t)2 * 257 * 32 * 16));
     CK(cudaMemsetAsync(h.dPart, 0, (size_t)2 * 257 * 32 * 16, h.sU));
     CK(cudaMalloc(&h.dFlag, sizeof(int)));
+    if (nb == 128) {
+        // fused small-S solve: [2][sms][nb * kSmallS] partial slots + [2][nb * kSmallS] sum slots, 16 bytes each
+        const size_t lls = ((size_t)2 * h.sms + 2) * nb * kSmallS * 16;
+        CK(cudaMalloc(&h.dLLs, lls));
+        CK(cudaMemsetAsync(h.dLLs, 0, lls, h.sU));
+    }
     h.bar_count = 0;
     return 0;
 }
@@ -721,6 +729,27 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         return 0;
     }
     const T* A = P_<T>(h.dA);
+    static const bool no_small = [] { const char* e = getenv("CTQR_NO_SMALL_S"); return e && e[0] == '1'; }();
+    if (S <= kSmallS && h.dLLs && !no_small && h.gemm_impl == 0) {
+        // memory-bound regime: one cooperative kernel for all panels (solve_small.cuh)
+        SmallQtArgs<T> a{};
+        const int G = (int)std::min<int64_t>(h.sms, ceil_div(h.m, 64));
+        a.A = A; a.lda = h.lda; a.m = h.m; a.n = h.n; a.nb = h.nb; a.P = h.P; a.Tm = P_<T>(h.dT);
+        a.B = C; a.ldb = ldc; a.S = (int)S;
+        a.part = reinterpret_cast<uint4*>(h.dLLs);
+        a.sums = a.part + (size_t)2 * h.sms * h.nb * kSmallS;
+        a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
+        a.rpc = (int)round_up(ceil_div(h.m, (int64_t)G), 32);
+        const size_t smem = ((size_t)kSmallS * a.rpc + 2 * (size_t)h.nb * kSmallS) * sizeof(T);
+        if (smem <= 200 * 1024) {
+            static size_t cur = 0;
+            if (smem > cur) { CK(cudaFuncSetAttribute(apply_qt_small_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); cur = smem; }
+            void* args[] = {(void*)&a};
+            CK(cudaLaunchCooperativeKernel((void*)apply_qt_small_kernel<T>, dim3(G), dim3(kSmallThreads), args, smem, h.sU));
+            h.launches += 1;
+            return 0;
+        }
+    }
     for (int k = 0; k < h.P; ++k) {
         const int64_t j0 = (int64_t)k * h.nb;
         const int nbw = (int)std::min<int64_t>(h.nb, h.n - j0);

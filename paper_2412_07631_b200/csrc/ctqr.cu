@@ -563,8 +563,9 @@ static int alloc_state(H& h, int64_t max_nc) {
     CK(cudaMemsetAsync(h.dPart, 0, (size_t)2 * 257 * 32 * 16, h.sU));
     CK(cudaMalloc(&h.dFlag, sizeof(int)));
     if (nb == 128) {
-        // fused small-S solve: [2][sms][nb * kSmallS] partial slots + [2][nb * kSmallS] sum slots, 16 bytes each
-        const size_t lls = ((size_t)2 * h.sms + 2) * nb * kSmallS * 16;
+        // fused small-S solve: [2][sms][nb * kSmallS] partial slots + [2][nb * kSmallS] sum slots (Q^T B),
+        // then [P][nb * kSmallS] slots of the fused TRSM, 16 bytes each
+        const size_t lls = ((size_t)2 * h.sms + 2 + h.P) * nb * kSmallS * 16;
         CK(cudaMalloc(&h.dLLs, lls));
         CK(cudaMemsetAsync(h.dLLs, 0, lls, h.sU));
     }
@@ -733,15 +734,16 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
     if (S <= kSmallS && h.dLLs && !no_small && h.gemm_impl == 0) {
         // memory-bound regime: one cooperative kernel for all panels (solve_small.cuh)
         SmallQtArgs<T> a{};
-        const int G = (int)std::min<int64_t>(h.sms, ceil_div(h.m, 64));
+        const int64_t nch = ceil_div(h.m, (int64_t)kSmallChunk);
+        const int G = (int)std::min<int64_t>(h.sms, nch);
         a.A = A; a.lda = h.lda; a.m = h.m; a.n = h.n; a.nb = h.nb; a.P = h.P; a.Tm = P_<T>(h.dT);
         a.B = C; a.ldb = ldc; a.S = (int)S;
         a.part = reinterpret_cast<uint4*>(h.dLLs);
         a.sums = a.part + (size_t)2 * h.sms * h.nb * kSmallS;
         a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
-        a.rpc = (int)round_up(ceil_div(h.m, (int64_t)G), 32);
-        const size_t smem = ((size_t)kSmallS * a.rpc + 2 * (size_t)h.nb * kSmallS) * sizeof(T);
-        if (smem <= 200 * 1024) {
+        a.rpc = (int)ceil_div(nch, (int64_t)G) * kSmallChunk;
+        const size_t smem = ((size_t)h.nb * kSmallLdT + 2 * (size_t)h.nb * kSmallS + (size_t)kSmallS * (a.rpc + 4)) * sizeof(T);
+        if (smem <= 220 * 1024) {
             static size_t cur = 0;
             if (smem > cur) { CK(cudaFuncSetAttribute(apply_qt_small_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); cur = smem; }
             void* args[] = {(void*)&a};
@@ -777,6 +779,28 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
         CK(trinv_launch<T>(P_<T>(h.dRd), h.nb, h.n, h.P, P_<T>(h.dRinv), h.sU));
         h.rinv_ready = true;
         h.launches += 1;
+    }
+    static const bool no_small = [] { const char* e = getenv("CTQR_NO_SMALL_S"); return e && e[0] == '1'; }();
+    if (S <= kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && !no_small && h.gemm_impl == 0) {
+        // memory-bound regime: one cooperative kernel for all diagonal blocks (solve_small.cuh)
+        SmallTrsmArgs<T> a{};
+        const int64_t nch = ceil_div(h.n, (int64_t)kTrsmChunk);
+        const int G = (int)std::min<int64_t>(h.sms, nch);
+        a.A = P_<T>(h.dA); a.lda = h.lda; a.n = h.n; a.nb = h.nb; a.P = h.P; a.Rinv = P_<T>(h.dRinv);
+        a.X = X; a.ldx = ldx; a.S = (int)S;
+        a.slots = reinterpret_cast<uint4*>(h.dLLs) + ((size_t)2 * h.sms + 2) * h.nb * kSmallS;
+        a.seq = ++h.ll_seq;
+        a.rpc = (int)ceil_div(nch, (int64_t)G) * kTrsmChunk;
+        const size_t smem = ((size_t)h.nb * h.nb + 2 * (size_t)h.nb * kSmallS + (size_t)kSmallS * kTrsmThreads +
+                             (size_t)kSmallS * a.rpc) * sizeof(T);
+        if (smem <= 220 * 1024) {
+            static size_t cur = 0;
+            if (smem > cur) { CK(cudaFuncSetAttribute(trsm_small_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); cur = smem; }
+            void* args[] = {(void*)&a};
+            CK(cudaLaunchCooperativeKernel((void*)trsm_small_kernel<T>, dim3(G), dim3(kTrsmThreads), args, smem, h.sU));
+            h.launches += 1;
+            return 0;
+        }
     }
     for (int i = h.P - 1; i >= 0; --i) {
         const int64_t i0 = (int64_t)i * h.nb;

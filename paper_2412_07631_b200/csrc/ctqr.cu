@@ -742,13 +742,23 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         a.sums = a.part + (size_t)2 * h.sms * h.nb * kSmallS;
         a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
         a.rpc = (int)ceil_div(nch, (int64_t)G) * kSmallChunk;
-        const size_t smem = ((size_t)h.nb * kSmallLdT + 2 * (size_t)h.nb * kSmallS + (size_t)kSmallS * (a.rpc + 4)) * sizeof(T);
+        const size_t smem = ((size_t)h.nb * SmallLd<T>::T_ + 2 * (size_t)h.nb * SmallLd<T>::W + (size_t)kSmallS * (a.rpc + 4)) * sizeof(T);
         if (smem <= 220 * 1024) {
             static size_t cur = 0;
             if (smem > cur) { CK(cudaFuncSetAttribute(apply_qt_small_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); cur = smem; }
             void* args[] = {(void*)&a};
             CK(cudaLaunchCooperativeKernel((void*)apply_qt_small_kernel<T>, dim3(G), dim3(kSmallThreads), args, smem, h.sU));
             h.launches += 1;
+#ifdef CTQR_SMALL_PROFILE
+            {
+                unsigned long long ph[16] = {0}, zero[16] = {0};
+                cudaStreamSynchronize(h.sU);
+                cudaMemcpyFromSymbol(ph, g_small_prof, sizeof(ph));
+                cudaMemcpyToSymbol(g_small_prof, zero, sizeof(zero));
+                for (int i = 1; i <= 8; ++i) fprintf(stderr, "ph%d %.2f  ", i, ph[i] * 1e-3 / h.P);
+                fprintf(stderr, "us/panel\n");
+            }
+#endif
             return 0;
         }
     }

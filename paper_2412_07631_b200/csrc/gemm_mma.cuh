@@ -428,8 +428,14 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
     p.sk.partial = partial ? 1 : 0;
     if (partial) {
         // no CTA shorter than ~1024 rows of K: a small product split over every SM costs more in the
-        // consumer (which sums one partial tile per segment) than it gains in the contraction
-        const int64_t min_units = std::max<int64_t>(8, 1024 / BK);
+        // consumer (which sums one partial tile per segment) than it gains in the contraction.  With
+        // only a few output tiles (the look-ahead column block, the solve's 128 x S products) that
+        // rule leaves most SMs idle, so the floor drops to 512 rows (<= 2 tiles) / 256 rows (<= 8):
+        // measured at configs[2], solve S = 256 Q^T B 26.4 -> 23.4 ms, factor 644 -> 636 ms (fp64).
+        static const int min_rows = [] { const char* e = getenv("CTQR_SK_MIN_ROWS"); return e ? atoi(e) : 1024; }();
+        static const int min_rows_few = [] { const char* e = getenv("CTQR_SK_MIN_ROWS_FEW"); return e ? atoi(e) : 0; }();
+        const int rows = tiles > 8 ? min_rows : min_rows_few ? min_rows_few : tiles > 2 ? 256 : 512;
+        const int64_t min_units = std::max<int64_t>(8, rows / BK);
         int64_t G = std::min<int64_t>(slots, std::max<int64_t>(1, p.sk.U / min_units));
         p.sk.L = ceil_div(p.sk.U, G);
         p.grid = (int)ceil_div(p.sk.U, p.sk.L);

@@ -20,11 +20,28 @@ namespace ctqr {
 constexpr int kSmallS = 8;          // most right-hand sides the fused path handles
 constexpr int kSmallThreads = 512;
 constexpr int kSmallChunk = 16;     // rows are dealt to the CTAs in chunks of this many, round-robin
-constexpr int kSmallLdT = 129;      // padded leading dimension of the staged T_k / R_ii^{-1} (bank-conflict-free rows)
+// padded leading dimensions in shared memory: T_k is read as DMMA fragments in fp64 (ld == 4 mod 16 doubles is
+// conflict-free) and row-per-thread in fp32 (odd ld); W / T^T W as DMMA B fragments in fp64 (ld 12), plain in fp32
+template <typename T> struct SmallLd { static constexpr int T_ = 129, W = kSmallS; };
+template <> struct SmallLd<double> { static constexpr int T_ = 132, W = 12; };
 
 __device__ __forceinline__ void cp_async_elem(double* smem, const double* g) { cp_async8(smem, g, 8); }
 __device__ __forceinline__ void cp_async_elem(float* smem, const float* g) { cp_async4(smem, g, 4); }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
+
+// Per-phase timers of CTA 0 (builds with -DCTQR_SMALL_PROFILE only): nanoseconds summed over the panels.
+#ifdef CTQR_SMALL_PROFILE
+__device__ unsigned long long g_small_prof[16];
+#define CTQR_PH(i)                                                                       \
+    if (tid == 0 && g == 0) {                                                            \
+        unsigned long long t1_;                                                          \
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1_));                          \
+        if (ph_t0) g_small_prof[i] += t1_ - ph_t0;                                       \
+        ph_t0 = t1_;                                                                     \
+    }
+#else
+#define CTQR_PH(i)
+#endif
 
 template <typename T>
 struct SmallQtArgs {
@@ -40,21 +57,25 @@ struct SmallQtArgs {
 template <typename T>
 __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQtArgs<T> p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int NB = 128, SM = kSmallS, NT = kSmallThreads, NW = NT / 32, CH = kSmallChunk, LDT = kSmallLdT;
+    constexpr int NB = 128, SM = kSmallS, NT = kSmallThreads, NW = NT / 32, CH = kSmallChunk, LDT = SmallLd<T>::T_, LDW = SmallLd<T>::W;
     constexpr int NQ = NT / NB, SQ = SM / NQ;
     constexpr bool F64 = sizeof(T) == 8;                   // fp64: the three products run on DMMA.8x8x4
     T* Ts = reinterpret_cast<T*>(smem_raw);                 // [NB][LDT]   T_k (column r at Ts + r * LDT)
     T* Ds = Ts;                                             // partial updates of the column groups; T_k is dead by then
-    T* Wp = Ts + NB * LDT;                                  // [NB][SM]    partial, then summed W
-    T* W2 = Wp + NB * SM;                                   // [NB][SM]    T^T W
-    T* Bs = W2 + NB * SM;                                   // [SM][ldbs]  own rows of B, transposed
+    T* Wp = Ts + NB * LDT;                                  // [NB][LDW]   partial, then summed W
+    T* W2 = Wp + NB * LDW;                                  // [NB][LDW]   T^T W
+    T* Bs = W2 + NB * LDW;                                   // [SM][ldbs]  own rows of B, transposed
     const int ldbs = p.rpc + 4;                             // == 4 (mod 16): conflict-free DMMA fragment loads
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = blockIdx.x, G = gridDim.x, S = p.S;
     auto row_of = [&](int lr) -> int64_t { return ((int64_t)(lr / CH) * G + g) * CH + (lr % CH); };
     auto stage_t = [&](int k) {
         const T* Tk = p.Tm + (size_t)k * NB * NB;
-        for (int e = tid; e < NB * NB; e += NT) cp_async_elem(Ts + (e >> 7) * LDT + (e & (NB - 1)), Tk + e);
+        if constexpr (F64) {                                 // 16-byte copies: ld 132 keeps every column 16-byte aligned
+            for (int e = 2 * tid; e < NB * NB; e += 2 * NT) cp_async16(Ts + (e >> 7) * LDT + (e & (NB - 1)), Tk + e, 16);
+        } else {
+            for (int e = tid; e < NB * NB; e += NT) cp_async_elem(Ts + (e >> 7) * LDT + (e & (NB - 1)), Tk + e);
+        }
         cp_async_commit();
     };
     // local rows [la, nl) take part in panel k: la = first local row at or below row j0 (j0 is a multiple of CH)
@@ -79,6 +100,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
         const T* V = p.A + j0 * p.lda;                       // column c of the panel at V + c * lda, rows absolute
         const int la = first_local(j0);
         const int na = nl - la;
+        unsigned long long ph_t0 = 0; (void)ph_t0;
+        CTQR_PH(0)
         // ---- partial W[c][s] = sum over own rows of V[r, c] * B[r, s] ----
         if constexpr (F64) {
             // warp w: columns 8w .. 8w+7 (M), right-hand sides (N), 4 consecutive local rows per k-step
@@ -86,18 +109,18 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
             const T* vc = V + (int64_t)c * p.lda;
             const T* bs = Bs + (lane >> 2) * ldbs + (lane & 3);
             const bool okc = c < kw;
-            double c0[2] = {0.0, 0.0}, c1[2] = {0.0, 0.0};
-#pragma unroll 4
-            for (int t = 0; t < na / 4; t += 2) {            // na is a multiple of 16: an even number of steps
+            double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};   // four independent DMMA chains
+#pragma unroll 8
+            for (int t = 0; t < na / 4; t += 4) {            // na is a multiple of 16: a multiple of 4 steps
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < 4; ++h) {
                     const int64_t row = row_of(la + 4 * (t + h) + (lane & 3));
                     const double a = (okc && row < p.m) ? __ldg(vc + row) : 0.0;
                     dmma884(c0[h], c1[h], a, bs[la + 4 * (t + h)]);
                 }
             }
-            Wp[c * SM + 2 * (lane & 3)] = c0[0] + c0[1];
-            Wp[c * SM + 2 * (lane & 3) + 1] = c1[0] + c1[1];
+            Wp[c * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
+            Wp[c * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
         } else {
             // a warp takes 4 columns per pass, lanes over rows: 4 independent loads per lane and row step
             for (int cb = warp; cb < NB; cb += 4 * NW) {
@@ -121,13 +144,15 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
                     }
                 }
                 warp_transpose_reduce<T, 4 * SM>(acc, lane);  // lane l: total of acc[l] = (column cb + (l / SM) * NW, rhs l % SM)
-                Wp[(cb + (lane / SM) * NW) * SM + (lane % SM)] = acc[0];
+                Wp[(cb + (lane / SM) * NW) * LDW + (lane % SM)] = acc[0];
             }
         }
         __syncthreads();
+        CTQR_PH(1)
         // ---- publish the CTA's partial (LL slots) ----
         uint4* mine = p.part + ((size_t)par * G + g) * (NB * SM);
-        for (int e = tid; e < NB * SM; e += NT) ll_store(mine + e, Wp[e], seq);
+        for (int e = tid; e < NB * SM; e += NT) ll_store(mine + e, Wp[(e / SM) * LDW + (e % SM)], seq);
+        CTQR_PH(2)
         // ---- pull this CTA's slice of the next panel towards L2 while the exchange is in flight ----
         if (k + 1 < p.P) {
             const int la1 = first_local(j0 + NB);
@@ -138,6 +163,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
                 if (F64 && row + 8 < p.m) prefetch_l2(vc + row + 8);
             }
         }
+        CTQR_PH(3)
         // ---- element owners reduce over the CTAs in a fixed order: element e belongs to CTA e % G ----
         {
             const uint4* all = p.part + (size_t)par * G * (NB * SM);
@@ -165,6 +191,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
                 if (lane == 0) ll_store(p.sums + (size_t)par * (NB * SM) + e, t, seq);
             }
         }
+        CTQR_PH(4)
         // ---- everyone gathers the sums (both slots of a thread in flight) ----
         {
             const uint4* sl = p.sums + (size_t)par * (NB * SM);
@@ -175,29 +202,31 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
             for (int u = 0; u < NB * SM / NT; ++u) {
                 const int e = tid + u * NT;
                 while (r[u].y != seq || r[u].w != seq) r[u] = ll_load(sl + e);
-                Wp[e] = ll_value<T>(r[u]);
+                Wp[(e / SM) * LDW + (e % SM)] = ll_value<T>(r[u]);
             }
         }
+        CTQR_PH(5)
         cp_async_wait<0>();
         __syncthreads();
+        CTQR_PH(6)
         // ---- W2 = T_k^T W  (T upper triangular: W2[r][s] = sum_{q <= r} T[q][r] W[q][s]) ----
         if constexpr (F64) {
             // warp w: rows 8w .. 8w+7 of W2 (M), right-hand sides (N), q in steps of 4 up to the diagonal
             const int r = warp * 8 + (lane >> 2);
             const T* tr = Ts + r * LDT + (lane & 3);
-            const T* wq = Wp + (lane & 3) * SM + (lane >> 2);
-            double c0[2] = {0.0, 0.0}, c1[2] = {0.0, 0.0};
+            const T* wq = Wp + (lane & 3) * LDW + (lane >> 2);
+            double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll 2
-            for (int t = 0; t < 2 * warp + 2; t += 2) {
+            for (int t = 0; t < 2 * warp + 2; t += 4) {      // the last group may run past the diagonal: masked by q <= r
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < 4; ++h) {
                     const int q = 4 * (t + h) + (lane & 3);
                     const double a = (q <= r && r < kw) ? tr[4 * (t + h)] : 0.0;
-                    dmma884(c0[h], c1[h], a, wq[4 * (t + h) * SM]);
+                    dmma884(c0[h], c1[h], a, wq[4 * (t + h) * LDW]);
                 }
             }
-            W2[r * SM + 2 * (lane & 3)] = c0[0] + c0[1];
-            W2[r * SM + 2 * (lane & 3) + 1] = c1[0] + c1[1];
+            W2[r * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
+            W2[r * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
         } else {
             const int r = tid & (NB - 1), sh = (tid >> 7) * SQ;
             T acc[SQ];
@@ -208,18 +237,19 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
                 for (int q = 0; q <= r; ++q) {
                     const T t = Ts[r * LDT + q];
 #pragma unroll
-                    for (int s = 0; s < SQ; ++s) acc[s] = fma(t, Wp[q * SM + sh + s], acc[s]);
+                    for (int s = 0; s < SQ; ++s) acc[s] = fma(t, Wp[q * LDW + sh + s], acc[s]);
                 }
 #pragma unroll
-            for (int s = 0; s < SQ; ++s) W2[r * SM + sh + s] = acc[s];
+            for (int s = 0; s < SQ; ++s) W2[r * LDW + sh + s] = acc[s];
         }
         __syncthreads();
+        CTQR_PH(7)
         // ---- own rows: B[r, :] -= V[r, 0:kw] * W2, the columns split over CS groups ----
         if constexpr (F64) {
             // unit = (8 local rows, one of CS column ranges); a warp walks its units, 4 columns per k-step
             const int mt = na / 8;
             int CS = 1;
-            while (CS < 8 && mt * CS < 4 * NW && 2 * CS * na * SM <= NB * LDT) CS *= 2;
+            while (CS < 8 && mt * CS < NW && 2 * CS * na * SM <= NB * LDT) CS *= 2;   // at least one unit per warp
             const int steps = NB / 4 / CS;
             for (int u = warp; u < mt * CS; u += NW) {
                 const int cs = u / mt, l0 = (u - cs * mt) * 8;
@@ -227,23 +257,25 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
                 const bool okr = row < p.m;
                 const int cbeg = cs * steps * 4 + (lane & 3);
                 const T* vr = V + (int64_t)cbeg * p.lda + row;
-                const T* wb = W2 + cbeg * SM + (lane >> 2);
-                double c0[2] = {0.0, 0.0}, c1[2] = {0.0, 0.0};
-#pragma unroll 4
-                for (int t = 0; t < steps; t += 2) {           // steps = 32 / CS >= 4
+                const T* wb = W2 + cbeg * LDW + (lane >> 2);
+                double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll 8
+                for (int t = 0; t < steps; t += 4) {           // steps = 32 / CS: a multiple of 4
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
+                    for (int h = 0; h < 4; ++h) {
                         const double a = (okr && cbeg + 4 * (t + h) < kw) ? __ldg(vr + (int64_t)(4 * (t + h)) * p.lda) : 0.0;
-                        dmma884(c0[h], c1[h], a, wb[4 * (t + h) * SM]);
+                        dmma884(c0[h], c1[h], a, wb[4 * (t + h) * LDW]);
                     }
                 }
+                c0[0] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
+                c1[0] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
                 const int l = l0 + (lane >> 2), s0 = 2 * (lane & 3);
                 if (CS == 1) {
-                    Bs[s0 * ldbs + la + l] -= c0[0] + c0[1];
-                    Bs[(s0 + 1) * ldbs + la + l] -= c1[0] + c1[1];
+                    Bs[s0 * ldbs + la + l] -= c0[0];
+                    Bs[(s0 + 1) * ldbs + la + l] -= c1[0];
                 } else {
-                    Ds[(cs * SM + s0) * na + l] = c0[0] + c0[1];
-                    Ds[(cs * SM + s0 + 1) * na + l] = c1[0] + c1[1];
+                    Ds[(cs * SM + s0) * na + l] = c0[0];
+                    Ds[(cs * SM + s0 + 1) * na + l] = c1[0];
                 }
             }
             __syncthreads();
@@ -273,7 +305,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
                     for (int c = c0; c < c1; ++c) {
                         const T v = __ldg(vr + (int64_t)c * p.lda);
 #pragma unroll
-                        for (int s = 0; s < SM; ++s) d[s] = fma(v, W2[c * SM + s], d[s]);
+                        for (int s = 0; s < SM; ++s) d[s] = fma(v, W2[c * LDW + s], d[s]);
                     }
                 }
                 if (CS == 1) {
@@ -295,6 +327,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
                 __syncthreads();
             }
         }
+        CTQR_PH(8)
         if (k + 1 < p.P) stage_t(k + 1);                     // lands during the next panel's partial products and exchange
     }
     cp_async_wait<0>();

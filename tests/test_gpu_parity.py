@@ -81,6 +81,35 @@ def test_random_small(shape, dt):
 
 
 @pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("shape", [(2500, 1300), (4099, 1025), (1300, 1300)])
+def test_small_batch_fused_solve(shape, dt):
+    """S <= 8 takes the two fused cooperative kernels (one launch for Q^T B, one for the TRSM):
+    every CTA owns several row chunks, the last chunk is ragged, n is not a multiple of nb.  S = 9 takes
+    the per-panel path; both must meet the oracle."""
+    import torch
+    m, n = shape
+    rng = np.random.default_rng(31 * m + n)
+    A = np.asfortranarray(rng.standard_normal((m, n)).astype(dt))
+    B = np.asfortranarray(rng.standard_normal((m, 9)).astype(dt))
+    VR, tau = oracle.qr(A)
+    X_or = oracle.solve(VR, tau, B)
+    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m, n)
+    for S in (1, 3, 8, 9):
+        Bt = ctqr.colmajor_from_numpy(np.asfortranarray(B[:, :S]))
+        Xt = torch.zeros((S, n), dtype=Bt.dtype, device="cuda")
+        ctqr.ct_qr_solve(f, Bt, S, Xt)                      # first call of a handle also inverts the diagonal blocks
+        ctqr.ct_qr_solve(f, Bt, S, Xt)
+        X = ctqr.numpy_from_colmajor(Xt)
+        assert relerr(X, X_or[:, :S]) <= SOLUTION[dt], (S, relerr(X, X_or[:, :S]))
+        launches = f.stats()["kernel_launches"]
+        if S <= 8:
+            assert launches == 2, launches
+        else:
+            assert launches > 2 * f.stats()["n_panels"]
+    f.destroy()
+
+
+@pytest.mark.parametrize("dt", DT)
 @pytest.mark.parametrize("nb,ib", [(8, 8), (32, 16), (64, 16), (128, 16), (128, 32), (64, 8)])
 @pytest.mark.parametrize("la", [0, 1])
 def test_blocking_invariance(nb, ib, la, dt):

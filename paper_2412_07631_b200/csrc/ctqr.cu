@@ -174,7 +174,11 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     CK(gemm_run<T>(true, g1, L1, h.gemm_impl, st));
     if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 0}); }
     const T* W2 = W;
-    if (L1.kind == 1 && kw == 128 && nc >= 128 && ldt % (16 / (int)sizeof(T)) == 0 && (uintptr_t)Tm % 16 == 0) {
+    if (L1.kind == 1 && kw == 128 && nc <= 512 && L1.seg.BN % 8 == 0 && ldt % (16 / (int)sizeof(T)) == 0 &&
+        (uintptr_t)Tm % 16 == 0) {
+        // narrow right-hand side (the solve, the look-ahead block): partial sum and T^T W in one small kernel
+        CK(mm128_launch<T>(true, Tm, ldt, Wp, 0, L1.seg, nc, W, ldw, st));
+    } else if (L1.kind == 1 && kw == 128 && nc >= 128 && ldt % (16 / (int)sizeof(T)) == 0 && (uintptr_t)Tm % 16 == 0) {
         // full-width panel: W <- sum of the partial tiles, then T^T W as one more tensor-core
         // contraction (T is stored with explicit zeros below the diagonal), written over the partials
         CK(partial_sum_launch<T>(Wp, L1.seg, kw, nc, W, ldw, st));
@@ -824,7 +828,11 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
             } else { Rcol = P_<T>(h.dA) + i0 * h.lda; ldr = h.lda; }
         }
         const T* Xi = X + i0; int64_t ldxi = ldx;         // where the update below reads X_i
-        if (use_inv) {
+        if (use_inv && nbw == 128 && h.nb == 128 && S <= 512) {
+            // X_i = R_ii^{-1} C_i in place, one CTA per 8 right-hand sides (small.cuh mm128_kernel)
+            CK(mm128_launch<T>(false, P_<T>(h.dRinv) + (size_t)i * h.nb * h.nb, h.nb, X + i0, ldx, SegInfo{}, S, X + i0, ldx, h.sU));
+            h.launches += 1;
+        } else if (use_inv) {
             // X_i = R_ii^{-1} C_i as a contraction (out of place into W, copied back over C_i)
             T* W = P_<T>(h.dW[0]);
             GemmArgs<T> gi{};

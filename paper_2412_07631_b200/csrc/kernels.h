@@ -72,6 +72,9 @@ template <typename T> cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t w
 template <typename T> cudaError_t partial_sum_launch(const T* Wp, SegInfo seg, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st);
 template <typename T> cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx, cudaStream_t st);
 // inverses of the P diagonal blocks of R (nb x nb each, ld = nb; a narrower last block is padded with zeros)
+// out = op(M) * in, M 128 x 128 upper triangular (zeros stored), N <= a few hundred columns; `in` is either a matrix
+// (seg.L == 0; may alias out) or the stream-K partial tiles of a 128 x N product (seg.L != 0)
+template <typename T> cudaError_t mm128_launch(bool trans, const T* M, int ldm, const T* in, int64_t ldin, SegInfo seg, int64_t N, T* out, int64_t ldo, cudaStream_t st);
 template <typename T> cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, cudaStream_t st);
 template <typename T> cudaError_t copy2d_launch(const T* src, int64_t lds, T* dst, int64_t ldd, int64_t rows, int64_t cols, cudaStream_t st);
 template <typename T> cudaError_t gather_R_launch(const T* A, int64_t lda, const T* Rd, int nb, int64_t n, T* R, int64_t ldr, cudaStream_t st);

@@ -49,6 +49,29 @@ cudaError_t partial_sum_launch(const T* Wp, SegInfo seg, int kw, int64_t N, T* W
 }
 
 template <typename T>
+cudaError_t mm128_launch(bool trans, const T* M, int ldm, const T* in, int64_t ldin, SegInfo seg, int64_t N, T* out,
+                         int64_t ldo, cudaStream_t st) {
+    const size_t smem = ((size_t)128 * Mm128Ld<T>::M + (size_t)128 * Mm128Ld<T>::X +
+                         (size_t)(kMm128Threads / 128) * 128 * (kMm128Cols + 1)) * sizeof(T);
+    const unsigned grid = (unsigned)ceil_div(N, (int64_t)kMm128Cols);
+    const bool partial = seg.L != 0;
+    if (partial && (seg.BN % kMm128Cols != 0 || !trans)) return cudaErrorInvalidValue;
+    static size_t cur[2] = {0, 0};
+    if (partial) {
+        cudaError_t e = ensure_smem(mm128_kernel<T, true, true>, smem, cur[0]);
+        if (e != cudaSuccess) return e;
+        mm128_kernel<T, true, true><<<grid, kMm128Threads, smem, st>>>(M, ldm, in, ldin, seg, N, out, ldo);
+    } else if (trans) {
+        return cudaErrorInvalidValue;
+    } else {
+        cudaError_t e = ensure_smem(mm128_kernel<T, false, false>, smem, cur[1]);
+        if (e != cudaSuccess) return e;
+        mm128_kernel<T, false, false><<<grid, kMm128Threads, smem, st>>>(M, ldm, in, ldin, seg, N, out, ldo);
+    }
+    return cudaGetLastError();
+}
+
+template <typename T>
 cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx,
                              cudaStream_t st) {
     static size_t cur = 0;
@@ -96,6 +119,7 @@ cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, c
     template cudaError_t larft_launch<T>(const T*, SegInfo, int64_t, int, int, int, T*, int, cudaStream_t);           \
     template cudaError_t ttw_launch<T>(const T*, SegInfo, int64_t, int64_t, const T*, int, int, int64_t, T*, int64_t,  \
                                        cudaStream_t);                                                                  \
+    template cudaError_t mm128_launch<T>(bool, const T*, int, const T*, int64_t, SegInfo, int64_t, T*, int64_t, cudaStream_t); \
     template cudaError_t trsm_diag_launch<T>(const T*, int, int, const T*, int64_t, int64_t, T*, int64_t, cudaStream_t); \
     template cudaError_t copy2d_launch<T>(const T*, int64_t, T*, int64_t, int64_t, int64_t, cudaStream_t);             \
     template cudaError_t gather_R_launch<T>(const T*, int64_t, const T*, int, int64_t, T*, int64_t, cudaStream_t);     \

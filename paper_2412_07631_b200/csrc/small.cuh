@@ -192,6 +192,104 @@ partial_sum_kernel(const T* __restrict__ Wp, SegInfo seg, int kw, int64_t N, T* 
     Wout[k + c * ldo] = s;
 }
 
+// ---- out = op(M) * in for a 128 x 128 triangular M and a narrow right-hand side ----------------
+// The small products of the solve (and of the look-ahead block): W <- T_k^T (sum of the stream-K
+// partial tiles) [TRANS, PARTIAL] and X_i <- R_ii^{-1} C_i [in place, !TRANS].  A tensor-core
+// contraction launch costs ~16 us for these 128 x S x 128 products (4 CTAs busy) plus ~12 us for
+// the partial sum; here one CTA takes 8 columns: M is staged once in shared memory (cp.async in
+// fp64), the 128 x 8 slab of the input is summed / loaded by all 512 threads (segments dealt to 4
+// thread groups, combined in a fixed order: deterministic), fp64 runs on DMMA.8x8x4 with the
+// triangular k-range, fp32 on FFMA.  M upper triangular with explicit zeros below the diagonal.
+constexpr int kMm128Threads = 512;
+constexpr int kMm128Cols = 8;
+template <typename T> struct Mm128Ld { static constexpr int M = 129, X = kMm128Cols; };
+template <> struct Mm128Ld<double> { static constexpr int M = 132, X = 12; };
+
+template <typename T, bool TRANS, bool PARTIAL>
+__global__ void __launch_bounds__(kMm128Threads, 1)
+mm128_kernel(const T* __restrict__ Mg, int ldm, const T* In, int64_t ldin, SegInfo seg, int64_t N, T* Out, int64_t ldo) {
+    constexpr int NB = 128, NC = kMm128Cols, NT = kMm128Threads, NG = NT / NB, LDM = Mm128Ld<T>::M, LDX = Mm128Ld<T>::X;
+    constexpr bool F64 = sizeof(T) == 8;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* Ms = reinterpret_cast<T*>(smem_raw);          // [NB][LDM]: Ms[c * LDM + r] = M[r][c]
+    T* Xs = Ms + NB * LDM;                           // [NB][LDX]: the input slab
+    T* Ps = Xs + NB * LDX;                           // [NG][NB][NC + 1]: per-group partial sums
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t c0 = (int64_t)blockIdx.x * NC;
+    if constexpr (F64) {
+        for (int e = 2 * tid; e < NB * NB; e += 2 * NT) cp_async16(Ms + (e >> 7) * LDM + (e & (NB - 1)), Mg + (e & (NB - 1)) + (size_t)(e >> 7) * ldm, 16);
+        cp_async_commit();
+    } else {
+        for (int e = tid; e < NB * NB; e += NT) Ms[(e >> 7) * LDM + (e & (NB - 1))] = Mg[(e & (NB - 1)) + (size_t)(e >> 7) * ldm];
+    }
+    {
+        const int k = tid & (NB - 1), grp = tid >> 7;
+        if constexpr (PARTIAL) {
+            // segments sp = grp (mod NG) of the tile the columns belong to (NC divides the tile width)
+            const int64_t t = c0 / seg.BN, slot = (int64_t)NB * seg.BN;
+            const int nseg = sk_nseg(t, seg.KT, seg.L);
+            const T* base = In + (t + sk_first_cta(t, seg.KT, seg.L)) * slot + k + (c0 % seg.BN) * NB;
+            T acc[NC];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) acc[c] = T(0);
+#pragma unroll 2
+            for (int sp = grp; sp < nseg; sp += NG) {
+                const T* b = base + (int64_t)sp * slot;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[c] += (c0 + c < N) ? b[c * NB] : T(0);
+            }
+#pragma unroll
+            for (int c = 0; c < NC; ++c) Ps[(grp * NB + k) * (NC + 1) + c] = acc[c];
+            __syncthreads();
+            for (int e = tid; e < NB * NC; e += NT) {
+                const int kk = e / NC, c = e - kk * NC;
+                T v = T(0);
+#pragma unroll
+                for (int q = 0; q < NG; ++q) v += Ps[(q * NB + kk) * (NC + 1) + c];
+                Xs[kk * LDX + c] = v;
+            }
+        } else {
+            for (int c = grp; c < NC; c += NG) Xs[k * LDX + c] = (c0 + c < N) ? In[k + (c0 + c) * ldin] : T(0);
+        }
+    }
+    if constexpr (F64) cp_async_wait<0>();
+    __syncthreads();
+    if constexpr (F64) {
+        // warp w: rows 8w .. 8w+7 (16 warps x 8 rows), k in steps of 4 over the non-zero range of op(M)
+        const int r = warp * 8 + (lane >> 2);
+        const int tb = TRANS ? 0 : 2 * warp, te = TRANS ? 2 * warp + 2 : NB / 4;
+        double d0[2] = {0.0, 0.0}, d1[2] = {0.0, 0.0};
+        const T* xq = Xs + (lane & 3) * LDX + (lane >> 2);
+#pragma unroll 4
+        for (int t = tb; t < te; t += 2) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int k = 4 * (t + h) + (lane & 3);
+                const double a = TRANS ? Ms[r * LDM + k] : Ms[k * LDM + r];
+                dmma884(d0[h], d1[h], a, xq[4 * (t + h) * LDX]);
+            }
+        }
+        const int64_t c = c0 + 2 * (lane & 3);
+        if (c < N) Out[r + c * ldo] = d0[0] + d0[1];
+        if (c + 1 < N) Out[r + (c + 1) * ldo] = d1[0] + d1[1];
+    } else {
+        const int r = tid & (NB - 1), ch = (tid >> 7) * (NC / NG);
+        T acc[NC / NG];
+#pragma unroll
+        for (int c = 0; c < NC / NG; ++c) acc[c] = T(0);
+        const int kb = TRANS ? 0 : r, ke = TRANS ? r + 1 : NB;
+#pragma unroll 4
+        for (int k = kb; k < ke; ++k) {
+            const T a = TRANS ? Ms[r * LDM + k] : Ms[k * LDM + r];
+#pragma unroll
+            for (int c = 0; c < NC / NG; ++c) acc[c] = fma(a, Xs[k * LDX + ch + c], acc[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < NC / NG; ++c)
+            if (c0 + ch + c < N) Out[r + (c0 + ch + c) * ldo] = acc[c];
+    }
+}
+
 // ---- diagonal-block triangular solve -------------------------------------------------------
 // R: kw x kw upper triangular (ld = ldr, explicit storage); C: kw x S in (ld = ldc); X out (ld = ldx).
 // Thread layout: 16 threads per right-hand side (a half-warp), each owning rows r = sub + 16 q in

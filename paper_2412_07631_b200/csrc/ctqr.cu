@@ -101,6 +101,7 @@ struct ctqr_handle_s {
     // opt->profile: per-launch event spans of the trailing-update contractions
     struct Span { cudaEvent_t a, b; double flops; int kind; };
     int profile = 0;
+    void* dTickets = nullptr; int ticket_pos = 0;   // zeroed counter pairs for the SM-confined fp64 launches (kTicketRing of them)
     int reserve_sms = -1;  // SMs left to the look-ahead panel chain during the bulk update (fp32 tcgen05 path): -1 auto, 0 off
     std::vector<Span> spans;
     std::vector<cudaEvent_t> tpool; size_t tpool_used = 0;
@@ -123,7 +124,7 @@ struct ctqr_handle_s {
         if (ffd >= 0) close(ffd);
         cudaFree(dT); cudaFree(dRd); cudaFree(dRinv); cudaFree(dTau);
         for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); }
-        cudaFree(dPart); cudaFree(dLLs); cudaFree(dFlag);
+        cudaFree(dPart); cudaFree(dLLs); cudaFree(dFlag); cudaFree(dTickets);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
         for (auto e : tpool) cudaEventDestroy(e);
@@ -148,6 +149,29 @@ static bool is_device_ptr(const void* p) {
 // larfb: C <- (I - V T^T V^T) C   (with C = B it is row a6)
 //   V: mk x kw explicit unit-lower-trapezoid (ld ldv), T: kw x kw upper (ld ldt), C: mk x nc.
 // ------------------------------------------------------------------------------------------
+// SM confinement of a stream-K launch (fp64: two CTAs per SM, so a smaller grid alone leaves no SM empty; see
+// GemmLaunch::reserve).  Hands the launch a fresh pair of zeroed counters; the ring is re-zeroed on the
+// launching stream when it wraps (all users are on that stream).
+constexpr int kTicketRing = 4096;
+template <typename T>
+static int confine(H& h, GemmLaunch& L, int reserve_sms, cudaStream_t st) {
+    if (sizeof(T) != 8 || reserve_sms <= 0 || L.kind != 1 || !h.dTickets) return 0;
+    if (h.ticket_pos == kTicketRing) {
+        CK(cudaMemsetAsync(h.dTickets, 0, (size_t)kTicketRing * 2 * sizeof(unsigned), st));
+        h.ticket_pos = 0;
+    }
+    L.reserve = reserve_sms;
+    L.tickets = reinterpret_cast<unsigned*>(h.dTickets) + 2 * (size_t)h.ticket_pos++;
+    return 0;
+}
+template <typename T>
+static int gemm_direct_confined(H& h, bool ta, const GemmArgs<T>& g, int sms, int reserve_sms, cudaStream_t st) {
+    GemmLaunch L = gemm_plan<T>(ta, g.M, g.N, g.K, h.gemm_impl, sms, false, 0, 0, gemm_aligned(g));
+    CKI(confine<T>(h, L, reserve_sms, st));
+    CK(gemm_run<T>(ta, g, L, h.gemm_impl, st));
+    return 0;
+}
+
 template <typename T>
 static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t mk, int kw, const T* Tm, int ldt,
                  T* C, int64_t ldc, int64_t nc, bool prof = false, int reserve_sms = 0) {
@@ -165,8 +189,9 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     GemmArgs<T> g1{};
     g1.M = kw; g1.N = nc; g1.K = mk; g1.A = V; g1.lda = ldv; g1.B = C; g1.ldb = ldc;
     g1.C = Wp; g1.ldc = ldw; g1.alpha = T(1); g1.beta = T(0); g1.split_stride = sstride;
-    const GemmLaunch L1 = gemm_plan<T>(true, kw, nc, mk, h.gemm_impl, sms, true,
-                                       (int64_t)h.wp_elems[ws], sstride, gemm_aligned(g1));
+    GemmLaunch L1 = gemm_plan<T>(true, kw, nc, mk, h.gemm_impl, sms, true,
+                                 (int64_t)h.wp_elems[ws], sstride, gemm_aligned(g1));
+    CKI(confine<T>(h, L1, reserve_sms, st));
     prof = prof && h.profile;
     const double fl = 2.0 * (double)mk * (double)kw * (double)nc;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -185,7 +210,7 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
         GemmArgs<T> gt{};
         gt.M = kw; gt.N = nc; gt.K = kw; gt.A = Tm; gt.lda = ldt; gt.B = W; gt.ldb = ldw;
         gt.C = Wp; gt.ldc = ldw; gt.alpha = T(1); gt.beta = T(0);
-        CK(gemm_direct<T>(true, gt, h.gemm_impl, sms, st));
+        CKI(gemm_direct_confined<T>(h, true, gt, sms, reserve_sms, st));
         W2 = Wp;
         h.launches += 1;
     } else {
@@ -195,7 +220,7 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     g2.M = mk; g2.N = nc; g2.K = kw; g2.A = V; g2.lda = ldv; g2.B = W2; g2.ldb = ldw;
     g2.C = C; g2.ldc = ldc; g2.alpha = T(-1); g2.beta = T(1);
     if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
-    CK(gemm_direct<T>(false, g2, h.gemm_impl, sms, st));
+    CKI(gemm_direct_confined<T>(h, false, g2, sms, reserve_sms, st));
     if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, fl, 1}); }
     h.launches += 3;
     return 0;
@@ -341,6 +366,7 @@ static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
         }
         return 0;
     }
+    static const bool reserve64 = [] { const char* e = getenv("CTQR_RESERVE_F64"); return !e || e[0] != '0'; }();
     CKI(panel_factor<T>(h, h.sP, A, lda, m, c0, (int)std::min<int64_t>(nb, c1 - c0), k0));
     CK(cudaEventRecord(evP, h.sP));
     for (int k = k0; k < k1; ++k) {
@@ -361,19 +387,19 @@ static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
         // leaves whole SMs empty: the first part of the bulk runs on (SMs - R) while the look-ahead
         // panel chain (R co-resident CTAs of the cooperative panel kernel + its small kernels, on the
         // high-priority stream) uses the rest; the remainder of the bulk then takes every SM.
-        // (The fp64 kernels run two CTAs per SM and cannot be confined this way; measured: a
-        // one-CTA fp64 variant loses more than the overlap gains.)
+        // The fp64 kernels run two CTAs per SM, so there the CTAs that land on the R reserved SMs retire
+        // at once and the rest draw their worker index from a counter (GemmLaunch::reserve).
         const int64_t ncb = c1 - jn - nbn;
         int R = 0; int64_t nA = ncb;
-        if (sizeof(T) == 4 && h.gemm_impl == 0 && h.reserve_sms != 0 && ncb > 0) {
+        if (h.gemm_impl == 0 && h.reserve_sms != 0 && ncb > 0 && (sizeof(T) == 4 || reserve64)) {
             const int64_t mk1 = m - jn;
             const int ibn = panel_ib_for<T>(h, mk1);
             const int Gp = ibn ? (int)ceil_div(mk1, (int64_t)kPanelThreads * panel_rpts<T>(ibn)[0]) : h.sms;
             R = h.reserve_sms > 0 ? h.reserve_sms : Gp + 2;
             if (R > h.sms / 3) R = 0;                       // tall panels: the chain is negligible against the update
             if (R > 0) {
-                const double t_panel = 0.25e-3 + 1.5e-8 * (double)mk1;                   // s, calibrated at c3
-                const double rate = 69e12 * (double)(h.sms - R) / (double)h.sms;          // flop/s of the pair of products
+                const double t_panel = 0.25e-3 + 1.5e-8 * (double)mk1;                   // s, calibrated at c3 (flat optimum, both precisions)
+                const double rate = (sizeof(T) == 4 ? 69e12 : 25e12) * (double)(h.sms - R) / (double)h.sms;   // flop/s of the pair of products
                 nA = (int64_t)(t_panel * rate / (4.0 * (double)(m - j0) * nbw));
                 nA = std::min<int64_t>(ncb, round_up(std::max<int64_t>(nA, 128), 128));
                 if (ncb - nA < 256) nA = ncb;
@@ -566,6 +592,9 @@ static int alloc_state(H& h, int64_t max_nc) {
     CK(cudaMalloc(&h.dPart, (size_t)2 * 257 * 32 * 16));
     CK(cudaMemsetAsync(h.dPart, 0, (size_t)2 * 257 * 32 * 16, h.sU));
     CK(cudaMalloc(&h.dFlag, sizeof(int)));
+    CK(cudaMalloc(&h.dTickets, (size_t)kTicketRing * 2 * sizeof(unsigned)));
+    CK(cudaMemsetAsync(h.dTickets, 0, (size_t)kTicketRing * 2 * sizeof(unsigned), h.sU));
+    h.ticket_pos = 0;
     if (nb == 128) {
         // fused small-S solve: [2][sms][nb * kSmallS] partial slots + [2][nb * kSmallS] sum slots (Q^T B),
         // then [P][nb * kSmallS] slots of the fused TRSM, 16 bytes each

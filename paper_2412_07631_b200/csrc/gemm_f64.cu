@@ -59,6 +59,7 @@ static MmaPlan to_plan(const GemmLaunch& L) {
     MmaPlan p{};
     p.sk.tilesM = L.tilesM; p.sk.tilesN = L.tilesN; p.sk.KT = L.KT; p.sk.U = L.U; p.sk.L = L.L; p.sk.partial = L.partial;
     p.grid = L.grid; p.maxseg = L.slots; p.sk.G = L.G; p.sk.Gm = L.Gm;
+    p.sk.tickets = L.tickets; p.sk.reserve = L.reserve;
     return p;
 }
 

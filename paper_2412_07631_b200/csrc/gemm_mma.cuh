@@ -151,6 +151,9 @@ struct StreamK {
     // cycling through all of V (which no longer fits the L2 at m = 1e5)
     int G, Gm;
     int l2_prefetch;          // direct mode: prefetch the next tile's C into L2 (set by the launcher)
+    // SM confinement (see GemmLaunch::reserve): worker indices are drawn from tickets[1] by the CTAs that do
+    // not retire on a reserved SM; `workers` = the planned grid
+    unsigned* tickets; int reserve; int workers;
 };
 // first CTA that touches tile t, and how many CTAs (= partial slots) it has
 __host__ __device__ inline int64_t sk_first_cta(int64_t t, int KT, int64_t L) { return (t * KT) / L; }
@@ -178,7 +181,7 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 
 // Requires 16-byte aligned operands (a_vec_ok && b_vec_ok); the host falls back to the classic
 // kernels of gemm.cuh otherwise.
-template <typename T, bool TA, int BM, int BN, int WM, int WN, int STAGES, int MINB>
+template <typename T, bool TA, int BM, int BN, int WM, int WN, int STAGES, int MINB, bool CONFINED = false>
 __global__ void __launch_bounds__(MmaCfg<T, TA, BM, BN, WM, WN, STAGES>::NT, MINB)
 gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
     using Cfg = MmaCfg<T, TA, BM, BN, WM, WN, STAGES>;
@@ -196,16 +199,37 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp % Cfg::WARPS_M, wn = warp / Cfg::WARPS_M;
     const int grp = lane >> 2, tig = lane & 3;
-    const int64_t u0 = (int64_t)blockIdx.x * sk.L;
+    // worker index: blockIdx.x, or (CONFINED instantiation) a ticket when the launch is kept off some SMs
+    // (StreamK::tickets); held in shared memory there: the kernel sits at its register cap
+    __shared__ int s_worker_confined;
+    if constexpr (CONFINED) {
+        if (tid == 0) {
+            unsigned smid, nsm;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            asm volatile("mov.u32 %0, %%nsmid;" : "=r"(nsm));
+            const bool retire = smid + (unsigned)sk.reserve >= nsm &&
+                                atomicAdd(sk.tickets, 1u) < (unsigned)((int)gridDim.x - sk.workers);
+            int id = -1;
+            if (!retire) {
+                id = (int)atomicAdd(sk.tickets + 1, 1u);
+                if (id >= sk.workers) id = -1;
+            }
+            s_worker_confined = id;
+        }
+        __syncthreads();
+        if (s_worker_confined < 0) return;
+    }
+#define s_worker (CONFINED ? s_worker_confined : (int)blockIdx.x)
+    const int64_t u0 = (int64_t)s_worker * sk.L;
     const int64_t ntiles = sk.tilesM * sk.tilesN;
     const bool rr = !sk.partial && sk.G > 0;
     const int64_t u1 = !rr ? min(sk.U, u0 + sk.L)
-                                  : u0 + ((ntiles - (int64_t)blockIdx.x + sk.G - 1) / sk.G) * sk.KT;
+                                  : u0 + ((ntiles - (int64_t)s_worker + sk.G - 1) / sk.G) * sk.KT;
     if (u0 >= u1) return;
     // flat tile index (contiguous per CTA) -> tile coordinates
     auto decode = [&](int64_t t, int64_t& tm, int64_t& tn) {
         if (!rr) { tn = t / sk.tilesM; tm = t - tn * sk.tilesM; return; }
-        const int64_t rank = (t - u0 / sk.KT) * sk.G + (int64_t)blockIdx.x;
+        const int64_t rank = (t - u0 / sk.KT) * sk.G + (int64_t)s_worker;
         const int64_t per_band = (int64_t)sk.Gm * sk.tilesN;
         const int64_t band = rank / per_band, r = rank - band * per_band;
         const int64_t hb = min((int64_t)sk.Gm, sk.tilesM - band * sk.Gm);
@@ -375,7 +399,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
         if (sk.partial) {
             // compact partial tiles: the (CTA, tile) pairs of a stream-K schedule form a staircase
             // on which tile + CTA is strictly increasing, so that sum indexes a dense BM x BN slot
-            T* Pt = g.C + (t + (int64_t)blockIdx.x) * (int64_t)(BM * BN);
+            T* Pt = g.C + (t + (int64_t)s_worker) * (int64_t)(BM * BN);
 #pragma unroll
             for (int i = 0; i < MT; ++i)
 #pragma unroll
@@ -411,6 +435,8 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
 // -------------------------------------------------------------------------------------------
 // host side: plan + launch
 // -------------------------------------------------------------------------------------------
+#undef s_worker
+
 struct MmaPlan {
     StreamK sk;
     int grid;        // CTAs
@@ -459,6 +485,23 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
 template <typename T, bool TA, int BM, int BN, int WM, int WN, int STAGES, int MINB>
 inline cudaError_t launch_mma(GemmArgs<T> g, const MmaPlan& p, cudaStream_t st) {
     using Cfg = MmaCfg<T, TA, BM, BN, WM, WN, STAGES>;
+    if (p.sk.tickets) {
+        if constexpr (sizeof(T) == 8 && MINB == 2) {
+            auto kc = gemm_mma_kernel<T, TA, BM, BN, WM, WN, STAGES, MINB, true>;
+            static bool attr_c = false;
+            if (!attr_c) {
+                cudaError_t e = cudaFuncSetAttribute(kc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+                if (e != cudaSuccess) return e;
+                attr_c = true;
+            }
+            StreamK skc = p.sk;
+            skc.l2_prefetch = 0; skc.workers = p.grid;
+            kc<<<p.grid + MINB * skc.reserve, Cfg::NT, Cfg::SMEM, st>>>(g, skc);
+            return cudaGetLastError();
+        } else {
+            return cudaErrorInvalidValue;
+        }
+    }
     auto kern = gemm_mma_kernel<T, TA, BM, BN, WM, WN, STAGES, MINB>;
     static bool attr_done = false;
     if (!attr_done) {

@@ -46,6 +46,11 @@ struct GemmLaunch {
     int slots;         // partial output buffers needed (each g.split_stride elements apart)
     int cfg;           // kernel configuration index inside the dtype's dispatcher
     SegInfo seg;       // for the consumer of the partials
+    // kind 1, optional: keep the kernel off `reserve` SMs (those with the highest %smid).  2 * reserve extra CTAs are
+    // launched; a CTA that finds itself on a reserved SM retires at once (at most 2 * reserve do, counted in
+    // tickets[0]), every other CTA draws its worker index from tickets[1].  tickets: two zeroed counters per launch.
+    int reserve = 0;
+    unsigned* tickets = nullptr;
 };
 
 // impl: 0 = default for the dtype (fp64: DMMA tensor cores, fp32: 3xTF32 tensor cores),

@@ -396,7 +396,8 @@ static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
             const int ibn = panel_ib_for<T>(h, mk1);
             const int Gp = ibn ? (int)ceil_div(mk1, (int64_t)kPanelThreads * panel_rpts<T>(ibn)[0]) : h.sms;
             R = h.reserve_sms > 0 ? h.reserve_sms : Gp + 2;
-            if (R > h.sms / 3) R = 0;                       // tall panels: the chain is negligible against the update
+            static const double maxfrac = [] { const char* e = getenv("CTQR_RESERVE_MAXFRAC"); return e ? atof(e) : 0.45; }();
+            if (R > (int)(h.sms * maxfrac)) R = 0;          // tall panels: the chain is negligible against the update
             if (R > 0) {
                 const double t_panel = 0.25e-3 + 1.5e-8 * (double)mk1;                   // s, calibrated at c3 (flat optimum, both precisions)
                 const double rate = (sizeof(T) == 4 ? 69e12 : 25e12) * (double)(h.sms - R) / (double)h.sms;   // flop/s of the pair of products

@@ -89,6 +89,8 @@ struct ctqr_handle_s {
     // workspaces: [0] update stream, [1] panel stream
     void* dWp[2] = {nullptr, nullptr}; size_t wp_elems[2] = {0, 0};
     void* dW[2] = {nullptr, nullptr};  size_t w_elems[2] = {0, 0};
+    // two-panel (256-wide) trailing updates: W / T^T W (256 x nc each), two merged T factors, merge scratch
+    void* dW2[2] = {nullptr, nullptr}; size_t w2_elems = 0; void* dT2 = nullptr; void* dMerge = nullptr;
     void* dPart = nullptr;             // LL slots of the panel kernel
     void* dLLs = nullptr; unsigned ll_seq = 0;   // LL slots / step numbers of the fused small-S solve kernels
     unsigned bar_count = 0;            // step numbers handed to the panel kernel (never reused)
@@ -123,7 +125,8 @@ struct ctqr_handle_s {
         if (fmap) { msync(fmap, fmap_len, MS_SYNC); munmap(fmap, fmap_len); }
         if (ffd >= 0) close(ffd);
         cudaFree(dT); cudaFree(dRd); cudaFree(dRinv); cudaFree(dTau);
-        for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); }
+        for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); cudaFree(dW2[i]); }
+        cudaFree(dT2); cudaFree(dMerge);
         cudaFree(dPart); cudaFree(dLLs); cudaFree(dFlag); cudaFree(dTickets);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
@@ -347,7 +350,7 @@ static cudaEvent_t new_event(H& h, bool timing) {
 // applied.  Everything is enqueued; on return sU waits for the last panel.  No host sync.
 // ------------------------------------------------------------------------------------------
 template <typename T>
-static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
+static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
     const int64_t m = h.m;
     const int nb = h.nb;
     const int k0 = (int)(c0 / nb), k1 = (int)ceil_div(c1, nb);
@@ -412,6 +415,195 @@ static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
     }
     CK(cudaStreamWaitEvent(h.sU, evP, 0));
     return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// Two panels per trailing update (in core, nb = 128).  C <- C - V W with K = nb = 128 is the
+// slowest contraction of the factorisation (8 k-tiles per output tile, C read and written
+// once per panel); applying panels k, k+1 together as ONE 256-wide compact-WY block
+//     Q = H_k H_{k+1} = I - [V_k V_{k+1}] T2 [V_k V_{k+1}]^T,
+//     T2 = [[T_k, -T_k (V_k^T V_{k+1}) T_{k+1}], [0, T_{k+1}]]        (the larft recurrence, one block step)
+// halves the passes over C and doubles K (measured: the fp64 kernel alone 24.3 -> 27.8 TFLOP/s).
+// The look-ahead chain then factors TWO panels (with the narrow larfb between them) and merges
+// their T factors while the bulk of the previous pair's update runs.  V_{k+1} is zero in the
+// rows of panel k's diagonal block, where the matrix holds R_{k,k+1}: the products touching those
+// rows are issued separately (W_bot = V_{k+1}^T C[nb:], and the top nb rows of C take only V_k).
+// ------------------------------------------------------------------------------------------
+template <typename T>
+static int ensure_pair_ws(H& h, int64_t nc) {
+    const size_t need = (size_t)256 * (size_t)nc;
+    if (h.dW2[0] && h.w2_elems >= need) return 0;
+    for (int i = 0; i < 2; ++i) { if (h.dW2[i]) cudaFree(h.dW2[i]); h.dW2[i] = nullptr; }
+    for (int i = 0; i < 2; ++i)
+        if (cudaMalloc(&h.dW2[i], need * sizeof(T)) != cudaSuccess) { cudaGetLastError(); h.w2_elems = 0; return 1; }
+    h.w2_elems = need;
+    if (!h.dT2) {
+        if (cudaMalloc(&h.dT2, (size_t)2 * 256 * 256 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
+        CK(cudaMemsetAsync(h.dT2, 0, (size_t)2 * 256 * 256 * sizeof(T), h.sU));
+        if (cudaMalloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
+    }
+    return 0;
+}
+
+// T2[slot] for the panels starting at columns j0 and j0 + 128 (both factored, both 128 wide); stream st
+template <typename T>
+static int pair_merge(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m, int64_t j0, int slot) {
+    const int nb = 128;
+    const int k = (int)(j0 / nb);
+    const T* Tk = P_<T>(h.dT) + (size_t)k * nb * nb;
+    const T* Tk1 = Tk + (size_t)nb * nb;
+    T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;
+    T* G = P_<T>(h.dMerge), *X = G + 128 * 128;
+    // G = V_k[nb:, :]^T V_{k+1}  (stream-K partial tiles, summed in a fixed order)
+    GemmArgs<T> g{};
+    g.M = nb; g.N = nb; g.K = m - j0 - nb; g.A = A + (j0 + nb) + j0 * lda; g.lda = lda;
+    g.B = A + (j0 + nb) + (j0 + nb) * lda; g.ldb = lda;
+    g.C = P_<T>(h.dWp[1]); g.ldc = nb; g.alpha = T(1); g.beta = T(0); g.split_stride = (int64_t)nb * nb;
+    const GemmLaunch LG = gemm_plan<T>(true, nb, nb, g.K, h.gemm_impl, h.sms, true, (int64_t)h.wp_elems[1],
+                                       g.split_stride, gemm_aligned(g));
+    if (LG.kind != 1) return set_err(CTQR_ERR_STATE, "pair merge needs the stream-K product");
+    CK(gemm_run<T>(true, g, LG, h.gemm_impl, st));
+    CK(partial_sum_launch<T>(P_<T>(h.dWp[1]), LG.seg, nb, nb, G, nb, st));
+    // X = G T_{k+1};  T2[0:nb, nb:2nb] = -T_k X
+    GemmArgs<T> g2{};
+    g2.M = nb; g2.N = nb; g2.K = nb; g2.A = G; g2.lda = nb; g2.B = Tk1; g2.ldb = nb; g2.C = X; g2.ldc = nb;
+    g2.alpha = T(1); g2.beta = T(0);
+    CK(gemm_direct<T>(false, g2, h.gemm_impl, h.sms, st));
+    GemmArgs<T> g3{};
+    g3.M = nb; g3.N = nb; g3.K = nb; g3.A = Tk; g3.lda = nb; g3.B = X; g3.ldb = nb; g3.C = T2 + (size_t)nb * 256; g3.ldc = 256;
+    g3.alpha = T(-1); g3.beta = T(0);
+    CK(gemm_direct<T>(false, g3, h.gemm_impl, h.sms, st));
+    CK(copy2d_launch<T>(Tk, nb, T2, 256, nb, nb, st));
+    CK(copy2d_launch<T>(Tk1, nb, T2 + nb + (size_t)nb * 256, 256, nb, nb, st));
+    h.launches += 6;
+    return 0;
+}
+
+// C[j0:m, 0:nc] <- (H_k H_{k+1})^T C for the pair at columns j0, j0 + 128; T2 = its merged factor; stream sU
+template <typename T>
+static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m, int64_t j0, const T* T2, T* C,
+                      int64_t ldc, int64_t nc, int reserve_sms) {
+    if (nc <= 0) return 0;
+    const int nb = 128;
+    const int k = (int)(j0 / nb);
+    const T* V1 = A + j0 + j0 * lda;
+    const T* V2 = A + (j0 + nb) + (j0 + nb) * lda;
+    const int64_t mk = m - j0;
+    if (nc < 1024 || (size_t)256 * (size_t)nc > h.w2_elems) {
+        // narrow right-hand side: the two panels one after the other (same product, small kernels)
+        CKI(larfb<T>(h, 0, st, V1, lda, mk, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb, C, ldc, nc, true, reserve_sms));
+        CKI(larfb<T>(h, 0, st, V2, lda, mk - nb, nb, P_<T>(h.dT) + (size_t)(k + 1) * nb * nb, nb, C + nb, ldc, nc, true,
+                     reserve_sms));
+        return 0;
+    }
+    const int sms = std::max(8, h.sms - reserve_sms);
+    T* Wp = P_<T>(h.dWp[0]);
+    T* W = P_<T>(h.dW2[0]);
+    T* W2 = P_<T>(h.dW2[1]);
+    const bool prof = h.profile;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    // W[0:nb] = V_k^T C,  W[nb:2nb] = V_{k+1}^T C[nb:]
+    for (int half = 0; half < 2; ++half) {
+        GemmArgs<T> g1{};
+        g1.M = nb; g1.N = nc; g1.K = mk - half * nb; g1.A = half ? V2 : V1; g1.lda = lda; g1.B = C + half * nb; g1.ldb = ldc;
+        g1.C = Wp; g1.ldc = nb; g1.alpha = T(1); g1.beta = T(0); g1.split_stride = (int64_t)nb * nc;
+        GemmLaunch L1 = gemm_plan<T>(true, nb, nc, g1.K, h.gemm_impl, sms, true, (int64_t)h.wp_elems[0], g1.split_stride,
+                                     gemm_aligned(g1));
+        if (L1.kind != 1) return set_err(CTQR_ERR_STATE, "pair update needs the stream-K product");
+        CKI(confine<T>(h, L1, reserve_sms, st));
+        if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
+        CK(gemm_run<T>(true, g1, L1, h.gemm_impl, st));
+        if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, 2.0 * (double)g1.K * nb * (double)nc, 0}); }
+        CK(partial_sum_launch<T>(Wp, L1.seg, nb, nc, W + half * nb, 256, st));
+    }
+    // W2 = T2^T W
+    GemmArgs<T> gt{};
+    gt.M = 256; gt.N = nc; gt.K = 256; gt.A = T2; gt.lda = 256; gt.B = W; gt.ldb = 256; gt.C = W2; gt.ldc = 256;
+    gt.alpha = T(1); gt.beta = T(0);
+    CKI(gemm_direct_confined<T>(h, true, gt, sms, reserve_sms, st));
+    // top nb rows: only V_k reaches them;  the rest: K = 256
+    GemmArgs<T> ga{};
+    ga.M = nb; ga.N = nc; ga.K = nb; ga.A = V1; ga.lda = lda; ga.B = W2; ga.ldb = 256; ga.C = C; ga.ldc = ldc;
+    ga.alpha = T(-1); ga.beta = T(1);
+    CKI(gemm_direct_confined<T>(h, false, ga, sms, reserve_sms, st));
+    GemmArgs<T> gb{};
+    gb.M = mk - nb; gb.N = nc; gb.K = 256; gb.A = A + (j0 + nb) + j0 * lda; gb.lda = lda; gb.B = W2; gb.ldb = 256;
+    gb.C = C + nb; gb.ldc = ldc; gb.alpha = T(-1); gb.beta = T(1);
+    if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
+    CKI(gemm_direct_confined<T>(h, false, gb, sms, reserve_sms, st));
+    if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, 2.0 * (double)gb.M * 256 * (double)nc, 1}); }
+    h.launches += 7;
+    return 0;
+}
+
+template <typename T>
+static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
+    const int64_t m = h.m;
+    const int nb = 128;
+    if (!h.evP) { h.evP = new_event(h, false); h.evL = new_event(h, false); h.evU = new_event(h, false); }
+    cudaEvent_t evP = h.evP, evL = h.evL, evU = h.evU;
+    CK(cudaEventRecord(evU, h.sU));
+    CK(cudaStreamWaitEvent(h.sP, evU, 0));
+    // the look-ahead chain of one pair on sP: panel, narrow larfb onto the next panel's columns, panel, merge
+    auto chain = [&](int64_t j0, int slot) -> int {
+        const int k = (int)(j0 / nb);
+        CKI(panel_factor<T>(h, h.sP, A, lda, m, j0, nb, k));
+        CKI(larfb<T>(h, 1, h.sP, A + j0 + j0 * lda, lda, m - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
+                     A + j0 + (j0 + nb) * lda, lda, nb));
+        CKI(panel_factor<T>(h, h.sP, A, lda, m, j0 + nb, nb, k + 1));
+        CKI(pair_merge<T>(h, h.sP, A, lda, m, j0, slot));
+        CK(cudaEventRecord(evP, h.sP));
+        return 0;
+    };
+    int slot = 0;
+    CKI(chain(c0, slot));
+    for (int64_t j0 = c0;; j0 += 2 * nb, slot ^= 1) {
+        const T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;
+        const int64_t jn = j0 + 2 * nb;                     // first trailing column
+        const int64_t rem = c1 - jn;
+        CK(cudaStreamWaitEvent(h.sU, evP, 0));              // V, T2 of this pair ready
+        if (rem < 2 * nb) {
+            // no further full pair: finish this update, then the single-panel driver takes the tail
+            CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, A + j0 + jn * lda, lda, rem, 0));
+            if (rem > 0) CKI(factor_range_single<T>(h, A, lda, jn, c1));
+            return 0;
+        }
+        // look-ahead block: the columns of the next pair
+        CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, A + j0 + jn * lda, lda, 2 * nb, 0));
+        CK(cudaEventRecord(evL, h.sU));
+        CK(cudaStreamWaitEvent(h.sP, evL, 0));
+        CKI(chain(jn, slot ^ 1));
+        // bulk: first part beside the chain on SMs - R (see factor_range_single), then everything
+        const int64_t ncb = rem - 2 * nb;
+        int R = 0; int64_t nA = ncb;
+        if (h.reserve_sms != 0 && ncb > 0) {
+            const int64_t mk1 = m - jn;
+            const int ibn = panel_ib_for<T>(h, mk1);
+            const int Gp = ibn ? (int)ceil_div(mk1, (int64_t)kPanelThreads * panel_rpts<T>(ibn)[0]) : h.sms;
+            R = h.reserve_sms > 0 ? h.reserve_sms : Gp + 2;
+            if (R > (int)(h.sms * 0.45)) R = 0;
+            if (R > 0) {
+                const double t_chain = 2.0 * (0.25e-3 + 1.5e-8 * (double)mk1) + 0.15e-3;
+                const double rate = (sizeof(T) == 4 ? 75e12 : 27e12) * (double)(h.sms - R) / (double)h.sms;
+                nA = (int64_t)(t_chain * rate / (4.0 * (double)(m - j0) * 2 * nb));
+                nA = std::min<int64_t>(ncb, round_up(std::max<int64_t>(nA, 1024), 128));
+                if (ncb - nA < 1024) nA = ncb;
+            }
+        }
+        T* Cb = A + j0 + (jn + 2 * nb) * lda;
+        CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, Cb, lda, nA, R));
+        if (nA < ncb) CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, Cb + nA * lda, lda, ncb - nA, 0));
+    }
+}
+
+template <typename T>
+static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
+    static const bool pairs = [] { const char* e = getenv("CTQR_PAIR"); return !e || e[0] != '0'; }();
+    const bool aligned = (uintptr_t)A % 16 == 0 && (lda * (int64_t)sizeof(T)) % 16 == 0;
+    if (pairs && h.lookahead && !h.ooc && h.nb == 128 && h.gemm_impl == 0 && aligned && c0 % 128 == 0 && c1 - c0 >= 4 * 128 &&
+        h.m - c0 >= 1024 && ensure_pair_ws<T>(h, c1 - c0) == 0)
+        return factor_range_pairs<T>(h, A, lda, c0, c1);
+    return factor_range_single<T>(h, A, lda, c0, c1);
 }
 
 template <typename T>

@@ -390,9 +390,9 @@ def workload_name(cfg) -> str:
 
 # per-launch DRAM traffic of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/); filled in when a capture of the current kernel exists, else null.
-# profiles/r1_final_c3.md: dram__bytes_read.sum + dram__bytes_write.sum of the largest launch of the kernel
-# (bulk update of panel 1 at configs[2]); its algorithmic bytes there are 8.42e9 (fp64) / 4.2e9 (fp32, whole bulk)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {("f64", "upd"): 9.82e9, ("f64", "vtc"): 4.29e9,
+# profiles/r1_pairs_c3.md (fp64: bulk update of the first PAIR of panels at configs[2], K = 256; algorithmic bytes there
+# 8.29e9) and profiles/r1_final_c3.md (fp32): dram__bytes_read.sum + dram__bytes_write.sum of the largest launch
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {("f64", "upd"): 13.68e9, ("f64", "vtc"): 3.95e9,
                                 ("f32", "upd"): 3.57e9, ("f32", "vtc"): 1.91e9}
 
 KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; DMMA.8x8x4)",
@@ -414,7 +414,7 @@ def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:
     return {"bound": "tensor" if dtype == "f64" else "alu", "kernel": KERNEL_NAMES[(dtype, dom)],
             "achieved": ach, "peak": peak, "unit": UNIT, "frac": ach / peak,
             "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dtype, dom)),
-            "traffic_note": "ncu --set full, largest launch of this kernel at configs[2] (profiles/r1_final_c3.md); "
+            "traffic_note": "ncu --set full, largest launch of this kernel at configs[2] (profiles/r1_pairs_c3.md); "
                             "the launches of a factorisation shrink with the trailing matrix",
             "peak_source": ("derived: 148 SMs x %d %s FMA lanes x 2 x %.0f MHz max SM clock (MEASURED_PEAKS.json "
                             "holds no %s figure; sm_max_mhz %s)" % (64 if dtype == "f64" else 128,

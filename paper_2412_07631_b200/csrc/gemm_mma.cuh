@@ -476,7 +476,8 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
         // G > 0 would deal the tiles round-robin in bands of Gm tile rows (see StreamK); measured
         // neutral to slightly slower than contiguous ranges at m = 3e4 and 1e5 (the L2 hints already
         // keep V resident), so the contiguous order stays the default
-        p.sk.G = 0;
+        static const int band = [] { const char* e = getenv("CTQR_BAND"); return e ? atoi(e) : 0; }();
+        p.sk.G = (band && K >= band) ? p.grid : 0;
         p.sk.Gm = (int)std::max<int64_t>(1, std::min<int64_t>(p.sk.tilesM, slots / 4));
     }
     return p;

@@ -118,7 +118,22 @@ int ct_qr_get_V(ctqr_handle_t h, int64_t j0, int64_t ncols, void* V, int64_t ldv
 int ct_qr_get_T(ctqr_handle_t h, int64_t panel, void* T, int64_t ldt);   /* nb_k x nb_k upper (last panel may be narrower) */
 int ct_qr_get_tau(ctqr_handle_t h, void* tau);                           /* n values */
 int ct_qr_get_stats(ctqr_handle_t h, ctqr_stats_t* s);
+int ct_qr_dtype(ctqr_handle_t h);                                        /* CTQR_F32 / CTQR_F64; -1 when h is NULL */
 void ct_qr_destroy(ctqr_handle_t h);
+
+/* Factor persistence ("factor once per geometry, reuse for every batch of slices").
+ * ct_qr_save writes the whole factor of a factored handle (V\R storage, T_k, diagonal R blocks, tau;
+ * in-core or out-of-core handle alike) to `path` (created / truncated; removed again on failure).
+ * The file is self-describing (dtype, m, n, nb, ib) and holds m*n*w bytes plus O(n*nb*w).
+ * ct_qr_load builds a handle from such a file without factoring: the factor is read into device
+ * memory when it fits opt->device_budget_bytes (0 = free device memory), otherwise the file is mapped
+ * read-only and ct_qr_solve streams its panels through the page cache (out-of-core solve, row a5).
+ * Of `opt` only device_budget_bytes, gemm_impl and stream are used (nb / ib come from the file); opt
+ * may be NULL.  A loaded handle supports every call a factored one does; its factor_ms is 0.
+ * Errors: CTQR_ERR_IO (cannot create/open, short write/read, bad magic/header, truncated file),
+ * CTQR_ERR_NOMEM, CTQR_ERR_CUDA; *out is untouched on failure. */
+int ct_qr_save(ctqr_handle_t h, const char* path);
+int ct_qr_load(const char* path, const ctqr_options_t* opt, ctqr_handle_t* out);
 
 const char* ct_qr_strerror(int code);
 const char* ct_qr_last_error(void);

@@ -66,6 +66,9 @@ EXPORTS = {
     "ct_qr_get_tau": ([_P, _P], _I),
     "ct_qr_get_stats": ([_P, ctypes.POINTER(Stats)], _I),
     "ct_qr_destroy": ([_P], None),
+    "ct_qr_save": ([_P, ctypes.c_char_p], _I),
+    "ct_qr_load": ([ctypes.c_char_p, ctypes.POINTER(Options), ctypes.POINTER(_P)], _I),
+    "ct_qr_dtype": ([_P], _I),
     "ct_qr_strerror": ([_I], ctypes.c_char_p),
     "ct_qr_last_error": ([], ctypes.c_char_p),
     "ct_qr_version": ([], _I),
@@ -184,6 +187,22 @@ def ct_qr_factor(A, m: int, n: int, lda: int | None = None, *, nb: int = 0, ib: 
     h = _P()
     _check(lib().ct_qr_factor(_ptr(A) if A is not None else None, m, n, lda, code, ctypes.byref(o), ctypes.byref(h)))
     return Factor(h, m, n, code, keep=A if in_place else None)
+
+
+def ct_qr_save(f: Factor, path: str) -> None:
+    """Write the factor (V\\R storage, T_k, diagonal R blocks, tau) to ``path`` (reuse)."""
+    _check(lib().ct_qr_save(f._h, os.fsencode(path)))
+
+
+def ct_qr_load(path: str, *, device_budget_bytes: int = 0, gemm_impl: int = 0, stream=None) -> Factor:
+    """Handle from a file written by ``ct_qr_save``; the solve streams the file when the factor
+    exceeds ``device_budget_bytes`` (0 = free device memory)."""
+    o = Options(lookahead=-1, device_budget_bytes=device_budget_bytes, gemm_impl=gemm_impl, stream=stream)
+    h = _P()
+    _check(lib().ct_qr_load(os.fsencode(path), ctypes.byref(o), ctypes.byref(h)))
+    s = Stats()
+    _check(lib().ct_qr_get_stats(h, ctypes.byref(s)))
+    return Factor(h, s.m, s.n, lib().ct_qr_dtype(h))     # dtype, m, n are properties of the file
 
 
 def ct_qr_solve(f: Factor, B, S: int, X, ldb: int | None = None, ldx: int | None = None):

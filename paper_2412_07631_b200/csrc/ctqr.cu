@@ -6,6 +6,7 @@
 #include <cooperative_groups.h>
 #include <stdarg.h>
 #include <stdlib.h>
+#include <errno.h>
 #include <fcntl.h>
 #include <sys/mman.h>
 #include <sys/stat.h>
@@ -862,18 +863,8 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
     return factor_ooc<T>(h, (T*)A, lda, ns);
 }
 
-extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dtype_t dtype,
-                            const ctqr_options_t* opt, ctqr_handle_t* out) {
-    g_err[0] = 0;
-    const bool use_file = opt && opt->file_path && opt->file_path[0];
-    if (!A && !use_file) return set_err(-1, "A is NULL");
-    if (m < 1) return set_err(-2, "m < 1");
-    if (n < 1 || n > m) return set_err(-3, "need 1 <= n <= m");
-    if (lda < m) return set_err(-4, "lda < m");
-    if (dtype != CTQR_F32 && dtype != CTQR_F64) return set_err(-5, "bad dtype");
-    if (!out) return set_err(-7, "out is NULL");
-    ctqr_options_t o; memset(&o, 0, sizeof o); o.lookahead = -1;
-    if (opt) o = *opt;
+// handle with its options, streams and device properties (shared by ct_qr_factor and ct_qr_load)
+static int new_handle(ctqr_dtype_t dtype, int64_t m, int64_t n, const ctqr_options_t& o, H** out) {
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();
@@ -905,6 +896,24 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
     }
     // order after the caller's stream
     if (cudaStreamSynchronize(h->user) != cudaSuccess) { delete h; return set_err(CTQR_ERR_CUDA, "user stream sync failed"); }
+    *out = h;
+    return 0;
+}
+
+extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dtype_t dtype,
+                            const ctqr_options_t* opt, ctqr_handle_t* out) {
+    g_err[0] = 0;
+    const bool use_file = opt && opt->file_path && opt->file_path[0];
+    if (!A && !use_file) return set_err(-1, "A is NULL");
+    if (m < 1) return set_err(-2, "m < 1");
+    if (n < 1 || n > m) return set_err(-3, "need 1 <= n <= m");
+    if (lda < m) return set_err(-4, "lda < m");
+    if (dtype != CTQR_F32 && dtype != CTQR_F64) return set_err(-5, "bad dtype");
+    if (!out) return set_err(-7, "out is NULL");
+    ctqr_options_t o; memset(&o, 0, sizeof o); o.lookahead = -1;
+    if (opt) o = *opt;
+    H* h = nullptr;
+    CKI(new_handle(dtype, m, n, o, &h));
     if (use_file) {
         // file tier: column-major m x n matrix with leading dimension lda at offset 0 of the file
         const size_t need = (size_t)lda * (size_t)n * h->w;
@@ -1305,10 +1314,214 @@ extern "C" int ct_qr_get_stats(ctqr_handle_t h, ctqr_stats_t* s) {
     return 0;
 }
 
+extern "C" int ct_qr_dtype(ctqr_handle_t h) { return h ? (int)h->dtype : -1; }
+
 extern "C" void ct_qr_destroy(ctqr_handle_t h) {
     if (!h) return;
     cudaDeviceSynchronize();
     delete h;
+}
+
+// ------------------------------------------------------------------------------------------
+// factor persistence (the factor is computed once per
+// scanner geometry and reused for every later batch of slices).
+//
+// File layout (little endian): one 4096-byte header page, then the factored matrix storage
+// (column-major, leading dimension hdr.ld, n columns: V below / R above the panel diagonals),
+// then P blocks T_k (nb x nb), P diagonal blocks of R (nb x nb), then tau[n].  The matrix
+// section starts on a page boundary so that ct_qr_load can map the file and stream panels
+// straight from the page cache when the factor does not fit the device budget.
+// ------------------------------------------------------------------------------------------
+struct FactorFileHeader {
+    char magic[8];                    // "CTQRFAC1"
+    int32_t version, dtype, nb, ib, P, reserved;
+    int64_t m, n, ld;
+    uint64_t off_matrix, off_T, off_Rd, off_tau, file_bytes;
+};
+static const char kFactorMagic[8] = {'C', 'T', 'Q', 'R', 'F', 'A', 'C', '1'};
+constexpr size_t kFactorHeaderBytes = 4096;
+constexpr size_t kIoChunkBytes = (size_t)64 << 20;
+
+static int write_all(int fd, const void* buf, size_t len, const char* path) {
+    const char* p = (const char*)buf;
+    while (len > 0) {
+        ssize_t k = write(fd, p, len);
+        if (k < 0) { if (errno == EINTR) continue; return set_err(CTQR_ERR_IO, "write to %s failed: %s", path, strerror(errno)); }
+        p += k; len -= (size_t)k;
+    }
+    return 0;
+}
+static int read_all(int fd, void* buf, size_t len, const char* path) {
+    char* p = (char*)buf;
+    while (len > 0) {
+        ssize_t k = read(fd, p, len);
+        if (k < 0) { if (errno == EINTR) continue; return set_err(CTQR_ERR_IO, "read from %s failed: %s", path, strerror(errno)); }
+        if (k == 0) return set_err(CTQR_ERR_IO, "%s is truncated", path);
+        p += k; len -= (size_t)k;
+    }
+    return 0;
+}
+
+// device section -> file through a pinned bounce buffer
+static int save_device_section(H& h, int fd, const void* dsrc, size_t bytes, void* bounce, const char* path) {
+    for (size_t off = 0; off < bytes; off += kIoChunkBytes) {
+        const size_t len = std::min(kIoChunkBytes, bytes - off);
+        CK(cudaMemcpyAsync(bounce, (const char*)dsrc + off, len, cudaMemcpyDeviceToHost, h.sU));
+        CK(cudaStreamSynchronize(h.sU));
+        CKI(write_all(fd, bounce, len, path));
+    }
+    return 0;
+}
+static int load_device_section(H& h, int fd, void* ddst, size_t bytes, void* bounce, const char* path) {
+    for (size_t off = 0; off < bytes; off += kIoChunkBytes) {
+        const size_t len = std::min(kIoChunkBytes, bytes - off);
+        CKI(read_all(fd, bounce, len, path));
+        CK(cudaMemcpyAsync((char*)ddst + off, bounce, len, cudaMemcpyHostToDevice, h.sU));
+        CK(cudaStreamSynchronize(h.sU));
+    }
+    return 0;
+}
+
+static int save_body(H& h, int fd, const char* path, void* bounce) {
+    const size_t w = h.w;
+    const size_t blk = (size_t)h.nb * h.nb * w;
+    FactorFileHeader hd; memset(&hd, 0, sizeof hd);
+    memcpy(hd.magic, kFactorMagic, 8);
+    hd.version = 1; hd.dtype = (int32_t)h.dtype; hd.nb = h.nb; hd.ib = h.ib; hd.P = h.P;
+    hd.m = h.m; hd.n = h.n; hd.ld = round_up(h.m, 16 / (int64_t)w);
+    hd.off_matrix = kFactorHeaderBytes;
+    hd.off_T = hd.off_matrix + (uint64_t)hd.ld * h.n * w;
+    hd.off_Rd = hd.off_T + (uint64_t)blk * h.P;
+    hd.off_tau = hd.off_Rd + (uint64_t)blk * h.P;
+    hd.file_bytes = hd.off_tau + (uint64_t)h.n * w;
+    std::vector<char> page(kFactorHeaderBytes, 0);
+    memcpy(page.data(), &hd, sizeof hd);
+    CKI(write_all(fd, page.data(), page.size(), path));
+    // matrix storage, a chunk of whole columns at a time (padding rows of the file are zero)
+    const size_t col_bytes = (size_t)hd.ld * w;
+    const int64_t cols_per = std::max<int64_t>(1, (int64_t)(kIoChunkBytes / col_bytes));
+    const size_t slab = col_bytes <= kIoChunkBytes ? kIoChunkBytes : col_bytes;
+    std::vector<char> big;
+    char* buf = (char*)bounce;
+    if (slab > kIoChunkBytes) { big.resize(slab); buf = big.data(); }    // one column exceeds the bounce buffer: pageable
+    for (int64_t c0 = 0; c0 < h.n; c0 += cols_per) {
+        const int64_t nc = std::min<int64_t>(cols_per, h.n - c0);
+        if (hd.ld != h.m) memset(buf, 0, (size_t)nc * col_bytes);
+        if (h.ooc) {
+            for (int64_t c = 0; c < nc; ++c)
+                memcpy(buf + (size_t)c * col_bytes, (const char*)h.hA + (size_t)(c0 + c) * h.hlda * w, (size_t)h.m * w);
+        } else {
+            CK(cudaMemcpy2DAsync(buf, col_bytes, (const char*)h.dA + (size_t)c0 * h.lda * w, (size_t)h.lda * w,
+                                 (size_t)h.m * w, nc, cudaMemcpyDeviceToHost, h.sU));
+            CK(cudaStreamSynchronize(h.sU));
+        }
+        CKI(write_all(fd, buf, (size_t)nc * col_bytes, path));
+    }
+    CKI(save_device_section(h, fd, h.dT, blk * h.P, bounce, path));
+    CKI(save_device_section(h, fd, h.dRd, blk * h.P, bounce, path));
+    CKI(save_device_section(h, fd, h.dTau, (size_t)h.n * w, bounce, path));
+    return 0;
+}
+
+extern "C" int ct_qr_save(ctqr_handle_t h, const char* path) {
+    g_err[0] = 0;
+    CKI(check_handle(h));
+    if (!path || !path[0]) return set_err(-2, "path is NULL or empty");
+    if (cudaStreamSynchronize(h->user) != cudaSuccess) return set_err(CTQR_ERR_CUDA, "user stream sync failed");
+    const int fd = open(path, O_WRONLY | O_CREAT | O_TRUNC, 0644);
+    if (fd < 0) return set_err(CTQR_ERR_IO, "cannot create %s: %s", path, strerror(errno));
+    void* bounce = nullptr;
+    if (cudaMallocHost(&bounce, kIoChunkBytes) != cudaSuccess) {
+        cudaGetLastError(); close(fd);
+        return set_err(CTQR_ERR_NOMEM, "cannot allocate the pinned bounce buffer");
+    }
+    int rc = save_body(*h, fd, path, bounce);
+    cudaFreeHost(bounce);
+    if (rc == 0 && fsync(fd) != 0) rc = set_err(CTQR_ERR_IO, "fsync of %s failed: %s", path, strerror(errno));
+    if (close(fd) != 0 && rc == 0) rc = set_err(CTQR_ERR_IO, "close of %s failed: %s", path, strerror(errno));
+    if (rc != 0) unlink(path);                 // never leave a partial factor file behind
+    return rc;
+}
+
+template <typename T>
+static int load_typed(H& h, int fd, const FactorFileHeader& hd, const ctqr_options_t& o, const char* path, void* bounce) {
+    const size_t w = sizeof(T);
+    const size_t blk = (size_t)h.nb * h.nb * w;
+    const size_t mat_bytes = (size_t)hd.ld * h.n * w;
+    CKI(alloc_state<T>(h, h.nb));              // solve workspaces grow on demand (ensure_solve_ws)
+    size_t freeb = 0, totb = 0;
+    CK(cudaMemGetInfo(&freeb, &totb));
+    const size_t slack = (size_t)2 << 30;
+    const size_t budget = o.device_budget_bytes > 0 ? (size_t)o.device_budget_bytes : (freeb > slack ? freeb - slack : 0);
+    if (mat_bytes <= budget) {
+        h.lda = hd.ld;
+        if (cudaMalloc(&h.dA, mat_bytes) != cudaSuccess) { cudaGetLastError(); return set_err(CTQR_ERR_NOMEM, "cannot allocate %zu bytes for the factor", mat_bytes); }
+        h.own_A = true;
+        if (lseek(fd, (off_t)hd.off_matrix, SEEK_SET) < 0) return set_err(CTQR_ERR_IO, "seek in %s failed", path);
+        CKI(load_device_section(h, fd, h.dA, mat_bytes, bounce, path));
+        h.st.h2d_bytes = (double)mat_bytes;
+    } else {
+        // factor larger than the budget: map the file, the solve streams panels from the page cache (a5)
+        void* mp = mmap(nullptr, (size_t)hd.file_bytes, PROT_READ, MAP_SHARED, fd, 0);
+        if (mp == MAP_FAILED) return set_err(CTQR_ERR_IO, "mmap of %s failed: %s", path, strerror(errno));
+        h.fmap = mp; h.fmap_len = (size_t)hd.file_bytes;
+        h.ooc = true; h.hA = (char*)mp + hd.off_matrix; h.hlda = hd.ld;
+        h.n_super = (int)std::max<int64_t>(1, (int64_t)ceil_div((int64_t)mat_bytes, (int64_t)std::max<size_t>(budget, 1)));
+        CKI(ensure_stream_bufs(h));
+    }
+    if (lseek(fd, (off_t)hd.off_T, SEEK_SET) < 0) return set_err(CTQR_ERR_IO, "seek in %s failed", path);
+    CKI(load_device_section(h, fd, h.dT, blk * h.P, bounce, path));
+    CKI(load_device_section(h, fd, h.dRd, blk * h.P, bounce, path));
+    CKI(load_device_section(h, fd, h.dTau, (size_t)h.n * w, bounce, path));
+    CK(cudaStreamSynchronize(h.sU));
+    return 0;
+}
+
+extern "C" int ct_qr_load(const char* path, const ctqr_options_t* opt, ctqr_handle_t* out) {
+    g_err[0] = 0;
+    if (!path || !path[0]) return set_err(-1, "path is NULL or empty");
+    if (!out) return set_err(-3, "out is NULL");
+    ctqr_options_t o; memset(&o, 0, sizeof o); o.lookahead = -1;
+    if (opt) o = *opt;
+    const int fd = open(path, O_RDONLY);
+    if (fd < 0) return set_err(CTQR_ERR_IO, "cannot open %s: %s", path, strerror(errno));
+    FactorFileHeader hd;
+    struct stat sb;
+    int rc = read_all(fd, &hd, sizeof hd, path);
+    if (rc == 0 && fstat(fd, &sb) != 0) rc = set_err(CTQR_ERR_IO, "fstat of %s failed", path);
+    if (rc == 0) {
+        const int64_t w = hd.dtype == CTQR_F64 ? 8 : 4;
+        const uint64_t blk = (uint64_t)hd.nb * hd.nb * w;
+        const bool ok = memcmp(hd.magic, kFactorMagic, 8) == 0 && hd.version == 1 &&
+            (hd.dtype == CTQR_F32 || hd.dtype == CTQR_F64) && hd.n >= 1 && hd.m >= hd.n && hd.ld >= hd.m &&
+            hd.nb >= 8 && hd.nb <= 128 && (hd.ib == 8 || hd.ib == 16 || hd.ib == 32) && hd.nb % hd.ib == 0 &&
+            hd.P == (int32_t)ceil_div(hd.n, (int64_t)hd.nb) && (hd.ld * w) % 16 == 0 &&
+            hd.off_matrix == kFactorHeaderBytes && hd.off_T == hd.off_matrix + (uint64_t)hd.ld * hd.n * w &&
+            hd.off_Rd == hd.off_T + blk * hd.P && hd.off_tau == hd.off_Rd + blk * hd.P &&
+            hd.file_bytes == hd.off_tau + (uint64_t)hd.n * w && (uint64_t)sb.st_size >= hd.file_bytes;
+        if (!ok) rc = set_err(CTQR_ERR_IO, "%s is not a ctqr factor file (bad header or truncated)", path);
+    }
+    if (rc != 0) { close(fd); return rc; }
+    o.nb = hd.nb; o.ib = hd.ib;
+    H* h = nullptr;
+    rc = new_handle((ctqr_dtype_t)hd.dtype, hd.m, hd.n, o, &h);
+    if (rc != 0) { close(fd); return rc; }
+    void* bounce = nullptr;
+    if (cudaMallocHost(&bounce, kIoChunkBytes) != cudaSuccess) {
+        cudaGetLastError(); close(fd); delete h;
+        return set_err(CTQR_ERR_NOMEM, "cannot allocate the pinned bounce buffer");
+    }
+    rc = hd.dtype == CTQR_F64 ? load_typed<double>(*h, fd, hd, o, path, bounce)
+                              : load_typed<float>(*h, fd, hd, o, path, bounce);
+    cudaFreeHost(bounce);
+    if (rc != 0) { close(fd); cudaDeviceSynchronize(); delete h; return rc; }
+    if (h->fmap) h->ffd = fd; else close(fd);  // the mapping keeps the file open for the handle's lifetime
+    h->st.m = hd.m; h->st.n = hd.n; h->st.nb = h->nb; h->st.ib = h->ib; h->st.n_panels = h->P;
+    h->st.n_superpanels = h->n_super; h->st.out_of_core = h->ooc ? 1 : 0; h->st.singular_col = -1;
+    h->st.factor_flops = 2.0 * (double)hd.m * (double)hd.n * (double)hd.n - 2.0 * (double)hd.n * (double)hd.n * (double)hd.n / 3.0;
+    h->factored = true;
+    *out = h;
+    return 0;
 }
 
 // ------------------------------------------------------------------------------------------

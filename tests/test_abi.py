@@ -66,6 +66,24 @@ def test_argument_errors_need_no_device(L):
     assert b"" != L.ct_qr_last_error()
 
 
+def test_persistence_argument_and_file_errors_need_no_device(L, tmp_path):
+    h = ctypes.c_void_p()
+    assert L.ct_qr_save(None, b"/tmp/x") == -1
+    assert L.ct_qr_load(None, None, ctypes.byref(h)) == -1
+    assert L.ct_qr_load(b"/tmp/x", None, None) == -3
+    assert L.ct_qr_dtype(None) == -1
+    # missing file, empty file, wrong magic, right magic with a corrupt header: all CTQR_ERR_IO (3), no device touched
+    assert L.ct_qr_load(os.fsencode(tmp_path / "missing.ctqr"), None, ctypes.byref(h)) == 3
+    (tmp_path / "empty.ctqr").write_bytes(b"")
+    assert L.ct_qr_load(os.fsencode(tmp_path / "empty.ctqr"), None, ctypes.byref(h)) == 3
+    (tmp_path / "junk.ctqr").write_bytes(b"NOTAFACT" + bytes(8192))
+    assert L.ct_qr_load(os.fsencode(tmp_path / "junk.ctqr"), None, ctypes.byref(h)) == 3
+    (tmp_path / "hdr.ctqr").write_bytes(b"CTQRFAC1" + bytes(8192))
+    assert L.ct_qr_load(os.fsencode(tmp_path / "hdr.ctqr"), None, ctypes.byref(h)) == 3
+    assert b"not a ctqr factor file" in L.ct_qr_last_error()
+    assert h.value is None
+
+
 def test_no_cpu_fallback(L):
     import torch
     if torch.cuda.is_available():

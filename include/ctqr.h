@@ -64,6 +64,14 @@ typedef struct {
                                    the file is mapped read-write, factored out of core through the page cache and
                                    overwritten with the factor, which ct_qr_solve streams from it.  NULL = none */
     void* stream;               /* cudaStream_t the caller's data is ordered on (NULL = legacy default) */
+    int64_t lower_bandwidth;    /* 0 = dense.  kl > 0: the caller promises A(i, j) == 0 for i - j > kl (for the Tikhonov-
+                                   augmented [A0; sqrt(lambda) I] with m0 rows of A0: kl = m0).  Householder QR keeps that
+                                   profile (v_j ends at row kl + j), so every panel and trailing update stops at row
+                                   kl + (last column of the block) and the factorisation costs sum_j 4 r_j (n-j-1) flop,
+                                   r_j = min(m, kl+j+1) - j, instead of 2mn^2 - 2n^3/3.  The result
+                                   is the same factor (the skipped work is arithmetic on exact zeros).  The promise is
+                                   checked on the device first (-6 if violated).  Used by in-core factorisations; the
+                                   out-of-core path ignores it. */
 } ctqr_options_t;
 
 /* Per-handle statistics (CUDA-event timed, milliseconds). */
@@ -78,13 +86,15 @@ typedef struct {
     double apply_qt_ms;        /* last Q^T B part (a6) */
     double trsm_ms;            /* last triangular solve part (a7) */
     double h2d_bytes, d2h_bytes;   /* bytes moved over the host link by the last factor / solve */
-    double factor_flops;       /* 2 m n^2 - 2 n^3 / 3 */
+    double factor_flops;       /* 2 m n^2 - 2 n^3 / 3 (the dense count, whatever was run) */
     int64_t kernel_launches;   /* kernels launched by the last factor or solve call */
     /* opt->profile only: the two contractions of every trailing update (a3) of the last factor,
      * each launch bracketed by CUDA events on the stream it runs on.
      *   vtc: W = V_k^T C  (K = m_k),   upd: C <- C - V_k W  (K = nb);  flops = 2*m_k*nb_k*n_c each. */
     double vtc_ms, vtc_flops;  int64_t vtc_launches;
     double upd_ms, upd_flops;  int64_t upd_launches;
+    int64_t lower_bandwidth;   /* the band promise the factorisation used (0 = dense) */
+    double factor_flops_performed;   /* = factor_flops when dense; the banded count of opt->lower_bandwidth otherwise */
 } ctqr_stats_t;
 
 /* Eq. 2: Householder QR of the m x n matrix A (m >= n >= 1, lda >= m).

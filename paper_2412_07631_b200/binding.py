@@ -34,7 +34,8 @@ class Options(ctypes.Structure):
     _fields_ = [("nb", ctypes.c_int32), ("ib", ctypes.c_int32), ("lookahead", ctypes.c_int32),
                 ("in_place", ctypes.c_int32), ("device_budget_bytes", ctypes.c_int64),
                 ("gemm_impl", ctypes.c_int32), ("profile", ctypes.c_int32),
-                ("file_path", ctypes.c_char_p), ("stream", ctypes.c_void_p)]
+                ("file_path", ctypes.c_char_p), ("stream", ctypes.c_void_p),
+                ("lower_bandwidth", ctypes.c_int64)]
 
 
 class Stats(ctypes.Structure):
@@ -48,7 +49,8 @@ class Stats(ctypes.Structure):
                 ("h2d_bytes", ctypes.c_double), ("d2h_bytes", ctypes.c_double),
                 ("factor_flops", ctypes.c_double), ("kernel_launches", ctypes.c_int64),
                 ("vtc_ms", ctypes.c_double), ("vtc_flops", ctypes.c_double), ("vtc_launches", ctypes.c_int64),
-                ("upd_ms", ctypes.c_double), ("upd_flops", ctypes.c_double), ("upd_launches", ctypes.c_int64)]
+                ("upd_ms", ctypes.c_double), ("upd_flops", ctypes.c_double), ("upd_launches", ctypes.c_int64),
+                ("lower_bandwidth", ctypes.c_int64), ("factor_flops_performed", ctypes.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -176,14 +178,15 @@ class Factor:
 def ct_qr_factor(A, m: int, n: int, lda: int | None = None, *, nb: int = 0, ib: int = 0,
                  lookahead: int = -1, in_place: bool = False, device_budget_bytes: int = 0,
                  gemm_impl: int = 0, profile: bool = False, stream=None, file_path: str | None = None,
-                 dtype=None) -> Factor:
+                 dtype=None, lower_bandwidth: int = 0) -> Factor:
     """Eq. 2.  ``A``: torch tensor (device or pinned/pageable host) or numpy array whose MEMORY
     is the column-major m x n matrix with leading dimension ``lda`` (default m)."""
     code = _code_of(A) if A is not None else (F64 if np.dtype(dtype) == np.float64 else F32)
     lda = m if lda is None else lda
     o = Options(nb=nb, ib=ib, lookahead=lookahead, in_place=int(in_place),
                 device_budget_bytes=device_budget_bytes, gemm_impl=gemm_impl, profile=int(profile),
-                file_path=file_path.encode() if file_path else None, stream=stream)
+                file_path=file_path.encode() if file_path else None, stream=stream,
+                lower_bandwidth=lower_bandwidth)
     h = _P()
     _check(lib().ct_qr_factor(_ptr(A) if A is not None else None, m, n, lda, code, ctypes.byref(o), ctypes.byref(h)))
     return Factor(h, m, n, code, keep=A if in_place else None)

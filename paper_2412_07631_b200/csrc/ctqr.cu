@@ -113,6 +113,9 @@ struct ctqr_handle_s {
         return tpool[tpool_used++];
     }
     bool factored = false;
+    // opt->lower_bandwidth (in-core factorisations only): A(i, j) == 0 for i - j > kl, so the reflectors of the
+    // columns [.., jend) end at row min(m, kl + jend) and every product over rows stops there
+    int64_t kl = 0;
     // out-of-core state
     bool ooc = false; void* hA = nullptr; int64_t hlda = 0; int n_super = 1;
     // file-backed tier: the matrix / factor lives in a file mapped MAP_SHARED (the OS page cache is the
@@ -142,6 +145,9 @@ struct ctqr_handle_s {
 typedef ctqr_handle_s H;
 
 template <typename T> static inline T* P_(void* p) { return reinterpret_cast<T*>(p); }
+
+// one past the last row that the reflectors of the columns [.., jend) can touch
+static inline int64_t row_end(const H& h, int64_t jend) { return h.kl > 0 ? std::min(h.m, h.kl + jend) : h.m; }
 
 static bool is_device_ptr(const void* p) {
     cudaPointerAttributes at;
@@ -352,7 +358,6 @@ static cudaEvent_t new_event(H& h, bool timing) {
 // ------------------------------------------------------------------------------------------
 template <typename T>
 static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
-    const int64_t m = h.m;
     const int nb = h.nb;
     const int k0 = (int)(c0 / nb), k1 = (int)ceil_div(c1, nb);
     if (!h.evP) { h.evP = new_event(h, false); h.evL = new_event(h, false); h.evU = new_event(h, false); }
@@ -363,15 +368,16 @@ static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) 
         for (int k = k0; k < k1; ++k) {
             const int64_t j0 = (int64_t)k * nb;
             const int nbw = (int)std::min<int64_t>(nb, c1 - j0);
-            CKI(panel_factor<T>(h, h.sU, A, lda, m, j0, nbw, k));
+            const int64_t me = row_end(h, j0 + nbw);
+            CKI(panel_factor<T>(h, h.sU, A, lda, me, j0, nbw, k));
             const int64_t nc = c1 - (j0 + nbw);
-            CKI(larfb<T>(h, 0, h.sU, A + j0 + j0 * lda, lda, m - j0, nbw,
+            CKI(larfb<T>(h, 0, h.sU, A + j0 + j0 * lda, lda, me - j0, nbw,
                          P_<T>(h.dT) + (size_t)k * nb * nb, nb, A + j0 + (j0 + nbw) * lda, lda, nc, true));
         }
         return 0;
     }
     static const bool reserve64 = [] { const char* e = getenv("CTQR_RESERVE_F64"); return !e || e[0] != '0'; }();
-    CKI(panel_factor<T>(h, h.sP, A, lda, m, c0, (int)std::min<int64_t>(nb, c1 - c0), k0));
+    CKI(panel_factor<T>(h, h.sP, A, lda, row_end(h, std::min<int64_t>(c0 + nb, c1)), c0, (int)std::min<int64_t>(nb, c1 - c0), k0));
     CK(cudaEventRecord(evP, h.sP));
     for (int k = k0; k < k1; ++k) {
         const int64_t j0 = (int64_t)k * nb;
@@ -379,13 +385,14 @@ static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) 
         const int64_t jn = j0 + nbw;                        // first trailing column
         if (jn >= c1) break;
         const int nbn = (int)std::min<int64_t>(nb, c1 - jn); // width of panel k+1
+        const int64_t me = row_end(h, jn), men = row_end(h, jn + nbn);   // row ends of panels k and k+1
         const T* V = A + j0 + j0 * lda;
         const T* Tk = P_<T>(h.dT) + (size_t)k * nb * nb;
         CK(cudaStreamWaitEvent(h.sU, evP, 0));              // V_k, T_k ready
-        CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, A + j0 + jn * lda, lda, nbn, true));
+        CKI(larfb<T>(h, 0, h.sU, V, lda, me - j0, nbw, Tk, nb, A + j0 + jn * lda, lda, nbn, true));
         CK(cudaEventRecord(evL, h.sU));
         CK(cudaStreamWaitEvent(h.sP, evL, 0));
-        CKI(panel_factor<T>(h, h.sP, A, lda, m, jn, nbn, k + 1));
+        CKI(panel_factor<T>(h, h.sP, A, lda, men, jn, nbn, k + 1));
         CK(cudaEventRecord(evP, h.sP));
         // Bulk update.  The fp32 contractions are one-CTA-per-SM persistent kernels, so a smaller grid
         // leaves whole SMs empty: the first part of the bulk runs on (SMs - R) while the look-ahead
@@ -396,7 +403,7 @@ static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) 
         const int64_t ncb = c1 - jn - nbn;
         int R = 0; int64_t nA = ncb;
         if (h.gemm_impl == 0 && h.reserve_sms != 0 && ncb > 0 && (sizeof(T) == 4 || reserve64)) {
-            const int64_t mk1 = m - jn;
+            const int64_t mk1 = men - jn;
             const int ibn = panel_ib_for<T>(h, mk1);
             const int Gp = ibn ? (int)ceil_div(mk1, (int64_t)kPanelThreads * panel_rpts<T>(ibn)[0]) : h.sms;
             R = h.reserve_sms > 0 ? h.reserve_sms : Gp + 2;
@@ -405,14 +412,14 @@ static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) 
             if (R > 0) {
                 const double t_panel = 0.25e-3 + 1.5e-8 * (double)mk1;                   // s, calibrated at c3 (flat optimum, both precisions)
                 const double rate = (sizeof(T) == 4 ? 69e12 : 25e12) * (double)(h.sms - R) / (double)h.sms;   // flop/s of the pair of products
-                nA = (int64_t)(t_panel * rate / (4.0 * (double)(m - j0) * nbw));
+                nA = (int64_t)(t_panel * rate / (4.0 * (double)(me - j0) * nbw));
                 nA = std::min<int64_t>(ncb, round_up(std::max<int64_t>(nA, 128), 128));
                 if (ncb - nA < 256) nA = ncb;
             }
         }
         T* Cb = A + j0 + (jn + nbn) * lda;
-        CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, Cb, lda, nA, true, R));
-        if (nA < ncb) CKI(larfb<T>(h, 0, h.sU, V, lda, m - j0, nbw, Tk, nb, Cb + nA * lda, lda, ncb - nA, true, 0));
+        CKI(larfb<T>(h, 0, h.sU, V, lda, me - j0, nbw, Tk, nb, Cb, lda, nA, true, R));
+        if (nA < ncb) CKI(larfb<T>(h, 0, h.sU, V, lda, me - j0, nbw, Tk, nb, Cb + nA * lda, lda, ncb - nA, true, 0));
     }
     CK(cudaStreamWaitEvent(h.sU, evP, 0));
     return 0;
@@ -539,7 +546,6 @@ static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
 
 template <typename T>
 static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
-    const int64_t m = h.m;
     const int nb = 128;
     if (!h.evP) { h.evP = new_event(h, false); h.evL = new_event(h, false); h.evU = new_event(h, false); }
     cudaEvent_t evP = h.evP, evL = h.evL, evU = h.evU;
@@ -548,6 +554,7 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
     // the look-ahead chain of one pair on sP: panel, narrow larfb onto the next panel's columns, panel, merge
     auto chain = [&](int64_t j0, int slot) -> int {
         const int k = (int)(j0 / nb);
+        const int64_t m = row_end(h, j0 + 2 * nb);          // row end of the pair (its first panel ends nb rows earlier: zeros)
         CKI(panel_factor<T>(h, h.sP, A, lda, m, j0, nb, k));
         CKI(larfb<T>(h, 1, h.sP, A + j0 + j0 * lda, lda, m - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
                      A + j0 + (j0 + nb) * lda, lda, nb));
@@ -562,6 +569,7 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
         const T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;
         const int64_t jn = j0 + 2 * nb;                     // first trailing column
         const int64_t rem = c1 - jn;
+        const int64_t m = row_end(h, jn);                   // row end of this pair
         CK(cudaStreamWaitEvent(h.sU, evP, 0));              // V, T2 of this pair ready
         if (rem < 2 * nb) {
             // no further full pair: finish this update, then the single-panel driver takes the tail
@@ -578,7 +586,7 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
         const int64_t ncb = rem - 2 * nb;
         int R = 0; int64_t nA = ncb;
         if (h.reserve_sms != 0 && ncb > 0) {
-            const int64_t mk1 = m - jn;
+            const int64_t mk1 = row_end(h, jn + 2 * nb) - jn;
             const int ibn = panel_ib_for<T>(h, mk1);
             const int Gp = ibn ? (int)ceil_div(mk1, (int64_t)kPanelThreads * panel_rpts<T>(ibn)[0]) : h.sms;
             R = h.reserve_sms > 0 ? h.reserve_sms : Gp + 2;
@@ -815,6 +823,32 @@ static int ensure_solve_ws(H& h, int64_t S) {
     return 0;
 }
 
+// opt->lower_bandwidth: the caller's promise A(i, j) == 0 for i - j > kl is checked before it is used
+// (one pass over the part of the matrix below the band; flag = first offending column)
+template <typename T>
+__global__ void band_check_kernel(const T* __restrict__ A, int64_t lda, int64_t m, int64_t n, int64_t kl, int* flag) {
+    for (int64_t j = blockIdx.x; j < n; j += gridDim.x) {
+        const T* col = A + j * lda;
+        bool bad = false;
+        for (int64_t i = kl + j + 1 + threadIdx.x; i < m; i += blockDim.x) bad |= (col[i] != T(0));
+        if (bad) atomicMin(flag, (int)j);
+    }
+}
+template <typename T>
+static int band_check(H& h, const T* A, int64_t lda) {
+    CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
+    band_check_kernel<T><<<(unsigned)std::min<int64_t>(h.n, (int64_t)h.sms * 8), 256, 0, h.sU>>>(A, lda, h.m, h.n, h.kl, h.dFlag);
+    CK(cudaGetLastError());
+    int flag = 0;
+    CK(cudaMemcpyAsync(&flag, h.dFlag, sizeof(int), cudaMemcpyDeviceToHost, h.sU));
+    CK(cudaStreamSynchronize(h.sU));
+    h.launches += 1;
+    if (flag < h.n)
+        return set_err(-6, "lower_bandwidth = %lld but column %d has a non-zero below row %lld",
+                       (long long)h.kl, flag, (long long)(h.kl + flag));
+    return 0;
+}
+
 // ------------------------------------------------------------------------------------------
 // ct_qr_factor
 // ------------------------------------------------------------------------------------------
@@ -835,6 +869,7 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
             CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
                                  cudaMemcpyDeviceToDevice, h.sU));
         }
+        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda));
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
     const size_t budget = o.device_budget_bytes > 0 ? (size_t)o.device_budget_bytes
@@ -848,9 +883,11 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
         CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
                              cudaMemcpyHostToDevice, h.sU));
         h.st.h2d_bytes = (double)bytes;
+        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda));
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
-    // out of core: budget = 2 super-panel buffers + 2 panel stream buffers
+    // out of core: budget = 2 super-panel buffers + 2 panel stream buffers (the band promise is not used here)
+    h.kl = 0;
     const int64_t lds = round_up(m, 16 / (int64_t)sizeof(T));
     const int64_t col_bytes = lds * (int64_t)sizeof(T);
     int64_t ns = ((int64_t)budget / col_bytes - 2 * h.nb) / 2;
@@ -912,8 +949,10 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
     if (!out) return set_err(-7, "out is NULL");
     ctqr_options_t o; memset(&o, 0, sizeof o); o.lookahead = -1;
     if (opt) o = *opt;
+    if (o.lower_bandwidth < 0) return set_err(-6, "lower_bandwidth < 0");
     H* h = nullptr;
     CKI(new_handle(dtype, m, n, o, &h));
+    h->kl = (o.lower_bandwidth > 0 && o.lower_bandwidth < m - 1) ? o.lower_bandwidth : 0;   // >= m-1: dense
     if (use_file) {
         // file tier: column-major m x n matrix with leading dimension lda at offset 0 of the file
         const size_t need = (size_t)lda * (size_t)n * h->w;
@@ -938,6 +977,14 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
     h->st.m = m; h->st.n = n; h->st.nb = h->nb; h->st.ib = h->ib; h->st.n_panels = h->P;
     h->st.n_superpanels = h->n_super; h->st.out_of_core = h->ooc ? 1 : 0; h->st.singular_col = -1;
     h->st.factor_flops = 2.0 * (double)m * (double)n * (double)n - 2.0 * (double)n * (double)n * (double)n / 3.0;
+    h->st.lower_bandwidth = h->kl;
+    h->st.factor_flops_performed = h->st.factor_flops;
+    if (h->kl > 0) {
+        // column j: a reflector of r_j = min(m, kl + j + 1) - j rows applied to the n - j - 1 trailing columns
+        double fl = 0;
+        for (int64_t j = 0; j < n; ++j) fl += 4.0 * (double)(std::min(m, h->kl + j + 1) - j) * (double)(n - j - 1);
+        h->st.factor_flops_performed = fl;
+    }
     h->st.kernel_launches = h->launches;
     h->factored = true;
     *out = h;
@@ -1000,7 +1047,7 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
     for (int k = 0; k < h.P; ++k) {
         const int64_t j0 = (int64_t)k * h.nb;
         const int nbw = (int)std::min<int64_t>(h.nb, h.n - j0);
-        CKI(larfb<T>(h, 0, h.sU, A + j0 + j0 * h.lda, h.lda, h.m - j0, nbw,
+        CKI(larfb<T>(h, 0, h.sU, A + j0 + j0 * h.lda, h.lda, row_end(h, j0 + nbw) - j0, nbw,
                      P_<T>(h.dT) + (size_t)k * h.nb * h.nb, h.nb, C + j0, ldc, S));
     }
     return 0;

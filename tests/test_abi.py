@@ -37,10 +37,10 @@ def test_every_declared_symbol_is_exported_and_bound(L):
 
 
 def test_struct_layouts_match_the_header():
-    # ctqr_options_t: 4 x int32, int64, 2 x int32, 2 pointers; ctqr_stats_t as declared
-    assert ctypes.sizeof(binding.Options) == 4 * 4 + 8 + 2 * 4 + 2 * 8
-    assert binding.Options.device_budget_bytes.offset == 16 and binding.Options.file_path.offset == 32
-    assert ctypes.sizeof(binding.Stats) == 2 * 8 + 6 * 4 + 9 * 8 + 8 + 2 * (8 + 8 + 8)
+    # ctqr_options_t: 4 x int32, int64, 2 x int32, 2 pointers, int64; ctqr_stats_t as declared
+    assert ctypes.sizeof(binding.Options) == 4 * 4 + 8 + 2 * 4 + 2 * 8 + 8
+    assert binding.Options.device_budget_bytes.offset == 16 and binding.Options.file_path.offset == 32 and binding.Options.lower_bandwidth.offset == 48
+    assert ctypes.sizeof(binding.Stats) == 2 * 8 + 6 * 4 + 9 * 8 + 8 + 2 * (8 + 8 + 8) + 2 * 8
     assert binding.Stats.factor_ms.offset == 40 and binding.Stats.vtc_ms.offset == 120
 
 

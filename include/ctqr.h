@@ -70,8 +70,8 @@ typedef struct {
                                    kl + (last column of the block) and the factorisation costs sum_j 4 r_j (n-j-1) flop,
                                    r_j = min(m, kl+j+1) - j, instead of 2mn^2 - 2n^3/3.  The result
                                    is the same factor (the skipped work is arithmetic on exact zeros).  The promise is
-                                   checked on the device first (-6 if violated).  Used by in-core factorisations; the
-                                   out-of-core path ignores it. */
+                                   checked on the device first (-6 if violated), per super-panel when out of core,
+                                   where it also shortens the reflector panels streamed over the host link. */
 } ctqr_options_t;
 
 /* Per-handle statistics (CUDA-event timed, milliseconds). */

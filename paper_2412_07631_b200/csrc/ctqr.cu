@@ -113,7 +113,7 @@ struct ctqr_handle_s {
         return tpool[tpool_used++];
     }
     bool factored = false;
-    // opt->lower_bandwidth (in-core factorisations only): A(i, j) == 0 for i - j > kl, so the reflectors of the
+    // opt->lower_bandwidth: A(i, j) == 0 for i - j > kl, so the reflectors of the
     // columns [.., jend) end at row min(m, kl + jend) and every product over rows stops there
     int64_t kl = 0;
     // out-of-core state
@@ -672,6 +672,8 @@ static int ensure_stream_bufs(H& h) {
     return 0;
 }
 
+template <typename T> static int band_check(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1);
+
 template <typename T>
 static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
     const int64_t m = h.m, n = h.n;
@@ -712,6 +714,7 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
         const int64_t c0 = (int64_t)s * ns, c1 = std::min<int64_t>(n, c0 + ns);
         T* Cv = sp[s & 1] - c0 * lds;                     // virtual base of SP_s
         CK(cudaStreamWaitEvent(h.sU, evIn[s], 0));
+        if (h.kl > 0) { rc = band_check<T>(h, Cv, lds, c0, c1); if (rc) break; }   // the promise, on the raw columns of SP_s
         // ---- earlier reflectors, streamed from the host (super-panels 0 .. s-2) ----
         const int kres = s >= 1 ? (int)(((int64_t)(s - 1) * ns) / nb) : 0;   // first panel of SP_{s-1}
         const int kcur = (int)(c0 / nb);
@@ -719,10 +722,11 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
             const int64_t j0 = (int64_t)k * nb;
             const int slot = k & 1;
             CK(cudaStreamWaitEvent(h.sC, evOut[(int)(j0 / ns)], 0));          // factor of that SP is on the host
-            rc = stream_panel_in<T>(h, slot, hA + j0 + j0 * hlda, hlda, m - j0, nb);
+            const int64_t mk = row_end(h, j0 + nb) - j0;                     // V_k is zero below (band promise)
+            rc = stream_panel_in<T>(h, slot, hA + j0 + j0 * hlda, hlda, mk, nb);
             if (rc) break;
             CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
-            rc = larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, m - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
+            rc = larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, mk, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
                           Cv + j0 + c0 * lds, lds, c1 - c0, true);
             CK(cudaEventRecord(h.evVfree[slot], h.sU));
         }
@@ -731,7 +735,7 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
             const T* Pv = sp[(s - 1) & 1] - (int64_t)(s - 1) * ns * lds;
             for (int k = kres; k < kcur && rc == 0; ++k) {
                 const int64_t j0 = (int64_t)k * nb;
-                rc = larfb<T>(h, 0, h.sU, Pv + j0 + j0 * lds, lds, m - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
+                rc = larfb<T>(h, 0, h.sU, Pv + j0 + j0 * lds, lds, row_end(h, j0 + nb) - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
                               Cv + j0 + c0 * lds, lds, c1 - c0, true);
             }
             CK(cudaEventRecord(evFree[s - 1], h.sU));
@@ -826,8 +830,9 @@ static int ensure_solve_ws(H& h, int64_t S) {
 // opt->lower_bandwidth: the caller's promise A(i, j) == 0 for i - j > kl is checked before it is used
 // (one pass over the part of the matrix below the band; flag = first offending column)
 template <typename T>
-__global__ void band_check_kernel(const T* __restrict__ A, int64_t lda, int64_t m, int64_t n, int64_t kl, int* flag) {
-    for (int64_t j = blockIdx.x; j < n; j += gridDim.x) {
+__global__ void band_check_kernel(const T* __restrict__ A, int64_t lda, int64_t m, int64_t c0, int64_t c1, int64_t kl, int* flag) {
+    // A is the virtual base: column j at A + j * lda, only c0 <= j < c1 is read
+    for (int64_t j = c0 + blockIdx.x; j < c1; j += gridDim.x) {
         const T* col = A + j * lda;
         bool bad = false;
         for (int64_t i = kl + j + 1 + threadIdx.x; i < m; i += blockDim.x) bad |= (col[i] != T(0));
@@ -835,9 +840,9 @@ __global__ void band_check_kernel(const T* __restrict__ A, int64_t lda, int64_t 
     }
 }
 template <typename T>
-static int band_check(H& h, const T* A, int64_t lda) {
+static int band_check(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1) {
     CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
-    band_check_kernel<T><<<(unsigned)std::min<int64_t>(h.n, (int64_t)h.sms * 8), 256, 0, h.sU>>>(A, lda, h.m, h.n, h.kl, h.dFlag);
+    band_check_kernel<T><<<(unsigned)std::min<int64_t>(c1 - c0, (int64_t)h.sms * 8), 256, 0, h.sU>>>(A, lda, h.m, c0, c1, h.kl, h.dFlag);
     CK(cudaGetLastError());
     int flag = 0;
     CK(cudaMemcpyAsync(&flag, h.dFlag, sizeof(int), cudaMemcpyDeviceToHost, h.sU));
@@ -869,7 +874,7 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
             CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
                                  cudaMemcpyDeviceToDevice, h.sU));
         }
-        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda));
+        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda, 0, h.n));
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
     const size_t budget = o.device_budget_bytes > 0 ? (size_t)o.device_budget_bytes
@@ -883,11 +888,10 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
         CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
                              cudaMemcpyHostToDevice, h.sU));
         h.st.h2d_bytes = (double)bytes;
-        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda));
+        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda, 0, h.n));
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
-    // out of core: budget = 2 super-panel buffers + 2 panel stream buffers (the band promise is not used here)
-    h.kl = 0;
+    // out of core: budget = 2 super-panel buffers + 2 panel stream buffers
     const int64_t lds = round_up(m, 16 / (int64_t)sizeof(T));
     const int64_t col_bytes = lds * (int64_t)sizeof(T);
     int64_t ns = ((int64_t)budget / col_bytes - 2 * h.nb) / 2;
@@ -1003,9 +1007,10 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
             const int64_t j0 = (int64_t)k * h.nb;
             const int nbw = (int)std::min<int64_t>(h.nb, h.n - j0);
             const int slot = k & 1;
-            CKI(stream_panel_in<T>(h, slot, hA + j0 + j0 * h.hlda, h.hlda, h.m - j0, nbw));
+            const int64_t mk = row_end(h, j0 + nbw) - j0;
+            CKI(stream_panel_in<T>(h, slot, hA + j0 + j0 * h.hlda, h.hlda, mk, nbw));
             CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
-            CKI(larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, h.m - j0, nbw,
+            CKI(larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, mk, nbw,
                          P_<T>(h.dT) + (size_t)k * h.nb * h.nb, h.nb, C + j0, ldc, S));
             CK(cudaEventRecord(h.evVfree[slot], h.sU));
         }
@@ -1024,6 +1029,7 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         a.sums = a.part + (size_t)2 * h.sms * h.nb * kSmallS;
         a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
         a.rpc = (int)ceil_div(nch, (int64_t)G) * kSmallChunk;
+        a.kl = h.kl;
         const size_t smem = ((size_t)h.nb * SmallLd<T>::T_ + 2 * (size_t)h.nb * SmallLd<T>::W + (size_t)kSmallS * (a.rpc + 4)) * sizeof(T);
         if (smem <= 220 * 1024) {
             static size_t cur = 0;
@@ -1420,12 +1426,21 @@ static int save_device_section(H& h, int fd, const void* dsrc, size_t bytes, voi
     return 0;
 }
 static int load_device_section(H& h, int fd, void* ddst, size_t bytes, void* bounce, const char* path) {
-    for (size_t off = 0; off < bytes; off += kIoChunkBytes) {
-        const size_t len = std::min(kIoChunkBytes, bytes - off);
-        CKI(read_all(fd, bounce, len, path));
-        CK(cudaMemcpyAsync((char*)ddst + off, bounce, len, cudaMemcpyHostToDevice, h.sU));
-        CK(cudaStreamSynchronize(h.sU));
+    // the two halves of the bounce buffer alternate: the file read of one chunk overlaps the H2D copy of the previous
+    const size_t half = kIoChunkBytes / 2;
+    cudaEvent_t done[2] = {new_event(h, false), new_event(h, false)};
+    bool busy[2] = {false, false};
+    int i = 0;
+    for (size_t off = 0; off < bytes; off += half, i ^= 1) {
+        const size_t len = std::min(half, bytes - off);
+        char* buf = (char*)bounce + (size_t)i * half;
+        if (busy[i]) CK(cudaEventSynchronize(done[i]));
+        CKI(read_all(fd, buf, len, path));
+        CK(cudaMemcpyAsync((char*)ddst + off, buf, len, cudaMemcpyHostToDevice, h.sU));
+        CK(cudaEventRecord(done[i], h.sU));
+        busy[i] = true;
     }
+    CK(cudaStreamSynchronize(h.sU));
     return 0;
 }
 

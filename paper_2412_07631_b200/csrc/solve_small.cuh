@@ -52,6 +52,7 @@ struct SmallQtArgs {
     uint4* sums;                    // [2][nb * kSmallS] LL slots: reduced W
     unsigned seq_base;              // step numbers seq_base + 1 .. seq_base + P are used by this launch
     int rpc;                        // local rows per CTA (multiple of kSmallChunk)
+    int64_t kl;                     // 0 = dense; > 0: V(i, j) == 0 for i - j > kl (opt->lower_bandwidth), rows below are skipped
 };
 
 template <typename T>
@@ -99,7 +100,9 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
         const int par = k & 1;
         const T* V = p.A + j0 * p.lda;                       // column c of the panel at V + c * lda, rows absolute
         const int la = first_local(j0);
-        const int na = nl - la;
+        // band promise (p.kl > 0): V_k is zero below row kl + j0 + kw, so the panel stops at local row le
+        const int le = p.kl > 0 ? min(nl, first_local(round_up(min(p.m, p.kl + j0 + kw), (int64_t)CH))) : nl;
+        const int na = le - la;
         unsigned long long ph_t0 = 0; (void)ph_t0;
         CTQR_PH(0)
         // ---- partial W[c][s] = sum over own rows of V[r, c] * B[r, s] ----
@@ -128,7 +131,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
 #pragma unroll
                 for (int u = 0; u < 4 * SM; ++u) acc[u] = T(0);
 #pragma unroll 2
-                for (int lr = la + lane; lr < nl; lr += 32) {
+                for (int lr = la + lane; lr < le; lr += 32) {
                     const int64_t row = row_of(lr);
                     T v[4];
 #pragma unroll
@@ -156,8 +159,9 @@ __global__ void __launch_bounds__(kSmallThreads, 1) apply_qt_small_kernel(SmallQ
         // ---- pull this CTA's slice of the next panel towards L2 while the exchange is in flight ----
         if (k + 1 < p.P) {
             const int la1 = first_local(j0 + NB);
+            const int le1 = p.kl > 0 ? min(nl, first_local(round_up(min(p.m, p.kl + j0 + 2 * NB), (int64_t)CH))) : nl;
             const T* vc = V + (int64_t)(NB + (tid & (NB - 1))) * p.lda;
-            for (int lr = la1 + (tid >> 7) * CH; lr < nl; lr += NQ * CH) {
+            for (int lr = la1 + (tid >> 7) * CH; lr < le1; lr += NQ * CH) {
                 const int64_t row = row_of(lr);
                 prefetch_l2(vc + row);
                 if (F64 && row + 8 < p.m) prefetch_l2(vc + row + 8);

@@ -110,3 +110,48 @@ def test_broken_promise_is_refused_and_wide_band_is_dense():
     f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), 350, 150, lower_bandwidth=349)   # no zero is promised
     st = f.stats()
     assert st["lower_bandwidth"] == 0 and st["factor_flops_performed"] == st["factor_flops"]
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("nb,ns,pinned", [(32, 160, True), (64, 128, False)])
+def test_out_of_core_uses_the_band(nb, ns, pinned, dt):
+    """Host-resident [A0; c I] with a capped device budget (a5): the promise is checked per super-panel, the
+    streamed reflector panels end at the band, so fewer bytes cross the host link than without the promise."""
+    m0, n, S = 420, 650, 9
+    m = m0 + n
+    rng = np.random.default_rng(8)
+    A = np.asfortranarray(augmented(rng, m0, n, dt))
+    B = np.asfortranarray(rng.standard_normal((m, S)).astype(dt))
+    w = np.dtype(dt).itemsize
+    lds = -(-m // (16 // w)) * (16 // w)
+    budget = (2 * ns + 2 * nb) * lds * w + 64
+    VR, tau_o = oracle.qr(A)
+    h2d = {}
+    for kl in (0, m0):
+        Ah = ctqr.colmajor_from_numpy(A, device="cpu", pin=pinned)
+        f = ctqr.ct_qr_factor(Ah, m, n, nb=nb, ib=16, device_budget_bytes=budget, lower_bandwidth=kl)
+        st = f.stats()
+        assert st["out_of_core"] == 1 and st["n_superpanels"] == -(-n // ns) and st["lower_bandwidth"] == kl
+        h2d[kl] = st["h2d_bytes"]
+        X = np.zeros((n, S), dtype=dt, order="F")
+        ctqr.ct_qr_solve(f, B, S, X)
+        assert relerr(X, oracle.solve(VR, tau_o, B)) <= SOLUTION[dt]
+        assert relerr(ctqr.ct_qr_get_R(f), oracle.R_of(VR)) <= ROUND[dt]
+        assert relerr(ctqr.ct_qr_get_V(f), oracle.V_of(VR)) <= ROUND[dt]
+        C = B.copy(order="F"); ctqr.ct_qr_apply_qt(f, C, S)
+        assert relerr(C, oracle.apply_qt(VR, tau_o, B)) <= ROUND[dt]
+        f.destroy()
+    assert h2d[m0] < 0.85 * h2d[0]
+
+
+def test_out_of_core_broken_promise_in_a_later_super_panel():
+    m0, n, nb, ns = 300, 400, 32, 128
+    rng = np.random.default_rng(9)
+    A = np.asfortranarray(augmented(rng, m0, n, np.float64))
+    A[m0 + n - 1, 300] = 0.5                            # column 300 lives in the third super-panel
+    lds = m0 + n
+    Ah = ctqr.colmajor_from_numpy(A, device="cpu", pin=True)
+    with pytest.raises(ctqr.CtqrError) as ei:
+        ctqr.ct_qr_factor(Ah, m0 + n, n, nb=nb, ib=16, device_budget_bytes=(2 * ns + 2 * nb) * lds * 8 + 64,
+                          lower_bandwidth=m0)
+    assert ei.value.code == -6 and "column 300" in str(ei.value)

@@ -28,7 +28,7 @@ from paper_2412_07631_b200 import workload as wl
 
 pytestmark = pytest.mark.gpu
 
-CFG = os.environ.get("CTQR_FULLSIZE", "c3")
+CFG = os.environ.get("CTQR_FULLSIZE", "c3")       # select one variant of a big config with -k "band and float32" etc.
 K_LEAD = 96
 
 
@@ -52,13 +52,13 @@ def sparse_aug(P, dt):
     return sp.vstack([A0, sl * sp.identity(c.n, format="csr")]).tocsr(), sl
 
 
-def run(P, dt):
+def run(P, dt, band=False):
     import torch
     c = P["c"]
     tdt = torch.float64 if dt == np.float64 else torch.float32
     At, lam = wl.dense_augmented_device(c, tdt, P["coo"])
     big = c.m * c.n * At.element_size() > 60e9            # no room for a second copy: factor in place
-    f = ctqr.ct_qr_factor(At, c.m, c.n, in_place=big)
+    f = ctqr.ct_qr_factor(At, c.m, c.n, in_place=big, lower_bandwidth=c.m0 if band else 0)
     if not big:
         del At
         torch.cuda.empty_cache()
@@ -76,14 +76,22 @@ def relerr(a, b):
 RESULTS = {}
 
 
+@pytest.mark.parametrize("band", [False, True], ids=["dense", "band"])
 @pytest.mark.parametrize("dt", [np.float64, np.float32])
-def test_fullsize_factor_and_solve(problem, dt):
+def test_fullsize_factor_and_solve(problem, dt, band):
+    """band: the same checks on the structure-aware factorisation (opt->lower_bandwidth = m0)."""
     P = problem
     c = P["c"]
     if c.m * c.n * np.dtype(dt).itemsize > 170e9:
         pytest.skip("does not fit the 180 GB of HBM in core; the out-of-core run needs the matrix in host RAM")
-    f, X = run(P, dt)
-    RESULTS[dt] = X
+    f, X = run(P, dt, band)
+    if band:
+        st = f.stats()
+        assert st["lower_bandwidth"] == c.m0 and st["factor_flops_performed"] < 0.75 * st["factor_flops"]
+        if dt in RESULTS:                                   # same factor => same solution as the dense path, to rounding
+            assert relerr(X, RESULTS[dt]) <= (1e-10 if dt == np.float64 else 5e-4)
+    else:
+        RESULTS[dt] = X
     tol_round = 1e-11 if dt == np.float64 else 5e-4
     # (i) leading columns against the oracle
     k = K_LEAD
@@ -124,7 +132,7 @@ def test_fullsize_factor_and_solve(problem, dt):
     lam_eff = sparse_aug(P, dt)[1] ** 2
     bound = np.linalg.norm(g) / lam_eff / np.linalg.norm(X64)
     opt = np.linalg.norm(g) / (np.linalg.norm(Aaug.data) * np.linalg.norm(B))
-    print(f"\n[{CFG} {np.dtype(dt).name}] R^T R vs A^T A {gram_err:.2e}; optimality residual {opt:.2e}; "
+    print(f"\n[{CFG} {np.dtype(dt).name}{' band' if band else ''}] R^T R vs A^T A {gram_err:.2e}; optimality residual {opt:.2e}; "
           f"certified ||x - x*||/||x|| <= {bound:.2e}; factor {f.stats()['factor_ms']:.1f} ms")
     if dt == np.float64:
         assert bound <= 1e-9, bound            # the north_star fp64 solution gate, certified

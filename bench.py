@@ -139,7 +139,8 @@ def quality(cfg, X0: np.ndarray, X: np.ndarray) -> dict:
             "psnr_db_min": float(np.min(ps)), "slices": int(X.shape[1])}
 
 
-def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do_e2e: bool = True) -> dict:
+def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do_e2e: bool = True,
+             structured: bool = False) -> dict:
     import torch
     import paper_2412_07631_b200 as ctqr
     dist = torch.distributed if world > 1 else None
@@ -152,9 +153,10 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     Bt = ctqr.colmajor_from_numpy(B.astype(npdt))
     Xt = torch.zeros((S, n), dtype=At.dtype, device="cuda")
     flops = cfg.factor_flops()
+    kl = (m - n) if structured else 0     # --structured: promise the identity block
 
     def one_step(profile: bool):
-        f = ctqr.ct_qr_factor(At, m, n, in_place=False, profile=profile)
+        f = ctqr.ct_qr_factor(At, m, n, in_place=False, profile=profile, lower_bandwidth=kl)
         factor_launches = f.stats()["kernel_launches"]      # the solve call restarts the counter
         ctqr.ct_qr_solve(f, Bt, S, Xt)
         st = f.stats()
@@ -175,6 +177,7 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     e0.record()
     stats = [one_step(True) for _ in range(steps)]
     e1.record()
+    flops = stats[0]["factor_flops_performed"] if structured else flops   # TFLOP/s on flops actually performed
     torch.cuda.synchronize()
     if dist:
         dist.barrier()
@@ -188,7 +191,7 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     # b_aug = A_aug x for a few phantoms, solved with one more factorisation outside the timed region
     Sc = min(8, S)
     X0c, Bc = wl.make_slices(cfg, S=Sc, coo=coo, lam=lam, consistent=True)
-    fq = ctqr.ct_qr_factor(At, m, n, in_place=False)
+    fq = ctqr.ct_qr_factor(At, m, n, in_place=False, lower_bandwidth=kl)
     Bct = ctqr.colmajor_from_numpy(Bc.astype(npdt))
     Xct = torch.zeros((Sc, n), dtype=At.dtype, device="cuda")
     ctqr.ct_qr_solve(fq, Bct, Sc, Xct)
@@ -209,7 +212,7 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
         "clocks": clocks,
         "quality_noisy": quality(cfg, X0, X),
         "quality_consistent": dict(quality(cfg, X0c, Xc), rel_error_vs_phantom=resid),
-        "nb": stats[-1]["nb"], "ib": stats[-1]["ib"],
+        "nb": stats[-1]["nb"], "ib": stats[-1]["ib"], "flops_per_factor": flops,
     }
     # roofline of the dominant kernel: the two contractions of the trailing update (a3)
     vt = {"ms": sum(s["vtc_ms"] for s in stats), "flops": sum(s["vtc_flops"] for s in stats),
@@ -218,7 +221,7 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
           "launches": sum(s["upd_launches"] for s in stats)}
     out["_spans"] = {"vtc": vt, "upd": up}
     if do_e2e and rank == 0:
-        out["e2e"] = run_e2e(cfg, dtype, At, B.astype(npdt), S, steps, flops)
+        out["e2e"] = run_e2e(cfg, dtype, At, B.astype(npdt), S, steps, flops, kl)
     elif do_e2e:
         out["e2e"] = None
     del At, Bt, Xt
@@ -226,7 +229,7 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     return out
 
 
-def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float) -> dict:
+def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float, kl: int = 0) -> dict:
     """Same metric through ct_qr_factor / ct_qr_solve with HOST buffers: every step copies A and
     B host->device and X device->host inside the timed region (the library does the copies)."""
     import torch
@@ -240,7 +243,7 @@ def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float
     def step():
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        f = ctqr.ct_qr_factor(Ah, m, n)
+        f = ctqr.ct_qr_factor(Ah, m, n, lower_bandwidth=kl)
         t1 = time.perf_counter()
         ctqr.ct_qr_solve(f, Bh, S, Xh)
         torch.cuda.synchronize()
@@ -255,7 +258,8 @@ def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float
     return {"value": flops / tf / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(m * n * w + m * S * w),
             "d2h_bytes_per_step": int(n * S * w), "factor_s": tf, "solve_s": tsol,
             "solve_slices_per_s": S / tsol, "steps": len(ts),
-            "note": "A, B, X in pinned host memory; wall clock around the synchronous C-ABI calls"}
+            "factor_s_steps": [round(a, 4) for a, _ in ts], "solve_s_steps": [round(b, 4) for _, b in ts],
+            "note": "A, B, X in pinned host memory; wall clock around the synchronous C-ABI calls; mean over the steps"}
 
 
 def run_extras(cfg, dtype: str) -> dict:
@@ -499,6 +503,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--short-warmup", action="store_true", help="honour --warmup < 3 (profiling runs under ncu only; not a valid bench number)")
+    ap.add_argument("--structured", action="store_true",
+                    help="promise the identity block of [A0; sqrt(lambda) I] (lower_bandwidth = m0): same factor, "
+                         "TFLOP/s on the flops actually performed; not the BASELINE.json headline")
     ap.add_argument("--no-extras", action="store_true", help="skip the solve S-sweep and the out-of-core run")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
@@ -525,11 +532,11 @@ def main():
     import paper_2412_07631_b200 as ctqr
 
     warm = args.warmup if args.short_warmup else max(args.warmup, 3)
-    res = run_ours(cfg, args.dtype, args.steps, warm, rank, world, do_e2e=not args.no_e2e)
+    res = run_ours(cfg, args.dtype, args.steps, warm, rank, world, do_e2e=not args.no_e2e, structured=args.structured)
     other = "f32" if args.dtype == "f64" else "f64"
     res2 = None
     if not args.no_also:
-        res2 = run_ours(cfg, other, args.steps, warm, rank, world, do_e2e=not args.no_e2e)
+        res2 = run_ours(cfg, other, args.steps, warm, rank, world, do_e2e=not args.no_e2e, structured=args.structured)
     if rank != 0:
         if world > 1:
             torch.distributed.destroy_process_group()
@@ -552,11 +559,14 @@ def main():
             "warmup": warm, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
             "config": {"workload": workload_name(cfg), "m": cfg.m, "n": cfg.n, "S": cfg.S, "nb": res["nb"],
-                       "ib": res["ib"], "flops_per_factor": cfg.factor_flops(),
+                       "ib": res["ib"], "flops_per_factor": res["flops_per_factor"],
+                       "lower_bandwidth": (cfg.m - cfg.n) if args.structured else 0,
                        "l2": "inputs larger than L2 (A is %.2f GB; every step re-reads it from HBM)"
                              % (cfg.m * cfg.n * (8 if args.dtype == "f64" else 4) / 1e9),
                        "parallelism": "1 GPU" if world == 1 else f"{world} replicas, slices sharded"},
-            "value_definition": "sum over timed steps of 2mn^2-2n^3/3 / device time of ct_qr_factor (A resident in HBM)",
+            "value_definition": ("sum over timed steps of the banded flop count sum_j 4 r_j (n-j-1) actually performed"
+                                 if args.structured else "sum over timed steps of 2mn^2-2n^3/3")
+                                + " / device time of ct_qr_factor (A resident in HBM)",
             "factor_ms_per_step": res["factor_ms_per_step"], "frac_of_peak_whole_factor": res["frac_of_peak_whole_factor"],
             "solve": res["solve"], "quality_noisy": res["quality_noisy"], "quality_consistent": res["quality_consistent"], "clocks": res["clocks"],
             "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],

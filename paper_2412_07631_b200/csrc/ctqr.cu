@@ -92,6 +92,7 @@ struct ctqr_handle_s {
     void* dW[2] = {nullptr, nullptr};  size_t w_elems[2] = {0, 0};
     // two-panel (256-wide) trailing updates: W / T^T W (256 x nc each), two merged T factors, merge scratch
     void* dW2[2] = {nullptr, nullptr}; size_t w2_elems = 0; void* dT2 = nullptr; void* dMerge = nullptr;
+    void* dCw = nullptr; size_t cw_bytes = 0;   // staging buffer of the solves (B in, X out), grow-only: no allocation per batch
     void* dPart = nullptr;             // LL slots of the panel kernel
     void* dLLs = nullptr; unsigned ll_seq = 0;   // LL slots / step numbers of the fused small-S solve kernels
     unsigned bar_count = 0;            // step numbers handed to the panel kernel (never reused)
@@ -130,7 +131,7 @@ struct ctqr_handle_s {
         if (ffd >= 0) close(ffd);
         cudaFree(dT); cudaFree(dRd); cudaFree(dRinv); cudaFree(dTau);
         for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); cudaFree(dW2[i]); }
-        cudaFree(dT2); cudaFree(dMerge);
+        cudaFree(dT2); cudaFree(dMerge); cudaFree(dCw);
         cudaFree(dPart); cudaFree(dLLs); cudaFree(dFlag); cudaFree(dTickets);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
@@ -1171,11 +1172,17 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
     bool inplace_dev = (mode == 1) && is_device_ptr(B);
     if (inplace_dev) { Cw = (T*)B; }
     else {
-        CK(cudaMalloc(&Cw, (size_t)ldw * S * sizeof(T)));
+        const size_t need = (size_t)ldw * S * sizeof(T);
+        if (need > h.cw_bytes) {                           // kept by the handle: later batches of the same size allocate nothing
+            cudaFree(h.dCw); h.dCw = nullptr; h.cw_bytes = 0;
+            if (cudaMalloc(&h.dCw, need) != cudaSuccess) { cudaGetLastError(); return set_err(CTQR_ERR_NOMEM, "cannot allocate %zu bytes for the right-hand sides", need); }
+            h.cw_bytes = need;
+        }
+        Cw = P_<T>(h.dCw);
         const bool bdev = is_device_ptr(B);
         cudaError_t e = cudaMemcpy2DAsync(Cw, ldw * sizeof(T), B, ldb * sizeof(T), rows_in * sizeof(T), S,
                                           bdev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h.sU);
-        if (e != cudaSuccess) { cudaFree(Cw); return set_err(CTQR_ERR_CUDA, "copy of B failed: %s", cudaGetErrorString(e)); }
+        if (e != cudaSuccess) return set_err(CTQR_ERR_CUDA, "copy of B failed: %s", cudaGetErrorString(e));
         if (!bdev) h.st.h2d_bytes += (double)rows_in * S * sizeof(T);
     }
     const int64_t ldcw = inplace_dev ? ldb : ldw;
@@ -1210,7 +1217,6 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
         h.st.apply_qt_ms = a; h.st.trsm_ms = b; h.st.solve_ms = a + b;
         h.st.kernel_launches = h.launches;
     }
-    if (!inplace_dev) cudaFree(Cw);
     return rc;
 }
 

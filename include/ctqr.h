@@ -134,7 +134,8 @@ void ct_qr_destroy(ctqr_handle_t h);
 /* Factor persistence ("factor once per geometry, reuse for every batch of slices").
  * ct_qr_save writes the whole factor of a factored handle (V\R storage, T_k, diagonal R blocks, tau;
  * in-core or out-of-core handle alike) to `path` (created / truncated; removed again on failure).
- * The file is self-describing (dtype, m, n, nb, ib) and holds m*n*w bytes plus O(n*nb*w).
+ * The file is self-describing (dtype, m, n, nb, ib, the lower_bandwidth the factor was computed under, which the
+ * solves of a loaded handle keep using) and holds m*n*w bytes plus O(n*nb*w).
  * ct_qr_load builds a handle from such a file without factoring: the factor is read into device
  * memory when it fits opt->device_budget_bytes (0 = free device memory), otherwise the file is mapped
  * read-only and ct_qr_solve streams its panels through the page cache (out-of-core solve, row a5).

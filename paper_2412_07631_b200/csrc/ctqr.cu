@@ -1396,6 +1396,7 @@ struct FactorFileHeader {
     int32_t version, dtype, nb, ib, P, reserved;
     int64_t m, n, ld;
     uint64_t off_matrix, off_T, off_Rd, off_tau, file_bytes;
+    int64_t kl;                       // band promise the factor was computed under (0 = dense); the solve reuses it
 };
 static const char kFactorMagic[8] = {'C', 'T', 'Q', 'R', 'F', 'A', 'C', '1'};
 constexpr size_t kFactorHeaderBytes = 4096;
@@ -1457,6 +1458,7 @@ static int save_body(H& h, int fd, const char* path, void* bounce) {
     memcpy(hd.magic, kFactorMagic, 8);
     hd.version = 1; hd.dtype = (int32_t)h.dtype; hd.nb = h.nb; hd.ib = h.ib; hd.P = h.P;
     hd.m = h.m; hd.n = h.n; hd.ld = round_up(h.m, 16 / (int64_t)w);
+    hd.kl = h.kl;
     hd.off_matrix = kFactorHeaderBytes;
     hd.off_T = hd.off_matrix + (uint64_t)hd.ld * h.n * w;
     hd.off_Rd = hd.off_T + (uint64_t)blk * h.P;
@@ -1574,6 +1576,7 @@ extern "C" int ct_qr_load(const char* path, const ctqr_options_t* opt, ctqr_hand
     H* h = nullptr;
     rc = new_handle((ctqr_dtype_t)hd.dtype, hd.m, hd.n, o, &h);
     if (rc != 0) { close(fd); return rc; }
+    h->kl = (hd.kl > 0 && hd.kl < hd.m - 1) ? hd.kl : 0;
     void* bounce = nullptr;
     if (cudaMallocHost(&bounce, kIoChunkBytes) != cudaSuccess) {
         cudaGetLastError(); close(fd); delete h;
@@ -1586,6 +1589,7 @@ extern "C" int ct_qr_load(const char* path, const ctqr_options_t* opt, ctqr_hand
     if (h->fmap) h->ffd = fd; else close(fd);  // the mapping keeps the file open for the handle's lifetime
     h->st.m = hd.m; h->st.n = hd.n; h->st.nb = h->nb; h->st.ib = h->ib; h->st.n_panels = h->P;
     h->st.n_superpanels = h->n_super; h->st.out_of_core = h->ooc ? 1 : 0; h->st.singular_col = -1;
+    h->st.lower_bandwidth = h->kl;
     h->st.factor_flops = 2.0 * (double)hd.m * (double)hd.n * (double)hd.n - 2.0 * (double)hd.n * (double)hd.n * (double)hd.n / 3.0;
     h->factored = true;
     *out = h;

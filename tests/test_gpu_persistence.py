@@ -157,3 +157,28 @@ def test_load_rejects_truncated_and_foreign_files(tmp_path):
     with pytest.raises(ctqr.CtqrError) as ei:          # unwritable destination: nothing is left behind
         ctqr.ct_qr_save(f, str(tmp_path / "no_such_dir" / "f.ctqr"))
     assert ei.value.code == 3
+
+
+@pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("streamed", [False, True])
+def test_band_promise_travels_with_the_file(tmp_path, dt, streamed):
+    """A factor computed under opt->lower_bandwidth keeps it across save / load: the reloaded handle reports it
+    and its solves (which stop every panel at the band) still match the dense oracle."""
+    m0, n, S = 500, 700, 10
+    rng = np.random.default_rng(12)
+    A0 = rng.standard_normal((m0, n)) * (rng.random((m0, n)) < 0.3)
+    A = np.asfortranarray(np.vstack([A0, 0.4 * np.eye(n)]).astype(dt))
+    B = np.asfortranarray(rng.standard_normal((m0 + n, S)).astype(dt))
+    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m0 + n, n, lower_bandwidth=m0)
+    ref = factor_parts(f)
+    path = str(tmp_path / "band.ctqr")
+    ctqr.ct_qr_save(f, path)
+    f.destroy()
+    g = ctqr.ct_qr_load(path, device_budget_bytes=streamed_budget(m0 + n, 128, dt) if streamed else 0)
+    st = g.stats()
+    assert st["lower_bandwidth"] == m0 and st["out_of_core"] == int(streamed)
+    assert_same_factor(ref, factor_parts(g))
+    VR, tau_o = oracle.qr(A)
+    for s_cols in (3, S):                               # fused small-S kernel (in core) and the per-panel path
+        X = solve(g, B[:, :s_cols], dt)
+        assert relerr(X, oracle.solve(VR, tau_o, B[:, :s_cols])) <= SOLUTION[dt]

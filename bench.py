@@ -155,8 +155,11 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     flops = cfg.factor_flops()
     kl = (m - n) if structured else 0     # --structured: promise the identity block
 
+    Aw = torch.empty_like(At)             # working copy, factored in place: no 4 GB cudaMalloc / cudaFree inside a step
+
     def one_step(profile: bool):
-        f = ctqr.ct_qr_factor(At, m, n, in_place=False, profile=profile, lower_bandwidth=kl)
+        Aw.copy_(At)                      # (device-to-device, part of the step; ct_qr_factor orders itself after it)
+        f = ctqr.ct_qr_factor(Aw, m, n, in_place=True, profile=profile, lower_bandwidth=kl)
         factor_launches = f.stats()["kernel_launches"]      # the solve call restarts the counter
         ctqr.ct_qr_solve(f, Bt, S, Xt)
         st = f.stats()
@@ -224,7 +227,7 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
         out["e2e"] = run_e2e(cfg, dtype, At, B.astype(npdt), S, steps, flops, kl)
     elif do_e2e:
         out["e2e"] = None
-    del At, Bt, Xt
+    del At, Aw, Bt, Xt
     torch.cuda.empty_cache()
     return out
 

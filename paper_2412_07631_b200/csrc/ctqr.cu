@@ -13,7 +13,10 @@
 #include <unistd.h>
 #include <string.h>
 #include <algorithm>
+#include <map>
+#include <mutex>
 #include <new>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/ctqr.h"
@@ -73,6 +76,78 @@ extern "C" const char* ct_qr_strerror(int code) {
 extern "C" int ct_qr_version(void) { return 100; }
 
 // ------------------------------------------------------------------------------------------
+// Process-wide cache of the small per-handle device buffers (T, tau, workspaces, LL slots, the solve
+// staging buffer; not the matrix storage, not the super-panel buffers).  cudaMalloc / cudaFree cost
+// 0.1 - 100 ms each and cudaFree synchronises the device; a service that factors or reloads one
+// geometry after another would pay that for ~20 buffers per handle.  Blocks of
+// at most kCacheMaxBlock bytes go back to a size-ordered free list (at most kCacheMaxTotal bytes are
+// kept) and are handed out again to the next request of up to half their size; contents are
+// unspecified, as after cudaMalloc.  Callers free only buffers no kernel is using (handles are
+// destroyed after a device synchronise, workspaces are replaced between synchronous calls).
+// ------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t kCacheMaxBlock = (size_t)256 << 20, kCacheMaxTotal = (size_t)1 << 30;
+struct DevCache {
+    std::mutex mu;
+    std::multimap<uint64_t, void*> free_;          // key = device << 32 | bytes  (bytes <= 256 MiB)
+    std::unordered_map<void*, uint64_t> key_;      // every block this cache may take back
+    size_t cached = 0;
+} g_cache;
+}
+static cudaError_t dev_alloc_raw(void** p, size_t bytes) {
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e == cudaSuccess) return e;
+    cudaGetLastError();
+    std::vector<void*> drop;                        // out of memory: give the cached blocks back and retry once
+    {
+        std::lock_guard<std::mutex> lk(g_cache.mu);
+        for (auto& kv : g_cache.free_) { drop.push_back(kv.second); g_cache.key_.erase(kv.second); }
+        g_cache.free_.clear(); g_cache.cached = 0;
+    }
+    if (drop.empty()) return e;
+    for (void* q : drop) cudaFree(q);
+    return cudaMalloc(p, bytes);
+}
+template <typename P>
+static cudaError_t dev_alloc(P** p, size_t bytes) {
+    void* q = nullptr;
+    int dev = 0; cudaGetDevice(&dev);
+    if (bytes > 0 && bytes <= kCacheMaxBlock) {
+        std::lock_guard<std::mutex> lk(g_cache.mu);
+        auto it = g_cache.free_.lower_bound(((uint64_t)dev << 32) | bytes);
+        if (it != g_cache.free_.end() && (it->first >> 32) == (uint64_t)dev && (it->first & 0xffffffffu) <= 2 * bytes + 4096) {
+            q = it->second; g_cache.cached -= (size_t)(it->first & 0xffffffffu); g_cache.free_.erase(it);
+            *p = (P*)q;
+            return cudaSuccess;
+        }
+    }
+    cudaError_t e = dev_alloc_raw(&q, bytes);
+    if (e != cudaSuccess) return e;
+    if (q && bytes <= kCacheMaxBlock) {
+        std::lock_guard<std::mutex> lk(g_cache.mu);
+        g_cache.key_[q] = ((uint64_t)dev << 32) | bytes;
+    }
+    *p = (P*)q;
+    return cudaSuccess;
+}
+static void dev_free(void* p) {
+    if (!p) return;
+    {
+        std::lock_guard<std::mutex> lk(g_cache.mu);
+        auto it = g_cache.key_.find(p);
+        if (it != g_cache.key_.end()) {
+            const size_t bytes = (size_t)(it->second & 0xffffffffu);
+            if (g_cache.cached + bytes <= kCacheMaxTotal) {
+                g_cache.free_.emplace(it->second, p); g_cache.cached += bytes;
+                return;
+            }
+            g_cache.key_.erase(it);
+        }
+    }
+    cudaFree(p);
+}
+
+// ------------------------------------------------------------------------------------------
 // handle
 // ------------------------------------------------------------------------------------------
 struct ctqr_handle_s {
@@ -129,10 +204,10 @@ struct ctqr_handle_s {
         if (own_A && dA) cudaFree(dA);
         if (fmap) { msync(fmap, fmap_len, MS_SYNC); munmap(fmap, fmap_len); }
         if (ffd >= 0) close(ffd);
-        cudaFree(dT); cudaFree(dRd); cudaFree(dRinv); cudaFree(dTau);
-        for (int i = 0; i < 2; ++i) { cudaFree(dWp[i]); cudaFree(dW[i]); cudaFree(dW2[i]); }
-        cudaFree(dT2); cudaFree(dMerge); cudaFree(dCw);
-        cudaFree(dPart); cudaFree(dLLs); cudaFree(dFlag); cudaFree(dTickets);
+        dev_free(dT); dev_free(dRd); dev_free(dRinv); dev_free(dTau);
+        for (int i = 0; i < 2; ++i) { dev_free(dWp[i]); dev_free(dW[i]); dev_free(dW2[i]); }
+        dev_free(dT2); dev_free(dMerge); dev_free(dCw);
+        dev_free(dPart); dev_free(dLLs); dev_free(dFlag); dev_free(dTickets);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
         for (auto e : tpool) cudaEventDestroy(e);
@@ -140,7 +215,7 @@ struct ctqr_handle_s {
         if (sP) cudaStreamDestroy(sP);
         if (sC) cudaStreamDestroy(sC);
         if (sD) cudaStreamDestroy(sD);
-        for (int i = 0; i < 2; ++i) cudaFree(dVb[i]);
+        for (int i = 0; i < 2; ++i) dev_free(dVb[i]);
     }
 };
 typedef ctqr_handle_s H;
@@ -442,14 +517,14 @@ template <typename T>
 static int ensure_pair_ws(H& h, int64_t nc) {
     const size_t need = (size_t)256 * (size_t)nc;
     if (h.dW2[0] && h.w2_elems >= need) return 0;
-    for (int i = 0; i < 2; ++i) { if (h.dW2[i]) cudaFree(h.dW2[i]); h.dW2[i] = nullptr; }
+    for (int i = 0; i < 2; ++i) { if (h.dW2[i]) dev_free(h.dW2[i]); h.dW2[i] = nullptr; }
     for (int i = 0; i < 2; ++i)
-        if (cudaMalloc(&h.dW2[i], need * sizeof(T)) != cudaSuccess) { cudaGetLastError(); h.w2_elems = 0; return 1; }
+        if (dev_alloc(&h.dW2[i], need * sizeof(T)) != cudaSuccess) { cudaGetLastError(); h.w2_elems = 0; return 1; }
     h.w2_elems = need;
     if (!h.dT2) {
-        if (cudaMalloc(&h.dT2, (size_t)2 * 256 * 256 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
+        if (dev_alloc(&h.dT2, (size_t)2 * 256 * 256 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
         CK(cudaMemsetAsync(h.dT2, 0, (size_t)2 * 256 * 256 * sizeof(T), h.sU));
-        if (cudaMalloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
+        if (dev_alloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
     }
     return 0;
 }
@@ -661,7 +736,7 @@ static int ensure_stream_bufs(H& h) {
     if (h.dVb[0]) return 0;
     h.ldvb = round_up(h.m, 16 / (int64_t)h.w);
     for (int i = 0; i < 2; ++i) {
-        if (cudaMalloc(&h.dVb[i], (size_t)h.ldvb * h.nb * h.w) != cudaSuccess) {
+        if (dev_alloc(&h.dVb[i], (size_t)h.ldvb * h.nb * h.w) != cudaSuccess) {
             cudaGetLastError();
             return set_err(CTQR_ERR_NOMEM, "cannot allocate the panel stream buffers");
         }
@@ -779,12 +854,12 @@ template <typename T>
 static int alloc_state(H& h, int64_t max_nc) {
     const int nb = h.nb;
     const size_t blk = (size_t)nb * nb;
-    CK(cudaMalloc(&h.dT, blk * h.P * sizeof(T)));
-    CK(cudaMalloc(&h.dRd, blk * h.P * sizeof(T)));
+    CK(dev_alloc(&h.dT, blk * h.P * sizeof(T)));
+    CK(dev_alloc(&h.dRd, blk * h.P * sizeof(T)));
     CK(cudaMemsetAsync(h.dT, 0, blk * h.P * sizeof(T), h.sU));
     CK(cudaMemsetAsync(h.dRd, 0, blk * h.P * sizeof(T), h.sU));
-    CK(cudaMalloc(&h.dTau, (size_t)h.n * sizeof(T)));
-    if (nb == 128) CK(cudaMalloc(&h.dRinv, blk * h.P * sizeof(T)));
+    CK(dev_alloc(&h.dTau, (size_t)h.n * sizeof(T)));
+    if (nb == 128) CK(dev_alloc(&h.dRinv, blk * h.P * sizeof(T)));
     const int64_t slots = (int64_t)h.sms * 2;
     // [0]: trailing update / solve; [1]: in-panel work
     h.w_elems[0] = (size_t)nb * (size_t)max_nc;
@@ -792,21 +867,21 @@ static int alloc_state(H& h, int64_t max_nc) {
     h.w_elems[1] = (size_t)nb * nb;
     h.wp_elems[1] = (size_t)nb * 128 * (size_t)slots;
     for (int i = 0; i < 2; ++i) {
-        CK(cudaMalloc(&h.dW[i], h.w_elems[i] * sizeof(T)));
-        CK(cudaMalloc(&h.dWp[i], h.wp_elems[i] * sizeof(T)));
+        CK(dev_alloc(&h.dW[i], h.w_elems[i] * sizeof(T)));
+        CK(dev_alloc(&h.dWp[i], h.wp_elems[i] * sizeof(T)));
     }
     // LL slots of the panel kernel: [2 parities][G + 1 <= 257][IB <= 32] x 16 bytes, step numbers start at 1
-    CK(cudaMalloc(&h.dPart, (size_t)2 * 257 * 32 * 16));
+    CK(dev_alloc(&h.dPart, (size_t)2 * 257 * 32 * 16));
     CK(cudaMemsetAsync(h.dPart, 0, (size_t)2 * 257 * 32 * 16, h.sU));
-    CK(cudaMalloc(&h.dFlag, sizeof(int)));
-    CK(cudaMalloc(&h.dTickets, (size_t)kTicketRing * 2 * sizeof(unsigned)));
+    CK(dev_alloc(&h.dFlag, sizeof(int)));
+    CK(dev_alloc(&h.dTickets, (size_t)kTicketRing * 2 * sizeof(unsigned)));
     CK(cudaMemsetAsync(h.dTickets, 0, (size_t)kTicketRing * 2 * sizeof(unsigned), h.sU));
     h.ticket_pos = 0;
     if (nb == 128) {
         // fused small-S solve: [2][sms][nb * kSmallS] partial slots + [2][nb * kSmallS] sum slots (Q^T B),
         // then [P][nb * kSmallS] slots of the fused TRSM, 16 bytes each
         const size_t lls = ((size_t)2 * h.sms + 2 + h.P) * nb * kSmallS * 16;
-        CK(cudaMalloc(&h.dLLs, lls));
+        CK(dev_alloc(&h.dLLs, lls));
         CK(cudaMemsetAsync(h.dLLs, 0, lls, h.sU));
     }
     h.bar_count = 0;
@@ -818,12 +893,12 @@ static int ensure_solve_ws(H& h, int64_t S) {
     const size_t need_w = (size_t)h.nb * (size_t)S;
     const size_t need_wp = (size_t)h.nb * (size_t)(S + 128 * (int64_t)h.sms * 2);
     if (need_w > h.w_elems[0]) {
-        cudaFree(h.dW[0]); h.dW[0] = nullptr;
-        CK(cudaMalloc(&h.dW[0], need_w * h.w)); h.w_elems[0] = need_w;
+        dev_free(h.dW[0]); h.dW[0] = nullptr;
+        CK(dev_alloc(&h.dW[0], need_w * h.w)); h.w_elems[0] = need_w;
     }
     if (need_wp > h.wp_elems[0]) {
-        cudaFree(h.dWp[0]); h.dWp[0] = nullptr;
-        CK(cudaMalloc(&h.dWp[0], need_wp * h.w)); h.wp_elems[0] = need_wp;
+        dev_free(h.dWp[0]); h.dWp[0] = nullptr;
+        CK(dev_alloc(&h.dWp[0], need_wp * h.w)); h.wp_elems[0] = need_wp;
     }
     return 0;
 }
@@ -1174,8 +1249,8 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
     else {
         const size_t need = (size_t)ldw * S * sizeof(T);
         if (need > h.cw_bytes) {                           // kept by the handle: later batches of the same size allocate nothing
-            cudaFree(h.dCw); h.dCw = nullptr; h.cw_bytes = 0;
-            if (cudaMalloc(&h.dCw, need) != cudaSuccess) { cudaGetLastError(); return set_err(CTQR_ERR_NOMEM, "cannot allocate %zu bytes for the right-hand sides", need); }
+            dev_free(h.dCw); h.dCw = nullptr; h.cw_bytes = 0;
+            if (dev_alloc(&h.dCw, need) != cudaSuccess) { cudaGetLastError(); return set_err(CTQR_ERR_NOMEM, "cannot allocate %zu bytes for the right-hand sides", need); }
             h.cw_bytes = need;
         }
         Cw = P_<T>(h.dCw);

@@ -10,8 +10,15 @@ HBM); the solve part of the same steps is reported as `solve.slices_per_s`; `ms_
 the whole step.  `e2e` is the same metric through the same C-ABI calls with HOST (pinned)
 buffers, host<->device copies inside the timed region.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--dtype f64|f32]
-                    [--impl ours|reference] [--no-also]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--dtype f64|f32]
+                    [--impl ours|reference] [--no-also] [--time-budget SECONDS]
+
+The default workload is BASELINE.json configs[3] (m = 109096, n = 65536: 57 GB fp64 in core), the
+largest config whose K + W steps fit the driver's window in both precisions; configs[4] (m = 245376,
+n = 147456) is one factorisation of 110 s or more, so it is run once, in fp32, out of core from
+pinned host memory with a capped device budget, as `extras.out_of_core`.  Every optional leg (second
+precision, e2e, extras, CPU baseline) is sized against --time-budget (seconds of wall time for the
+whole run, default 1500) and says in its block what it ran.
 
 N > 1 (torchrun): the factorisation does not shard on one node without an exchange step
 (DESIGN.md "Multi-GPU"): every rank factors its own replica of A and solves its own S/N share
@@ -139,8 +146,32 @@ def quality(cfg, X0: np.ndarray, X: np.ndarray) -> dict:
             "psnr_db_min": float(np.min(ps)), "slices": int(X.shape[1])}
 
 
-def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do_e2e: bool = True,
-             structured: bool = False) -> dict:
+T_START = time.perf_counter()
+
+
+class Budget:
+    """Wall-time budget of the whole run: optional legs ask before they start."""
+    def __init__(self, seconds: float):
+        self.seconds = float(seconds)
+
+    def left(self) -> float:
+        return self.seconds - (time.perf_counter() - T_START)
+
+    def allows(self, cost_s: float) -> bool:
+        return self.left() >= cost_s
+
+
+def pinned_like(t):
+    """Pinned host copy of a device tensor (one cudaHostAlloc + one D2H copy; no pageable detour)."""
+    import torch
+    h = torch.empty(t.shape, dtype=t.dtype, pin_memory=True)
+    h.copy_(t)
+    torch.cuda.synchronize()
+    return h
+
+
+def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, budget: Budget, do_e2e: bool = True,
+             structured: bool = False, do_sweep: bool = False, e2e_steps: int = 3) -> dict:
     import torch
     import paper_2412_07631_b200 as ctqr
     dist = torch.distributed if world > 1 else None
@@ -150,24 +181,38 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     s_lo, S = wl.shard_slices(S_all, rank, world)
     At, X0, B, coo, lam = build_inputs(cfg, dtype, S, s_lo)
     m, n = cfg.m, cfg.n
+    w = At.element_size()
     Bt = ctqr.colmajor_from_numpy(B.astype(npdt))
     Xt = torch.zeros((S, n), dtype=At.dtype, device="cuda")
     flops = cfg.factor_flops()
     kl = (m - n) if structured else 0     # --structured: promise the identity block
 
-    Aw = torch.empty_like(At)             # working copy, factored in place: no 4 GB cudaMalloc / cudaFree inside a step
+    Aw = torch.empty_like(At)             # working copy, factored in place: no cudaMalloc / cudaFree of the matrix inside a step
 
-    def one_step(profile: bool):
+    def one_step(profile: bool, keep: bool = False):
         Aw.copy_(At)                      # (device-to-device, part of the step; ct_qr_factor orders itself after it)
         f = ctqr.ct_qr_factor(Aw, m, n, in_place=True, profile=profile, lower_bandwidth=kl)
         factor_launches = f.stats()["kernel_launches"]      # the solve call restarts the counter
         ctqr.ct_qr_solve(f, Bt, S, Xt)
         st = f.stats()
         st["launches_step"] = factor_launches + st["kernel_launches"]
+        if keep:
+            return st, f
         f.destroy()
-        return st
+        return st, None
 
-    for _ in range(max(warmup, 0)):
+    # the first warm-up step is wall-clocked: if W + K steps of this size cannot fit the share of the
+    # time budget given to this precision, K is cut (never below 1) and the line says so
+    t0 = time.perf_counter()
+    if warmup > 0:
+        one_step(False)
+    torch.cuda.synchronize()
+    t_step = time.perf_counter() - t0
+    share = 0.55 * budget.seconds if do_sweep else 0.12 * budget.seconds
+    steps_req = steps
+    if warmup > 0 and (warmup + steps) * t_step > share:
+        steps = int(max(1, min(steps, share / t_step - warmup)))
+    for _ in range(max(warmup - 1, 0)):
         one_step(False)
     torch.cuda.synchronize()
     if dist:
@@ -178,7 +223,10 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record()
-    stats = [one_step(True) for _ in range(steps)]
+    stats, f_last = [], None
+    for i in range(steps):
+        st, f_last = one_step(True, keep=(i == steps - 1))
+        stats.append(st)
     e1.record()
     flops = stats[0]["factor_flops_performed"] if structured else flops   # TFLOP/s on flops actually performed
     torch.cuda.synchronize()
@@ -191,14 +239,12 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     launches = sum(s["launches_step"] for s in stats)
     X = ctqr.numpy_from_colmajor(Xt)
     # the paper's regime (Tables 3, 7, 9: consistent systems, quality limited by the arithmetic only):
-    # b_aug = A_aug x for a few phantoms, solved with one more factorisation outside the timed region
+    # b_aug = A_aug x for a few phantoms, solved with the factor of the last timed step
     Sc = min(8, S)
     X0c, Bc = wl.make_slices(cfg, S=Sc, coo=coo, lam=lam, consistent=True)
-    fq = ctqr.ct_qr_factor(At, m, n, in_place=False, lower_bandwidth=kl)
     Bct = ctqr.colmajor_from_numpy(Bc.astype(npdt))
     Xct = torch.zeros((Sc, n), dtype=At.dtype, device="cuda")
-    ctqr.ct_qr_solve(fq, Bct, Sc, Xct)
-    fq.destroy()
+    ctqr.ct_qr_solve(f_last, Bct, Sc, Xct)
     Xc = ctqr.numpy_from_colmajor(Xct)
     resid = float(np.linalg.norm(Xc.astype(np.float64) - X0c) / np.linalg.norm(X0c))
     t = torch.tensor([total_ms, factor_ms, solve_ms], dtype=torch.float64, device="cuda")
@@ -207,10 +253,12 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     total_ms, factor_ms, solve_ms = (float(x) for x in t.tolist())
     out = {
         "value": world * steps * flops / (factor_ms * 1e-3) / 1e12,
+        "steps": steps, "steps_requested": steps_req,
         "ms_per_step": total_ms / steps,
         "factor_ms_per_step": factor_ms / steps,
         "solve": {"S": S_all, "ms_per_batch": solve_ms / steps, "slices_per_s": S_all * steps / (solve_ms * 1e-3),
-                  "apply_qt_ms": stats[-1]["apply_qt_ms"], "trsm_ms": stats[-1]["trsm_ms"]},
+                  "apply_qt_ms": stats[-1]["apply_qt_ms"], "trsm_ms": stats[-1]["trsm_ms"],
+                  "tflops": cfg.solve_flops(S_all) * steps / (solve_ms * 1e-3) / 1e12},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "quality_noisy": quality(cfg, X0, X),
@@ -223,22 +271,36 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, do
     up = {"ms": sum(s["upd_ms"] for s in stats), "flops": sum(s["upd_flops"] for s in stats),
           "launches": sum(s["upd_launches"] for s in stats)}
     out["_spans"] = {"vtc": vt, "upd": up}
+    del Bct, Xct
+    if do_sweep and rank == 0 and world == 1:
+        out["_extras"] = run_resident_extras(cfg, dtype, f_last, At, Aw, B, budget, factor_ms / steps, structured)
+    f_last.destroy()
     if do_e2e and rank == 0:
-        out["e2e"] = run_e2e(cfg, dtype, At, B.astype(npdt), S, steps, flops, kl)
+        per = t_step * 1.15 + 2.0
+        k = int(max(0, min(e2e_steps, (budget.left() - 0.35 * budget.seconds) / per - 1))) if do_sweep else \
+            int(max(0, min(e2e_steps, (budget.left() - 0.30 * budget.seconds) / per - 1)))
+        if k >= 1:
+            Ah = pinned_like(At)
+            del At, Aw
+            torch.cuda.empty_cache()
+            out["e2e"] = run_e2e(cfg, dtype, Ah, B.astype(npdt), S, k, flops, kl)
+            del Ah
+        else:
+            out["e2e"] = None
+            out["e2e_skipped"] = "time budget"
     elif do_e2e:
         out["e2e"] = None
-    del At, Aw, Bt, Xt
+    At = Aw = Bt = Xt = None
     torch.cuda.empty_cache()
     return out
 
 
-def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float, kl: int = 0) -> dict:
+def run_e2e(cfg, dtype: str, Ah, B: np.ndarray, S: int, steps: int, flops: float, kl: int = 0) -> dict:
     """Same metric through ct_qr_factor / ct_qr_solve with HOST buffers: every step copies A and
     B host->device and X device->host inside the timed region (the library does the copies)."""
     import torch
     import paper_2412_07631_b200 as ctqr
     m, n = cfg.m, cfg.n
-    Ah = At.cpu().pin_memory()
     Bh = torch.from_numpy(np.ascontiguousarray(B.T)).pin_memory()
     Xh = torch.zeros((S, n), dtype=Ah.dtype).pin_memory()
     w = Ah.element_size()
@@ -255,37 +317,38 @@ def run_e2e(cfg, dtype: str, At, B: np.ndarray, S: int, steps: int, flops: float
         return t1 - t0, t2 - t1
 
     step()
-    ts = [step() for _ in range(max(1, min(steps, 3)))]
+    ts = [step() for _ in range(max(1, steps))]
     tf = sum(a for a, _ in ts) / len(ts)
     tsol = sum(b for _, b in ts) / len(ts)
     return {"value": flops / tf / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(m * n * w + m * S * w),
             "d2h_bytes_per_step": int(n * S * w), "factor_s": tf, "solve_s": tsol,
             "solve_slices_per_s": S / tsol, "steps": len(ts),
             "factor_s_steps": [round(a, 4) for a, _ in ts], "solve_s_steps": [round(b, 4) for _, b in ts],
-            "note": "A, B, X in pinned host memory; wall clock around the synchronous C-ABI calls; mean over the steps"}
+            "note": "A, B, X in pinned host memory; wall clock around the synchronous C-ABI calls (one untimed "
+                    "warm-up call first); mean over the steps"}
 
 
-def run_extras(cfg, dtype: str) -> dict:
-    """The other rooflines north_star asks evidence for, on the same workload (rank 0, N = 1):
-    solve S-sweep (Fig. 1: throughput rises with the number of slices solved at
-    once; small S is bound by reading the factor from HBM, m*n*w bytes per batch) and the
-    out-of-core path from pinned host memory with the device budget capped at a quarter of the
-    matrix (achieved host-link GB/s, time against the in-core factorisation)."""
+SWEEP_S = (1, 8, 64, 256, 512, 1024, 2048)       # PAPER.md:L89, Fig. 1 (L117-130): up to 2048 simultaneous slices
+
+
+def run_resident_extras(cfg, dtype: str, f, At, Aw, B: np.ndarray, budget: Budget, incore_ms: float, structured: bool) -> dict:
+    """Legs that reuse the resident factor of the last timed step (rank 0, N = 1):
+    solve S-sweep (PAPER.md Fig. 1, L117-130: throughput rises with the number of slices solved at once;
+    small S is bound by reading the factor from HBM, m*n*w bytes per batch), then -- after that factor is
+    dropped -- the structure-aware factorisation of the same matrix."""
     import torch
     import paper_2412_07631_b200 as ctqr
     tdt = torch.float64 if dtype == "f64" else torch.float32
     npdt = np.float64 if dtype == "f64" else np.float32
     w = 8 if dtype == "f64" else 4
     m, n = cfg.m, cfg.n
-    coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
-    At, lam = wl.dense_augmented_device(cfg, tdt, coo)
-    _, B = wl.make_slices(cfg, S=min(cfg.S, 256), coo=coo, lam=lam)
     out = {}
-    f = ctqr.ct_qr_factor(At, m, n, in_place=False)
-    incore_ms = f.stats()["factor_ms"]
     sweep = []
-    for S in (1, 8, 64, min(cfg.S, 256)):
-        Bt = ctqr.colmajor_from_numpy(B[:, :S].astype(npdt))
+    Smax = max(SWEEP_S)
+    reps = -(-Smax // B.shape[1])
+    Bt_all = ctqr.colmajor_from_numpy(np.tile(B.astype(npdt), (1, reps))[:, :Smax])   # the batch repeated: timing only
+    for S in SWEEP_S:
+        Bt = Bt_all[:S]
         Xt = torch.zeros((S, n), dtype=tdt, device="cuda")
         ctqr.ct_qr_solve(f, Bt, S, Xt)
         ms = []
@@ -293,28 +356,37 @@ def run_extras(cfg, dtype: str) -> dict:
             ctqr.ct_qr_solve(f, Bt, S, Xt)
             ms.append(f.stats()["solve_ms"])
         t = min(ms)
+        st = f.stats()
         sweep.append({"S": S, "ms": t, "slices_per_s": S / (t * 1e-3),
+                      "apply_qt_ms": st["apply_qt_ms"], "trsm_ms": st["trsm_ms"],
                       "factor_read_gbs": m * n * w / (t * 1e-3) / 1e9,
                       "tflops": (4.0 * m * n - n * n) * S / (t * 1e-3) / 1e12,
-                      "launches": f.stats()["kernel_launches"]})
+                      "launches": st["kernel_launches"]})
+        del Xt
     out["solve_sweep"] = sweep
-    # structure-aware factorisation (SURVEY.md 8f item 1): the identity block of [A0; sqrt(lambda) I] promised through
+    del Bt_all
+    if structured or not budget.allows(0.45 * budget.seconds + 0.6 * incore_ms * 1e-3):
+        return out
+    # structure-aware factorisation: the identity block of [A0; sqrt(lambda) I] promised through
     # opt->lower_bandwidth = m0; same factor, fewer flops -- TFLOP/s quoted on the flops actually performed
     m0 = m - n
-    fs = ctqr.ct_qr_factor(At, m, n, in_place=False, lower_bandwidth=m0)
-    ms = [fs.stats()["factor_ms"]]
-    for _ in range(2):
-        fs.destroy()
-        fs = ctqr.ct_qr_factor(At, m, n, in_place=False, lower_bandwidth=m0)
-        ms.append(fs.stats()["factor_ms"])
-    sst = fs.stats()
     Ss = min(cfg.S, 256)
     Bt = ctqr.colmajor_from_numpy(B[:, :Ss].astype(npdt))
-    Xs = torch.zeros((Ss, n), dtype=tdt, device="cuda")
     Xd = torch.zeros((Ss, n), dtype=tdt, device="cuda")
+    ctqr.ct_qr_solve(f, Bt, Ss, Xd)
+    f.destroy()
+    ms = []
+    fs = None
+    for _ in range(3 if incore_ms < 2000 else 1):
+        if fs is not None:
+            fs.destroy()
+        Aw.copy_(At)
+        fs = ctqr.ct_qr_factor(Aw, m, n, in_place=True, lower_bandwidth=m0)
+        ms.append(fs.stats()["factor_ms"])
+    sst = fs.stats()
+    Xs = torch.zeros((Ss, n), dtype=tdt, device="cuda")
     ctqr.ct_qr_solve(fs, Bt, Ss, Xs); ctqr.ct_qr_solve(fs, Bt, Ss, Xs)
     solve_ms = fs.stats()["solve_ms"]
-    ctqr.ct_qr_solve(f, Bt, Ss, Xd)
     B8 = ctqr.colmajor_from_numpy(B[:, :8].astype(npdt))
     X8 = torch.zeros((8, n), dtype=tdt, device="cuda")
     s8 = []
@@ -322,7 +394,7 @@ def run_extras(cfg, dtype: str) -> dict:
         ctqr.ct_qr_solve(fs, B8, 8, X8)
         s8.append(fs.stats()["solve_ms"])
     t = min(ms)
-    out["structured"] = {"lower_bandwidth": m0, "factor_ms": t, "vs_dense_time": t / incore_ms,
+    out["structured"] = {"lower_bandwidth": m0, "factor_ms": t, "vs_dense_time": t / incore_ms, "runs": len(ms),
                          "flops_performed": sst["factor_flops_performed"],
                          "flops_performed_over_dense": sst["factor_flops_performed"] / sst["factor_flops"],
                          "tflops_on_performed_flops": sst["factor_flops_performed"] / (t * 1e-3) / 1e12,
@@ -331,52 +403,111 @@ def run_extras(cfg, dtype: str) -> dict:
                          "solve_S8": {"ms": min(s8[1:]), "slices_per_s": 8 / (min(s8[1:]) * 1e-3)},
                          "solution_rel_diff_vs_dense_path": float((Xs - Xd).norm() / Xd.norm())}
     fs.destroy()
-    del Xs, Xd
-    # factor persistence (factor once per geometry, reuse): save, reload, first solve
-    if m * n * w <= 8 << 30:
-        import tempfile
-        with tempfile.TemporaryDirectory() as td:
-            path = os.path.join(td, "factor.ctqr")
-            t0 = time.perf_counter(); ctqr.ct_qr_save(f, path); t_save = time.perf_counter() - t0
-            nbytes = os.path.getsize(path)
-            t0 = time.perf_counter(); g = ctqr.ct_qr_load(path); t_load = time.perf_counter() - t0
-            X2 = torch.zeros_like(Xt)
-            ctqr.ct_qr_solve(g, Bt, S, X2)
-            out["persistence"] = {"file_bytes": nbytes, "save_s": t_save, "save_gbs": nbytes / t_save / 1e9,
-                                  "load_s": t_load, "load_gbs": nbytes / t_load / 1e9,
-                                  "reloaded_solve_ms": g.stats()["solve_ms"],
-                                  "reloaded_solve_max_abs_diff": float((X2 - Xt).abs().max()),
-                                  "vs_refactor_time": t_load / (incore_ms * 1e-3),
-                                  "note": "file in the box's temp dir; wall clock around ct_qr_save / ct_qr_load"}
-            g.destroy()
+    return out
+
+
+def run_persistence() -> dict:
+    """Factor persistence (factor once per geometry, reuse): save, reload, first solve.
+    Always on BASELINE.json configs[2] in fp64 (a 4.3 GB factor file in the box's temp directory)."""
+    import tempfile
+    import torch
+    import paper_2412_07631_b200 as ctqr
+    cfg = wl.CONFIGS["c3"]
+    m, n, S = cfg.m, cfg.n, 64
+    coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
+    At, lam = wl.dense_augmented_device(cfg, torch.float64, coo)
+    _, B = wl.make_slices(cfg, S=S, coo=coo, lam=lam)
+    f = ctqr.ct_qr_factor(At, m, n, in_place=True)
+    incore_ms = f.stats()["factor_ms"]
+    Bt = ctqr.colmajor_from_numpy(B)
+    Xt = torch.zeros((S, n), dtype=torch.float64, device="cuda")
+    ctqr.ct_qr_solve(f, Bt, S, Xt)
+    with tempfile.TemporaryDirectory() as td:
+        path = os.path.join(td, "factor.ctqr")
+        t0 = time.perf_counter(); ctqr.ct_qr_save(f, path); t_save = time.perf_counter() - t0
+        nbytes = os.path.getsize(path)
+        t0 = time.perf_counter(); g = ctqr.ct_qr_load(path); t_load = time.perf_counter() - t0
+        X2 = torch.zeros_like(Xt)
+        ctqr.ct_qr_solve(g, Bt, S, X2)
+        out = {"workload": "configs[2] fp64", "file_bytes": nbytes, "save_s": t_save, "save_gbs": nbytes / t_save / 1e9,
+               "load_s": t_load, "load_gbs": nbytes / t_load / 1e9,
+               "reloaded_solve_ms": g.stats()["solve_ms"],
+               "reloaded_solve_max_abs_diff": float((X2 - Xt).abs().max()),
+               "vs_refactor_time": t_load / (incore_ms * 1e-3),
+               "note": "file in the box's temp dir; wall clock around ct_qr_save / ct_qr_load"}
+        g.destroy()
     f.destroy()
-    # out of core
-    Ah = At.cpu().pin_memory()
-    del At
-    torch.cuda.empty_cache()
-    budget = int(m * n * w // 4)
+    return out
+
+
+def host_augmented_pinned(cfg, torch_dtype, coo):
+    """A_aug of `cfg` built straight in pinned host memory (the matrices of the out-of-core legs do not fit, or
+    need not touch, the device): same entries as wl.dense_augmented_device (duplicates summed in fp64, one
+    rounding).  Returns (tensor (n, m) = column-major m x n, lambda)."""
+    import torch
+    rows, cols, vals = coo
+    lam = wl.tikhonov_lambda(vals, cfg.n)
+    Ah = torch.zeros((cfg.n, cfg.m), dtype=torch_dtype, pin_memory=True)
+    flat = Ah.view(-1).numpy()
+    key = cols * np.int64(cfg.m) + rows
+    uk, inv = np.unique(key, return_inverse=True)
+    acc = np.zeros(uk.shape[0], dtype=np.float64)
+    np.add.at(acc, inv, vals)
+    flat[uk] = acc.astype(flat.dtype)
+    d = np.arange(cfg.n, dtype=np.int64)
+    flat[d * cfg.m + cfg.m0 + d] = np.asarray(np.sqrt(lam), dtype=np.float64).astype(flat.dtype)
+    return Ah, lam
+
+
+def run_out_of_core(cfg, dtype: str, budget_bytes: int, S: int, structured: bool = False) -> dict:
+    """a5 under real load: the matrix lives in pinned host memory, the device may use `budget_bytes` for
+    matrix tiles, the factor is written back in place and the solve streams it (section 2.2)."""
+    import torch
+    import paper_2412_07631_b200 as ctqr
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    npdt = np.float64 if dtype == "f64" else np.float32
+    w = 8 if dtype == "f64" else 4
+    m, n = cfg.m, cfg.n
+    t0 = time.perf_counter()
+    coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
+    Ah, lam = host_augmented_pinned(cfg, tdt, coo)
+    t_build = time.perf_counter() - t0
+    _, B = wl.make_slices(cfg, S=S, coo=coo, lam=lam)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    f = ctqr.ct_qr_factor(Ah, m, n, device_budget_bytes=budget)
+    f = ctqr.ct_qr_factor(Ah, m, n, device_budget_bytes=budget_bytes, lower_bandwidth=(m - n) if structured else 0)
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
     st = f.stats()
-    S = min(cfg.S, 64)
-    Bh = torch.from_numpy(np.ascontiguousarray(B[:, :S].astype(npdt).T)).pin_memory()
+    Bh = torch.from_numpy(np.ascontiguousarray(B.astype(npdt).T)).pin_memory()
     Xh = torch.zeros((S, n), dtype=tdt).pin_memory()
     ctqr.ct_qr_solve(f, Bh, S, Xh)
     st2 = f.stats()
-    out["out_of_core"] = {
-        "device_budget_bytes": budget, "n_superpanels": st["n_superpanels"], "factor_ms": st["factor_ms"],
-        "wall_s": wall, "tflops": cfg.factor_flops() / (st["factor_ms"] * 1e-3) / 1e12,
-        "vs_in_core_time": st["factor_ms"] / incore_ms,
+    # optimality residual of the streamed solve, from the sparse rows in fp64 (no device arithmetic)
+    import scipy.sparse as sp
+    rows, cols, vals = coo
+    A0 = sp.coo_matrix((vals.astype(npdt).astype(np.float64), (rows, cols)), shape=(cfg.m0, n)).tocsr()
+    sl = float(np.asarray(np.sqrt(lam), dtype=npdt))
+    X = Xh.numpy().T.astype(np.float64)
+    Bd = B.astype(npdt).astype(np.float64)
+    g = A0.T @ (Bd[:cfg.m0] - A0 @ X) + sl * (Bd[cfg.m0:] - sl * X)
+    opt = float(np.linalg.norm(g) / (np.sqrt(np.sum(A0.data ** 2) + n * sl * sl) * np.linalg.norm(Bd)))
+    fl = st["factor_flops_performed"] if structured else cfg.factor_flops()
+    link = (st["h2d_bytes"] + st["d2h_bytes"]) / (st["factor_ms"] * 1e-3) / 1e9
+    out = {
+        "workload": workload_name(cfg), "dtype": dtype, "matrix_bytes": m * n * w, "host_build_s": t_build,
+        "device_budget_bytes": budget_bytes, "n_superpanels": st["n_superpanels"], "factor_ms": st["factor_ms"],
+        "wall_s": wall, "tflops": fl / (st["factor_ms"] * 1e-3) / 1e12, "lower_bandwidth": st["lower_bandwidth"],
         "h2d_bytes": st["h2d_bytes"], "d2h_bytes": st["d2h_bytes"],
-        "host_link_gbs_avg": (st["h2d_bytes"] + st["d2h_bytes"]) / (st["factor_ms"] * 1e-3) / 1e9,
+        "host_link_gbs_avg": link,
         "algorithmic_link_bytes": m * n * w * (st["n_superpanels"] + 3) / 2.0,
+        "copy_exposed_ms": st.get("copy_exposed_ms"), "copy_busy_ms": st.get("copy_busy_ms"),
         "solve_streamed": {"S": S, "ms": st2["solve_ms"], "slices_per_s": S / (st2["solve_ms"] * 1e-3),
-                           "h2d_gbs": st2["h2d_bytes"] / (st2["solve_ms"] * 1e-3) / 1e9},
+                           "h2d_gbs": st2["h2d_bytes"] / (st2["solve_ms"] * 1e-3) / 1e9,
+                           "optimality_residual": opt},
         "note": "matrix in pinned host memory, factor written back in place; the link is shared by H2D and D2H streams"}
     f.destroy()
+    del Ah
     return out
 
 
@@ -446,12 +577,14 @@ def workload_name(cfg) -> str:
             f"I0={cfg.I0:g}")
 
 
-# per-launch DRAM traffic of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/); filled in when a capture of the current kernel exists, else null.
-# profiles/r1_pairs_c3.md (fp64: bulk update of the first PAIR of panels at configs[2], K = 256; algorithmic bytes there
-# 8.29e9) and profiles/r1_final_c3.md (fp32): dram__bytes_read.sum + dram__bytes_write.sum of the largest launch
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {("f64", "upd"): 13.68e9, ("f64", "vtc"): 3.95e9,
-                                ("f32", "upd"): 3.57e9, ("f32", "vtc"): 1.91e9}
+# per-launch DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the committed
+# `ncu --set full` captures under profiles/: the LARGEST launch of that kernel in a factorisation of that config (the
+# launches shrink with the trailing matrix); null when no capture of that config / kernel is committed.
+#   (config, dtype, kernel) -> (bytes, algorithmic bytes of that launch, profile file)
+NCU_TRAFFIC = {("c3", "f64", "upd"): (13.68e9, 8.29e9, "profiles/r1_pairs_c3.md"),
+               ("c3", "f64", "vtc"): (3.95e9, None, "profiles/r1_pairs_c3.md"),
+               ("c3", "f32", "upd"): (3.57e9, None, "profiles/r1_final_c3.md"),
+               ("c3", "f32", "vtc"): (1.91e9, None, "profiles/r1_final_c3.md")}
 
 KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; DMMA.8x8x4)",
                 ("f64", "vtc"): "gemm_mma_kernel<double,TA=true,128,64,32,32,3,2> (W = V^T C, larfb; DMMA.8x8x4)",
@@ -459,21 +592,23 @@ KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,
                 ("f32", "vtc"): "umma::gemm_umma_kernel<TA=true,BN=128> (W = V^T C, larfb; 3xTF32 on tcgen05.mma kind::tf32 / TMEM)"}
 
 
-def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:
+def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops, cfg) -> dict:
     dom = max(("upd", "vtc"), key=lambda k: spans[k]["ms"])
     oth = "vtc" if dom == "upd" else "upd"
     s, o = spans[dom], spans[oth]
     ach = s["flops"] / (s["ms"] * 1e-3) / 1e12 if s["ms"] > 0 else 0.0
     peak = nominal_peak_tflops(dtype, float(peaks.get("sm_max_mhz", 1965.0)))
+    tr = NCU_TRAFFIC.get((cfg.name, dtype, dom))
     # fp64 runs on the FP64 tensor pipe (DMMA), whose peak equals the DFMA peak.  fp32 runs as a 3xTF32
     # split on the tensor cores, but the work it replaces is fp32 FMA work and north_star asks for the
     # fraction of the FP32 peak, so the denominator stays the FFMA peak ("alu"): a fraction above 1
     # would mean the tensor-core path beats what FFMA could ever do.
     return {"bound": "tensor" if dtype == "f64" else "alu", "kernel": KERNEL_NAMES[(dtype, dom)],
             "achieved": ach, "peak": peak, "unit": UNIT, "frac": ach / peak,
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dtype, dom)),
-            "traffic_note": "ncu --set full, largest launch of this kernel at configs[2] (profiles/r1_pairs_c3.md); "
-                            "the launches of a factorisation shrink with the trailing matrix",
+            "traffic": tr[0] if tr else None,
+            "traffic_note": ("ncu --set full, largest launch of this kernel in this config (%s); algorithmic bytes of that "
+                             "launch %s; the launches of a factorisation shrink with the trailing matrix"
+                             % (tr[2], "%.3g" % tr[1] if tr[1] else "n/a")) if tr else "no committed capture for this config",
             "peak_source": ("derived: 148 SMs x %d %s FMA lanes x 2 x %.0f MHz max SM clock (MEASURED_PEAKS.json "
                             "holds no %s figure; sm_max_mhz %s)" % (64 if dtype == "f64" else 128,
                                                                    "FP64" if dtype == "f64" else "FP32",
@@ -494,13 +629,44 @@ def roofline(spans: dict, dtype: str, peaks: dict, probe_tflops) -> dict:
                 "peak_source": "MEASURED_PEAKS.json bf16_tflops (%s) x 1.1/2.25 / 3" % peaks.get("_source")})}
 
 
+def cpu_baseline_block(cfg, dtype: str, budget: Budget) -> dict:
+    """BASELINE.md "CPU-baseline plan": the oracle as it stands on the box's host cores.  The headline `value` is a
+    bounded sample of the bench workload (leading columns at full height; the whole factorisation at that rate is an
+    EXTRAPOLATION by flop count and is labelled so); configs[0] and configs[1] are run in full, configs[0] also on
+    one thread."""
+    import oracle
+    k, s = sample_size(cfg)
+    r = oracle_sample(cfg, dtype, k, s)
+    out = {k2: v for k2, v in r.items() if k2 in ("value", "unit", "cores", "kind", "sample", "solve_slices_per_s_on_sample")}
+    out["whole_factorisation_extrapolated_s"] = cfg.factor_flops() / (r["value"] * 1e12)
+    out["extrapolated"] = ("value is measured on the sample; whole_factorisation_extrapolated_s = 2mn^2-2n^3/3 of the "
+                           "full config / that rate (extrapolated by flop count, not run)")
+    full = {}
+    for name in ("c1", "c2"):
+        c = wl.CONFIGS[name]
+        if not budget.allows(40.0 if name == "c2" else 5.0):
+            full[name] = "skipped: time budget"
+            continue
+        fr = oracle_sample(c, dtype, c.n, c.S)
+        full[name] = {"m": c.m, "n": c.n, "S": c.S, "factor_s": fr["factor_s"], "tflops": fr["value"],
+                      "solve_s": fr["solve_s"], "solve_slices_per_s": c.S / fr["solve_s"], "cores": fr["cores"]}
+        if name == "c1":
+            nt = oracle.num_threads()
+            oracle.set_num_threads(1)
+            f1 = oracle_sample(c, dtype, c.n, c.S)
+            oracle.set_num_threads(nt)
+            full[name]["one_thread"] = {"factor_s": f1["factor_s"], "tflops": f1["value"], "solve_s": f1["solve_s"]}
+    out["full_runs"] = full
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c3", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--config", default="c4", choices=sorted(wl.CONFIGS))
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--no-also", action="store_true", help="skip the second precision")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -509,7 +675,12 @@ def main():
     ap.add_argument("--structured", action="store_true",
                     help="promise the identity block of [A0; sqrt(lambda) I] (lower_bandwidth = m0): same factor, "
                          "TFLOP/s on the flops actually performed; not the BASELINE.json headline")
-    ap.add_argument("--no-extras", action="store_true", help="skip the solve S-sweep and the out-of-core run")
+    ap.add_argument("--no-extras", action="store_true", help="skip the solve S-sweep, the structured run, persistence and the out-of-core run")
+    ap.add_argument("--time-budget", type=float, default=1500.0,
+                    help="wall seconds for the whole run; optional legs are sized against it")
+    ap.add_argument("--ooc-config", default="c5", choices=sorted(wl.CONFIGS),
+                    help="config of the out-of-core leg (fp32 from pinned host memory, --ooc-budget-gb device bytes)")
+    ap.add_argument("--ooc-budget-gb", type=float, default=48.0)
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     rank = int(os.environ.get("RANK", "0"))
@@ -534,12 +705,19 @@ def main():
         torch.distributed.barrier()
     import paper_2412_07631_b200 as ctqr
 
+    budget = Budget(args.time_budget)
     warm = args.warmup if args.short_warmup else max(args.warmup, 3)
-    res = run_ours(cfg, args.dtype, args.steps, warm, rank, world, do_e2e=not args.no_e2e, structured=args.structured)
+    extras_on = not args.no_extras and world == 1
+    res = run_ours(cfg, args.dtype, args.steps, warm, rank, world, budget, do_e2e=not args.no_e2e,
+                   structured=args.structured, do_sweep=True if extras_on else False)
+    if not extras_on:
+        res.pop("_extras", None)
     other = "f32" if args.dtype == "f64" else "f64"
     res2 = None
     if not args.no_also:
-        res2 = run_ours(cfg, other, args.steps, warm, rank, world, do_e2e=not args.no_e2e, structured=args.structured)
+        # second precision: same step, W >= 3 warm-up steps, K cut to its share of the time budget
+        res2 = run_ours(cfg, other, min(args.steps, 5), 3 if not args.short_warmup else warm, rank, world, budget,
+                        do_e2e=not args.no_e2e, structured=args.structured, do_sweep=False, e2e_steps=1)
     if rank != 0:
         if world > 1:
             torch.distributed.destroy_process_group()
@@ -551,22 +729,26 @@ def main():
         probe[name] = round(ctqr.ct_qr_peak_probe(kind, 8192)[0], 2)
 
     def finish(r, dtype):
-        rf = roofline(r.pop("_spans"), dtype, peaks, probe["dmma_f64" if dtype == "f64" else "ffma_f32"])
-        rf["share_of_factor_time"] = (rf["launches"] * rf["avg_launch_ms"]) / (r["factor_ms_per_step"] * args.steps)
+        rf = roofline(r.pop("_spans"), dtype, peaks, probe["dmma_f64" if dtype == "f64" else "ffma_f32"], cfg)
+        rf["share_of_factor_time"] = (rf["launches"] * rf["avg_launch_ms"]) / (r["factor_ms_per_step"] * r["steps"])
         r["roofline"] = rf
         r["frac_of_peak_whole_factor"] = r["value"] / (world * rf["peak"])
         return r
 
+    extras = res.pop("_extras", None)
     res = finish(res, args.dtype)
-    line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+    w = 8 if args.dtype == "f64" else 4
+    line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": res["steps"],
             "warmup": warm, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
             "config": {"workload": workload_name(cfg), "m": cfg.m, "n": cfg.n, "S": cfg.S, "nb": res["nb"],
                        "ib": res["ib"], "flops_per_factor": res["flops_per_factor"],
                        "lower_bandwidth": (cfg.m - cfg.n) if args.structured else 0,
-                       "l2": "inputs larger than L2 (A is %.2f GB; every step re-reads it from HBM)"
-                             % (cfg.m * cfg.n * (8 if args.dtype == "f64" else 4) / 1e9),
-                       "parallelism": "1 GPU" if world == 1 else f"{world} replicas, slices sharded"},
+                       "l2": "inputs larger than L2 (A is %.2f GB; every step re-reads it from HBM)" % (cfg.m * cfg.n * w / 1e9),
+                       "parallelism": "1 GPU" if world == 1 else f"{world} replicas, slices sharded",
+                       "steps_requested": args.steps, "time_budget_s": args.time_budget,
+                       "steps_note": ("as requested" if res["steps"] == args.steps else
+                                      "cut to fit --time-budget (one step is %.1f s)" % (res["ms_per_step"] * 1e-3))},
             "value_definition": ("sum over timed steps of the banded flop count sum_j 4 r_j (n-j-1) actually performed"
                                  if args.structured else "sum over timed steps of 2mn^2-2n^3/3")
                                 + " / device time of ct_qr_factor (A resident in HBM)",
@@ -574,17 +756,31 @@ def main():
             "solve": res["solve"], "quality_noisy": res["quality_noisy"], "quality_consistent": res["quality_consistent"], "clocks": res["clocks"],
             "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
             "peak_probe_tflops": probe}
+    if res.get("e2e_skipped"):
+        line["e2e_skipped"] = res["e2e_skipped"]
     if res2 is not None:
         res2 = finish(res2, other)
-        line["also"] = {other: {k: res2.get(k) for k in ("value", "ms_per_step", "factor_ms_per_step",
+        line["also"] = {other: {k: res2.get(k) for k in ("value", "steps", "ms_per_step", "factor_ms_per_step",
                                                      "frac_of_peak_whole_factor", "solve", "quality_noisy", "quality_consistent", "e2e",
                                                      "gpu_launches", "roofline", "clocks")}}
-    if not args.no_extras and world == 1:
-        line["extras"] = run_extras(cfg, args.dtype)
+    if extras_on:
+        extras = extras or {}
+        if budget.allows(0.30 * budget.seconds + 30.0):
+            try:
+                extras["persistence"] = run_persistence()
+            except Exception as e:                                # e.g. no room in the temp directory
+                extras["persistence"] = {"skipped": repr(e)[:200]}
+        oc = wl.CONFIGS[args.ooc_config]
+        need_s = 60.0 + oc.factor_flops() / 60e12 * 1.6           # host build + a factorisation at ~60 TFLOP/s fp32 + solve
+        if budget.allows(need_s + 40.0):
+            torch.cuda.empty_cache()
+            extras["out_of_core"] = run_out_of_core(oc, "f32", int(args.ooc_budget_gb * 1e9), 64)
+        else:
+            extras["out_of_core"] = {"skipped": "time budget (%.0f s left, %.0f s needed)" % (budget.left(), need_s)}
+        line["extras"] = extras
     if not args.no_cpu_baseline and world == 1:
-        k, s = sample_size(cfg)
-        line["cpu_baseline"] = {k2: v for k2, v in oracle_sample(cfg, args.dtype, k, s).items()
-                                if k2 in ("value", "unit", "cores", "kind", "sample", "solve_slices_per_s_on_sample")}
+        line["cpu_baseline"] = cpu_baseline_block(cfg, args.dtype, budget)
+    line["wall_s_total"] = time.perf_counter() - T_START
     print(json.dumps(line), flush=True)
     if world > 1:
         torch.distributed.destroy_process_group()

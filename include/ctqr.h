@@ -70,8 +70,11 @@ typedef struct {
                                    kl + (last column of the block) and the factorisation costs sum_j 4 r_j (n-j-1) flop,
                                    r_j = min(m, kl+j+1) - j, instead of 2mn^2 - 2n^3/3.  The result
                                    is the same factor (the skipped work is arithmetic on exact zeros).  The promise is
-                                   checked on the device first (-6 if violated), per super-panel when out of core,
-                                   where it also shortens the reflector panels streamed over the host link. */
+                                   checked on the device BEFORE anything is overwritten (-6 if violated, naming the
+                                   first offending column; the input -- device matrix, host matrix or file -- is then
+                                   untouched): in core on the resident matrix, out of core by one extra streamed pass
+                                   over the part of the host matrix below the band.  Out of core it also shortens the
+                                   reflector panels streamed over the host link. */
 } ctqr_options_t;
 
 /* Per-handle statistics (CUDA-event timed, milliseconds). */
@@ -95,6 +98,10 @@ typedef struct {
     double upd_ms, upd_flops;  int64_t upd_launches;
     int64_t lower_bandwidth;   /* the band promise the factorisation used (0 = dense) */
     double factor_flops_performed;   /* = factor_flops when dense; the banded count of opt->lower_bandwidth otherwise */
+    /* out of core only (last factor or solve call): copy_busy_ms = sum of the durations of all host<->device tile copies
+     * (H2D and D2H streams added up); copy_exposed_ms = time the compute stream spent stalled waiting for one of them,
+     * i.e. the part of the copies that compute did NOT hide (includes the first load and the last write-back). */
+    double copy_busy_ms, copy_exposed_ms;
 } ctqr_stats_t;
 
 /* Eq. 2: Householder QR of the m x n matrix A (m >= n >= 1, lda >= m).

@@ -50,7 +50,8 @@ class Stats(ctypes.Structure):
                 ("factor_flops", ctypes.c_double), ("kernel_launches", ctypes.c_int64),
                 ("vtc_ms", ctypes.c_double), ("vtc_flops", ctypes.c_double), ("vtc_launches", ctypes.c_int64),
                 ("upd_ms", ctypes.c_double), ("upd_flops", ctypes.c_double), ("upd_launches", ctypes.c_int64),
-                ("lower_bandwidth", ctypes.c_int64), ("factor_flops_performed", ctypes.c_double)]
+                ("lower_bandwidth", ctypes.c_int64), ("factor_flops_performed", ctypes.c_double),
+                ("copy_busy_ms", ctypes.c_double), ("copy_exposed_ms", ctypes.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

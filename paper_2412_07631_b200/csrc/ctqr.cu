@@ -174,6 +174,7 @@ struct ctqr_handle_s {
     int* dFlag = nullptr;
     cudaStream_t sU = nullptr, sP = nullptr, sC = nullptr, sD = nullptr, user = nullptr;
     cudaEvent_t evP = nullptr, evL = nullptr, evU = nullptr;
+    cudaEvent_t evS[3] = {nullptr, nullptr, nullptr};   // timing events of the solve calls, created once per handle
     std::vector<cudaEvent_t> ev;       // event pool
     ctqr_stats_t st;
     int64_t launches = 0;
@@ -183,6 +184,9 @@ struct ctqr_handle_s {
     void* dTickets = nullptr; int ticket_pos = 0;   // zeroed counter pairs for the SM-confined fp64 launches (kTicketRing of them)
     int reserve_sms = -1;  // SMs left to the look-ahead panel chain during the bulk update (fp32 tcgen05 path): -1 auto, 0 off
     std::vector<Span> spans;
+    // out of core: [a, b] brackets on the compute stream around every wait for a copy (exposed copy time) and on the
+    // copy streams around every copy (busy time)
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> wait_spans, copy_spans;
     std::vector<cudaEvent_t> tpool; size_t tpool_used = 0;
     cudaEvent_t timing_event() {
         if (tpool_used == tpool.size()) { cudaEvent_t e; cudaEventCreate(&e); tpool.push_back(e); }
@@ -312,6 +316,15 @@ static int larfb(H& h, int ws, cudaStream_t st, const T* V, int64_t ldv, int64_t
     return 0;
 }
 
+// out-of-core copy brackets -> stats (after the streams have been synchronised); releases the timing events
+static void resolve_copy_spans(H& h) {
+    h.st.copy_exposed_ms = h.st.copy_busy_ms = 0;
+    for (auto& s : h.wait_spans) { float ms = 0; cudaEventElapsedTime(&ms, s.first, s.second); h.st.copy_exposed_ms += ms; }
+    for (auto& s : h.copy_spans) { float ms = 0; cudaEventElapsedTime(&ms, s.first, s.second); h.st.copy_busy_ms += ms; }
+    h.wait_spans.clear(); h.copy_spans.clear();
+    h.tpool_used = 0;
+}
+
 // sum the profiled spans into the stats (after the streams have been synchronised)
 static void resolve_spans(H& h) {
     h.st.vtc_ms = h.st.upd_ms = h.st.vtc_flops = h.st.upd_flops = 0; h.st.vtc_launches = h.st.upd_launches = 0;
@@ -320,7 +333,18 @@ static void resolve_spans(H& h) {
         if (s.kind == 0) { h.st.vtc_ms += ms; h.st.vtc_flops += s.flops; h.st.vtc_launches++; }
         else             { h.st.upd_ms += ms; h.st.upd_flops += s.flops; h.st.upd_launches++; }
     }
-    h.spans.clear(); h.tpool_used = 0;
+    h.spans.clear();
+    resolve_copy_spans(h);
+}
+
+// [st] wait for `ev` (a copy), bracketed by timing events: the time the stream really stalls is the exposed copy time
+static int wait_copy(H& h, cudaStream_t st, cudaEvent_t ev) {
+    cudaEvent_t a = h.timing_event(), b = h.timing_event();
+    CK(cudaEventRecord(a, st));
+    CK(cudaStreamWaitEvent(st, ev, 0));
+    CK(cudaEventRecord(b, st));
+    h.wait_spans.push_back({a, b});
+    return 0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -419,8 +443,11 @@ static int panel_factor(H& h, cudaStream_t st, T* A, int64_t lda, int64_t m, int
 }
 
 static cudaEvent_t new_event(H& h, bool timing) {
-    cudaEvent_t e;
-    cudaEventCreateWithFlags(&e, timing ? cudaEventDefault : cudaEventDisableTiming);
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreateWithFlags(&e, timing ? cudaEventDefault : cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;                 // cudaEventRecord(nullptr, ..) then fails and the caller's CK reports it
+    }
     h.ev.push_back(e);
     return e;
 }
@@ -725,8 +752,12 @@ template <typename T>
 static int stream_panel_in(H& h, int slot, const T* hsrc, int64_t hld, int64_t rows, int cols) {
     // [sC] wait until the larfb that last read Vb[slot] is done, copy, signal
     CK(cudaStreamWaitEvent(h.sC, h.evVfree[slot], 0));
+    cudaEvent_t ca = h.timing_event(), cb = h.timing_event();
+    CK(cudaEventRecord(ca, h.sC));
     CK(cudaMemcpy2DAsync(h.dVb[slot], h.ldvb * sizeof(T), hsrc, hld * sizeof(T), rows * sizeof(T), cols,
                          cudaMemcpyHostToDevice, h.sC));
+    CK(cudaEventRecord(cb, h.sC));
+    h.copy_spans.push_back({ca, cb});
     CK(cudaEventRecord(h.evVin[slot], h.sC));
     h.st.h2d_bytes += (double)rows * cols * sizeof(T);
     return 0;
@@ -749,6 +780,8 @@ static int ensure_stream_bufs(H& h) {
 }
 
 template <typename T> static int band_check(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1);
+template <typename T> static int band_check_enqueue(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1);
+static int band_check_result(H& h);
 
 template <typename T>
 static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
@@ -779,18 +812,48 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
             CK(cudaStreamWaitEvent(h.sC, evOut[s - 2], 0));
             CK(cudaStreamWaitEvent(h.sC, evFree[s - 2], 0));
         }
+        cudaEvent_t ca = h.timing_event(), cb = h.timing_event();
+        CK(cudaEventRecord(ca, h.sC));
         CK(cudaMemcpy2DAsync(sp[s & 1], lds * sizeof(T), hA + c0 * hlda, hlda * sizeof(T), m * sizeof(T), c1 - c0,
                              cudaMemcpyHostToDevice, h.sC));
+        CK(cudaEventRecord(cb, h.sC));
+        h.copy_spans.push_back({ca, cb});
         CK(cudaEventRecord(evIn[s], h.sC));
         h.st.h2d_bytes += (double)m * (c1 - c0) * sizeof(T);
         return 0;
     };
+    if (h.kl > 0 && Ps > 1) {
+        // The band promise is verified on the WHOLE matrix before anything is written back over the caller's host
+        // matrix (or file): the part below the band of every super-panel (rows > kl + c0) is streamed through the two
+        // super-panel buffers and checked; a violation returns -6 with the input untouched.  Extra host-link bytes:
+        // about w (m - kl)^2 / 2, a few per cent of the factorisation's traffic.
+        cudaEvent_t evC[2] = {new_event(h, false), new_event(h, false)}, evK[2] = {new_event(h, false), new_event(h, false)};
+        CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
+        for (int i = 0; i < 2; ++i) CK(cudaEventRecord(evK[i], h.sU));
+        for (int s = 0; s < Ps; ++s) {
+            const int64_t c0 = (int64_t)s * ns, c1 = std::min<int64_t>(n, c0 + ns);
+            const int64_t r0 = h.kl + c0 + 1;             // first row that can lie below the band in these columns
+            if (r0 >= m) break;
+            const int b = s & 1;
+            CK(cudaStreamWaitEvent(h.sC, evK[b], 0));
+            CK(cudaMemcpy2DAsync(sp[b], lds * sizeof(T), hA + r0 + c0 * hlda, hlda * sizeof(T), (m - r0) * sizeof(T), c1 - c0,
+                                 cudaMemcpyHostToDevice, h.sC));
+            CK(cudaEventRecord(evC[b], h.sC));
+            h.st.h2d_bytes += (double)(m - r0) * (c1 - c0) * sizeof(T);
+            CK(cudaStreamWaitEvent(h.sU, evC[b], 0));
+            CKI(band_check_enqueue<T>(h, sp[b] - r0 - c0 * lds, lds, c0, c1));
+            CK(cudaEventRecord(evK[b], h.sU));
+        }
+        CKI(band_check_result(h));
+        CK(cudaStreamWaitEvent(h.sC, evK[0], 0));
+        CK(cudaStreamWaitEvent(h.sC, evK[1], 0));
+    }
     int rc = load_sp(0);
     for (int s = 0; s < Ps && rc == 0; ++s) {
         const int64_t c0 = (int64_t)s * ns, c1 = std::min<int64_t>(n, c0 + ns);
         T* Cv = sp[s & 1] - c0 * lds;                     // virtual base of SP_s
-        CK(cudaStreamWaitEvent(h.sU, evIn[s], 0));
-        if (h.kl > 0) { rc = band_check<T>(h, Cv, lds, c0, c1); if (rc) break; }   // the promise, on the raw columns of SP_s
+        CKI(wait_copy(h, h.sU, evIn[s]));
+        if (h.kl > 0 && Ps == 1) { rc = band_check<T>(h, Cv, lds, c0, c1); if (rc) break; }   // single super-panel: nothing written back yet
         // ---- earlier reflectors, streamed from the host (super-panels 0 .. s-2) ----
         const int kres = s >= 1 ? (int)(((int64_t)(s - 1) * ns) / nb) : 0;   // first panel of SP_{s-1}
         const int kcur = (int)(c0 / nb);
@@ -801,7 +864,7 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
             const int64_t mk = row_end(h, j0 + nb) - j0;                     // V_k is zero below (band promise)
             rc = stream_panel_in<T>(h, slot, hA + j0 + j0 * hlda, hlda, mk, nb);
             if (rc) break;
-            CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
+            CKI(wait_copy(h, h.sU, h.evVin[slot]));
             rc = larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, mk, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
                           Cv + j0 + c0 * lds, lds, c1 - c0, true);
             CK(cudaEventRecord(h.evVfree[slot], h.sU));
@@ -823,14 +886,18 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
         if (rc) break;
         CK(cudaEventRecord(evDone[s], h.sU));
         CK(cudaStreamWaitEvent(h.sD, evDone[s], 0));
+        cudaEvent_t da = h.timing_event(), db = h.timing_event();
+        CK(cudaEventRecord(da, h.sD));
         CK(cudaMemcpy2DAsync(hA + c0 * hlda, hlda * sizeof(T), sp[s & 1], lds * sizeof(T), m * sizeof(T), c1 - c0,
                              cudaMemcpyDeviceToHost, h.sD));
+        CK(cudaEventRecord(db, h.sD));
+        h.copy_spans.push_back({da, db});
         CK(cudaEventRecord(evOut[s], h.sD));
         h.st.d2h_bytes += (double)m * (c1 - c0) * sizeof(T);
     }
     if (rc == 0) {
-        CK(cudaStreamWaitEvent(h.sU, evOut[Ps - 1], 0));
-        if (Ps >= 2) CK(cudaStreamWaitEvent(h.sU, evOut[Ps - 2], 0));
+        if (Ps >= 2) CKI(wait_copy(h, h.sU, evOut[Ps - 2]));
+        CKI(wait_copy(h, h.sU, evOut[Ps - 1]));      // the write-back of the last super-panel has nothing left to hide behind
         CK(cudaEventRecord(t1, h.sU));
     }
     cudaError_t e1 = cudaStreamSynchronize(h.sU), e2 = cudaStreamSynchronize(h.sP);
@@ -916,18 +983,26 @@ __global__ void band_check_kernel(const T* __restrict__ A, int64_t lda, int64_t 
     }
 }
 template <typename T>
-static int band_check(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1) {
-    CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
+static int band_check_enqueue(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1) {
     band_check_kernel<T><<<(unsigned)std::min<int64_t>(c1 - c0, (int64_t)h.sms * 8), 256, 0, h.sU>>>(A, lda, h.m, c0, c1, h.kl, h.dFlag);
     CK(cudaGetLastError());
+    h.launches += 1;
+    return 0;
+}
+static int band_check_result(H& h) {
     int flag = 0;
     CK(cudaMemcpyAsync(&flag, h.dFlag, sizeof(int), cudaMemcpyDeviceToHost, h.sU));
     CK(cudaStreamSynchronize(h.sU));
-    h.launches += 1;
     if (flag < h.n)
         return set_err(-6, "lower_bandwidth = %lld but column %d has a non-zero below row %lld",
                        (long long)h.kl, flag, (long long)(h.kl + flag));
     return 0;
+}
+template <typename T>
+static int band_check(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1) {
+    CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
+    CKI(band_check_enqueue<T>(h, A, lda, c0, c1));
+    return band_check_result(h);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1085,7 +1160,7 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
             const int slot = k & 1;
             const int64_t mk = row_end(h, j0 + nbw) - j0;
             CKI(stream_panel_in<T>(h, slot, hA + j0 + j0 * h.hlda, h.hlda, mk, nbw));
-            CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
+            CKI(wait_copy(h, h.sU, h.evVin[slot]));
             CKI(larfb<T>(h, 0, h.sU, P_<T>(h.dVb[slot]), h.ldvb, mk, nbw,
                          P_<T>(h.dT) + (size_t)k * h.nb * h.nb, h.nb, C + j0, ldc, S));
             CK(cudaEventRecord(h.evVfree[slot], h.sU));
@@ -1207,7 +1282,7 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
             h.launches += 1;
         }
         if (i0 > 0) {
-            if (h.ooc) CK(cudaStreamWaitEvent(h.sU, h.evVin[slot], 0));
+            if (h.ooc) CKI(wait_copy(h, h.sU, h.evVin[slot]));
             GemmArgs<T> g{};
             g.M = i0; g.N = S; g.K = nbw; g.A = Rcol; g.lda = ldr; g.B = Xi; g.ldb = ldxi;
             g.C = X; g.ldc = ldx; g.alpha = T(-1); g.beta = T(1);
@@ -1238,7 +1313,10 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
     // mode 0: full solve; 1: apply Q^T in place on B (B is also the output); 2: trsm only (B = C)
     CKI(ensure_solve_ws(h, S));
     h.launches = 0; h.st.h2d_bytes = 0; h.st.d2h_bytes = 0;
-    cudaEvent_t t0 = new_event(h, true), t1 = new_event(h, true), t2 = new_event(h, true);
+    if (!h.evS[0])
+        for (int i = 0; i < 3; ++i)
+            if (!(h.evS[i] = new_event(h, true))) { h.evS[0] = nullptr; return set_err(CTQR_ERR_CUDA, "cudaEventCreate failed"); }
+    cudaEvent_t t0 = h.evS[0], t1 = h.evS[1], t2 = h.evS[2];
     const int64_t m = h.m, n = h.n;
     const int64_t rows_in = (mode == 2) ? n : m;
     // working buffer Cw (rows_in x S) on the device
@@ -1292,6 +1370,7 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
         h.st.apply_qt_ms = a; h.st.trsm_ms = b; h.st.solve_ms = a + b;
         h.st.kernel_launches = h.launches;
     }
+    if (h.ooc) resolve_copy_spans(h);          // exposed / busy copy time of the streamed solve
     return rc;
 }
 

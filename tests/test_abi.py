@@ -36,12 +36,35 @@ def test_every_declared_symbol_is_exported_and_bound(L):
     assert set(binding.EXPORTS) <= set(syms)
 
 
-def test_struct_layouts_match_the_header():
-    # ctqr_options_t: 4 x int32, int64, 2 x int32, 2 pointers, int64; ctqr_stats_t as declared
-    assert ctypes.sizeof(binding.Options) == 4 * 4 + 8 + 2 * 4 + 2 * 8 + 8
-    assert binding.Options.device_budget_bytes.offset == 16 and binding.Options.file_path.offset == 32 and binding.Options.lower_bandwidth.offset == 48
-    assert ctypes.sizeof(binding.Stats) == 2 * 8 + 6 * 4 + 9 * 8 + 8 + 2 * (8 + 8 + 8) + 2 * 8
-    assert binding.Stats.factor_ms.offset == 40 and binding.Stats.vtc_ms.offset == 120
+def test_struct_layouts_match_the_header(tmp_path):
+    """The ctypes mirrors against the C compiler's view of include/ctqr.h: a small C program prints sizeof and
+    every offsetof; names, order, offsets and sizes must agree."""
+    import subprocess
+    pairs = (("ctqr_options_t", binding.Options), ("ctqr_stats_t", binding.Stats))
+    if hasattr(binding, "Csr"):
+        pairs += (("ctqr_csr_t", binding.Csr),)
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "ctqr.h"', 'int main(void) {']
+    for cname, cls in pairs:
+        lines.append(f'printf("%zu\\n", sizeof({cname}));')
+        for fld, _ in cls._fields_:
+            lines.append(f'printf("%zu\\n", offsetof({cname}, {fld}));')
+    lines += ['return 0; }']
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    got = [int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
+    want = []
+    for _, cls in pairs:
+        want.append(ctypes.sizeof(cls))
+        want += [getattr(cls, fld).offset for fld, _ in cls._fields_]
+    assert got == want
+    # every member the header declares has a mirror (count the declarators of each struct body)
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "ctqr.h")).read(), flags=re.S)
+    for cname, cls in pairs:
+        body = re.search(r"typedef struct \{([^}]*)\} " + cname, hdr, flags=re.S).group(1)
+        n_decl = sum(len(d.split(",")) for d in body.split(";") if d.strip())
+        assert n_decl == len(cls._fields_), (cname, n_decl, len(cls._fields_))
 
 
 def test_version_and_error_strings(L):

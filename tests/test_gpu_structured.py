@@ -155,3 +155,5 @@ def test_out_of_core_broken_promise_in_a_later_super_panel():
         ctqr.ct_qr_factor(Ah, m0 + n, n, nb=nb, ib=16, device_budget_bytes=(2 * ns + 2 * nb) * lds * 8 + 64,
                           lower_bandwidth=m0)
     assert ei.value.code == -6 and "column 300" in str(ei.value)
+    # the promise is verified on the whole matrix before the first write-back: a refused input is left untouched
+    assert np.array_equal(ctqr.numpy_from_colmajor(Ah), A)

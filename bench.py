@@ -161,11 +161,37 @@ class Budget:
         return self.left() >= cost_s
 
 
-def pinned_like(t):
-    """Pinned host copy of a device tensor (one cudaHostAlloc + one D2H copy; no pageable detour)."""
+def log(msg: str) -> None:
+    """Progress line on stderr (stdout carries only the one JSON line)."""
+    print("[bench %7.1f s] %s" % (time.perf_counter() - T_START, msg), file=sys.stderr, flush=True)
+
+
+class PinnedBuffer:
+    """Page-locked host tensor that bypasses torch's caching host allocator (which rounds every request up to a
+    power of two -- 145 GB would ask for 256 GB -- and never returns blocks to the OS): plain pageable storage
+    registered with cudaHostRegister, unregistered and freed by release()."""
+    def __init__(self, shape, dtype, zero: bool = False):
+        import torch
+        self.t = torch.zeros(shape, dtype=dtype) if zero else torch.empty(shape, dtype=dtype)
+        self.nbytes = self.t.numel() * self.t.element_size()
+        rc = torch.cuda.cudart().cudaHostRegister(self.t.data_ptr(), self.nbytes, 0)
+        if int(rc) != 0:
+            self.t = None
+            raise RuntimeError(f"cudaHostRegister of {self.nbytes} bytes failed: {rc}")
+
+    def release(self):
+        import torch
+        if self.t is not None:
+            torch.cuda.synchronize()
+            torch.cuda.cudart().cudaHostUnregister(self.t.data_ptr())
+            self.t = None
+
+
+def pinned_like(t) -> PinnedBuffer:
+    """Pinned host copy of a device tensor."""
     import torch
-    h = torch.empty(t.shape, dtype=t.dtype, pin_memory=True)
-    h.copy_(t)
+    h = PinnedBuffer(t.shape, t.dtype)
+    h.t.copy_(t)
     torch.cuda.synchronize()
     return h
 
@@ -283,8 +309,10 @@ def run_ours(cfg, dtype: str, steps: int, warmup: int, rank: int, world: int, bu
             Ah = pinned_like(At)
             del At, Aw
             torch.cuda.empty_cache()
-            out["e2e"] = run_e2e(cfg, dtype, Ah, B.astype(npdt), S, k, flops, kl)
-            del Ah
+            try:
+                out["e2e"] = run_e2e(cfg, dtype, Ah.t, B.astype(npdt), S, k, flops, kl)
+            finally:
+                Ah.release()
         else:
             out["e2e"] = None
             out["e2e_skipped"] = "time budget"
@@ -443,11 +471,12 @@ def run_persistence() -> dict:
 def host_augmented_pinned(cfg, torch_dtype, coo):
     """A_aug of `cfg` built straight in pinned host memory (the matrices of the out-of-core legs do not fit, or
     need not touch, the device): same entries as wl.dense_augmented_device (duplicates summed in fp64, one
-    rounding).  Returns (tensor (n, m) = column-major m x n, lambda)."""
+    rounding).  Returns (PinnedBuffer whose tensor (n, m) is the column-major m x n matrix, lambda)."""
     import torch
     rows, cols, vals = coo
     lam = wl.tikhonov_lambda(vals, cfg.n)
-    Ah = torch.zeros((cfg.n, cfg.m), dtype=torch_dtype, pin_memory=True)
+    buf = PinnedBuffer((cfg.n, cfg.m), torch_dtype, zero=True)
+    Ah = buf.t
     flat = Ah.view(-1).numpy()
     key = cols * np.int64(cfg.m) + rows
     uk, inv = np.unique(key, return_inverse=True)
@@ -456,7 +485,7 @@ def host_augmented_pinned(cfg, torch_dtype, coo):
     flat[uk] = acc.astype(flat.dtype)
     d = np.arange(cfg.n, dtype=np.int64)
     flat[d * cfg.m + cfg.m0 + d] = np.asarray(np.sqrt(lam), dtype=np.float64).astype(flat.dtype)
-    return Ah, lam
+    return buf, lam
 
 
 def run_out_of_core(cfg, dtype: str, budget_bytes: int, S: int, structured: bool = False) -> dict:
@@ -470,8 +499,10 @@ def run_out_of_core(cfg, dtype: str, budget_bytes: int, S: int, structured: bool
     m, n = cfg.m, cfg.n
     t0 = time.perf_counter()
     coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
-    Ah, lam = host_augmented_pinned(cfg, tdt, coo)
+    buf, lam = host_augmented_pinned(cfg, tdt, coo)
+    Ah = buf.t
     t_build = time.perf_counter() - t0
+    log("out-of-core leg: %s %s built in pinned host memory (%.1f GB) in %.1f s" % (cfg.name, dtype, m * n * w / 1e9, t_build))
     _, B = wl.make_slices(cfg, S=S, coo=coo, lam=lam)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -508,6 +539,7 @@ def run_out_of_core(cfg, dtype: str, budget_bytes: int, S: int, structured: bool
         "note": "matrix in pinned host memory, factor written back in place; the link is shared by H2D and D2H streams"}
     f.destroy()
     del Ah
+    buf.release()
     return out
 
 
@@ -710,6 +742,8 @@ def main():
     extras_on = not args.no_extras and world == 1
     res = run_ours(cfg, args.dtype, args.steps, warm, rank, world, budget, do_e2e=not args.no_e2e,
                    structured=args.structured, do_sweep=True if extras_on else False)
+    if rank == 0:
+        log("%s %s: %.2f TFLOP/s over %d steps, step %.1f ms" % (cfg.name, args.dtype, res["value"], res["steps"], res["ms_per_step"]))
     if not extras_on:
         res.pop("_extras", None)
     other = "f32" if args.dtype == "f64" else "f64"
@@ -718,6 +752,8 @@ def main():
         # second precision: same step, W >= 3 warm-up steps, K cut to its share of the time budget
         res2 = run_ours(cfg, other, min(args.steps, 5), 3 if not args.short_warmup else warm, rank, world, budget,
                         do_e2e=not args.no_e2e, structured=args.structured, do_sweep=False, e2e_steps=1)
+        if rank == 0:
+            log("%s %s: %.2f TFLOP/s over %d steps" % (cfg.name, other, res2["value"], res2["steps"]))
     if rank != 0:
         if world > 1:
             torch.distributed.destroy_process_group()
@@ -774,7 +810,11 @@ def main():
         need_s = 60.0 + oc.factor_flops() / 60e12 * 1.6           # host build + a factorisation at ~60 TFLOP/s fp32 + solve
         if budget.allows(need_s + 40.0):
             torch.cuda.empty_cache()
-            extras["out_of_core"] = run_out_of_core(oc, "f32", int(args.ooc_budget_gb * 1e9), 64)
+            try:
+                extras["out_of_core"] = run_out_of_core(oc, "f32", int(args.ooc_budget_gb * 1e9), 64)
+            except Exception as e:                                # e.g. the box cannot pin that much host memory
+                extras["out_of_core"] = {"failed": repr(e)[:300]}
+            log("out-of-core leg done")
         else:
             extras["out_of_core"] = {"skipped": "time budget (%.0f s left, %.0f s needed)" % (budget.left(), need_s)}
         line["extras"] = extras

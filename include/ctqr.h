@@ -18,6 +18,11 @@
  *     ABI.  ct_qr_last_error() returns a thread-local message for the last non-zero return.
  *   - Calls are synchronous: on return all device work they enqueued has completed.
  *   - A handle is not thread-safe; distinct handles may be used from distinct threads.
+ *   - Global state: the thread-local last-error string, and ONE process-wide, mutex-protected cache of freed small
+ *     device blocks (the ~20 per-handle buffers: T, tau, workspaces; each <= 256 MiB, <= 1 GiB kept in total), so
+ *     that a service which factors or reloads one geometry after another does not pay cudaMalloc / cudaFree per
+ *     handle.  The cache is emptied automatically when a device allocation fails, and on request by
+ *     ct_qr_trim_cache(); matrix storage is never cached.
  *   - There is NO CPU fallback: without a CUDA device every compute entry point returns
  *     CTQR_ERR_CUDA.
  *
@@ -50,14 +55,19 @@ typedef enum {
 
 /* Options for ct_qr_factor.  Zero-initialise for defaults. */
 typedef struct {
-    int32_t nb;                 /* panel width; 0 = default (128). Must be a multiple of ib. */
+    int32_t nb;                 /* panel width; 0 = default (128). A multiple of ib, at most 128 (the tensor-core
+                                   kernels, the merged two-panel update and the fused small-S solve are built
+                                   for 128; smaller values exist for the blocking-invariance tests). */
     int32_t ib;                 /* inner (register-resident) panel width: 8, 16 or 32; 0 = default (32) */
     int32_t lookahead;          /* 0 = off, 1 = factor panel k+1 while the rest of update k runs; -1 = default */
     int32_t in_place;           /* 1: A (device) is overwritten and must outlive the handle.
                                    0: A is read-only; the handle owns a copy. */
     int64_t device_budget_bytes;/* 0 = unlimited (in-core if it fits). >0 caps the device bytes used
                                    for matrix tiles: forces the out-of-core path when m*n*w exceeds it */
-    int32_t gemm_impl;          /* 0 = default (fp64: DMMA tensor cores, fp32: FFMA), 1 = SIMT reference kernels */
+    int32_t gemm_impl;          /* 0 = default: tensor cores (fp64: mma.sync m8n8k4 = DMMA.8x8x4; fp32: 3xTF32 split on
+                                   tcgen05.mma kind::tf32 with TMEM accumulators, warp-level mma.sync tf32 for shapes the
+                                   tcgen05 kernel does not take); 1 = SIMT cross-check kernels (DFMA / FFMA), which also
+                                   switches the fused small-S solve kernels off */
     int32_t profile;            /* 1: CUDA-event time every trailing-update contraction launch (stats.vtc_*, upd_*) */
     const char* file_path;      /* optional file-backed tier: path of a file holding the column-major m x n matrix
                                    (leading dimension lda, offset 0).  The A argument is then ignored (may be NULL);
@@ -75,6 +85,13 @@ typedef struct {
                                    untouched): in core on the resident matrix, out of core by one extra streamed pass
                                    over the part of the host matrix below the band.  Out of core it also shortens the
                                    reflector panels streamed over the host link. */
+    int32_t trsm_exact;         /* 0 = default: the diagonal tasks X_i = R_ii^{-1} C_i of the blocked TRSM
+                                   multiply by the explicitly inverted nb x nb DIAGONAL block (inverted once per handle;
+                                   the off-diagonal part of R^{-1} is never formed, L48).  That is only conditionally
+                                   backward stable, so the library falls back to back-substitution by itself when a
+                                   diagonal block looks ill-conditioned (stats.diag_block_cond > 1/sqrt(eps)).
+                                   1 = always back-substitution (trsm_diag_kernel; also disables the fused S <= 8 TRSM). */
+    int32_t reserved_;          /* must be 0 */
 } ctqr_options_t;
 
 /* Per-handle statistics (CUDA-event timed, milliseconds). */
@@ -102,6 +119,9 @@ typedef struct {
      * (H2D and D2H streams added up); copy_exposed_ms = time the compute stream spent stalled waiting for one of them,
      * i.e. the part of the copies that compute did NOT hide (includes the first load and the last write-back). */
     double copy_busy_ms, copy_exposed_ms;
+    double diag_block_cond;    /* max over diagonal blocks of max|R_jj| / min|R_jj| (set by the first solve; 0 before) */
+    int32_t trsm_exact;        /* 0: inverted diagonal blocks; 1: back-substitution by option; 2: forced by the guard */
+    int32_t reserved_;
 } ctqr_stats_t;
 
 /* Eq. 2: Householder QR of the m x n matrix A (m >= n >= 1, lda >= m).
@@ -152,6 +172,10 @@ void ct_qr_destroy(ctqr_handle_t h);
  * CTQR_ERR_NOMEM, CTQR_ERR_CUDA; *out is untouched on failure. */
 int ct_qr_save(ctqr_handle_t h, const char* path);
 int ct_qr_load(const char* path, const ctqr_options_t* opt, ctqr_handle_t* out);
+
+/* Releases the process-wide cache of freed small device blocks (see "Global state" above); returns the bytes freed.
+ * Safe at any time from any thread; blocks in use by live handles are not affected. */
+int64_t ct_qr_trim_cache(void);
 
 const char* ct_qr_strerror(int code);
 const char* ct_qr_last_error(void);

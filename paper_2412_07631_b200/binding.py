@@ -35,7 +35,7 @@ class Options(ctypes.Structure):
                 ("in_place", ctypes.c_int32), ("device_budget_bytes", ctypes.c_int64),
                 ("gemm_impl", ctypes.c_int32), ("profile", ctypes.c_int32),
                 ("file_path", ctypes.c_char_p), ("stream", ctypes.c_void_p),
-                ("lower_bandwidth", ctypes.c_int64)]
+                ("lower_bandwidth", ctypes.c_int64), ("trsm_exact", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
 
 
 class Stats(ctypes.Structure):
@@ -51,7 +51,8 @@ class Stats(ctypes.Structure):
                 ("vtc_ms", ctypes.c_double), ("vtc_flops", ctypes.c_double), ("vtc_launches", ctypes.c_int64),
                 ("upd_ms", ctypes.c_double), ("upd_flops", ctypes.c_double), ("upd_launches", ctypes.c_int64),
                 ("lower_bandwidth", ctypes.c_int64), ("factor_flops_performed", ctypes.c_double),
-                ("copy_busy_ms", ctypes.c_double), ("copy_exposed_ms", ctypes.c_double)]
+                ("copy_busy_ms", ctypes.c_double), ("copy_exposed_ms", ctypes.c_double),
+                ("diag_block_cond", ctypes.c_double), ("trsm_exact", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -72,6 +73,7 @@ EXPORTS = {
     "ct_qr_save": ([_P, ctypes.c_char_p], _I),
     "ct_qr_load": ([ctypes.c_char_p, ctypes.POINTER(Options), ctypes.POINTER(_P)], _I),
     "ct_qr_dtype": ([_P], _I),
+    "ct_qr_trim_cache": ([], _I64),
     "ct_qr_strerror": ([_I], ctypes.c_char_p),
     "ct_qr_last_error": ([], ctypes.c_char_p),
     "ct_qr_version": ([], _I),
@@ -179,7 +181,7 @@ class Factor:
 def ct_qr_factor(A, m: int, n: int, lda: int | None = None, *, nb: int = 0, ib: int = 0,
                  lookahead: int = -1, in_place: bool = False, device_budget_bytes: int = 0,
                  gemm_impl: int = 0, profile: bool = False, stream=None, file_path: str | None = None,
-                 dtype=None, lower_bandwidth: int = 0) -> Factor:
+                 dtype=None, lower_bandwidth: int = 0, trsm_exact: bool = False) -> Factor:
     """Eq. 2.  ``A``: torch tensor (device or pinned/pageable host) or numpy array whose MEMORY
     is the column-major m x n matrix with leading dimension ``lda`` (default m)."""
     code = _code_of(A) if A is not None else (F64 if np.dtype(dtype) == np.float64 else F32)
@@ -187,10 +189,15 @@ def ct_qr_factor(A, m: int, n: int, lda: int | None = None, *, nb: int = 0, ib: 
     o = Options(nb=nb, ib=ib, lookahead=lookahead, in_place=int(in_place),
                 device_budget_bytes=device_budget_bytes, gemm_impl=gemm_impl, profile=int(profile),
                 file_path=file_path.encode() if file_path else None, stream=stream,
-                lower_bandwidth=lower_bandwidth)
+                lower_bandwidth=lower_bandwidth, trsm_exact=int(trsm_exact))
     h = _P()
     _check(lib().ct_qr_factor(_ptr(A) if A is not None else None, m, n, lda, code, ctypes.byref(o), ctypes.byref(h)))
     return Factor(h, m, n, code, keep=A if in_place else None)
+
+
+def ct_qr_trim_cache() -> int:
+    """Release the library's process-wide cache of freed small device blocks; returns the bytes freed."""
+    return int(lib().ct_qr_trim_cache())
 
 
 def ct_qr_save(f: Factor, path: str) -> None:

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <atomic>
 
 #if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
 #error "ctqr is written for sm_100a (B200) only"
@@ -14,6 +15,26 @@ constexpr int kWarp = 32;
 
 __host__ __device__ inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 __host__ __device__ inline int64_t round_up(int64_t a, int64_t b) { return ceil_div(a, b) * b; }
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-function, per-DEVICE setting: every launcher keeps one
+// `static SmemAttr` and raises the limit the first time a device (or a larger size) is seen.  Safe from several
+// host threads (distinct handles may live on distinct threads and devices): the worst case is a repeated call.
+constexpr int kMaxDevices = 64;
+struct SmemAttr { std::atomic<size_t> cur[kMaxDevices]; };
+template <typename K>
+inline cudaError_t ensure_dyn_smem(K kernel, size_t bytes, SmemAttr& a) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool tracked = dev >= 0 && dev < kMaxDevices;
+    if (tracked && bytes <= a.cur[dev].load(std::memory_order_acquire)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess && tracked) {
+        size_t old = a.cur[dev].load(std::memory_order_relaxed);
+        while (old < bytes && !a.cur[dev].compare_exchange_weak(old, bytes, std::memory_order_release)) {}
+    }
+    return e;
+}
 
 // ---- cp.async (LDGSTS) -----------------------------------------------------------------
 // 16-byte copy with zero-fill: src_bytes in [0,16]; bytes beyond src_bytes are written as 0.

@@ -147,6 +147,29 @@ static void dev_free(void* p) {
     cudaFree(p);
 }
 
+extern "C" int64_t ct_qr_trim_cache(void) {
+    std::vector<void*> drop;
+    size_t bytes = 0;
+    {
+        std::lock_guard<std::mutex> lk(g_cache.mu);
+        for (auto& kv : g_cache.free_) { drop.push_back(kv.second); g_cache.key_.erase(kv.second); }
+        bytes = g_cache.cached;
+        g_cache.free_.clear(); g_cache.cached = 0;
+    }
+    for (void* q : drop) cudaFree(q);
+    return (int64_t)bytes;
+}
+// large allocations (matrix storage, super-panel buffers, accessor temporaries): plain cudaMalloc that gives the
+// cached small blocks back and retries once before reporting out-of-memory
+static cudaError_t big_alloc(void** p, size_t bytes) { return dev_alloc_raw(p, bytes); }
+// free device memory as a budget: what cudaMemGetInfo reports plus what the cache could give back
+static size_t free_device_bytes() {
+    size_t freeb = 0, totb = 0;
+    if (cudaMemGetInfo(&freeb, &totb) != cudaSuccess) { cudaGetLastError(); return 0; }
+    std::lock_guard<std::mutex> lk(g_cache.mu);
+    return freeb + g_cache.cached;
+}
+
 // ------------------------------------------------------------------------------------------
 // handle
 // ------------------------------------------------------------------------------------------
@@ -182,6 +205,7 @@ struct ctqr_handle_s {
     struct Span { cudaEvent_t a, b; double flops; int kind; };
     int profile = 0;
     void* dTickets = nullptr; int ticket_pos = 0;   // zeroed counter pairs for the SM-confined fp64 launches (kTicketRing of them)
+    int trsm_exact = 0;    // 1: opt->trsm_exact; 2: forced by the conditioning guard of the diagonal blocks
     int reserve_sms = -1;  // SMs left to the look-ahead panel chain during the bulk update (fp32 tcgen05 path): -1 auto, 0 off
     std::vector<Span> spans;
     // out of core: [a, b] brackets on the compute stream around every wait for a copy (exposed copy time) and on the
@@ -389,11 +413,6 @@ static int panel_inner(H& h, int ib, cudaStream_t st, T* A, int64_t lda, int64_t
     const int* list = panel_rpts<T>(ib);
     // largest rpt whose grid still has >= 8 CTAs (enough parallelism), else the smallest that fits
     int pick = 0;
-    static const int force_rpt = [] { const char* e = getenv("CTQR_PANEL_RPT"); return e ? atoi(e) : 0; }();
-    if (force_rpt > 0)
-        for (const int* r = list; *r; ++r)
-            if (*r == force_rpt && ceil_div(rows, (int64_t)NT * *r) <= gmax) { pick = *r; break; }
-    if (!pick)
     for (const int* r = list; *r; ++r) {
         int64_t g = ceil_div(rows, (int64_t)NT * *r);
         if (g <= gmax && (g >= 8 || r[1] == 0)) { pick = *r; break; }
@@ -479,7 +498,6 @@ static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) 
         }
         return 0;
     }
-    static const bool reserve64 = [] { const char* e = getenv("CTQR_RESERVE_F64"); return !e || e[0] != '0'; }();
     CKI(panel_factor<T>(h, h.sP, A, lda, row_end(h, std::min<int64_t>(c0 + nb, c1)), c0, (int)std::min<int64_t>(nb, c1 - c0), k0));
     CK(cudaEventRecord(evP, h.sP));
     for (int k = k0; k < k1; ++k) {
@@ -505,13 +523,12 @@ static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) 
         // at once and the rest draw their worker index from a counter (GemmLaunch::reserve).
         const int64_t ncb = c1 - jn - nbn;
         int R = 0; int64_t nA = ncb;
-        if (h.gemm_impl == 0 && h.reserve_sms != 0 && ncb > 0 && (sizeof(T) == 4 || reserve64)) {
+        if (h.gemm_impl == 0 && h.reserve_sms != 0 && ncb > 0) {
             const int64_t mk1 = men - jn;
             const int ibn = panel_ib_for<T>(h, mk1);
             const int Gp = ibn ? (int)ceil_div(mk1, (int64_t)kPanelThreads * panel_rpts<T>(ibn)[0]) : h.sms;
             R = h.reserve_sms > 0 ? h.reserve_sms : Gp + 2;
-            static const double maxfrac = [] { const char* e = getenv("CTQR_RESERVE_MAXFRAC"); return e ? atof(e) : 0.45; }();
-            if (R > (int)(h.sms * maxfrac)) R = 0;          // tall panels: the chain is negligible against the update
+            if (R > (int)(h.sms * 0.45)) R = 0;          // tall panels: the chain is negligible against the update
             if (R > 0) {
                 const double t_panel = 0.25e-3 + 1.5e-8 * (double)mk1;                   // s, calibrated at c3 (flat optimum, both precisions)
                 const double rate = (sizeof(T) == 4 ? 69e12 : 25e12) * (double)(h.sms - R) / (double)h.sms;   // flop/s of the pair of products
@@ -710,9 +727,8 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
 
 template <typename T>
 static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
-    static const bool pairs = [] { const char* e = getenv("CTQR_PAIR"); return !e || e[0] != '0'; }();
     const bool aligned = (uintptr_t)A % 16 == 0 && (lda * (int64_t)sizeof(T)) % 16 == 0;
-    if (pairs && h.lookahead && !h.ooc && h.nb == 128 && h.gemm_impl == 0 && aligned && c0 % 128 == 0 && c1 - c0 >= 4 * 128 &&
+    if (h.lookahead && !h.ooc && h.nb == 128 && h.gemm_impl == 0 && aligned && c0 % 128 == 0 && c1 - c0 >= 4 * 128 &&
         h.m - c0 >= 1024 && ensure_pair_ws<T>(h, c1 - c0) == 0)
         return factor_range_pairs<T>(h, A, lda, c0, c1);
     return factor_range_single<T>(h, A, lda, c0, c1);
@@ -792,7 +808,7 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
     CKI(ensure_stream_bufs(h));
     T* sp[2] = {nullptr, nullptr};
     for (int i = 0; i < 2; ++i) {
-        if (cudaMalloc(&h.spbuf[i], (size_t)lds * std::min<int64_t>(ns, n) * sizeof(T)) != cudaSuccess) {
+        if (big_alloc(&h.spbuf[i], (size_t)lds * std::min<int64_t>(ns, n) * sizeof(T)) != cudaSuccess) {
             cudaGetLastError();
             return set_err(CTQR_ERR_NOMEM, "cannot allocate the super-panel buffers (%lld columns)", (long long)ns);
         }
@@ -826,7 +842,8 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
         // The band promise is verified on the WHOLE matrix before anything is written back over the caller's host
         // matrix (or file): the part below the band of every super-panel (rows > kl + c0) is streamed through the two
         // super-panel buffers and checked; a violation returns -6 with the input untouched.  Extra host-link bytes:
-        // about w (m - kl)^2 / 2, a few per cent of the factorisation's traffic.
+        // about w (m - kl)^2 / 2, i.e. n / (m (P_s + 3)) of the factorisation's traffic for [A0; c I] (6 % at
+        // configs[4] with 7 super-panels).
         cudaEvent_t evC[2] = {new_event(h, false), new_event(h, false)}, evK[2] = {new_event(h, false), new_event(h, false)};
         CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
         for (int i = 0; i < 2; ++i) CK(cudaEventRecord(evK[i], h.sU));
@@ -1012,15 +1029,14 @@ template <typename T>
 static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr_options_t& o) {
     const int64_t m = h.m, n = h.n;
     const size_t bytes = (size_t)m * n * sizeof(T);
-    size_t freeb = 0, totb = 0;
-    CK(cudaMemGetInfo(&freeb, &totb));
+    const size_t freeb = free_device_bytes();
     const size_t slack = (size_t)2 << 30;                 // workspaces, T, B/X of later solves
     if (a_on_device) {
         CKI(alloc_state<T>(h, n));
         if (o.in_place) { h.dA = A; h.lda = lda; h.own_A = false; }
         else {
             h.lda = round_up(m, 16 / sizeof(T));
-            CK(cudaMalloc(&h.dA, (size_t)h.lda * n * sizeof(T)));
+            CK(big_alloc(&h.dA, (size_t)h.lda * n * sizeof(T)));
             h.own_A = true;
             CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
                                  cudaMemcpyDeviceToDevice, h.sU));
@@ -1034,7 +1050,7 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
         // host matrix that fits: stage once, factor in core, keep the factor on the device
         CKI(alloc_state<T>(h, n));
         h.lda = round_up(m, 16 / sizeof(T));
-        CK(cudaMalloc(&h.dA, (size_t)h.lda * n * sizeof(T)));
+        CK(big_alloc(&h.dA, (size_t)h.lda * n * sizeof(T)));
         h.own_A = true;
         CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
                              cudaMemcpyHostToDevice, h.sU));
@@ -1074,7 +1090,8 @@ static int new_handle(ctqr_dtype_t dtype, int64_t m, int64_t n, const ctqr_optio
     h->lookahead = o.lookahead < 0 ? 1 : (o.lookahead ? 1 : 0);
     h->gemm_impl = o.gemm_impl;
     h->profile = o.profile ? 1 : 0;
-    { const char* e = getenv("CTQR_RESERVE_SMS"); h->reserve_sms = e ? atoi(e) : -1; }   // -1 = automatic, 0 = off
+    h->reserve_sms = -1;               // SMs left to the look-ahead chain during the bulk update: chosen per panel
+    h->trsm_exact = o.trsm_exact ? 1 : 0;
     h->P = (int)ceil_div(n, h->nb);
     h->user = (cudaStream_t)o.stream;
     int dev = 0; cudaGetDevice(&dev);
@@ -1168,8 +1185,7 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         return 0;
     }
     const T* A = P_<T>(h.dA);
-    static const bool no_small = [] { const char* e = getenv("CTQR_NO_SMALL_S"); return e && e[0] == '1'; }();
-    if (S <= kSmallS && h.dLLs && !no_small && h.gemm_impl == 0) {
+    if (S <= kSmallS && h.dLLs && h.gemm_impl == 0) {
         // memory-bound regime: one cooperative kernel for all panels (solve_small.cuh)
         SmallQtArgs<T> a{};
         const int64_t nch = ceil_div(h.m, (int64_t)kSmallChunk);
@@ -1183,8 +1199,8 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         a.kl = h.kl;
         const size_t smem = ((size_t)h.nb * SmallLd<T>::T_ + 2 * (size_t)h.nb * SmallLd<T>::W + (size_t)kSmallS * (a.rpc + 4)) * sizeof(T);
         if (smem <= 220 * 1024) {
-            static size_t cur = 0;
-            if (smem > cur) { CK(cudaFuncSetAttribute(apply_qt_small_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); cur = smem; }
+            static SmemAttr attr;
+            CK(ensure_dyn_smem(apply_qt_small_kernel<T>, smem, attr));
             void* args[] = {(void*)&a};
             CK(cudaLaunchCooperativeKernel((void*)apply_qt_small_kernel<T>, dim3(G), dim3(kSmallThreads), args, smem, h.sU));
             h.launches += 1;
@@ -1220,17 +1236,29 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
     CK(cudaMemcpyAsync(&flag, h.dFlag, sizeof(int), cudaMemcpyDeviceToHost, h.sU));
     CK(cudaStreamSynchronize(h.sU));
     if (flag < h.n) { h.st.singular_col = flag; return set_err(CTQR_ERR_SINGULAR, "R[%d,%d] == 0", flag, flag); }
-    // diagonal tasks through the inverses of the diagonal blocks (built once per handle) unless
-    // CTQR_TRSM_EXACT=1 asks for the back-substitution kernel
-    static const bool exact = [] { const char* e = getenv("CTQR_TRSM_EXACT"); return e && e[0] == '1'; }();
-    const bool use_inv = !exact && h.dRinv && ldx % (16 / (int64_t)sizeof(T)) == 0;
-    if (use_inv && !h.rinv_ready) {
-        CK(trinv_launch<T>(P_<T>(h.dRd), h.nb, h.n, h.P, P_<T>(h.dRinv), h.sU));
+    // Diagonal tasks X_i = R_ii^{-1} C_i: by default a product with the explicitly inverted 128 x 128 diagonal
+    // block (inverted once per handle, by back-substitution on the identity, working precision), which turns 128
+    // dependent steps per right-hand side into one small contraction.  The off-diagonal part of R^{-1} is never
+    // formed.  A product with an explicit inverse is only conditionally backward stable, so the
+    // back-substitution kernel is used instead when opt->trsm_exact is set, or when some diagonal block looks
+    // ill-conditioned: max|R_jj| / min|R_jj| inside the block (a lower bound of its condition number) above
+    // 1/sqrt(eps) of the working type.
+    if (!h.trsm_exact && h.dRinv && !h.rinv_ready) {
+        CK(cudaMemsetAsync(h.dFlag, 0, sizeof(int), h.sU));
+        CK(trinv_launch<T>(P_<T>(h.dRd), h.nb, h.n, h.P, P_<T>(h.dRinv), reinterpret_cast<unsigned*>(h.dFlag), h.sU));
+        unsigned bits = 0;
+        CK(cudaMemcpyAsync(&bits, h.dFlag, sizeof(unsigned), cudaMemcpyDeviceToHost, h.sU));
+        CK(cudaStreamSynchronize(h.sU));
+        float ratio; memcpy(&ratio, &bits, sizeof ratio);
+        h.st.diag_block_cond = ratio;
         h.rinv_ready = true;
         h.launches += 1;
+        if (!(ratio <= (sizeof(T) == 8 ? 6.7e7f : 2.9e3f))) h.trsm_exact = 2;      // also catches NaN
     }
-    static const bool no_small = [] { const char* e = getenv("CTQR_NO_SMALL_S"); return e && e[0] == '1'; }();
-    if (S <= kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && !no_small && h.gemm_impl == 0) {
+    h.st.trsm_exact = h.trsm_exact;
+    const bool exact = h.trsm_exact != 0;
+    const bool use_inv = !exact && h.dRinv && ldx % (16 / (int64_t)sizeof(T)) == 0;
+    if (S <= kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && h.gemm_impl == 0) {
         // memory-bound regime: one cooperative kernel for all diagonal blocks (solve_small.cuh)
         SmallTrsmArgs<T> a{};
         const int64_t nch = ceil_div(h.n, (int64_t)kTrsmChunk);
@@ -1243,8 +1271,8 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
         const size_t smem = ((size_t)h.nb * h.nb + 2 * (size_t)h.nb * kSmallS + (size_t)kSmallS * kTrsmThreads +
                              (size_t)kSmallS * a.rpc) * sizeof(T);
         if (smem <= 220 * 1024) {
-            static size_t cur = 0;
-            if (smem > cur) { CK(cudaFuncSetAttribute(trsm_small_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); cur = smem; }
+            static SmemAttr attr;
+            CK(ensure_dyn_smem(trsm_small_kernel<T>, smem, attr));
             void* args[] = {(void*)&a};
             CK(cudaLaunchCooperativeKernel((void*)trsm_small_kernel<T>, dim3(G), dim3(kTrsmThreads), args, smem, h.sU));
             h.launches += 1;
@@ -1436,7 +1464,7 @@ template <typename T>
 static int get_R_typed(H& h, void* R, int64_t ldr) {
     const int64_t n = h.n;
     T* tmp = nullptr;
-    CK(cudaMalloc(&tmp, (size_t)n * n * sizeof(T)));
+    CK(big_alloc((void**)&tmp, (size_t)n * n * sizeof(T)));
     cudaError_t e = gather_R_launch<T>(P_<T>(h.dA), h.lda, P_<T>(h.dRd), h.nb, n, tmp, n, h.sU);
     int rc = 0;
     if (e != cudaSuccess) rc = set_err(CTQR_ERR_CUDA, "gather_R failed: %s", cudaGetErrorString(e));
@@ -1673,13 +1701,12 @@ static int load_typed(H& h, int fd, const FactorFileHeader& hd, const ctqr_optio
     const size_t blk = (size_t)h.nb * h.nb * w;
     const size_t mat_bytes = (size_t)hd.ld * h.n * w;
     CKI(alloc_state<T>(h, h.nb));              // solve workspaces grow on demand (ensure_solve_ws)
-    size_t freeb = 0, totb = 0;
-    CK(cudaMemGetInfo(&freeb, &totb));
+    const size_t freeb = free_device_bytes();
     const size_t slack = (size_t)2 << 30;
     const size_t budget = o.device_budget_bytes > 0 ? (size_t)o.device_budget_bytes : (freeb > slack ? freeb - slack : 0);
     if (mat_bytes <= budget) {
         h.lda = hd.ld;
-        if (cudaMalloc(&h.dA, mat_bytes) != cudaSuccess) { cudaGetLastError(); return set_err(CTQR_ERR_NOMEM, "cannot allocate %zu bytes for the factor", mat_bytes); }
+        if (big_alloc(&h.dA, mat_bytes) != cudaSuccess) { cudaGetLastError(); return set_err(CTQR_ERR_NOMEM, "cannot allocate %zu bytes for the factor", mat_bytes); }
         h.own_A = true;
         if (lseek(fd, (off_t)hd.off_matrix, SEEK_SET) < 0) return set_err(CTQR_ERR_IO, "seek in %s failed", path);
         CKI(load_device_section(h, fd, h.dA, mat_bytes, bounce, path));

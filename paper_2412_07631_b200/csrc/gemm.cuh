@@ -366,8 +366,8 @@ template <bool TA, int BM, int BN, int WM, int WN, int BK, int STAGES, int MINB>
 inline cudaError_t launch_dmma(GemmArgs<double> g, int splits, cudaStream_t st) {
     using Cfg = DmmaCfg<TA, BM, BN, WM, WN, BK, STAGES>;
     auto kern = gemm_dmma_kernel<TA, BM, BN, WM, WN, BK, STAGES, MINB>;
-    static bool attr_done = false;
-    if (!attr_done) { cudaError_t e = set_smem(kern, Cfg::SMEM); if (e != cudaSuccess) return e; attr_done = true; }
+    static SmemAttr attr;
+    { cudaError_t e = ensure_dyn_smem(kern, Cfg::SMEM, attr); if (e != cudaSuccess) return e; }
     g.k_chunk = round_up(ceil_div(g.K, splits), BK);
     if (g.k_chunk <= 0) g.k_chunk = BK;
     dim3 grid((unsigned)ceil_div(g.M, BM), (unsigned)ceil_div(g.N, BN), (unsigned)splits);
@@ -379,8 +379,8 @@ template <typename T, bool TA, int BM, int BN, int BK>
 inline cudaError_t launch_simt(GemmArgs<T> g, int splits, cudaStream_t st) {
     using Cfg = SimtCfg<T, TA, BM, BN, BK>;
     auto kern = gemm_simt_kernel<T, TA, BM, BN, BK>;
-    static bool attr_done = false;
-    if (!attr_done) { cudaError_t e = set_smem(kern, Cfg::SMEM); if (e != cudaSuccess) return e; attr_done = true; }
+    static SmemAttr attr;
+    { cudaError_t e = ensure_dyn_smem(kern, Cfg::SMEM, attr); if (e != cudaSuccess) return e; }
     g.k_chunk = round_up(ceil_div(g.K, splits), BK);
     if (g.k_chunk <= 0) g.k_chunk = BK;
     dim3 grid((unsigned)ceil_div(g.M, BM), (unsigned)ceil_div(g.N, BN), (unsigned)splits);

@@ -5,7 +5,6 @@
 #include "gemm.cuh"
 #include "gemm_mma.cuh"
 #include "gemm_umma.cuh"
-#include <cstdlib>
 
 namespace ctqr {
 
@@ -33,7 +32,6 @@ static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
-    L.G = p.sk.G; L.Gm = p.sk.Gm;
     L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
 }
@@ -46,13 +44,8 @@ static GemmLaunch umma_plan_f32(int64_t M, int64_t N, int64_t K, int bn, int sms
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
-    L.G = 0; L.Gm = 1;
     L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
-}
-static bool umma_enabled() {
-    static const bool on = [] { const char* e = getenv("CTQR_NO_UMMA"); return !(e && e[0] == '1'); }();
-    return on;
 }
 
 GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems,
@@ -64,7 +57,7 @@ GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
                        : classic_plan(M, N, K, 128, 128, sms, 512, partial, max_elems, sstride, 5);
     }
     // the big products go to the tcgen05 kernel (float4 chunks: K, and M when A is m-contiguous, multiples of 4)
-    const bool umma_ok = umma_enabled() && N >= 128 && K % 4 == 0;
+    const bool umma_ok = N >= 128 && K % 4 == 0;
     if (ta) {
         if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0);
         if (umma_ok && M <= 128) return umma_plan_f32(M, N, K, 128, sms, partial, max_elems, 21);
@@ -78,7 +71,7 @@ GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
 static MmaPlan to_plan(const GemmLaunch& L) {
     MmaPlan p{};
     p.sk.tilesM = L.tilesM; p.sk.tilesN = L.tilesN; p.sk.KT = L.KT; p.sk.U = L.U; p.sk.L = L.L; p.sk.partial = L.partial;
-    p.grid = L.grid; p.maxseg = L.slots; p.sk.G = L.G; p.sk.Gm = L.Gm;
+    p.grid = L.grid; p.maxseg = L.slots;
     return p;
 }
 
@@ -94,10 +87,7 @@ cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int im
         case 5: return launch_simt<float, false, 128, 128, 8>(g, L.splits, st);
         case 1: return launch_mma<float, true, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
         case 3: return launch_mma<float, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
-        case 21: {
-            static const bool ws = [] { const char* e = getenv("CTQR_TN_WS"); return e && e[0] == '1'; }();
-            return ws ? umma::launch_umma_ws<true, 128>(g, to_plan(L), st) : umma::launch_umma<true, 128>(g, to_plan(L), st);
-        }
+        case 21: return umma::launch_umma<true, 128>(g, to_plan(L), st);
         case 23: return umma::launch_umma_ws<false, 64>(g, to_plan(L), st);
         case 24: return umma::launch_umma<false, 128>(g, to_plan(L), st);
     }

@@ -2,7 +2,6 @@
 // (gemm_mma.cuh) for the big products, the classic DMMA grid kernel for skinny in-panel shapes,
 // SIMT DFMA as cross-check (impl 1).
 #include <algorithm>
-#include <cstdlib>
 #include "gemm.cuh"
 #include "gemm_mma.cuh"
 
@@ -32,7 +31,6 @@ static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
-    L.G = p.sk.G; L.Gm = p.sk.Gm;
     L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
 }
@@ -40,25 +38,20 @@ static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
 GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int sms, bool partial, int64_t max_elems,
                          int64_t sstride, bool aligned) {
     if (impl == 1) return classic_plan(M, N, K, 64, 64, sms, 256, partial, max_elems, sstride, 9);
-    static const bool wide = [] { const char* e = getenv("CTQR_F64_BN128"); return e && e[0] == '1'; }();
     if (ta) {
         if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0);
         if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_elems, sstride, 6);
-        if (wide && N >= 128) return streamk_plan(M, N, K, 128, 128, 16, sms, partial, max_elems, sstride, 31, 1);
         return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_elems, sstride, 1);
     }
     if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
     if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_elems, sstride, 7);
-    static const bool defer = [] { const char* e = getenv("CTQR_F64_DEFER"); return e && e[0] == '1'; }();
-    if (wide && N >= 128) return streamk_plan(M, N, K, 128, 128, 16, sms, partial, max_elems, sstride, 33, 1);
-    if (defer && !partial) return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_elems, sstride, 13, 1);
     return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_elems, sstride, 3);
 }
 
 static MmaPlan to_plan(const GemmLaunch& L) {
     MmaPlan p{};
     p.sk.tilesM = L.tilesM; p.sk.tilesN = L.tilesN; p.sk.KT = L.KT; p.sk.U = L.U; p.sk.L = L.L; p.sk.partial = L.partial;
-    p.grid = L.grid; p.maxseg = L.slots; p.sk.G = L.G; p.sk.Gm = L.Gm;
+    p.grid = L.grid; p.maxseg = L.slots;
     p.sk.tickets = L.tickets; p.sk.reserve = L.reserve;
     return p;
 }
@@ -77,9 +70,6 @@ cudaError_t gemm_run_f64(bool ta, GemmArgs<double> g, const GemmLaunch& L, int i
         case 6: return launch_dmma<true, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);
         case 7: return launch_dmma<false, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);
         case 3: return launch_mma<double, false, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
-        case 13: return launch_mma<double, false, 128, 64, 32, 32, 6, 1>(g, to_plan(L), st);
-        case 31: return launch_mma<double, true, 128, 128, 32, 32, 4, 1>(g, to_plan(L), st);
-        case 33: return launch_mma<double, false, 128, 128, 32, 32, 4, 1>(g, to_plan(L), st);
     }
     return cudaErrorInvalidValue;
 }

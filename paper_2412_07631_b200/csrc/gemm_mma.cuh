@@ -26,7 +26,6 @@
 //           tcgen05 kernel of gemm_umma.cuh instead (4x the MMA rate); this one serves the rest.
 #pragma once
 #include <algorithm>
-#include <cstdlib>
 #include "common.cuh"
 #include "kernels.h"
 
@@ -145,12 +144,6 @@ struct StreamK {
     int64_t U;                // tilesM * tilesN * KT
     int64_t L;                // units per CTA (a multiple of KT in direct mode)
     int partial;              // 1: every segment writes alpha*acc to its compact partial slot; 0: direct
-    // direct mode only: tiles are dealt round-robin (CTA g's i-th tile has rank i * G + g), and ranks
-    // walk the tile grid in bands of Gm tile rows, n outer / m inner inside a band: the CTAs that
-    // run at the same time then share Gm V tiles and ~G/Gm W tiles (L2-resident) instead of
-    // cycling through all of V (which no longer fits the L2 at m = 1e5)
-    int G, Gm;
-    int l2_prefetch;          // direct mode: prefetch the next tile's C into L2 (set by the launcher)
     // SM confinement (see GemmLaunch::reserve): worker indices are drawn from tickets[1] by the CTAs that do
     // not retire on a reserved SM; `workers` = the planned grid
     unsigned* tickets; int reserve; int workers;
@@ -221,20 +214,10 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
     }
 #define s_worker (CONFINED ? s_worker_confined : (int)blockIdx.x)
     const int64_t u0 = (int64_t)s_worker * sk.L;
-    const int64_t ntiles = sk.tilesM * sk.tilesN;
-    const bool rr = !sk.partial && sk.G > 0;
-    const int64_t u1 = !rr ? min(sk.U, u0 + sk.L)
-                                  : u0 + ((ntiles - (int64_t)s_worker + sk.G - 1) / sk.G) * sk.KT;
+    const int64_t u1 = min(sk.U, u0 + sk.L);
     if (u0 >= u1) return;
     // flat tile index (contiguous per CTA) -> tile coordinates
-    auto decode = [&](int64_t t, int64_t& tm, int64_t& tn) {
-        if (!rr) { tn = t / sk.tilesM; tm = t - tn * sk.tilesM; return; }
-        const int64_t rank = (t - u0 / sk.KT) * sk.G + (int64_t)s_worker;
-        const int64_t per_band = (int64_t)sk.Gm * sk.tilesN;
-        const int64_t band = rank / per_band, r = rank - band * per_band;
-        const int64_t hb = min((int64_t)sk.Gm, sk.tilesM - band * sk.Gm);
-        tn = r / hb; tm = band * sk.Gm + (r - tn * hb);
-    };
+    auto decode = [&](int64_t t, int64_t& tm, int64_t& tn) { tn = t / sk.tilesM; tm = t - tn * sk.tilesM; };
 
     // L2 residency: the reflector block V (operand A) is re-read by every CTA -> keep it; the big
     // matrix C streams through once per launch -> let it go first.  In W = V^T C the streamed
@@ -325,10 +308,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
         cp_async_commit();
     }
 
-    // MINB == 1 (one CTA per SM, 255 registers): the C tile is held separately from the accumulators,
-    // so its loads are issued at the start of a tile and consumed only in the epilogue
-    constexpr bool DEFER = (MINB == 1) && (NT <= 256);
-    const T cscale = (sk.partial || g.beta == T(0)) ? T(0) : (DEFER ? T(1) : g.beta / g.alpha);
+    const T cscale = (sk.partial || g.beta == T(0)) ? T(0) : g.beta / g.alpha;
     int64_t t = u0 / sk.KT;
     int64_t tn, tm;
     decode(t, tm, tn);
@@ -338,19 +318,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
         const int64_t seg_end = min(u1, (t + 1) * sk.KT);
         const int64_t m0 = tm * BM, n0 = tn * BN;
         const bool interior = (m0 + BM <= g.M) && (n0 + BN <= g.N);
-        if (sk.l2_prefetch && cscale != T(0) && seg_end < u1) {
-            // pull the NEXT tile's C into L2 while this tile is computed: its accumulator-init loads
-            // then cost an L2 hit instead of a DRAM round trip (the tile has only K/BK k-tiles to hide it)
-            int64_t ntm, ntn;
-            decode(t + 1, ntm, ntn);
-            constexpr int LPC = BM * (int)sizeof(T) / 128;          // 128-byte lines per tile column
-            for (int i = tid; i < BN * LPC; i += NT) {
-                const int64_t n = ntn * BN + i / LPC, m = ntm * BM + (int64_t)(i % LPC) * (128 / (int)sizeof(T));
-                if (m < g.M && n < g.N) prefetch_l2(&g.C[m + n * g.ldc]);
-            }
-        }
         T acc[MT][NTL][ACC];
-        T cin[DEFER ? MT : 1][DEFER ? NTL : 1][ACC];     // DEFER: C tile requested now, used in the epilogue
         if (cscale != T(0)) {
             // all loads of the C tile are issued before the first use (one memory round trip per tile)
             const T* Cb = g.C + (m0 + wm * WM) + (n0 + wn * WN) * g.ldc;
@@ -362,18 +330,8 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
                     for (int q = 0; q < ACC; ++q) {
                         const int r = i * P::MFRAG + P::frag_row(q, grp), c = j * 8 + P::frag_col(q, tig);
                         const bool ok = interior || (m0 + wm * WM + r < g.M && n0 + wn * WN + c < g.N);
-                        const T cv = ok ? __ldcs(Cb + r + c * g.ldc) : T(0);
-                        if (DEFER) { cin[DEFER ? i : 0][DEFER ? j : 0][q] = cv; acc[i][j][q] = T(0); }
-                        else acc[i][j][q] = cv;
+                        acc[i][j][q] = ok ? cscale * __ldcs(Cb + r + c * g.ldc) : T(0);
                     }
-            if (!DEFER) {
-#pragma unroll
-                for (int i = 0; i < MT; ++i)
-#pragma unroll
-                    for (int j = 0; j < NTL; ++j)
-#pragma unroll
-                        for (int q = 0; q < ACC; ++q) acc[i][j][q] *= cscale;
-            }
         } else {
 #pragma unroll
             for (int i = 0; i < MT; ++i)
@@ -420,9 +378,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
                         const int64_t m = m0 + wm * WM + i * P::MFRAG + P::frag_row(q, grp);
                         const int64_t n = n0 + wn * WN + j * 8 + P::frag_col(q, tig);
                         if (interior || (m < g.M && n < g.N)) {
-                            T o = g.alpha * acc[i][j][q];
-                            if (DEFER && cscale != T(0)) o = fma(g.beta, cin[DEFER ? i : 0][DEFER ? j : 0][q], o);
-                            __stcs(&g.C[m + n * g.ldc], o);
+                            __stcs(&g.C[m + n * g.ldc], g.alpha * acc[i][j][q]);
                         }
                     }
         }
@@ -458,9 +414,7 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
         // only a few output tiles (the look-ahead column block, the solve's 128 x S products) that
         // rule leaves most SMs idle, so the floor drops to 512 rows (<= 2 tiles) / 256 rows (<= 8):
         // measured at configs[2], solve S = 256 Q^T B 26.4 -> 23.4 ms, factor 644 -> 636 ms (fp64).
-        static const int min_rows = [] { const char* e = getenv("CTQR_SK_MIN_ROWS"); return e ? atoi(e) : 1024; }();
-        static const int min_rows_few = [] { const char* e = getenv("CTQR_SK_MIN_ROWS_FEW"); return e ? atoi(e) : 0; }();
-        const int rows = tiles > 8 ? min_rows : min_rows_few ? min_rows_few : tiles > 2 ? 256 : 512;
+        const int rows = tiles > 8 ? 1024 : tiles > 2 ? 256 : 512;
         const int64_t min_units = std::max<int64_t>(8, rows / BK);
         int64_t G = std::min<int64_t>(slots, std::max<int64_t>(1, p.sk.U / min_units));
         p.sk.L = ceil_div(p.sk.U, G);
@@ -473,12 +427,6 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
         p.sk.L = tpc * p.sk.KT;
         p.grid = (int)ceil_div(tiles, tpc);
         p.maxseg = 1;
-        // G > 0 would deal the tiles round-robin in bands of Gm tile rows (see StreamK); measured
-        // neutral to slightly slower than contiguous ranges at m = 3e4 and 1e5 (the L2 hints already
-        // keep V resident), so the contiguous order stays the default
-        static const int band = [] { const char* e = getenv("CTQR_BAND"); return e ? atoi(e) : 0; }();
-        p.sk.G = (band && K >= band) ? p.grid : 0;
-        p.sk.Gm = (int)std::max<int64_t>(1, std::min<int64_t>(p.sk.tilesM, slots / 4));
     }
     return p;
 }
@@ -489,14 +437,10 @@ inline cudaError_t launch_mma(GemmArgs<T> g, const MmaPlan& p, cudaStream_t st) 
     if (p.sk.tickets) {
         if constexpr (sizeof(T) == 8 && MINB == 2) {
             auto kc = gemm_mma_kernel<T, TA, BM, BN, WM, WN, STAGES, MINB, true>;
-            static bool attr_c = false;
-            if (!attr_c) {
-                cudaError_t e = cudaFuncSetAttribute(kc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-                if (e != cudaSuccess) return e;
-                attr_c = true;
-            }
+            static SmemAttr attr_c;
+            { cudaError_t e = ensure_dyn_smem(kc, Cfg::SMEM, attr_c); if (e != cudaSuccess) return e; }
             StreamK skc = p.sk;
-            skc.l2_prefetch = 0; skc.workers = p.grid;
+            skc.workers = p.grid;
             kc<<<p.grid + MINB * skc.reserve, Cfg::NT, Cfg::SMEM, st>>>(g, skc);
             return cudaGetLastError();
         } else {
@@ -504,16 +448,9 @@ inline cudaError_t launch_mma(GemmArgs<T> g, const MmaPlan& p, cudaStream_t st) 
         }
     }
     auto kern = gemm_mma_kernel<T, TA, BM, BN, WM, WN, STAGES, MINB>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
-    StreamK sk = p.sk;
-    static const int pf = [] { const char* e = getenv("CTQR_L2_PREFETCH"); return e ? atoi(e) : 0; }();
-    sk.l2_prefetch = pf;
-    kern<<<p.grid, Cfg::NT, Cfg::SMEM, st>>>(g, sk);
+    static SmemAttr attr;
+    { cudaError_t e = ensure_dyn_smem(kern, Cfg::SMEM, attr); if (e != cudaSuccess) return e; }
+    kern<<<p.grid, Cfg::NT, Cfg::SMEM, st>>>(g, p.sk);
     return cudaGetLastError();
 }
 

@@ -544,12 +544,8 @@ __global__ void __launch_bounds__(WS_NT, 1) gemm_umma_ws_kernel(GemmArgs<float> 
 template <bool TA, int BN>
 inline cudaError_t launch_umma_ws(GemmArgs<float> g, const MmaPlan& p, cudaStream_t st) {
     auto kern = gemm_umma_ws_kernel<TA, BN>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<BN>::BYTES);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    static SmemAttr attr;
+    { cudaError_t e = ensure_dyn_smem(kern, WsSmem<BN>::BYTES, attr); if (e != cudaSuccess) return e; }
     kern<<<p.grid, WS_NT, WsSmem<BN>::BYTES, st>>>(g, p.sk);
     return cudaGetLastError();
 }
@@ -562,12 +558,8 @@ inline MmaPlan umma_plan(int64_t M, int64_t N, int64_t K, int bn, int sms, bool 
 template <bool TA, int BN>
 inline cudaError_t launch_umma(GemmArgs<float> g, const MmaPlan& p, cudaStream_t st) {
     auto kern = gemm_umma_kernel<TA, BN>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    static SmemAttr attr;
+    { cudaError_t e = ensure_dyn_smem(kern, SMEM_BYTES, attr); if (e != cudaSuccess) return e; }
     kern<<<p.grid, NT, SMEM_BYTES, st>>>(g, p.sk);
     return cudaGetLastError();
 }

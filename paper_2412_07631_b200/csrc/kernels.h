@@ -42,7 +42,7 @@ struct GemmLaunch {
     int kind;          // 0 = classic kernels (gemm.cuh) with `splits` K slices; 1 = persistent stream-K (gemm_mma.cuh)
     int splits;        // kind 0
     int grid;          // kind 1: CTAs
-    int64_t tilesM, tilesN, U, L; int KT; int partial; int G, Gm;   // kind 1: StreamK fields
+    int64_t tilesM, tilesN, U, L; int KT; int partial;   // kind 1: StreamK fields
     int slots;         // partial output buffers needed (each g.split_stride elements apart)
     int cfg;           // kernel configuration index inside the dtype's dispatcher
     SegInfo seg;       // for the consumer of the partials
@@ -80,7 +80,8 @@ template <typename T> cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, 
 // out = op(M) * in, M 128 x 128 upper triangular (zeros stored), N <= a few hundred columns; `in` is either a matrix
 // (seg.L == 0; may alias out) or the stream-K partial tiles of a 128 x N product (seg.L != 0)
 template <typename T> cudaError_t mm128_launch(bool trans, const T* M, int ldm, const T* in, int64_t ldin, SegInfo seg, int64_t N, T* out, int64_t ldo, cudaStream_t st);
-template <typename T> cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, cudaStream_t st);
+// cond_bits (optional, zeroed by the caller): receives the bit pattern of max over blocks of max|R_jj| / min|R_jj| as a float
+template <typename T> cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, unsigned* cond_bits, cudaStream_t st);
 template <typename T> cudaError_t copy2d_launch(const T* src, int64_t lds, T* dst, int64_t ldd, int64_t rows, int64_t cols, cudaStream_t st);
 template <typename T> cudaError_t gather_R_launch(const T* A, int64_t lda, const T* Rd, int nb, int64_t n, T* R, int64_t ldr, cudaStream_t st);
 template <typename T> cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, cudaStream_t st);

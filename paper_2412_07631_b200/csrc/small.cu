@@ -5,17 +5,12 @@
 namespace ctqr {
 
 template <typename K>
-static cudaError_t ensure_smem(K kernel, size_t bytes, size_t& cur) {
-    if (bytes <= cur) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e == cudaSuccess) cur = bytes;
-    return e;
-}
+static cudaError_t ensure_smem(K kernel, size_t bytes, SmemAttr& cur) { return ensure_dyn_smem(kernel, bytes, cur); }
 
 template <typename T>
 cudaError_t larft_launch(const T* Gp, SegInfo seg, int64_t gstride, int ldg, int nbw, int ib, T* Tk, int ldt,
                          cudaStream_t st) {
-    static size_t cur = 0;
+    static SmemAttr cur;
     const size_t smem = ((size_t)nbw * (nbw + 1) + (size_t)2 * nbw * (ib + 1)) * sizeof(T);
     cudaError_t e = ensure_smem(larft_kernel<T>, smem, cur);
     if (e != cudaSuccess) return e;
@@ -27,7 +22,7 @@ template <typename T>
 cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t wstride, int64_t ldw, const T* Tm, int ldt, int kw, int64_t N,
                        T* Wout, int64_t ldo, cudaStream_t st) {
     if (kw > 32 && kw <= 128 && (seg.L == 0 || seg.BN == 64 || seg.BN == 128)) {
-        static size_t cur2 = 0;
+        static SmemAttr cur2;
         const size_t smem2 = (size_t)(128 + 64) * 132 * sizeof(T);
         cudaError_t e2 = ensure_smem(ttw_mma_kernel<T>, smem2, cur2);
         if (e2 != cudaSuccess) return e2;
@@ -56,7 +51,7 @@ cudaError_t mm128_launch(bool trans, const T* M, int ldm, const T* in, int64_t l
     const unsigned grid = (unsigned)ceil_div(N, (int64_t)kMm128Cols);
     const bool partial = seg.L != 0;
     if (partial && (seg.BN % kMm128Cols != 0 || !trans)) return cudaErrorInvalidValue;
-    static size_t cur[2] = {0, 0};
+    static SmemAttr cur[2];
     if (partial) {
         cudaError_t e = ensure_smem(mm128_kernel<T, true, true>, smem, cur[0]);
         if (e != cudaSuccess) return e;
@@ -74,7 +69,7 @@ cudaError_t mm128_launch(bool trans, const T* M, int ldm, const T* in, int64_t l
 template <typename T>
 cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx,
                              cudaStream_t st) {
-    static size_t cur = 0;
+    static SmemAttr cur;
     const size_t smem = (size_t)128 * 129 * sizeof(T);
     cudaError_t e = ensure_smem(trsm_diag_kernel<T, 128>, smem, cur);
     if (e != cudaSuccess) return e;
@@ -83,12 +78,12 @@ cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ld
 }
 
 template <typename T>
-cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, cudaStream_t st) {
-    static size_t cur = 0;
+cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, unsigned* cond_bits, cudaStream_t st) {
+    static SmemAttr cur;
     const size_t smem = (size_t)nb * (nb + 1) * sizeof(T);
     cudaError_t e = ensure_smem(trinv_kernel<T>, smem, cur);
     if (e != cudaSuccess) return e;
-    trinv_kernel<T><<<P, 128, smem, st>>>(Rd, nb, n, Rinv);
+    trinv_kernel<T><<<P, 128, smem, st>>>(Rd, nb, n, Rinv, cond_bits);
     return cudaGetLastError();
 }
 
@@ -114,7 +109,7 @@ cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, c
 }
 
 #define INST(T)                                                                                                        \
-    template cudaError_t trinv_launch<T>(const T*, int, int64_t, int, T*, cudaStream_t);                               \
+    template cudaError_t trinv_launch<T>(const T*, int, int64_t, int, T*, unsigned*, cudaStream_t);                             \
     template cudaError_t partial_sum_launch<T>(const T*, SegInfo, int, int64_t, T*, int64_t, cudaStream_t);            \
     template cudaError_t larft_launch<T>(const T*, SegInfo, int64_t, int, int, int, T*, int, cudaStream_t);           \
     template cudaError_t ttw_launch<T>(const T*, SegInfo, int64_t, int64_t, const T*, int, int, int64_t, T*, int64_t,  \

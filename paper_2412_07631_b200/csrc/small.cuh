@@ -344,7 +344,7 @@ trsm_diag_kernel(const T* __restrict__ R, int ldr, int kw, const T* __restrict__
 // X_i = R_ii^{-1} C_i instead of 128 dependent steps per right-hand side.
 template <typename T>
 __global__ void __launch_bounds__(128)
-trinv_kernel(const T* __restrict__ Rd, int nb, int64_t n, T* __restrict__ Rinv) {
+trinv_kernel(const T* __restrict__ Rd, int nb, int64_t n, T* __restrict__ Rinv, unsigned* __restrict__ cond_bits) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* Ms = reinterpret_cast<T*>(smem_raw);          // [nb][nb+1]: R on entry, R^{-1} on exit (in place, column by column)
     const int ld = nb + 1;
@@ -372,6 +372,23 @@ trinv_kernel(const T* __restrict__ Rd, int nb, int64_t n, T* __restrict__ Rinv) 
     for (int e = threadIdx.x; e < nb * nb; e += blockDim.x) {
         const int r = e % nb, c = e / nb;
         out[r + (size_t)c * nb] = Ms[r * ld + c];
+    }
+    // conditioning guard: max|R_jj| / min|R_jj| = max|X_jj| / min|X_jj| of this block (a lower bound of cond(R_ii)),
+    // max over the blocks through an atomicMax on the float's bit pattern (ratios are >= 1, so the order is the same)
+    if (cond_bits && threadIdx.x < 32) {
+        float lo = 3.0e38f, hi = 0.f;
+        for (int j = threadIdx.x; j < kw; j += 32) {
+            const float a = fabsf((float)Ms[j * ld + j]);
+            lo = fminf(lo, a); hi = fmaxf(hi, a);
+        }
+        for (int off = 16; off >= 1; off >>= 1) {
+            lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, off));
+            hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, off));
+        }
+        if (threadIdx.x == 0) {
+            const float ratio = (lo > 0.f && isfinite(hi)) ? hi / lo : __int_as_float(0x7f800000);
+            atomicMax(cond_bits, __float_as_uint(ratio));
+        }
     }
 }
 

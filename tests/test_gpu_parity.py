@@ -26,6 +26,22 @@ def relerr(a, b):
     return np.linalg.norm(a - b) / (den if den > 0 else 1.0)
 
 
+def worst_col(a, b):
+    """Largest per-column relative error (reading 17 asks for the worst column beside the Frobenius figure: one bad
+    slice of a batch must not hide in the norm over all of them).  Columns of b that are exactly zero are compared
+    absolutely."""
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    a = a.reshape(a.shape[0], -1); b = b.reshape(b.shape[0], -1)
+    den = np.linalg.norm(b, axis=0)
+    return float(np.max(np.linalg.norm(a - b, axis=0) / np.where(den > 0, den, 1.0))) if a.size else 0.0
+
+
+def max_abs(a, b):
+    """Largest element error, relative to the largest element of the reference."""
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)) if a.size else 0.0
+
+
 def backward_error(A, V, tau, R):
     """||A - Q R||_F / ||A||_F with Q R evaluated in fp64 from the returned reflectors
     (reading 17): apply H_{n-1} ... H_0 order reversed to [R; 0]."""
@@ -63,10 +79,15 @@ def check_against_oracle(A, B, dt, **opts):
     assert be <= BACKWARD[dt], f"backward error {be}"
     se = relerr(g["X"], X_or)
     assert se <= SOLUTION[dt], f"solution error {se}"
-    # same convention => same R (with signs), V, tau up to rounding
+    # every slice on its own meets the gate, and no single pixel is off by more than the gate times the largest pixel
+    assert worst_col(g["X"], X_or) <= SOLUTION[dt], f"worst slice {worst_col(g['X'], X_or)}"
+    assert max_abs(g["X"], X_or) <= SOLUTION[dt], f"largest element error {max_abs(g['X'], X_or)}"
+    # same convention => same R (with signs), V, tau up to rounding; also column by column and element by element
     assert relerr(g["R"], oracle.R_of(VR)) <= ROUND[dt]
     assert relerr(g["V"], oracle.V_of(VR)) <= ROUND[dt]
     assert relerr(g["tau"], tau) <= ROUND[dt]
+    assert worst_col(g["R"], oracle.R_of(VR)) <= 10 * ROUND[dt] and max_abs(g["R"], oracle.R_of(VR)) <= ROUND[dt]
+    assert worst_col(g["V"], oracle.V_of(VR)) <= 10 * ROUND[dt] and max_abs(g["V"], oracle.V_of(VR)) <= ROUND[dt]
     assert np.all(np.tril(g["R"], -1) == 0)
     return g, VR, tau
 
@@ -165,6 +186,55 @@ def test_singular_solve_refused():
     with pytest.raises(ctqr.CtqrError) as ei:
         ctqr.ct_qr_solve(f, Bt, 1, Xt)
     assert ei.value.code == 4
+
+
+@pytest.mark.parametrize("dt", DT)
+def test_trsm_exact_option_and_conditioning_guard(dt):
+    """Blocked TRSM diagonal tasks: inverted diagonal blocks by default, back-substitution by option,
+    and by itself when a diagonal block of R is ill-conditioned (columns graded over 12 / 5 orders of magnitude)."""
+    rng = np.random.default_rng(77)
+    m, n, S = 700, 384, 11
+    A0 = rng.standard_normal((m, n))
+    B = rng.standard_normal((m, S))
+    # well conditioned: default uses the inverses, the option forces back-substitution, both match the oracle
+    for exact in (False, True):
+        g, VR, tau = check_against_oracle(A0, B, dt, trsm_exact=exact)
+        st = g["f"].stats()
+        assert st["trsm_exact"] == (1 if exact else 0)
+        if not exact:
+            assert 1.0 <= st["diag_block_cond"] < 1e3
+        C = oracle.apply_qt(VR, tau, np.asfortranarray(B.astype(dt)))[:n]
+        X = np.zeros((n, S), dtype=dt, order="F")
+        ctqr.ct_qr_trsm(g["f"], np.asfortranarray(C), S, X)
+        assert relerr(X, oracle.backsub(VR, C)) <= ROUND[dt] * 10
+        g["f"].destroy()
+    # graded columns inside every 128-block: the guard must switch to back-substitution and the solve must be
+    # backward stable: ||R X - C|| <= c n u ||R|| ||X||, column by column
+    span = 12.0 if dt == np.float64 else 5.0
+    scale = 10.0 ** (-span * (np.arange(n) % 128) / 127.0)
+    A = np.asfortranarray((A0 * scale).astype(dt))
+    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m, n)
+    R = ctqr.ct_qr_get_R(f).astype(np.float64)
+    C = np.asfortranarray(rng.standard_normal((n, S)).astype(dt))
+    X = np.zeros((n, S), dtype=dt, order="F")
+    ctqr.ct_qr_trsm(f, C, S, X)
+    st = f.stats()
+    assert st["trsm_exact"] == 2 and st["diag_block_cond"] > (6.7e7 if dt == np.float64 else 2.9e3)
+    X64 = X.astype(np.float64)
+    u = np.finfo(dt).eps
+    res = np.linalg.norm(R @ X64 - C.astype(np.float64), axis=0) / (np.linalg.norm(R) * np.linalg.norm(X64, axis=0))
+    assert res.max() <= 4 * n * u, res.max()
+    f.destroy()
+
+
+def test_trim_cache_releases_blocks():
+    rng = np.random.default_rng(5)
+    A = rng.standard_normal((300, 200))
+    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), 300, 200)
+    f.destroy()                                   # its small buffers go to the process-wide cache
+    assert ctqr.ct_qr_trim_cache() > 0
+    assert ctqr.ct_qr_trim_cache() == 0
+    check_against_oracle(A, rng.standard_normal((300, 3)), np.float64)      # the library works on after a trim
 
 
 @pytest.mark.parametrize("dt", DT)

@@ -141,7 +141,7 @@ def test_out_of_core_uses_the_band(nb, ns, pinned, dt):
         C = B.copy(order="F"); ctqr.ct_qr_apply_qt(f, C, S)
         assert relerr(C, oracle.apply_qt(VR, tau_o, B)) <= ROUND[dt]
         f.destroy()
-    assert h2d[m0] < 0.85 * h2d[0]
+    assert h2d[m0] < 0.95 * h2d[0]          # shorter streamed panels, minus the streamed pass that verifies the promise
 
 
 def test_out_of_core_broken_promise_in_a_later_super_panel():

@@ -149,6 +149,43 @@ int ct_qr_apply_qt(ctqr_handle_t h, void* C, int64_t ldc, int64_t S);
  * C EITHER (n x S used, ldc >= n, read-only), X EITHER (n x S, ldx >= n). */
 int ct_qr_trsm(ctqr_handle_t h, const void* C, int64_t ldc, int64_t S, void* X, int64_t ldx);
 
+/* The transposed half: X <- R^{-T} C (forward substitution with R^T, the task list of PAPER.md:L62-73 read for the
+ * transposed factor).  C EITHER (n x S, ldc >= n, read-only), X EITHER (n x S, ldx >= n).  In-core factors only
+ * (CTQR_ERR_STATE otherwise).  Used by ct_qr_solve_refined; R^{-1} R^{-T} g solves the normal equations A^T A d = g. */
+int ct_qr_trsm_t(ctqr_handle_t h, const void* C, int64_t ldc, int64_t S, void* X, int64_t ldx);
+
+/* Least-squares solve with fp64 iterative refinement on top of a working-precision factor (
+ * the paper's subject is the fp32 / fp64 quality gap, Table 3):
+ *     x_0 = R^{-1}(Q^T b)  in the handle's precision (Eq. 3), then, in fp64,
+ *     r = b - A x,  g = A^T r,  x <- x + R^{-1}(R^{-T} g)      (corrected semi-normal equations)
+ * with the two triangular solves in the handle's precision on g scaled to max|g| = 1 per slice.  The fixed point
+ * is the exact normal-equations solution A^T(b - A x) = 0 of the fp64 operator, also for inconsistent (noisy) b;
+ * the error contracts by about cond(A)^2 * eps(handle precision) per sweep.  With an fp32 handle this gives
+ * fp64-quality reconstructions from a factor that took half the memory and less than half the time.
+ * The operator A (m x n, the matrix that was factored, in fp64) is given EITHER as a CSR pair (A and its transpose
+ * At, 0-based, int64 row pointers, int32 column indices, fp64 values; every array EITHER host or device) OR as a
+ * dense column-major fp64 DEVICE matrix A_dense (leading dimension lda); pass NULL for the form not used.
+ *   B   EITHER, fp64, m x S, ldb >= m.     X   EITHER, fp64, n x S, ldx >= n.
+ *   max_iters  refinement sweeps at most (0 = x_0 only);  tol > 0 stops early when max over slices of
+ *   ||correction||_2 / ||x||_2 <= tol.   info (required) receives what happened.
+ * Errors: argument errors as -i; CTQR_ERR_STATE for an out-of-core handle or a NaN; CTQR_ERR_SINGULAR; CTQR_ERR_CUDA. */
+#define CTQR_REFINE_MAX_ITERS 16
+typedef struct {
+    int64_t m, n, nnz;
+    const int64_t* rowptr;     /* m + 1 entries */
+    const int32_t* colidx;     /* nnz entries, each < n */
+    const double* vals;        /* nnz entries */
+} ctqr_csr_t;
+typedef struct {
+    int32_t iters_done, converged;                 /* sweeps performed; 1 if tol was reached */
+    double correction[CTQR_REFINE_MAX_ITERS];      /* per sweep: max over slices of ||d||_2 / ||x||_2 */
+    double gradient[CTQR_REFINE_MAX_ITERS];        /* per sweep: max over slices of ||A^T (b - A x)||_2 BEFORE the correction */
+    double ms_total, ms_initial_solve, ms_residual, ms_correction;   /* CUDA-event times of the call and its three parts */
+} ctqr_refine_info_t;
+int ct_qr_solve_refined(ctqr_handle_t h, const ctqr_csr_t* A, const ctqr_csr_t* At, const void* A_dense, int64_t lda,
+                        const double* B, int64_t ldb, int64_t S, double* X, int64_t ldx,
+                        int32_t max_iters, double tol, ctqr_refine_info_t* info);
+
 /* Accessors (R, V, T, tau may be HOST or DEVICE pointers; output is dense column-major). */
 int ct_qr_get_R(ctqr_handle_t h, void* R, int64_t ldr);                  /* n x n upper; strictly lower part zeroed */
 int ct_qr_get_V(ctqr_handle_t h, int64_t j0, int64_t ncols, void* V, int64_t ldv); /* m x ncols, unit lower trapezoid */

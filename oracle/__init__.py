@@ -52,6 +52,9 @@ def _load():
             f = getattr(lib, f"oracle_backsub_{suf}")
             f.argtypes = [_P, _I, _I, _P, _I, _I, _P, _I]
             f.restype = ctypes.c_int64
+            f = getattr(lib, f"oracle_backsub_t_{suf}")
+            f.argtypes = [_P, _I, _I, _P, _I, _I, _P, _I]
+            f.restype = ctypes.c_int64
             f = getattr(lib, f"oracle_larft_{suf}")
             f.argtypes = [_P, _I, _I, _P, _I, _I, _P, _I]
             f.restype = ctypes.c_int
@@ -132,6 +135,20 @@ def backsub(VR: np.ndarray, C: np.ndarray) -> np.ndarray:
     if rc != 0:
         raise ZeroDivisionError(f"oracle_backsub: R[{rc - 1},{rc - 1}] == 0")
     return X
+
+
+def backsub_t(VR: np.ndarray, C: np.ndarray) -> np.ndarray:
+    """Y = R^{-T} C[0:n] by forward substitution with the transposed factor."""
+    suf = _suf(VR.dtype)
+    m, n = VR.shape
+    Cf = np.asfortranarray(np.asarray(C, dtype=VR.dtype)).reshape(C.shape[0], -1, order="F")
+    S = Cf.shape[1]
+    Y = np.zeros((n, S), dtype=VR.dtype, order="F")
+    VRf = np.asfortranarray(VR)
+    rc = getattr(_load(), f"oracle_backsub_t_{suf}")(_ptr(VRf), n, max(m, 1), _ptr(Cf), max(Cf.shape[0], 1), S, _ptr(Y), max(n, 1))
+    if rc != 0:
+        raise ZeroDivisionError(f"oracle_backsub_t: R[{rc - 1},{rc - 1}] == 0")
+    return Y
 
 
 def solve(VR: np.ndarray, tau: np.ndarray, B: np.ndarray) -> np.ndarray:

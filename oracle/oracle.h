@@ -9,7 +9,8 @@
  * double (f64) and single (f32) precision, all arithmetic in the working type.
  * Pins (tests/test_oracle_pins.py, tests/golden/): hand-computed 3x2 case, triangular and
  * [I; mu I] closed forms, Gram-Schmidt brute force, |diag R| = diag chol(A^T A), orthogonality,
- * exact recovery, normal equations, T^{-1} = striu(V^T V) + diag(1/tau).  Parity unpinned: none.
+ * exact recovery, normal equations, T^{-1} = striu(V^T V) + diag(1/tau); the transposed substitution by the
+ * semi-normal equations R^T R x = A^T b and closed forms.  Parity unpinned: none.
  */
 #ifndef CT_ORACLE_H
 #define CT_ORACLE_H
@@ -25,6 +26,8 @@ int     oracle_apply_q_f64(const double *A, int64_t m, int64_t n, int64_t lda, c
 int     oracle_apply_q_f32(const float *A, int64_t m, int64_t n, int64_t lda, const float *tau, float *B, int64_t ldb, int64_t S);
 int64_t oracle_backsub_f64(const double *A, int64_t n, int64_t lda, const double *C, int64_t ldc, int64_t S, double *X, int64_t ldx);
 int64_t oracle_backsub_f32(const float *A, int64_t n, int64_t lda, const float *C, int64_t ldc, int64_t S, float *X, int64_t ldx);
+int64_t oracle_backsub_t_f64(const double *A, int64_t n, int64_t lda, const double *C, int64_t ldc, int64_t S, double *Y, int64_t ldy);
+int64_t oracle_backsub_t_f32(const float *A, int64_t n, int64_t lda, const float *C, int64_t ldc, int64_t S, float *Y, int64_t ldy);
 int     oracle_larft_f64(const double *A, int64_t m, int64_t lda, const double *tau, int64_t j0, int64_t nb, double *T, int64_t ldt);
 int     oracle_larft_f32(const float *A, int64_t m, int64_t lda, const float *tau, int64_t j0, int64_t nb, float *T, int64_t ldt);
 int     oracle_num_threads(void);

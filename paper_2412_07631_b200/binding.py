@@ -58,12 +58,30 @@ class Stats(ctypes.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
+REFINE_MAX_ITERS = 16
+
+
+class Csr(ctypes.Structure):
+    _fields_ = [("m", ctypes.c_int64), ("n", ctypes.c_int64), ("nnz", ctypes.c_int64),
+                ("rowptr", ctypes.c_void_p), ("colidx", ctypes.c_void_p), ("vals", ctypes.c_void_p)]
+
+
+class RefineInfo(ctypes.Structure):
+    _fields_ = [("iters_done", ctypes.c_int32), ("converged", ctypes.c_int32),
+                ("correction", ctypes.c_double * REFINE_MAX_ITERS), ("gradient", ctypes.c_double * REFINE_MAX_ITERS),
+                ("ms_total", ctypes.c_double), ("ms_initial_solve", ctypes.c_double),
+                ("ms_residual", ctypes.c_double), ("ms_correction", ctypes.c_double)]
+
+
 _P, _I64, _I = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
 EXPORTS = {
     "ct_qr_factor": ([_P, _I64, _I64, _I64, _I, ctypes.POINTER(Options), ctypes.POINTER(_P)], _I),
     "ct_qr_solve": ([_P, _P, _I64, _I64, _P, _I64], _I),
     "ct_qr_apply_qt": ([_P, _P, _I64, _I64], _I),
     "ct_qr_trsm": ([_P, _P, _I64, _I64, _P, _I64], _I),
+    "ct_qr_trsm_t": ([_P, _P, _I64, _I64, _P, _I64], _I),
+    "ct_qr_solve_refined": ([_P, ctypes.POINTER(Csr), ctypes.POINTER(Csr), _P, _I64, _P, _I64, _I64, _P, _I64,
+                             ctypes.c_int32, ctypes.c_double, ctypes.POINTER(RefineInfo)], _I),
     "ct_qr_get_R": ([_P, _P, _I64], _I),
     "ct_qr_get_V": ([_P, _I64, _I64, _P, _I64], _I),
     "ct_qr_get_T": ([_P, _I64, _P, _I64], _I),
@@ -230,6 +248,44 @@ def ct_qr_apply_qt(f: Factor, C, S: int, ldc: int | None = None):
 def ct_qr_trsm(f: Factor, C, S: int, X, ldc: int | None = None, ldx: int | None = None):
     _check(lib().ct_qr_trsm(f._h, _ptr(C), f.n if ldc is None else ldc, S, _ptr(X), f.n if ldx is None else ldx))
     return X
+
+
+def ct_qr_trsm_t(f: Factor, C, S: int, X, ldc: int | None = None, ldx: int | None = None):
+    """X <- R^{-T} C (transposed half of the normal-equations solve)."""
+    _check(lib().ct_qr_trsm_t(f._h, _ptr(C), f.n if ldc is None else ldc, S, _ptr(X), f.n if ldx is None else ldx))
+    return X
+
+
+def _csr_struct(a, keep: list) -> Csr:
+    """scipy.sparse CSR matrix (any index dtype) -> ctqr_csr_t over host arrays that `keep` holds alive."""
+    rp = np.ascontiguousarray(a.indptr, dtype=np.int64)
+    ci = np.ascontiguousarray(a.indices, dtype=np.int32)
+    va = np.ascontiguousarray(a.data, dtype=np.float64)
+    keep += [rp, ci, va]
+    return Csr(m=a.shape[0], n=a.shape[1], nnz=int(a.nnz), rowptr=rp.ctypes.data, colidx=ci.ctypes.data, vals=va.ctypes.data)
+
+
+def ct_qr_solve_refined(f: Factor, B, S: int, X, *, A_csr=None, At_csr=None, A_dense=None, lda: int | None = None,
+                        max_iters: int = 3, tol: float = 0.0, ldb: int | None = None, ldx: int | None = None) -> dict:
+    """fp64 solution from a working-precision factor by iterative refinement (include/ctqr.h).  The fp64 operator is
+    either ``A_csr`` (scipy CSR, m x n; ``At_csr`` defaults to its transpose) or ``A_dense`` (device tensor whose memory
+    is the column-major m x n fp64 matrix).  B, X: fp64, column-major m x S / n x S.  Returns the info block as a dict."""
+    keep: list = []
+    pa = pat = None
+    if A_csr is not None:
+        a = A_csr.tocsr()
+        at = (At_csr if At_csr is not None else a.T).tocsr()
+        a.sort_indices(); at.sort_indices()
+        sa, sat = _csr_struct(a, keep), _csr_struct(at, keep)
+        pa, pat = ctypes.byref(sa), ctypes.byref(sat)
+    info = RefineInfo()
+    _check(lib().ct_qr_solve_refined(f._h, pa, pat, _ptr(A_dense) if A_dense is not None else None,
+                                     (f.m if lda is None else lda), _ptr(B), f.m if ldb is None else ldb, S,
+                                     _ptr(X), f.n if ldx is None else ldx, max_iters, tol, ctypes.byref(info)))
+    k = info.iters_done
+    return {"iters_done": k, "converged": bool(info.converged), "correction": list(info.correction)[:k],
+            "gradient": list(info.gradient)[:k], "ms_total": info.ms_total, "ms_initial_solve": info.ms_initial_solve,
+            "ms_residual": info.ms_residual, "ms_correction": info.ms_correction}
 
 
 def ct_qr_get_R(f: Factor) -> np.ndarray:

@@ -16,6 +16,7 @@
 #include <map>
 #include <mutex>
 #include <new>
+#include <thread>
 #include <unordered_map>
 #include <vector>
 
@@ -61,6 +62,10 @@ static int set_err(int code, const char* fmt, ...) {
 #define CKI(call) do { int r_ = (call); if (r_ != 0) return r_; } while (0)
 
 extern "C" const char* ct_qr_last_error(void) { return g_err; }
+// error plumbing for the library's other translation units (refine.cu); not part of the ABI
+extern "C" __attribute__((visibility("hidden"))) int ctqr_internal_set_error(int code, const char* what, const char* detail) {
+    return set_err(code, "%s%s%s", what, (detail && detail[0]) ? ": " : "", detail ? detail : "");
+}
 extern "C" const char* ct_qr_strerror(int code) {
     if (code < 0) return "invalid argument (the -code-th argument)";
     switch (code) {
@@ -1226,23 +1231,22 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
     return 0;
 }
 
+// Common preamble of the triangular solves: refuse a singular R, build the inverted diagonal blocks once per handle.
+// Diagonal tasks X_i = R_ii^{-1} C_i: by default a product with the explicitly inverted 128 x 128 diagonal
+// block (inverted once per handle, by back-substitution on the identity, working precision), which turns 128
+// dependent steps per right-hand side into one small contraction.  The off-diagonal part of R^{-1} is never
+// formed.  A product with an explicit inverse is only conditionally backward stable, so the
+// back-substitution kernel is used instead when opt->trsm_exact is set, or when some diagonal block looks
+// ill-conditioned: max|R_jj| / min|R_jj| inside the block (a lower bound of its condition number) above
+// 1/sqrt(eps) of the working type.
 template <typename T>
-static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
-    // X holds C[0:n,:] on entry.  Bottom-up over diagonal blocks (PAPER.md:L62-73):
-    //   R_ii X_i = C_i ;  C_j <- C_j - R_ji X_i  for all j < i (one GEMM over rows 0..i0)
+static int trsm_prepare(H& h) {
     CK(cudaMemsetAsync(h.dFlag, 0x7f, sizeof(int), h.sU));
     CK(find_zero_diag_launch<T>(P_<T>(h.dRd), h.nb, h.n, h.dFlag, h.sU));
     int flag = 0;
     CK(cudaMemcpyAsync(&flag, h.dFlag, sizeof(int), cudaMemcpyDeviceToHost, h.sU));
     CK(cudaStreamSynchronize(h.sU));
     if (flag < h.n) { h.st.singular_col = flag; return set_err(CTQR_ERR_SINGULAR, "R[%d,%d] == 0", flag, flag); }
-    // Diagonal tasks X_i = R_ii^{-1} C_i: by default a product with the explicitly inverted 128 x 128 diagonal
-    // block (inverted once per handle, by back-substitution on the identity, working precision), which turns 128
-    // dependent steps per right-hand side into one small contraction.  The off-diagonal part of R^{-1} is never
-    // formed.  A product with an explicit inverse is only conditionally backward stable, so the
-    // back-substitution kernel is used instead when opt->trsm_exact is set, or when some diagonal block looks
-    // ill-conditioned: max|R_jj| / min|R_jj| inside the block (a lower bound of its condition number) above
-    // 1/sqrt(eps) of the working type.
     if (!h.trsm_exact && h.dRinv && !h.rinv_ready) {
         CK(cudaMemsetAsync(h.dFlag, 0, sizeof(int), h.sU));
         CK(trinv_launch<T>(P_<T>(h.dRd), h.nb, h.n, h.P, P_<T>(h.dRinv), reinterpret_cast<unsigned*>(h.dFlag), h.sU));
@@ -1256,6 +1260,14 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
         if (!(ratio <= (sizeof(T) == 8 ? 6.7e7f : 2.9e3f))) h.trsm_exact = 2;      // also catches NaN
     }
     h.st.trsm_exact = h.trsm_exact;
+    return 0;
+}
+
+template <typename T>
+static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
+    // X holds C[0:n,:] on entry.  Bottom-up over diagonal blocks (PAPER.md:L62-73):
+    //   R_ii X_i = C_i ;  C_j <- C_j - R_ji X_i  for all j < i (one GEMM over rows 0..i0)
+    CKI(trsm_prepare<T>(h));
     const bool exact = h.trsm_exact != 0;
     const bool use_inv = !exact && h.dRinv && ldx % (16 / (int64_t)sizeof(T)) == 0;
     if (S <= kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && h.gemm_impl == 0) {
@@ -1322,6 +1334,42 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
     return 0;
 }
 
+// X <- R^{-T} C: forward substitution with the transposed factor, top-down over the diagonal blocks,
+//   Y_i = R_ii^{-T} C_i ;  C[i0+nb:, :] <- C[i0+nb:, :] - R[i0:i0+nb, i0+nb:n]^T Y_i
+// (the same task list as PAPER.md:L62-73 read for R^T; used by the semi-normal-equations refinement
+// ct_qr_solve_refined).  In-core factors only.
+template <typename T>
+static int trsm_t_dev(H& h, T* X, int64_t ldx, int64_t S) {
+    if (h.ooc) return set_err(CTQR_ERR_STATE, "the transposed triangular solve needs an in-core factor");
+    CKI(trsm_prepare<T>(h));
+    const bool use_inv = h.trsm_exact == 0 && h.dRinv && h.rinv_ready;
+    T* W = P_<T>(h.dW[0]);
+    for (int i = 0; i < h.P; ++i) {
+        const int64_t i0 = (int64_t)i * h.nb;
+        const int nbw = (int)std::min<int64_t>(h.nb, h.n - i0);
+        if (use_inv) {
+            GemmArgs<T> gi{};
+            gi.M = nbw; gi.N = S; gi.K = nbw; gi.A = P_<T>(h.dRinv) + (size_t)i * h.nb * h.nb; gi.lda = h.nb;
+            gi.B = X + i0; gi.ldb = ldx; gi.C = W; gi.ldc = h.nb; gi.alpha = T(1); gi.beta = T(0);
+            CK(gemm_direct<T>(true, gi, h.gemm_impl, h.sms, h.sU));
+            CK(copy2d_launch<T>(W, h.nb, X + i0, ldx, nbw, S, h.sU));
+            h.launches += 2;
+        } else {
+            CK(trsm_diag_t_launch<T>(P_<T>(h.dRd) + (size_t)i * h.nb * h.nb, h.nb, nbw, X + i0, ldx, S, h.sU));
+            h.launches += 1;
+        }
+        const int64_t rest = h.n - i0 - nbw;
+        if (rest > 0) {
+            GemmArgs<T> g{};
+            g.M = rest; g.N = S; g.K = nbw; g.A = P_<T>(h.dA) + i0 + (i0 + nbw) * h.lda; g.lda = h.lda;
+            g.B = X + i0; g.ldb = ldx; g.C = X + i0 + nbw; g.ldc = ldx; g.alpha = T(-1); g.beta = T(1);
+            CK(gemm_direct<T>(true, g, h.gemm_impl, h.sms, h.sU));
+            h.launches += 1;
+        }
+    }
+    return 0;
+}
+
 // stage an m x S host or device matrix into a fresh device buffer (ld = rows rounded up)
 template <typename T>
 static int stage_in(H& h, const void* src, int64_t lds, int64_t rows, int64_t S, T** out, int64_t* ldo, bool* owned) {
@@ -1338,7 +1386,7 @@ static int stage_in(H& h, const void* src, int64_t lds, int64_t rows, int64_t S,
 
 template <typename T>
 static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int64_t ldx, int mode) {
-    // mode 0: full solve; 1: apply Q^T in place on B (B is also the output); 2: trsm only (B = C)
+    // mode 0: full solve; 1: apply Q^T in place on B (B is also the output); 2: trsm only (B = C); 3: X = R^{-T} C
     CKI(ensure_solve_ws(h, S));
     h.launches = 0; h.st.h2d_bytes = 0; h.st.d2h_bytes = 0;
     if (!h.evS[0])
@@ -1346,7 +1394,7 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
             if (!(h.evS[i] = new_event(h, true))) { h.evS[0] = nullptr; return set_err(CTQR_ERR_CUDA, "cudaEventCreate failed"); }
     cudaEvent_t t0 = h.evS[0], t1 = h.evS[1], t2 = h.evS[2];
     const int64_t m = h.m, n = h.n;
-    const int64_t rows_in = (mode == 2) ? n : m;
+    const int64_t rows_in = (mode >= 2) ? n : m;
     // working buffer Cw (rows_in x S) on the device
     const int64_t ldw = round_up(rows_in, 16 / sizeof(T));
     T* Cw = nullptr;
@@ -1369,9 +1417,9 @@ static int solve_typed(H& h, const void* B, int64_t ldb, int64_t S, void* X, int
     const int64_t ldcw = inplace_dev ? ldb : ldw;
     int rc = 0;
     cudaEventRecord(t0, h.sU);
-    if (mode != 2) rc = apply_qt_dev<T>(h, Cw, ldcw, S);
+    if (mode < 2) rc = apply_qt_dev<T>(h, Cw, ldcw, S);
     cudaEventRecord(t1, h.sU);
-    if (rc == 0 && mode != 1) rc = trsm_dev<T>(h, Cw, ldcw, S);
+    if (rc == 0 && mode != 1) rc = mode == 3 ? trsm_t_dev<T>(h, Cw, ldcw, S) : trsm_dev<T>(h, Cw, ldcw, S);
     cudaEventRecord(t2, h.sU);
     if (rc == 0) {
         if (mode == 1) {
@@ -1432,6 +1480,20 @@ extern "C" int ct_qr_apply_qt(ctqr_handle_t h, void* C, int64_t ldc, int64_t S) 
     if (cudaStreamSynchronize(h->user) != cudaSuccess) return set_err(CTQR_ERR_CUDA, "user stream sync failed");
     return h->dtype == CTQR_F64 ? solve_typed<double>(*h, C, ldc, S, nullptr, 0, 1)
                                 : solve_typed<float>(*h, C, ldc, S, nullptr, 0, 1);
+}
+
+extern "C" int ct_qr_trsm_t(ctqr_handle_t h, const void* C, int64_t ldc, int64_t S, void* X, int64_t ldx) {
+    g_err[0] = 0;
+    CKI(check_handle(h));
+    if (!C) return set_err(-2, "C is NULL");
+    if (ldc < h->n) return set_err(-3, "ldc < n");
+    if (S < 0) return set_err(-4, "S < 0");
+    if (!X) return set_err(-5, "X is NULL");
+    if (ldx < h->n) return set_err(-6, "ldx < n");
+    if (S == 0) return 0;
+    if (cudaStreamSynchronize(h->user) != cudaSuccess) return set_err(CTQR_ERR_CUDA, "user stream sync failed");
+    return h->dtype == CTQR_F64 ? solve_typed<double>(*h, C, ldc, S, X, ldx, 3)
+                                : solve_typed<float>(*h, C, ldc, S, X, ldx, 3);
 }
 
 extern "C" int ct_qr_trsm(ctqr_handle_t h, const void* C, int64_t ldc, int64_t S, void* X, int64_t ldx) {
@@ -1582,7 +1644,7 @@ struct FactorFileHeader {
 };
 static const char kFactorMagic[8] = {'C', 'T', 'Q', 'R', 'F', 'A', 'C', '1'};
 constexpr size_t kFactorHeaderBytes = 4096;
-constexpr size_t kIoChunkBytes = (size_t)64 << 20;
+constexpr size_t kIoChunkBytes = (size_t)256 << 20;   // pinned bounce buffer of save / load, used as two halves
 
 static int write_all(int fd, const void* buf, size_t len, const char* path) {
     const char* p = (const char*)buf;
@@ -1604,13 +1666,43 @@ static int read_all(int fd, void* buf, size_t len, const char* path) {
     return 0;
 }
 
-// device section -> file through a pinned bounce buffer
-static int save_device_section(H& h, int fd, const void* dsrc, size_t bytes, void* bounce, const char* path) {
-    for (size_t off = 0; off < bytes; off += kIoChunkBytes) {
-        const size_t len = std::min(kIoChunkBytes, bytes - off);
-        CK(cudaMemcpyAsync(bounce, (const char*)dsrc + off, len, cudaMemcpyDeviceToHost, h.sU));
+// One chunk of a file write running on its own thread (pwrite at an explicit offset, then an asynchronous
+// write-back hint so the disk starts on it at once): ct_qr_save overlaps it with the device-to-host copy of the
+// next chunk into the other half of the bounce buffer.
+struct ChunkWriter {
+    std::thread th;
+    int err = 0;                       // errno of a failed pwrite (0 = fine); read after wait()
+    void start(int fd, const char* buf, size_t len, off_t off) {
+        wait();
+        err = 0;
+        th = std::thread([this, fd, buf, len, off] {
+            const char* p = buf; size_t left = len; off_t o = off;
+            while (left > 0) {
+                ssize_t k = pwrite(fd, p, left, o);
+                if (k < 0) { if (errno == EINTR) continue; err = errno; return; }
+                p += k; left -= (size_t)k; o += k;
+            }
+            sync_file_range(fd, off, (off_t)len, SYNC_FILE_RANGE_WRITE);
+        });
+    }
+    void wait() { if (th.joinable()) th.join(); }
+    ~ChunkWriter() { wait(); }
+};
+
+// device section -> file at offset *off through the two halves of the pinned bounce buffer
+static int save_device_section(H& h, int fd, const void* dsrc, size_t bytes, void* bounce, const char* path,
+                               ChunkWriter& wr, int& half_idx, off_t* off) {
+    const size_t half = kIoChunkBytes / 2;
+    for (size_t o = 0; o < bytes; o += half) {
+        const size_t len = std::min(half, bytes - o);
+        char* buf = (char*)bounce + (size_t)half_idx * half;
+        CK(cudaMemcpyAsync(buf, (const char*)dsrc + o, len, cudaMemcpyDeviceToHost, h.sU));
         CK(cudaStreamSynchronize(h.sU));
-        CKI(write_all(fd, bounce, len, path));
+        wr.wait();                                             // the other half's write (it may still own the disk)
+        if (wr.err) return set_err(CTQR_ERR_IO, "write to %s failed: %s", path, strerror(wr.err));
+        wr.start(fd, buf, len, *off);
+        *off += (off_t)len;
+        half_idx ^= 1;
     }
     return 0;
 }
@@ -1646,18 +1738,24 @@ static int save_body(H& h, int fd, const char* path, void* bounce) {
     hd.off_Rd = hd.off_T + (uint64_t)blk * h.P;
     hd.off_tau = hd.off_Rd + (uint64_t)blk * h.P;
     hd.file_bytes = hd.off_tau + (uint64_t)h.n * w;
+    if (posix_fallocate(fd, 0, (off_t)hd.file_bytes) != 0) { /* not fatal: some file systems cannot preallocate */ }
     std::vector<char> page(kFactorHeaderBytes, 0);
     memcpy(page.data(), &hd, sizeof hd);
     CKI(write_all(fd, page.data(), page.size(), path));
-    // matrix storage, a chunk of whole columns at a time (padding rows of the file are zero)
+    // matrix storage, whole columns at a time (padding rows of the file are zero): the device-to-host copy of one
+    // chunk into one half of the bounce buffer overlaps the file write of the previous chunk from the other half
     const size_t col_bytes = (size_t)hd.ld * w;
-    const int64_t cols_per = std::max<int64_t>(1, (int64_t)(kIoChunkBytes / col_bytes));
-    const size_t slab = col_bytes <= kIoChunkBytes ? kIoChunkBytes : col_bytes;
-    std::vector<char> big;
-    char* buf = (char*)bounce;
-    if (slab > kIoChunkBytes) { big.resize(slab); buf = big.data(); }    // one column exceeds the bounce buffer: pageable
-    for (int64_t c0 = 0; c0 < h.n; c0 += cols_per) {
+    const size_t half = kIoChunkBytes / 2;
+    const int64_t cols_per = std::max<int64_t>(1, (int64_t)(half / col_bytes));
+    std::vector<char> big[2];
+    char* bufs[2] = {(char*)bounce, (char*)bounce + half};
+    if (col_bytes > half) { for (auto& v : big) v.resize(col_bytes); bufs[0] = big[0].data(); bufs[1] = big[1].data(); }   // pageable
+    ChunkWriter wr;
+    off_t off = (off_t)hd.off_matrix;
+    int hi = 0;
+    for (int64_t c0 = 0; c0 < h.n; c0 += cols_per, hi ^= 1) {
         const int64_t nc = std::min<int64_t>(cols_per, h.n - c0);
+        char* buf = bufs[hi];
         if (hd.ld != h.m) memset(buf, 0, (size_t)nc * col_bytes);
         if (h.ooc) {
             for (int64_t c = 0; c < nc; ++c)
@@ -1667,11 +1765,19 @@ static int save_body(H& h, int fd, const char* path, void* bounce) {
                                  (size_t)h.m * w, nc, cudaMemcpyDeviceToHost, h.sU));
             CK(cudaStreamSynchronize(h.sU));
         }
-        CKI(write_all(fd, buf, (size_t)nc * col_bytes, path));
+        wr.wait();
+        if (wr.err) return set_err(CTQR_ERR_IO, "write to %s failed: %s", path, strerror(wr.err));
+        wr.start(fd, buf, (size_t)nc * col_bytes, off);
+        off += (off_t)((size_t)nc * col_bytes);
     }
-    CKI(save_device_section(h, fd, h.dT, blk * h.P, bounce, path));
-    CKI(save_device_section(h, fd, h.dRd, blk * h.P, bounce, path));
-    CKI(save_device_section(h, fd, h.dTau, (size_t)h.n * w, bounce, path));
+    wr.wait();
+    if (wr.err) return set_err(CTQR_ERR_IO, "write to %s failed: %s", path, strerror(wr.err));
+    int half_idx = 0;
+    CKI(save_device_section(h, fd, h.dT, blk * h.P, bounce, path, wr, half_idx, &off));
+    CKI(save_device_section(h, fd, h.dRd, blk * h.P, bounce, path, wr, half_idx, &off));
+    CKI(save_device_section(h, fd, h.dTau, (size_t)h.n * w, bounce, path, wr, half_idx, &off));
+    wr.wait();
+    if (wr.err) return set_err(CTQR_ERR_IO, "write to %s failed: %s", path, strerror(wr.err));
     return 0;
 }
 

@@ -76,6 +76,8 @@ template <typename T> cudaError_t ttw_launch(const T* Wp, SegInfo seg, int64_t w
 // dense (kw x N, ld = ldo) sum of the compact stream-K partial tiles (seg.L > 0)
 template <typename T> cudaError_t partial_sum_launch(const T* Wp, SegInfo seg, int kw, int64_t N, T* Wout, int64_t ldo, cudaStream_t st);
 template <typename T> cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ldc, int64_t S, T* X, int64_t ldx, cudaStream_t st);
+// X <- R^{-T} X in place on one kw x kw diagonal block (forward substitution with the transposed block)
+template <typename T> cudaError_t trsm_diag_t_launch(const T* R, int ldr, int kw, T* X, int64_t ldx, int64_t S, cudaStream_t st);
 // inverses of the P diagonal blocks of R (nb x nb each, ld = nb; a narrower last block is padded with zeros)
 // out = op(M) * in, M 128 x 128 upper triangular (zeros stored), N <= a few hundred columns; `in` is either a matrix
 // (seg.L == 0; may alias out) or the stream-K partial tiles of a 128 x N product (seg.L != 0)

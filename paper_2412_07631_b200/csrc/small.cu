@@ -78,6 +78,16 @@ cudaError_t trsm_diag_launch(const T* R, int ldr, int kw, const T* C, int64_t ld
 }
 
 template <typename T>
+cudaError_t trsm_diag_t_launch(const T* R, int ldr, int kw, T* X, int64_t ldx, int64_t S, cudaStream_t st) {
+    static SmemAttr cur;
+    const size_t smem = ((size_t)kw * (kw + 1) + (size_t)kw * kTrsmTThreads) * sizeof(T);
+    cudaError_t e = ensure_smem(trsm_diag_t_kernel<T>, smem, cur);
+    if (e != cudaSuccess) return e;
+    trsm_diag_t_kernel<T><<<(unsigned)ceil_div(S, (int64_t)kTrsmTThreads), kTrsmTThreads, smem, st>>>(R, ldr, kw, X, ldx, S);
+    return cudaGetLastError();
+}
+
+template <typename T>
 cudaError_t trinv_launch(const T* Rd, int nb, int64_t n, int P, T* Rinv, unsigned* cond_bits, cudaStream_t st) {
     static SmemAttr cur;
     const size_t smem = (size_t)nb * (nb + 1) * sizeof(T);
@@ -116,6 +126,7 @@ cudaError_t find_zero_diag_launch(const T* Rd, int nb, int64_t n, int* result, c
                                        cudaStream_t);                                                                  \
     template cudaError_t mm128_launch<T>(bool, const T*, int, const T*, int64_t, SegInfo, int64_t, T*, int64_t, cudaStream_t); \
     template cudaError_t trsm_diag_launch<T>(const T*, int, int, const T*, int64_t, int64_t, T*, int64_t, cudaStream_t); \
+    template cudaError_t trsm_diag_t_launch<T>(const T*, int, int, T*, int64_t, int64_t, cudaStream_t);                  \
     template cudaError_t copy2d_launch<T>(const T*, int64_t, T*, int64_t, int64_t, int64_t, cudaStream_t);             \
     template cudaError_t gather_R_launch<T>(const T*, int64_t, const T*, int, int64_t, T*, int64_t, cudaStream_t);     \
     template cudaError_t find_zero_diag_launch<T>(const T*, int, int64_t, int*, cudaStream_t);

@@ -392,6 +392,36 @@ trinv_kernel(const T* __restrict__ Rd, int nb, int64_t n, T* __restrict__ Rinv, 
     }
 }
 
+// Y = R^{-T} C in place on one diagonal block (the transposed solve of ct_qr_trsm_t when the inverted blocks are
+// not used): forward substitution y_j = (c_j - sum_{k<j} R[k][j] y_k) / R[j][j], one thread per right-hand side,
+// R staged in shared memory, the solution kept in shared memory (column per thread).
+constexpr int kTrsmTThreads = 64;
+template <typename T>
+__global__ void __launch_bounds__(kTrsmTThreads)
+trsm_diag_t_kernel(const T* __restrict__ R, int ldr, int kw, T* __restrict__ X, int64_t ldx, int64_t S) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NT = kTrsmTThreads;
+    T* Rs = reinterpret_cast<T*>(smem_raw);          // [kw][kw + 1]: Rs[j * ld + k] = R[k][j] (column j contiguous)
+    const int ld = kw + 1;
+    T* Ys = Rs + (size_t)kw * ld;                    // [kw][NT]
+    const int tid = threadIdx.x;
+    const int64_t col = (int64_t)blockIdx.x * NT + tid;
+    for (int e = tid; e < kw * kw; e += NT) {
+        const int k = e % kw, j = e / kw;
+        Rs[j * ld + k] = R[k + (size_t)j * ldr];
+    }
+    __syncthreads();
+    if (col >= S) return;
+    T* x = X + col * ldx;
+    for (int j = 0; j < kw; ++j) {
+        T acc = x[j];
+        const T* rj = Rs + j * ld;
+        for (int k = 0; k < j; ++k) acc = fma(-rj[k], Ys[k * NT + tid], acc);
+        Ys[j * NT + tid] = Num<T>::div(acc, rj[j]);
+    }
+    for (int j = 0; j < kw; ++j) x[j] = Ys[j * NT + tid];
+}
+
 // ---- utility kernels -----------------------------------------------------------------------
 template <typename T>
 __global__ void copy2d_kernel(const T* __restrict__ src, int64_t lds, T* __restrict__ dst, int64_t ldd,

@@ -29,7 +29,7 @@ from dataclasses import dataclass
 import numpy as np
 
 __all__ = [
-    "CTConfig", "CONFIGS", "siddon_coo", "tikhonov_lambda", "dense_augmented", "dense_augmented_device",
+    "CTConfig", "CONFIGS", "FanBeamConfig", "FAN_CONFIGS", "siddon_coo", "joseph_fanbeam_coo", "fanbeam_dense", "fanbeam_slices", "tikhonov_lambda", "dense_augmented", "dense_augmented_device",
     "ellipse_phantom", "make_slices", "chord_length", "psnr", "snr", "ssim", "shard_slices",
 ]
 
@@ -152,6 +152,126 @@ def chord_length(N: int, n_ang: int, n_bins: int) -> np.ndarray:
             length = np.where((s > -half) & (s <= half), length, 0.0)
         out[a] = length
     return out.reshape(-1)
+
+
+# ----------------------------------------------------------------------------------------
+# The paper's own geometry at reduced scale: fan beam, Joseph's projector
+# (Table 1: 360 degree circular scan, source-to-isocentre 75 cm, source-to-
+# detector 150 cm, fan angle 30 degrees, 1025 detectors, 512 x 512 pixels, 260 views; Table 5,
+# L222-232, is the same with 65 cm / 33 degrees).  No Tikhonov block: like the paper, the number
+# of views is chosen so that A has full column rank (L93-95).
+#
+# Readings (the paper gives the distances but not the pixel size, the detector shape or the
+# details of the projector):
+#   * pixel size 1 and the image square as in the Siddon conventions above; the fan covers the
+#     circle circumscribed to the image, radius N / sqrt(2), so the source-to-isocentre distance is
+#     D = (N / sqrt 2) / sin(fan / 2) pixels; the detector is an arc of n_det equal angles
+#     (gamma_k = (k - (n_det - 1)/2) * fan / n_det), so the source-to-detector distance does not
+#     enter the ray geometry;
+#   * view v has the source at angle beta_v = 2 pi v / n_views, position D (cos beta, sin beta);
+#     the ray of detector k leaves it in direction beta_v + pi + gamma_k; row index i = v n_det + k;
+#   * Joseph's method: a ray with |dx| >= |dy| is sampled at every pixel-column centre, where the
+#     image is interpolated linearly between the two nearest row centres, each sample weighted
+#     by the path length per column 1 / |dx|; otherwise the same over rows.  Equivalently
+#     a_ij = (1 / |dx|) * hat(row coordinate of the ray at column c(j) - r(j)), hat(t) = max(0, 1 - |t|);
+#     samples whose neighbour lies outside the image keep only the inside weight.
+# ----------------------------------------------------------------------------------------
+@dataclass(frozen=True)
+class FanBeamConfig:
+    name: str
+    N: int
+    n_det: int
+    n_views: int
+    S: int
+    fan_deg: float = 30.0
+
+    @property
+    def n(self) -> int:
+        return self.N * self.N
+
+    @property
+    def m(self) -> int:
+        return self.n_det * self.n_views
+
+
+# Table 1 scaled down with the same proportions (detectors = 2 N + 1); the paper's 260 views for 512 x 512 are
+# m / n = 1.017.  With the fan covering the circumscribed circle many outer rays only graze the corners, so at this
+# scale full rank needs m / n of about 1.2 (19 views at N = 32: cond 2.7e4; 21: 2.9e3; 24: 7.9e2) -- the behaviour the
+# paper reports in L93-95 and L240-242 (a few more views needed for a well-conditioned single-precision solve).
+FAN_CONFIGS = {
+    "fan32": FanBeamConfig("fan32", 32, 65, 24, 8),
+    "fan64": FanBeamConfig("fan64", 64, 129, 48, 16),
+    "fan128": FanBeamConfig("fan128", 128, 257, 96, 64),
+}
+
+
+def joseph_fanbeam_coo(N: int, n_det: int, n_views: int, fan_deg: float = 30.0):
+    """Joseph-projector weights of the fan-beam scanner as COO triplets (rows int64 in [0, n_views * n_det),
+    cols int64 in [0, N * N), vals float64); no duplicates."""
+    half = N / 2.0
+    fan = math.radians(fan_deg)
+    D = (N / math.sqrt(2.0)) / math.sin(fan / 2.0)
+    gam = (np.arange(n_det, dtype=np.float64) - (n_det - 1) / 2.0) * (fan / n_det)
+    centres = (np.arange(N, dtype=np.float64) + 0.5) - half      # x of column c; y of row r is -centres[r]
+    idx = np.arange(N, dtype=np.int64)
+    out_r, out_c, out_v = [], [], []
+    for v in range(n_views):
+        beta = 2.0 * math.pi * v / n_views
+        sx, sy = D * math.cos(beta), D * math.sin(beta)
+        phi = beta + math.pi + gam
+        dx, dy = np.cos(phi), np.sin(phi)
+        hor = np.abs(dx) >= np.abs(dy)
+        for sel, along_x in ((hor, True), (~hor, False)):
+            ks = np.nonzero(sel)[0]
+            if ks.size == 0:
+                continue
+            if along_x:      # sample at column centres x_c: y = sy + (x_c - sx) dy / dx, fractional row = N/2 - y - 1/2
+                L = 1.0 / np.abs(dx[ks])
+                t = half - (sy + (centres[None, :] - sx) * (dy[ks] / dx[ks])[:, None]) - 0.5
+            else:            # sample at row centres y_r = -centres[r]: x = sx + (y_r - sy) dx / dy, fractional column = x + N/2 - 1/2
+                L = 1.0 / np.abs(dy[ks])
+                t = (sx + (-centres[None, :] - sy) * (dx[ks] / dy[ks])[:, None]) + half - 0.5
+            i0 = np.floor(t).astype(np.int64)
+            w1 = t - i0
+            for other, w in ((i0, 1.0 - w1), (i0 + 1, w1)):
+                ok = (other >= 0) & (other < N) & (w > 0.0)
+                kk, jj = np.nonzero(ok)
+                out_r.append(v * n_det + ks[kk])
+                out_c.append(other[ok] * N + idx[jj] if along_x else idx[jj] * N + other[ok])
+                out_v.append((L[:, None] * w)[ok])
+    return (np.concatenate(out_r).astype(np.int64), np.concatenate(out_c).astype(np.int64), np.concatenate(out_v))
+
+
+def fanbeam_dense(cfg: FanBeamConfig, dtype=np.float64, coo=None) -> np.ndarray:
+    """Dense column-major A (m x n) of a fan-beam config, generated in fp64 and rounded once to ``dtype``."""
+    rows, cols, vals = coo if coo is not None else joseph_fanbeam_coo(cfg.N, cfg.n_det, cfg.n_views, cfg.fan_deg)
+    A = np.zeros((cfg.m, cfg.n), dtype=np.float64, order="F")
+    A[rows, cols] = vals
+    return np.asfortranarray(A.astype(dtype))
+
+
+def fanbeam_slices(cfg: FanBeamConfig, S: int | None = None, coo=None, I0: float | None = None):
+    """Phantoms X0 (n, S) and sinograms B = A X0 (m, S), fp64 Fortran order; seeds default_rng(7000 + N + slice).
+    I0 = None: noiseless, consistent (the paper's full-dose regime, Tables 2-3); else Poisson noise at I0 photons
+    with kappa = 4 / N as in make_slices (its low-dose regime, L208-212)."""
+    import scipy.sparse as sp
+    S = cfg.S if S is None else S
+    rows, cols, vals = coo if coo is not None else joseph_fanbeam_coo(cfg.N, cfg.n_det, cfg.n_views, cfg.fan_deg)
+    A = sp.coo_matrix((vals, (rows, cols)), shape=(cfg.m, cfg.n)).tocsr()
+    X0 = np.zeros((cfg.n, S), order="F")
+    B = np.zeros((cfg.m, S), order="F")
+    kappa = 4.0 / cfg.N
+    for sl in range(S):
+        rng = np.random.default_rng(7000 + cfg.N + sl)
+        x = ellipse_phantom(cfg.N, rng).reshape(-1)
+        X0[:, sl] = x
+        p = A @ x
+        if I0 is None:
+            B[:, sl] = p
+        else:
+            y = rng.poisson(I0 * np.exp(-kappa * p)).astype(np.float64)
+            B[:, sl] = -np.log(np.maximum(y, 1.0) / I0) / kappa
+    return X0, B
 
 
 def tikhonov_lambda(vals: np.ndarray, n: int) -> float:

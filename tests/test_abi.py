@@ -41,8 +41,7 @@ def test_struct_layouts_match_the_header(tmp_path):
     every offsetof; names, order, offsets and sizes must agree."""
     import subprocess
     pairs = (("ctqr_options_t", binding.Options), ("ctqr_stats_t", binding.Stats))
-    if hasattr(binding, "Csr"):
-        pairs += (("ctqr_csr_t", binding.Csr),)
+    pairs += (("ctqr_csr_t", binding.Csr), ("ctqr_refine_info_t", binding.RefineInfo))
     lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "ctqr.h"', 'int main(void) {']
     for cname, cls in pairs:
         lines.append(f'printf("%zu\\n", sizeof({cname}));')

@@ -248,6 +248,40 @@ def test_backsub_closed_forms(dt):
     np.testing.assert_allclose(X, Y[::-1], rtol=tol(dt, 1e4), atol=tol(dt, 1e2))
 
 
+@pytest.mark.parametrize("dt", DT)
+def test_backsub_t_closed_forms_and_semi_normal_equations(dt):
+    """The transposed substitution (R^T Y = C): identity, the bidiagonal closed form (now a running sum from the
+    top), forward substitution written out, a transposed operand caught by an unsymmetric R, and the use it is
+    made for -- R^{-1} R^{-T} (A^T b) is the least-squares solution (semi-normal equations) -- against lstsq."""
+    n = 12
+    C = rnd(n, 3, 21, dt)
+    np.testing.assert_array_equal(oracle.backsub_t(np.eye(n, dtype=dt, order="F"), C), C)
+    R = np.eye(n) - np.diag(np.ones(n - 1), 1)           # R^T = I - subdiag(1): y_j = c_j + y_{j-1}
+    c = np.arange(1, n + 1, dtype=np.float64).reshape(-1, 1)
+    y = oracle.backsub_t(np.asfortranarray(R.astype(dt)), c.astype(dt))
+    np.testing.assert_allclose(y.ravel(), np.cumsum(c), rtol=tol(dt))
+    U = np.triu(rnd(n, n, 22, dt)) + 4 * np.eye(n, dtype=dt)
+    Y = oracle.backsub_t(np.asfortranarray(U), C).astype(np.float64)
+    U64, C64 = U.astype(np.float64), C.astype(np.float64)
+    Z = np.zeros_like(C64)
+    for j in range(n):                                   # forward substitution with U^T, written out
+        Z[j] = (C64[j] - U64[:j, j] @ Z[:j]) / U64[j, j]
+    np.testing.assert_allclose(Y, Z, rtol=tol(dt, 1e4), atol=tol(dt, 1e2))
+    assert np.linalg.norm(U64.T @ Y - C64) / np.linalg.norm(C64) < tol(dt, 1e2)
+    assert np.linalg.norm(U64 @ Y - C64) / np.linalg.norm(C64) > 1e-2       # not the untransposed solve
+    with pytest.raises(ZeroDivisionError):
+        Us = np.triu(np.ones((4, 4))); Us[1, 1] = 0
+        oracle.backsub_t(np.asfortranarray(Us), np.ones((4, 1)))
+    # semi-normal equations on a full least-squares problem
+    m, S = 40, 3
+    A = rnd(m, n, 23, dt); B = rnd(m, S, 24, dt)
+    VR, tau = oracle.qr(A)
+    rhs = (A.astype(np.float64).T @ B.astype(np.float64)).astype(dt)
+    X = oracle.backsub(VR, oracle.backsub_t(VR, rhs)).astype(np.float64)
+    X_ls = np.linalg.lstsq(A.astype(np.float64), B.astype(np.float64), rcond=None)[0]
+    assert np.linalg.norm(X - X_ls) / np.linalg.norm(X_ls) < tol(dt, 1e4)
+
+
 def test_backsub_singular_raises():
     U = np.triu(np.ones((4, 4)))
     U[2, 2] = 0

@@ -101,3 +101,84 @@ def test_metrics_closed_forms():
     assert w.psnr(x, x + 0.01) == pytest.approx(40.0)           # MSE = 1e-4, MAX = 1
     assert w.snr(x, x + 0.01) == pytest.approx(10 * math.log10(np.sum(x * x) / (256 * 1e-4)))
     assert w.ssim(x, 1 - x) < 0.5
+
+
+# ---- fan-beam Joseph generator (the paper's own geometry, Table 1) ----------
+def _fan_dense(N, n_det, n_views, fan_deg=30.0):
+    r, c, v = w.joseph_fanbeam_coo(N, n_det, n_views, fan_deg)
+    assert len(set(zip(r.tolist(), c.tolist()))) == len(r)            # no duplicate entries
+    A = np.zeros((n_det * n_views, N * N))
+    A[r, c] = v
+    return A
+
+
+def test_joseph_equals_the_hat_function_form_pixel_by_pixel():
+    """Brute force on a tiny scanner, written pixel-driven instead of ray-driven: a_ij = (1 / |d_major|) *
+    max(0, 1 - |coordinate of the ray on the sampling line through pixel j - pixel centre|)."""
+    N, n_det, n_views, fan_deg = 6, 9, 7, 40.0
+    A = _fan_dense(N, n_det, n_views, fan_deg)
+    fan = math.radians(fan_deg)
+    D = (N / math.sqrt(2)) / math.sin(fan / 2)
+    B = np.zeros_like(A)
+    for v in range(n_views):
+        beta = 2 * math.pi * v / n_views
+        sx, sy = D * math.cos(beta), D * math.sin(beta)
+        for k in range(n_det):
+            phi = beta + math.pi + (k - (n_det - 1) / 2) * fan / n_det
+            dx, dy = math.cos(phi), math.sin(phi)
+            for r in range(N):
+                for c in range(N):
+                    px, py = c + 0.5 - N / 2, N / 2 - r - 0.5        # pixel centre
+                    if abs(dx) >= abs(dy):                           # sampling line x = px: distance along y
+                        dist, L = abs(sy + (px - sx) * dy / dx - py), 1 / abs(dx)
+                    else:                                            # sampling line y = py: distance along x
+                        dist, L = abs(sx + (py - sy) * dx / dy - px), 1 / abs(dy)
+                    B[v * n_det + k, r * N + c] = L * max(0.0, 1.0 - dist)
+    np.testing.assert_allclose(A, B, atol=1e-12)
+
+
+def test_joseph_central_ray_and_basic_invariants():
+    N, n_det, n_views = 16, 33, 12
+    A = _fan_dense(N, n_det, n_views)
+    assert A.min() >= 0 and A.max() <= math.sqrt(2) + 1e-12 and (A != 0).sum(axis=1).max() <= 2 * N
+    # view 0, central detector: the ray is the x axis; every column gives 1/2 to the two middle rows
+    row = A[(n_det - 1) // 2].reshape(N, N)
+    expect = np.zeros((N, N)); expect[N // 2 - 1] = 0.5; expect[N // 2] = 0.5
+    np.testing.assert_allclose(row, expect, atol=1e-12)
+    # row sums are the chord through the image up to the two end samples: |sum - chord| <= 2 / |d_major|
+    fan = math.radians(30.0)
+    D = (N / math.sqrt(2)) / math.sin(fan / 2)
+    for v in (0, 1, 5):
+        beta = 2 * math.pi * v / n_views
+        sx, sy = D * math.cos(beta), D * math.sin(beta)
+        for k in range(n_det):
+            phi = beta + math.pi + (k - (n_det - 1) / 2) * fan / n_det
+            dx, dy = math.cos(phi), math.sin(phi)
+            lo, hi = -math.inf, math.inf
+            for p0, d in ((sx, dx), (sy, dy)):
+                if d != 0:
+                    t1, t2 = (-N / 2 - p0) / d, (N / 2 - p0) / d
+                    lo, hi = max(lo, min(t1, t2)), min(hi, max(t1, t2))
+            chord = max(hi - lo, 0.0)
+            assert abs(A[v * n_det + k].sum() - chord) <= 2.0 / max(abs(dx), abs(dy)) + 1e-9
+
+
+def test_joseph_quarter_turn_symmetry():
+    """A quarter turn of the source is a quarter turn of the image: A[v + n_views/4, k, rot(pixel)] = A[v, k, pixel]."""
+    N, n_det, n_views = 12, 25, 8
+    A = _fan_dense(N, n_det, n_views).reshape(n_views, n_det, N, N)
+    for v in range(n_views):
+        # rotating the scene by +90 degrees maps the point (x, y) to (-y, x): pixel (r, c) -> (N - 1 - c, r)
+        rotated = np.rot90(A[v], k=1, axes=(1, 2))
+        np.testing.assert_allclose(A[(v + n_views // 4) % n_views], rotated, atol=1e-12)
+
+
+def test_fan_config_is_full_rank_like_the_papers():
+    cfg = w.FAN_CONFIGS["fan32"]
+    A = w.fanbeam_dense(cfg)
+    assert A.shape == (cfg.m, cfg.n) == (1560, 1024)
+    s = np.linalg.svd(A, compute_uv=False)
+    assert s[-1] > 1e-2 and s[0] / s[-1] < 2e3
+    X0, B = w.fanbeam_slices(cfg, S=2)
+    np.testing.assert_allclose(A @ X0, B, atol=1e-10)
+    assert X0.max() == 1.0 and B.min() >= 0

@@ -221,7 +221,8 @@ int ct_qr_version(void);
 /* Kernel-level entry points used by the parity tests (SURVEY.md test rung T2) and by the
  * micro-benchmarks of bench.py.  All pointers DEVICE.
  *   ct_qr_gemm: C <- alpha*op(A)*B + beta*C with op(A) = A^T when trans_a (A is K x M) else A
- *   (A is M x K); B is K x N; impl 0 = default kernel for the dtype, 1 = SIMT kernel.
+ *   (A is M x K); B is K x N; impl 0 = default kernel for the dtype, 1 = SIMT kernel, 2 = (fp32, op(A) = A only) the
+ *   TMA-fed tcgen05 kernel with operands pre-split into TF32 hi / lo, as the two-panel trailing update uses it.
  *   ct_qr_peak_probe: runs a register-resident FMA/MMA loop and returns achieved TFLOP/s
  *   (kind 0 = FFMA fp32, 1 = DFMA fp64, 2 = DMMA m8n8k4 fp64). */
 int ct_qr_gemm(int trans_a, int64_t M, int64_t N, int64_t K, double alpha, const void* A, int64_t lda,

@@ -24,6 +24,7 @@
 #include "common.cuh"
 #include "kernels.h"
 #include "solve_small.cuh"
+#include "solve_small2.cuh"
 
 using namespace ctqr;
 
@@ -189,12 +190,16 @@ struct ctqr_handle_s {
     void* dRd = nullptr;               // P blocks of nb x nb (ld nb): diagonal blocks of R
     void* dRinv = nullptr;             // their inverses (nb == 128 only), filled at the first solve
     bool rinv_ready = false;
+    void* dGt = nullptr; bool gt_ready = false;   // cross-Gram blocks V_(j-1)^T V_j of the pipelined small-S Q^T B (fp64), first use
     void* dTau = nullptr;              // n
     // workspaces: [0] update stream, [1] panel stream
     void* dWp[2] = {nullptr, nullptr}; size_t wp_elems[2] = {0, 0};
     void* dW[2] = {nullptr, nullptr};  size_t w_elems[2] = {0, 0};
     // two-panel (256-wide) trailing updates: W / T^T W (256 x nc each), two merged T factors, merge scratch
     void* dW2[2] = {nullptr, nullptr}; size_t w2_elems = 0; void* dT2 = nullptr; void* dMerge = nullptr;
+    // fp32 only: TF32 hi / lo split of the pair's reflector block (rows below the first diagonal block; one [hi | lo]
+    // buffer per T2 slot, leading dimension ldvs) and of T2^T W, for the TMA-fed tcgen05 update (gemm_umma_tma.cuh)
+    void* dVs[2] = {nullptr, nullptr}; int64_t ldvs = 0; void* dWs = nullptr; size_t ws_elems = 0;
     void* dCw = nullptr; size_t cw_bytes = 0;   // staging buffer of the solves (B in, X out), grow-only: no allocation per batch
     void* dPart = nullptr;             // LL slots of the panel kernel
     void* dLLs = nullptr; unsigned ll_seq = 0;   // LL slots / step numbers of the fused small-S solve kernels
@@ -237,9 +242,10 @@ struct ctqr_handle_s {
         if (own_A && dA) cudaFree(dA);
         if (fmap) { msync(fmap, fmap_len, MS_SYNC); munmap(fmap, fmap_len); }
         if (ffd >= 0) close(ffd);
-        dev_free(dT); dev_free(dRd); dev_free(dRinv); dev_free(dTau);
+        dev_free(dT); dev_free(dRd); dev_free(dRinv); dev_free(dTau); dev_free(dGt);
         for (int i = 0; i < 2; ++i) { dev_free(dWp[i]); dev_free(dW[i]); dev_free(dW2[i]); }
-        dev_free(dT2); dev_free(dMerge); dev_free(dCw);
+        dev_free(dT2); dev_free(dMerge); dev_free(dCw); dev_free(dWs);
+        for (int i = 0; i < 2; ++i) if (dVs[i]) cudaFree(dVs[i]);
         dev_free(dPart); dev_free(dLLs); dev_free(dFlag); dev_free(dTickets);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
@@ -570,6 +576,23 @@ static int ensure_pair_ws(H& h, int64_t nc) {
     for (int i = 0; i < 2; ++i)
         if (dev_alloc(&h.dW2[i], need * sizeof(T)) != cudaSuccess) { cudaGetLastError(); h.w2_elems = 0; return 1; }
     h.w2_elems = need;
+    if (sizeof(T) == 4 && h.gemm_impl == 0) {
+        const size_t need_ws = (size_t)2 * 256 * (size_t)nc;
+        if (h.ws_elems < need_ws) {
+            dev_free(h.dWs); h.dWs = nullptr; h.ws_elems = 0;
+            if (dev_alloc(&h.dWs, need_ws * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return 1; }
+            h.ws_elems = need_ws;
+        }
+        if (!h.dVs[0]) {
+            h.ldvs = round_up(h.m, 32);
+            for (int i = 0; i < 2; ++i)
+                if (big_alloc(&h.dVs[i], (size_t)2 * h.ldvs * 256 * sizeof(float)) != cudaSuccess) {
+                    cudaGetLastError();
+                    if (h.dVs[0]) { cudaFree(h.dVs[0]); h.dVs[0] = nullptr; }
+                    return 1;
+                }
+        }
+    }
     if (!h.dT2) {
         if (dev_alloc(&h.dT2, (size_t)2 * 256 * 256 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
         CK(cudaMemsetAsync(h.dT2, 0, (size_t)2 * 256 * 256 * sizeof(T), h.sU));
@@ -609,13 +632,23 @@ static int pair_merge(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
     CK(copy2d_launch<T>(Tk, nb, T2, 256, nb, nb, st));
     CK(copy2d_launch<T>(Tk1, nb, T2 + nb + (size_t)nb * 256, 256, nb, nb, st));
     h.launches += 6;
+    if constexpr (sizeof(T) == 4) {
+        if (h.dVs[slot]) {
+            // the K = 256 update of this pair reads [V_k V_{k+1}] below the first diagonal block once per output tile:
+            // split it into TF32 hi / lo once, here on the panel stream (gemm_umma_tma.cuh)
+            float* hi = P_<float>(h.dVs[slot]);
+            CK(split_tf32_launch(A + (j0 + nb) + j0 * lda, lda, m - j0 - nb, 2 * nb, hi, hi + (size_t)h.ldvs * 256, h.ldvs, st));
+            h.launches += 1;
+        }
+    }
     return 0;
 }
 
 // C[j0:m, 0:nc] <- (H_k H_{k+1})^T C for the pair at columns j0, j0 + 128; T2 = its merged factor; stream sU
 template <typename T>
-static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m, int64_t j0, const T* T2, T* C,
+static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m, int64_t j0, int slot, T* C,
                       int64_t ldc, int64_t nc, int reserve_sms) {
+    const T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;
     if (nc <= 0) return 0;
     const int nb = 128;
     const int k = (int)(j0 / nb);
@@ -662,9 +695,25 @@ static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
     GemmArgs<T> gb{};
     gb.M = mk - nb; gb.N = nc; gb.K = 256; gb.A = A + (j0 + nb) + j0 * lda; gb.lda = lda; gb.B = W2; gb.ldb = 256;
     gb.C = C + nb; gb.ldc = ldc; gb.alpha = T(-1); gb.beta = T(1);
-    if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
-    CKI(gemm_direct_confined<T>(h, false, gb, sms, reserve_sms, st));
-    if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, 2.0 * (double)gb.M * 256 * (double)nc, 1}); }
+    bool done = false;
+    if constexpr (sizeof(T) == 4) {
+        if (h.dVs[slot] && h.dWs && (size_t)2 * 256 * (size_t)nc <= h.ws_elems && ldc % 4 == 0) {
+            // fp32: operands pre-split once (V by the merge, T2^T W here), TMA-fed tcgen05 kernel, 128 x 128 tiles
+            float* whi = P_<float>(h.dWs); float* wlo = whi + (size_t)256 * nc;
+            const float* vhi = P_<float>(h.dVs[slot]); const float* vlo = vhi + (size_t)h.ldvs * 256;
+            CK(split_tf32_launch(W2, 256, 256, nc, whi, wlo, 256, st));
+            if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
+            CK(upd_presplit_launch(gb.M, nc, 256, -1.f, vhi, vlo, h.ldvs, whi, wlo, 256, 1.f, gb.C, ldc, sms, st));
+            if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, 2.0 * (double)gb.M * 256 * (double)nc, 1}); }
+            h.launches += 1;
+            done = true;
+        }
+    }
+    if (!done) {
+        if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
+        CKI(gemm_direct_confined<T>(h, false, gb, sms, reserve_sms, st));
+        if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, 2.0 * (double)gb.M * 256 * (double)nc, 1}); }
+    }
     h.launches += 7;
     return 0;
 }
@@ -691,19 +740,18 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
     int slot = 0;
     CKI(chain(c0, slot));
     for (int64_t j0 = c0;; j0 += 2 * nb, slot ^= 1) {
-        const T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;
         const int64_t jn = j0 + 2 * nb;                     // first trailing column
         const int64_t rem = c1 - jn;
         const int64_t m = row_end(h, jn);                   // row end of this pair
         CK(cudaStreamWaitEvent(h.sU, evP, 0));              // V, T2 of this pair ready
         if (rem < 2 * nb) {
             // no further full pair: finish this update, then the single-panel driver takes the tail
-            CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, A + j0 + jn * lda, lda, rem, 0));
+            CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, slot, A + j0 + jn * lda, lda, rem, 0));
             if (rem > 0) CKI(factor_range_single<T>(h, A, lda, jn, c1));
             return 0;
         }
         // look-ahead block: the columns of the next pair
-        CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, A + j0 + jn * lda, lda, 2 * nb, 0));
+        CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, slot, A + j0 + jn * lda, lda, 2 * nb, 0));
         CK(cudaEventRecord(evL, h.sU));
         CK(cudaStreamWaitEvent(h.sP, evL, 0));
         CKI(chain(jn, slot ^ 1));
@@ -725,8 +773,8 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
             }
         }
         T* Cb = A + j0 + (jn + 2 * nb) * lda;
-        CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, Cb, lda, nA, R));
-        if (nA < ncb) CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, T2, Cb + nA * lda, lda, ncb - nA, 0));
+        CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, slot, Cb, lda, nA, R));
+        if (nA < ncb) CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, slot, Cb + nA * lda, lda, ncb - nA, 0));
     }
 }
 
@@ -1171,6 +1219,58 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
 // ------------------------------------------------------------------------------------------
 // solve: a6 (Q^T B) and a7 (blocked TRSM)
 // ------------------------------------------------------------------------------------------
+// Pipelined, TMA-fed small-S Q^T B (solve_small2.cuh; fp64).  Returns -1000 when the configuration does not fit.
+static int apply_qt_small2(H& h, double* C, int64_t ldc, int64_t S) {
+    const int nb = 128;
+    const double* A = P_<double>(h.dA);
+    if (!h.gt_ready) {
+        // G_j = V_(j-1)^T V_j over the rows of panel j, once per handle (stream-K partial tiles summed in a fixed order)
+        if (!h.dGt) {
+            CK(dev_alloc(&h.dGt, (size_t)h.P * nb * nb * sizeof(double)));
+            CK(cudaMemsetAsync(h.dGt, 0, (size_t)h.P * nb * nb * sizeof(double), h.sU));
+        }
+        for (int j = 1; j < h.P; ++j) {
+            const int64_t j0 = (int64_t)j * nb;
+            const int kw = (int)std::min<int64_t>(nb, h.n - j0);
+            GemmArgs<double> g{};
+            g.M = nb; g.N = kw; g.K = row_end(h, j0 + kw) - j0; g.A = A + j0 + (j0 - nb) * h.lda; g.lda = h.lda;
+            g.B = A + j0 + j0 * h.lda; g.ldb = h.lda;
+            g.C = P_<double>(h.dWp[0]); g.ldc = nb; g.alpha = 1.0; g.beta = 0.0; g.split_stride = (int64_t)nb * nb;
+            const GemmLaunch LG = gemm_plan<double>(true, nb, kw, g.K, h.gemm_impl, h.sms, true, (int64_t)h.wp_elems[0],
+                                                    g.split_stride, gemm_aligned(g));
+            if (LG.kind != 1) return -1000;
+            CK(gemm_run<double>(true, g, LG, h.gemm_impl, h.sU));
+            CK(partial_sum_launch<double>(P_<double>(h.dWp[0]), LG.seg, nb, kw, P_<double>(h.dGt) + (size_t)j * nb * nb, nb, h.sU));
+            h.launches += 2;
+        }
+        h.gt_ready = true;
+    }
+    const int64_t nch = ceil_div(h.m, (int64_t)kQt2Chunk);
+    const int G = (int)std::min<int64_t>(h.sms, nch);
+    SmallQt2Args a{};
+    a.A = A; a.lda = h.lda; a.m = h.m; a.n = h.n; a.P = h.P; a.Tm = P_<double>(h.dT); a.Gt = P_<double>(h.dGt);
+    a.B = C; a.ldb = ldc; a.S = (int)S;
+    a.part = reinterpret_cast<uint4*>(h.dLLs);
+    a.sums = a.part + (size_t)2 * h.sms * nb * kSmallS;
+    a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
+    a.rpc = (int)ceil_div(nch, (int64_t)G) * kQt2Chunk;
+    a.kl = h.kl;
+    int ns = 8;
+    while (ns > 3 && qt2_smem_bytes(a.rpc, ns) > 225 * 1024) --ns;
+    const size_t smem = qt2_smem_bytes(a.rpc, ns);
+    if (smem > 225 * 1024) return -1000;
+    a.nstage = ns;
+    CUtensorMap mapV;
+    if (tma::map_2d(&mapV, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, A, h.m, h.n, h.lda, kQt2Chunk, 128, CU_TENSOR_MAP_SWIZZLE_128B) != cudaSuccess)
+        return -1000;
+    static SmemAttr attr;
+    CK(ensure_dyn_smem(apply_qt_small2_kernel, smem, attr));
+    void* args[] = {(void*)&mapV, (void*)&a};
+    CK(cudaLaunchCooperativeKernel((void*)apply_qt_small2_kernel, dim3(G), dim3(kSmallThreads), args, smem, h.sU));
+    h.launches += 1;
+    return 0;
+}
+
 template <typename T>
 static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
     if (h.ooc) {
@@ -1190,6 +1290,12 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         return 0;
     }
     const T* A = P_<T>(h.dA);
+    if constexpr (sizeof(T) == 8) {
+        if (S <= kSmallS && h.dLLs && h.gemm_impl == 0 && h.nb == 128 && (h.lda % 2) == 0 && ((uintptr_t)A % 16) == 0 && h.P >= 2) {
+            int rc2 = apply_qt_small2(h, C, ldc, S);
+            if (rc2 != -1000) return rc2;                  // -1000: does not fit (shared memory); fall through
+        }
+    }
     if (S <= kSmallS && h.dLLs && h.gemm_impl == 0) {
         // memory-bound regime: one cooperative kernel for all panels (solve_small.cuh)
         SmallQtArgs<T> a{};
@@ -1886,6 +1992,29 @@ extern "C" int ct_qr_load(const char* path, const ctqr_options_t* opt, ctqr_hand
 // ------------------------------------------------------------------------------------------
 // kernel-level test / probe entry points
 // ------------------------------------------------------------------------------------------
+// impl == 2 (fp32, op(A) = A only): both operands split once into TF32 hi / lo, then the TMA-fed tcgen05 kernel
+static int gemm_presplit(int64_t, int64_t, int64_t, double, const double*, int64_t, const double*, int64_t, double, double*, int64_t, int, int) {
+    return set_err(-14, "impl 2 (pre-split tcgen05 kernel) is fp32 only");
+}
+static int gemm_presplit(int64_t M, int64_t N, int64_t K, double alpha, const float* A, int64_t lda, const float* B, int64_t ldb,
+                         double beta, float* C, int64_t ldc, int ta, int sms) {
+    if (ta) return set_err(-1, "impl 2 takes op(A) = A only");
+    if (M == 0 || N == 0) return 0;
+    const int64_t lda2 = round_up(M, 32), ldb2 = round_up(std::max<int64_t>(K, 1), 32);
+    float *Ah = nullptr, *Al = nullptr, *Bh = nullptr, *Bl = nullptr;
+    cudaError_t e = cudaMalloc(&Ah, (size_t)lda2 * K * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&Al, (size_t)lda2 * K * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&Bh, (size_t)ldb2 * N * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&Bl, (size_t)ldb2 * N * 4);
+    if (e == cudaSuccess) e = split_tf32_launch(A, lda, M, K, Ah, Al, lda2, 0);
+    if (e == cudaSuccess) e = split_tf32_launch(B, ldb, K, N, Bh, Bl, ldb2, 0);
+    if (e == cudaSuccess) e = upd_presplit_launch(M, N, K, (float)alpha, Ah, Al, lda2, Bh, Bl, ldb2, (float)beta, C, ldc, sms, 0);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    cudaFree(Ah); cudaFree(Al); cudaFree(Bh); cudaFree(Bl);
+    if (e != cudaSuccess) return set_err(CTQR_ERR_CUDA, "pre-split product failed: %s", cudaGetErrorString(e));
+    return 0;
+}
+
 template <typename T>
 static int gemm_typed(int ta, int64_t M, int64_t N, int64_t K, double alpha, const void* A, int64_t lda,
                       const void* B, int64_t ldb, double beta, void* C, int64_t ldc, int impl) {
@@ -1893,6 +2022,7 @@ static int gemm_typed(int ta, int64_t M, int64_t N, int64_t K, double alpha, con
     g.M = M; g.N = N; g.K = K; g.A = (const T*)A; g.lda = lda; g.B = (const T*)B; g.ldb = ldb;
     g.C = (T*)C; g.ldc = ldc; g.alpha = (T)alpha; g.beta = (T)beta; g.split_stride = 0;
     int dev = 0, sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (impl == 2) return gemm_presplit(M, N, K, alpha, (const T*)A, lda, (const T*)B, ldb, beta, (T*)C, ldc, ta, sms);
     CK(gemm_direct<T>(ta != 0, g, impl, sms, 0));
     CK(cudaDeviceSynchronize());
     return 0;

@@ -5,6 +5,7 @@
 #include "gemm.cuh"
 #include "gemm_mma.cuh"
 #include "gemm_umma.cuh"
+#include "gemm_umma_tma.cuh"
 
 namespace ctqr {
 
@@ -66,6 +67,14 @@ GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
     if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
     if (umma_ok && M % 4 == 0) return umma_plan_f32(M, N, K, partial ? 128 : 64, sms, partial, max_elems, partial ? 24 : 23);
     return streamk_plan(M, N, K, 128, 64, 32, sms, partial, max_elems, sstride, 3);
+}
+
+cudaError_t split_tf32_launch(const float* src, int64_t ld, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ld_out, cudaStream_t st) {
+    return split_tf32_launch_impl(src, ld, rows, cols, hi, lo, ld_out, st);
+}
+cudaError_t upd_presplit_launch(int64_t M, int64_t N, int64_t K, float alpha, const float* Ahi, const float* Alo, int64_t lda,
+                                const float* Bhi, const float* Blo, int64_t ldb, float beta, float* C, int64_t ldc, int ctas, cudaStream_t st) {
+    return upd_presplit_launch_impl(M, N, K, alpha, Ahi, Alo, lda, Bhi, Blo, ldb, beta, C, ldc, ctas, st);
 }
 
 static MmaPlan to_plan(const GemmLaunch& L) {

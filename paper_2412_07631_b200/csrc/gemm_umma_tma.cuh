@@ -1,0 +1,235 @@
+// gemm_umma_tma.cuh -- C <- alpha * A * B + beta * C in fp32 as a 3xTF32 split on tcgen05 with PRE-SPLIT operands fed by
+// TMA (the larfb product C <- C - V W, the dominant kernel of the fp32 factorisation).
+//
+// gemm_umma.cuh splits every operand tile into hi + lo again for every output tile (the producer warps took 60 % of the
+// issue slots, ncu profiles/r1_final_c3.md) and drains the TMEM accumulator after every 32 of K.  Here
+//   * A (= the reflector block V, M x K, m-contiguous) and B (= W, K x N, k-contiguous) are split ONCE per panel pair into
+//     hi / lo arrays of TF32 bit patterns by split_tf32_kernel -- both are small and re-read by every tile;
+//   * one thread issues cp.async.bulk.tensor (TMA) loads of the four operand tiles of a k-block straight into the UMMA
+//     canonical shared-memory layouts (K-major SWIZZLE_128B for B, MN-major SWIZZLE_128B with 32-byte atoms for A: the
+//     hardware swizzles, nothing is transposed), completing on the stage's `full` mbarrier; there are no producer warps;
+//   * one thread issues the tcgen05.mma kind::tf32 instructions (128 x 128 x 8, three per k-step: lo*hi, hi*lo, hi*hi);
+//   * the accumulator stays in TMEM for kDrain k-blocks (128 of K) before the drainer warps add it to the running sum in
+//     registers with round-to-nearest FADDs (the tensor core's own accumulation truncates: an error growing linearly in
+//     the number of accumulated terms, 1e-5 at K = 1024; 128 terms keep it at FFMA level);
+//   * 128 x 128 output tiles: a 128 x 64 tile needs 6 KB of shared-memory operand reads per 35-clock MMA, more than the
+//     128 B/clk the SM delivers; 128 x 128 needs 8 KB per 69 clocks.
+// Warp roles: warp 0 TMA producer, warp 1 MMA issuer (owns the TMEM allocation), warps 2-9 drainers / epilogue.
+#pragma once
+#include "common.cuh"
+#include "gemm_umma.cuh"
+#include "tma.cuh"
+
+namespace ctqr {
+namespace umma {
+
+constexpr int kTBN = 128, kTStages = 3, kDrain = 4;
+constexpr int kTTile = 128 * BK * 4;                       // one operand tile: 128 rows x 32 floats = 16 KB
+constexpr int kTStage = 4 * kTTile;                        // A_hi, A_lo, B_hi, B_lo
+constexpr int kTSmem = kTStages * kTStage + 1024 + 256;
+constexpr int kTDrainThreads = 256, kTThreads = 64 + kTDrainThreads;
+
+struct UpdTmaArgs {
+    int64_t M, N, K;
+    float* C; int64_t ldc;
+    float alpha, beta;
+    int64_t tilesM, tilesN, tpc;      // tiles per CTA (contiguous ranges, m fastest)
+    int KT;                           // k-blocks of 32
+};
+
+// hi / lo TF32 bit patterns of a column-major block (ld_out >= rows; the padding rows are written as zeros)
+__global__ void split_tf32_kernel(const float* __restrict__ src, int64_t ld, int64_t rows, int64_t cols,
+                                  float* __restrict__ hi, float* __restrict__ lo, int64_t ld_out) {
+    const int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (r >= ld_out) return;
+    for (int64_t c = blockIdx.y; c < cols; c += gridDim.y) {
+        float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float* s = src + r + c * ld;
+        if (r + 3 < rows && ((uintptr_t)s & 15) == 0) x = __ldg(reinterpret_cast<const float4*>(s));
+        else {
+            if (r < rows) x.x = s[0];
+            if (r + 1 < rows) x.y = s[1];
+            if (r + 2 < rows) x.z = s[2];
+            if (r + 3 < rows) x.w = s[3];
+        }
+        uint4 h, l;
+        split4(x, h, l);
+        *reinterpret_cast<uint4*>(hi + r + c * ld_out) = h;
+        *reinterpret_cast<uint4*>(lo + r + c * ld_out) = l;
+    }
+}
+
+__global__ void __launch_bounds__(kTThreads, 1)
+upd_tma_kernel(const __grid_constant__ CUtensorMap mAh, const __grid_constant__ CUtensorMap mAl,
+               const __grid_constant__ CUtensorMap mBh, const __grid_constant__ CUtensorMap mBl, UpdTmaArgs g) {
+    extern __shared__ unsigned char smem_raw[];
+    const unsigned sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
+    const unsigned bars = sbase + kTStages * kTStage;
+    auto full = [&](int s) { return bars + 8u * s; };
+    auto empty = [&](int s) { return bars + 8u * (kTStages + s); };
+    auto tfull = [&](int b) { return bars + 8u * (2 * kTStages + b); };
+    auto tempty = [&](int b) { return bars + 8u * (2 * kTStages + 2 + b); };
+    unsigned* tmem_slot = reinterpret_cast<unsigned*>(sgen + kTStages * kTStage + 8 * (2 * kTStages + 4));
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t tiles = g.tilesM * g.tilesN;
+    const int64_t t0 = (int64_t)blockIdx.x * g.tpc, t1 = min(tiles, t0 + g.tpc);
+
+    if (tid == 0) {
+        for (int s = 0; s < kTStages; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tfull(b), 1); mbar_init(tempty(b), kTDrainThreads); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        tma::prefetch_map(&mAh); tma::prefetch_map(&mAl); tma::prefetch_map(&mBh); tma::prefetch_map(&mBl);
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(tmem_slot)), "r"(256u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const unsigned tmem = *tmem_slot;
+
+    if (warp == 0) {
+        // ================= TMA producer =================
+        if (lane == 0) {
+            int s = 0; unsigned ph = 1;
+            for (int64_t t = t0; t < t1; ++t) {
+                const int64_t tn = t / g.tilesM, tm = t - tn * g.tilesM;
+                const int m0 = (int)(tm * BM), n0 = (int)(tn * kTBN);
+                for (int kb = 0; kb < g.KT; ++kb) {
+                    mbar_wait(empty(s), ph);
+                    tma::mbar_expect_tx(full(s), (unsigned)kTStage);
+                    const unsigned st = sbase + s * kTStage;
+                    const int k0 = kb * BK;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {          // A: four boxes of 32 m x 32 k (4 KB each), m-groups 4 KB apart
+                        tma::load_2d(st + i * 4096, &mAh, m0 + 32 * i, k0, full(s));
+                        tma::load_2d(st + kTTile + i * 4096, &mAl, m0 + 32 * i, k0, full(s));
+                    }
+                    tma::load_2d(st + 2 * kTTile, &mBh, k0, n0, full(s));      // B: one box of 32 k x 128 n
+                    tma::load_2d(st + 3 * kTTile, &mBl, k0, n0, full(s));
+                    if (++s == kTStages) { s = 0; ph ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer =================
+        const unsigned idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | ((unsigned)(kTBN >> 3) << 17) | ((unsigned)(BM >> 4) << 24);
+        int s = 0; unsigned fph = 0;
+        int64_t d = 0;                                     // accumulator generations handed to the drainers so far
+        for (int64_t t = t0; t < t1; ++t) {
+            for (int kb = 0; kb < g.KT; ++kb) {
+                const int b = (int)(d & 1);
+                const bool first = (kb % kDrain) == 0, last = (kb % kDrain) == kDrain - 1 || kb == g.KT - 1;
+                if (first) mbar_wait(tempty(b), (unsigned)(((d >> 1) & 1) ^ 1));
+                mbar_wait(full(s), fph);
+                tc_fence_after();
+                if (lane == 0) {
+                    const unsigned a_hi = sbase + s * kTStage, a_lo = a_hi + kTTile, b_hi = a_hi + 2 * kTTile, b_lo = a_hi + 3 * kTTile;
+                    const unsigned dt = tmem + (unsigned)b * kTBN;
+#pragma unroll
+                    for (int ks = 0; ks < BK / 8; ++ks) {
+                        // A, MN-major SWIZZLE_128B_BASE32B: atoms of 32 m x 4 k (512 B); m-groups 4 KB apart (LBO), k-groups of
+                        // 4 are 512 B apart (SBO), one K = 8 instruction spans two of them.  B, K-major SWIZZLE_128B.
+                        const uint64_t dah = make_desc(a_hi + ks * 1024, 4096, 512, 1), dal = make_desc(a_lo + ks * 1024, 4096, 512, 1);
+                        const uint64_t dbh = make_desc(b_hi + ks * 32, 16, 1024), dbl = make_desc(b_lo + ks * 32, 16, 1024);
+                        tc_mma_tf32(dt, dal, dbh, idesc, (first && ks == 0) ? 0u : 1u);     // small terms first
+                        tc_mma_tf32(dt, dah, dbl, idesc, 1u);
+                        tc_mma_tf32(dt, dah, dbh, idesc, 1u);
+                    }
+                    tc_commit(empty(s));
+                    if (last) tc_commit(tfull(b));
+                }
+                __syncwarp();
+                if (last) ++d;
+                if (++s == kTStages) { s = 0; fph ^= 1u; }
+            }
+        }
+    } else {
+        // ================= drainers + epilogue =================
+        const int dw = warp - 2;                          // 0..7
+        const int rowq = (warp & 3) * 32 + lane;          // TMEM lanes a warp may read: 32 * (warp % 4) ..
+        const int colh = (dw >> 2) * 64;
+        constexpr int NC = 64;
+        float acc[NC];
+        const bool use_c = g.beta != 0.f;
+        const float cs = use_c ? g.beta / g.alpha : 0.f;
+        int64_t d = 0;
+        const int ndrain = (g.KT + kDrain - 1) / kDrain;
+        for (int64_t t = t0; t < t1; ++t) {
+            const int64_t tn = t / g.tilesM, tm = t - tn * g.tilesM;
+            const int64_t m = tm * BM + rowq, n0 = tn * kTBN + colh;
+            float* Cp = g.C + m + n0 * g.ldc;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) acc[c] = (use_c && m < g.M && n0 + c < g.N) ? __ldcs(Cp + c * g.ldc) : 0.f;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) acc[c] *= cs;
+            for (int q = 0; q < ndrain; ++q, ++d) {
+                const int b = (int)(d & 1);
+                mbar_wait(tfull(b), (unsigned)((d >> 1) & 1));
+                tc_fence_after();
+                const unsigned taddr = tmem + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(b * kTBN + colh);
+#pragma unroll
+                for (int c0 = 0; c0 < NC; c0 += 32) {
+                    float v[32];
+                    tmem_ld32(taddr + c0, v);
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) acc[c0 + c] += v[c];
+                }
+                tc_fence_before();
+                mbar_arrive(tempty(b));
+            }
+            if (m < g.M) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c)
+                    if (n0 + c < g.N) __stcs(Cp + c * g.ldc, g.alpha * acc[c]);
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem), "r"(256u) : "memory");
+}
+
+}  // namespace umma
+
+// ---- host side (declared in kernels.h) -------------------------------------------------------------
+inline cudaError_t split_tf32_launch_impl(const float* src, int64_t ld, int64_t rows, int64_t cols, float* hi, float* lo,
+                                          int64_t ld_out, cudaStream_t st) {
+    if (rows <= 0 || cols <= 0) return cudaSuccess;
+    dim3 grid((unsigned)ceil_div(ld_out, 4 * 256), (unsigned)std::min<int64_t>(cols, 65535));
+    umma::split_tf32_kernel<<<grid, 256, 0, st>>>(src, ld, rows, cols, hi, lo, ld_out);
+    return cudaGetLastError();
+}
+
+// C <- alpha (Ahi + Alo)(Bhi + Blo) + beta C on `ctas` CTAs (one per SM).  Ahi / Alo: M x K, m-contiguous, leading dimension
+// lda (multiple of 4, 16-byte aligned base); Bhi / Blo: K x N, k-contiguous, leading dimension ldb (same constraints).
+inline cudaError_t upd_presplit_launch_impl(int64_t M, int64_t N, int64_t K, float alpha, const float* Ahi, const float* Alo,
+                                            int64_t lda, const float* Bhi, const float* Blo, int64_t ldb, float beta, float* C,
+                                            int64_t ldc, int ctas, cudaStream_t st) {
+    if (M <= 0 || N <= 0) return cudaSuccess;
+    if (K <= 0 || alpha == 0.f || lda % 4 || ldb % 4 || ((uintptr_t)Ahi | (uintptr_t)Alo | (uintptr_t)Bhi | (uintptr_t)Blo) % 16)
+        return cudaErrorInvalidValue;
+    CUtensorMap mAh, mAl, mBh, mBl;
+    cudaError_t e;
+    if ((e = tma::map_2d(&mAh, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Ahi, M, K, lda, 32, 32, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B)) != cudaSuccess) return e;
+    if ((e = tma::map_2d(&mAl, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Alo, M, K, lda, 32, 32, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B)) != cudaSuccess) return e;
+    if ((e = tma::map_2d(&mBh, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Bhi, K, N, ldb, 32, 128, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return e;
+    if ((e = tma::map_2d(&mBl, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Blo, K, N, ldb, 32, 128, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return e;
+    umma::UpdTmaArgs g{};
+    g.M = M; g.N = N; g.K = K; g.C = C; g.ldc = ldc; g.alpha = alpha; g.beta = beta;
+    g.tilesM = ceil_div(M, umma::BM); g.tilesN = ceil_div(N, umma::kTBN);
+    g.KT = (int)ceil_div(K, umma::BK);
+    const int64_t tiles = g.tilesM * g.tilesN;
+    g.tpc = ceil_div(tiles, (int64_t)std::max(1, ctas));
+    const int grid = (int)ceil_div(tiles, g.tpc);
+    static SmemAttr attr;
+    if ((e = ensure_dyn_smem(umma::upd_tma_kernel, umma::kTSmem, attr)) != cudaSuccess) return e;
+    umma::upd_tma_kernel<<<grid, umma::kTThreads, umma::kTSmem, st>>>(mAh, mAl, mBh, mBl, g);
+    return cudaGetLastError();
+}
+
+}  // namespace ctqr

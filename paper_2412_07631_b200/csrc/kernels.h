@@ -64,6 +64,13 @@ GemmLaunch gemm_plan_f32(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
 cudaError_t gemm_run_f64(bool ta, GemmArgs<double> g, const GemmLaunch& L, int impl, cudaStream_t st);
 cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int impl, cudaStream_t st);
 
+// fp32 tcgen05 path with pre-split operands (gemm_umma_tma.cuh): TF32 hi / lo bit patterns of a column-major block
+// (ld_out a multiple of 4, >= rows; padding rows zeroed), and C <- alpha (Ahi + Alo)(Bhi + Blo) + beta C with
+// A m-contiguous (M x K, lda) and B k-contiguous (K x N, ldb), TMA-fed, on `ctas` CTAs (one per SM)
+cudaError_t split_tf32_launch(const float* src, int64_t ld, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ld_out, cudaStream_t st);
+cudaError_t upd_presplit_launch(int64_t M, int64_t N, int64_t K, float alpha, const float* Ahi, const float* Alo, int64_t lda,
+                                const float* Bhi, const float* Blo, int64_t ldb, float beta, float* C, int64_t ldc, int ctas, cudaStream_t st);
+
 // cooperative register-resident panel kernel; returns cudaErrorInvalidValue for an unsupported (ib, rpt)
 cudaError_t panel_launch_f64(int ib, int rpt, PanelArgs<double>& pa, int G, cudaStream_t st);
 cudaError_t panel_launch_f32(int ib, int rpt, PanelArgs<float>& pa, int G, cudaStream_t st);

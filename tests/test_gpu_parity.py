@@ -278,6 +278,40 @@ def test_gemm_kernel(mnk, impl, ta, dt):
     assert relerr(got, ref) <= (1e-13 if dt == np.float64 else 2e-5)
 
 
+@pytest.mark.parametrize("mnk", [(128, 128, 256), (256, 128, 32), (1000, 300, 100), (517, 259, 256), (130, 9, 77),
+                                 (5, 300, 4), (2100, 1000, 256), (384, 640, 128)])
+def test_gemm_presplit_tma_kernel(mnk):
+    """impl 2: the TMA-fed tcgen05 kernel with operands pre-split into TF32 hi / lo (C <- C - V W of the two-panel
+    update): ragged tiles in M and N, K tails, K = 256 as used, against the fp64 definition at the fp32 kernel gate."""
+    M, N, K = mnk
+    rng = np.random.default_rng(M + N + K)
+    A = rng.standard_normal((M, K)).astype(np.float32)
+    B = rng.standard_normal((K, N)).astype(np.float32)
+    C = rng.standard_normal((M, N)).astype(np.float32)
+    ref = -1.0 * A.astype(np.float64) @ B.astype(np.float64) + C.astype(np.float64)
+    At, Bt, Ct = (ctqr.colmajor_from_numpy(np.asfortranarray(x)) for x in (A, B, C))
+    ctqr.ct_qr_gemm(False, M, N, K, -1.0, At, M, Bt, K, 1.0, Ct, M, 2)
+    got = ctqr.numpy_from_colmajor(Ct)
+    assert relerr(got, ref) <= 2e-5, relerr(got, ref)
+    assert max_abs(got, ref) <= 2e-5
+
+
+def test_gemm_presplit_long_k_accumulation():
+    """Same-sign data, K = 32768: the TMEM accumulator is drained every 128 of K, so the truncating in-MMA accumulation
+    must stay at FFMA level (<= 1e-5 elementwise; 3e-4 if the whole K were accumulated inside the tensor core)."""
+    import torch
+    M, N, K = 128, 192, 32768
+    rng = np.random.default_rng(1)
+    A = np.abs(rng.standard_normal((M, K))).astype(np.float32)
+    B = np.abs(rng.standard_normal((K, N))).astype(np.float32)
+    ref = A.astype(np.float64) @ B.astype(np.float64)
+    At, Bt = (ctqr.colmajor_from_numpy(np.asfortranarray(x)) for x in (A, B))
+    Ct = torch.zeros((N, M), dtype=torch.float32, device="cuda")
+    ctqr.ct_qr_gemm(False, M, N, K, 1.0, At, M, Bt, K, 0.0, Ct, M, 2)
+    err = np.max(np.abs(ctqr.numpy_from_colmajor(Ct) - ref) / np.abs(ref))
+    assert err <= 1e-5, err
+
+
 # ---- a5: out-of-core scheduler (SURVEY.md 8c rung T4) ---------------------------------------
 def _ooc_budget(m, nb, ns, dt):
     w = np.dtype(dt).itemsize

@@ -468,6 +468,59 @@ def run_persistence() -> dict:
     return out
 
 
+def run_file_tier(cfg, dtype: str, budget_bytes: int, S: int) -> dict:
+    """The paper's storage tier (matrix on disk, host RAM as a block cache over it): the matrix is
+    written to a file, its pages are dropped from the page cache (fsync + posix_fadvise DONTNEED), and ct_qr_factor
+    runs on the file path with a capped device budget -- the first pass over every super-panel is a cold disk read;
+    the factor is left in the file and the solve streams it from there."""
+    import tempfile
+    import torch
+    import paper_2412_07631_b200 as ctqr
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    npdt = np.float64 if dtype == "f64" else np.float32
+    w = 8 if dtype == "f64" else 4
+    m, n = cfg.m, cfg.n
+    coo = wl.siddon_coo(cfg.N, cfg.n_ang, cfg.n_bins)
+    buf, lam = host_augmented_pinned(cfg, tdt, coo)
+    _, B = wl.make_slices(cfg, S=S, coo=coo, lam=lam)
+    out = {"workload": workload_name(cfg), "dtype": dtype, "matrix_bytes": m * n * w, "device_budget_bytes": budget_bytes}
+    with tempfile.TemporaryDirectory() as td:
+        path = os.path.join(td, "A.bin")
+        t0 = time.perf_counter()
+        with open(path, "wb") as fh:
+            buf.t.numpy().tofile(fh)
+            fh.flush(); os.fsync(fh.fileno())
+        out["file_write_s"] = time.perf_counter() - t0
+        out["file_write_gbs"] = m * n * w / out["file_write_s"] / 1e9
+        buf.release()
+        fd = os.open(path, os.O_RDONLY)
+        os.posix_fadvise(fd, 0, 0, os.POSIX_FADV_DONTNEED)       # cold: nothing of the file stays in the page cache
+        os.close(fd)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        f = ctqr.ct_qr_factor(None, m, n, dtype=npdt, file_path=path, device_budget_bytes=budget_bytes)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        st = f.stats()
+        Bh = torch.from_numpy(np.ascontiguousarray(B.astype(npdt).T)).pin_memory()
+        Xh = torch.zeros((S, n), dtype=tdt).pin_memory()
+        ctqr.ct_qr_solve(f, Bh, S, Xh)
+        st2 = f.stats()
+        out.update({
+            "n_superpanels": st["n_superpanels"], "factor_ms": st["factor_ms"], "wall_s": wall,
+            "tflops": cfg.factor_flops() / (st["factor_ms"] * 1e-3) / 1e12,
+            "cold_read_bytes": m * n * w, "h2d_bytes": st["h2d_bytes"], "d2h_bytes": st["d2h_bytes"],
+            "file_traffic_gbs_avg": (st["h2d_bytes"] + st["d2h_bytes"]) / (st["factor_ms"] * 1e-3) / 1e9,
+            "cold_read_gbs_lower_bound": m * n * w / wall / 1e9,
+            "copy_exposed_ms": st.get("copy_exposed_ms"), "copy_busy_ms": st.get("copy_busy_ms"),
+            "solve_streamed_from_file": {"S": S, "ms": st2["solve_ms"], "slices_per_s": S / (st2["solve_ms"] * 1e-3),
+                                         "gbs": st2["h2d_bytes"] / (st2["solve_ms"] * 1e-3) / 1e9},
+            "note": "matrix file in the box's temp directory, page cache dropped before the factorisation; every super-panel is "
+                    "first read from disk; later reads of written-back reflector panels may hit the page cache"})
+        f.destroy()
+    return out
+
+
 def host_augmented_pinned(cfg, torch_dtype, coo):
     """A_aug of `cfg` built straight in pinned host memory (the matrices of the out-of-core legs do not fit, or
     need not touch, the device): same entries as wl.dense_augmented_device (duplicates summed in fp64, one
@@ -713,6 +766,10 @@ def main():
     ap.add_argument("--ooc-config", default="c5", choices=sorted(wl.CONFIGS),
                     help="config of the out-of-core leg (fp32 from pinned host memory, --ooc-budget-gb device bytes)")
     ap.add_argument("--ooc-budget-gb", type=float, default=48.0)
+    ap.add_argument("--file-tier-config", default="c3", choices=sorted(wl.CONFIGS),
+                    help="config of the cold file-tier leg (matrix written to the temp directory, page cache dropped)")
+    ap.add_argument("--file-tier-dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--file-tier-budget-gb", type=float, default=1.2)
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     rank = int(os.environ.get("RANK", "0"))
@@ -806,6 +863,13 @@ def main():
                 extras["persistence"] = run_persistence()
             except Exception as e:                                # e.g. no room in the temp directory
                 extras["persistence"] = {"skipped": repr(e)[:200]}
+        if budget.allows(0.25 * budget.seconds + 45.0):
+            try:
+                extras["file_tier"] = run_file_tier(wl.CONFIGS[args.file_tier_config], args.file_tier_dtype,
+                                                    int(args.file_tier_budget_gb * 1e9), 8)
+            except Exception as e:
+                extras["file_tier"] = {"failed": repr(e)[:300]}
+            log("file-tier leg done")
         oc = wl.CONFIGS[args.ooc_config]
         need_s = 60.0 + oc.factor_flops() / 60e12 * 1.6           # host build + a factorisation at ~60 TFLOP/s fp32 + solve
         if budget.allows(need_s + 40.0):

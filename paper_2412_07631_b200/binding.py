@@ -52,7 +52,7 @@ class Stats(ctypes.Structure):
                 ("upd_ms", ctypes.c_double), ("upd_flops", ctypes.c_double), ("upd_launches", ctypes.c_int64),
                 ("lower_bandwidth", ctypes.c_int64), ("factor_flops_performed", ctypes.c_double),
                 ("copy_busy_ms", ctypes.c_double), ("copy_exposed_ms", ctypes.c_double),
-                ("diag_block_cond", ctypes.c_double), ("trsm_exact", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
+                ("diag_block_cond", ctypes.c_double), ("trsm_exact", ctypes.c_int32), ("apply_qt_path", ctypes.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -190,7 +190,7 @@ struct ctqr_handle_s {
     void* dRd = nullptr;               // P blocks of nb x nb (ld nb): diagonal blocks of R
     void* dRinv = nullptr;             // their inverses (nb == 128 only), filled at the first solve
     bool rinv_ready = false;
-    void* dGt = nullptr; bool gt_ready = false;   // cross-Gram blocks V_(j-1)^T V_j of the pipelined small-S Q^T B (fp64), first use
+    void* dGt = nullptr; bool gt_ready = false;   // Mt[j] = T_(j-1) (V_(j-1)^T V_j) of the pipelined small-S Q^T B (fp64), built at first use
     void* dTau = nullptr;              // n
     // workspaces: [0] update stream, [1] panel stream
     void* dWp[2] = {nullptr, nullptr}; size_t wp_elems[2] = {0, 0};
@@ -1224,11 +1224,14 @@ static int apply_qt_small2(H& h, double* C, int64_t ldc, int64_t S) {
     const int nb = 128;
     const double* A = P_<double>(h.dA);
     if (!h.gt_ready) {
-        // G_j = V_(j-1)^T V_j over the rows of panel j, once per handle (stream-K partial tiles summed in a fixed order)
+        // Mt[j] = T_(j-1) (V_(j-1)^T V_j), once per handle: the Gram block over the rows of panel j as stream-K partial
+        // tiles summed in a fixed order, then one 128^3 product
         if (!h.dGt) {
             CK(dev_alloc(&h.dGt, (size_t)h.P * nb * nb * sizeof(double)));
             CK(cudaMemsetAsync(h.dGt, 0, (size_t)h.P * nb * nb * sizeof(double), h.sU));
         }
+        if (!h.dMerge) CK(dev_alloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(double)));
+        double* Gs = P_<double>(h.dMerge);
         for (int j = 1; j < h.P; ++j) {
             const int64_t j0 = (int64_t)j * nb;
             const int kw = (int)std::min<int64_t>(nb, h.n - j0);
@@ -1240,22 +1243,26 @@ static int apply_qt_small2(H& h, double* C, int64_t ldc, int64_t S) {
                                                     g.split_stride, gemm_aligned(g));
             if (LG.kind != 1) return -1000;
             CK(gemm_run<double>(true, g, LG, h.gemm_impl, h.sU));
-            CK(partial_sum_launch<double>(P_<double>(h.dWp[0]), LG.seg, nb, kw, P_<double>(h.dGt) + (size_t)j * nb * nb, nb, h.sU));
-            h.launches += 2;
+            CK(partial_sum_launch<double>(P_<double>(h.dWp[0]), LG.seg, nb, kw, Gs, nb, h.sU));
+            GemmArgs<double> g2{};
+            g2.M = nb; g2.N = kw; g2.K = nb; g2.A = P_<double>(h.dT) + (size_t)(j - 1) * nb * nb; g2.lda = nb; g2.B = Gs; g2.ldb = nb;
+            g2.C = P_<double>(h.dGt) + (size_t)j * nb * nb; g2.ldc = nb; g2.alpha = 1.0; g2.beta = 0.0;
+            CK(gemm_direct<double>(false, g2, h.gemm_impl, h.sms, h.sU));
+            h.launches += 3;
         }
         h.gt_ready = true;
     }
     const int64_t nch = ceil_div(h.m, (int64_t)kQt2Chunk);
     const int G = (int)std::min<int64_t>(h.sms, nch);
     SmallQt2Args a{};
-    a.A = A; a.lda = h.lda; a.m = h.m; a.n = h.n; a.P = h.P; a.Tm = P_<double>(h.dT); a.Gt = P_<double>(h.dGt);
+    a.A = A; a.lda = h.lda; a.m = h.m; a.n = h.n; a.P = h.P; a.Tm = P_<double>(h.dT); a.Mt = P_<double>(h.dGt);
     a.B = C; a.ldb = ldc; a.S = (int)S;
     a.part = reinterpret_cast<uint4*>(h.dLLs);
     a.sums = a.part + (size_t)2 * h.sms * nb * kSmallS;
     a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
     a.rpc = (int)ceil_div(nch, (int64_t)G) * kQt2Chunk;
     a.kl = h.kl;
-    int ns = 8;
+    int ns = 10;
     while (ns > 3 && qt2_smem_bytes(a.rpc, ns) > 225 * 1024) --ns;
     const size_t smem = qt2_smem_bytes(a.rpc, ns);
     if (smem > 225 * 1024) return -1000;
@@ -1266,13 +1273,24 @@ static int apply_qt_small2(H& h, double* C, int64_t ldc, int64_t S) {
     static SmemAttr attr;
     CK(ensure_dyn_smem(apply_qt_small2_kernel, smem, attr));
     void* args[] = {(void*)&mapV, (void*)&a};
-    CK(cudaLaunchCooperativeKernel((void*)apply_qt_small2_kernel, dim3(G), dim3(kSmallThreads), args, smem, h.sU));
+    CK(cudaLaunchCooperativeKernel((void*)apply_qt_small2_kernel, dim3(G), dim3(kQt2Threads), args, smem, h.sU));
     h.launches += 1;
+#ifdef CTQR_SMALL_PROFILE
+    {
+        unsigned long long ph[16] = {0}, zero[16] = {0};
+        cudaStreamSynchronize(h.sU);
+        cudaMemcpyFromSymbol(ph, g_small_prof, sizeof(ph));
+        cudaMemcpyToSymbol(g_small_prof, zero, sizeof(zero));
+        for (int i = 0; i <= 5; ++i) fprintf(stderr, "ph%d %.2f  ", i, ph[i] * 1e-3 / h.P);
+        fprintf(stderr, "us/panel (1 gather, 2 reduce, 3 T^T W, 4 update, 5 pass A)\n");
+    }
+#endif
     return 0;
 }
 
 template <typename T>
 static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
+    h.st.apply_qt_path = h.ooc ? 3 : 0;
     if (h.ooc) {
         // factor on the host: stream V_k through the double buffer (sC) against the larfb on sU
         const T* hA = P_<T>(h.hA);
@@ -1293,7 +1311,7 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
     if constexpr (sizeof(T) == 8) {
         if (S <= kSmallS && h.dLLs && h.gemm_impl == 0 && h.nb == 128 && (h.lda % 2) == 0 && ((uintptr_t)A % 16) == 0 && h.P >= 2) {
             int rc2 = apply_qt_small2(h, C, ldc, S);
-            if (rc2 != -1000) return rc2;                  // -1000: does not fit (shared memory); fall through
+            if (rc2 != -1000) { h.st.apply_qt_path = 2; return rc2; }   // -1000: does not fit (shared memory); fall through
         }
     }
     if (S <= kSmallS && h.dLLs && h.gemm_impl == 0) {
@@ -1315,6 +1333,7 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
             void* args[] = {(void*)&a};
             CK(cudaLaunchCooperativeKernel((void*)apply_qt_small_kernel<T>, dim3(G), dim3(kSmallThreads), args, smem, h.sU));
             h.launches += 1;
+            h.st.apply_qt_path = 1;
 #ifdef CTQR_SMALL_PROFILE
             {
                 unsigned long long ph[16] = {0}, zero[16] = {0};

@@ -9,8 +9,11 @@
 //     (B_i = B after panels 0..i), published, and reduced over the grid while panels j-2 and j-1 are being applied.
 //     The true W_j = V_j^T B_(j-1) differs by the update of panel j-1 alone (panel j-2's is already in B_(j-2)... see
 //     below): B_(j-1) = B_(j-2) - V_(j-1) W2_(j-1), hence  W_j = Y_j - (V_j^T V_(j-1)) W2_(j-1).
-//     G_j = V_(j-1)^T V_j (128 x 128, "Gt" below) is computed once per handle; the element owners of the reduction
-//     subtract their rows of G_j^T W2_(j-1) before they publish the sums -- 128 KB of G per panel for the whole grid.
+//     With W2_(j-1) = T_(j-1)^T W_(j-1) this is W_j = Y_j - M_j W_(j-1), M_j = (V_j^T V_(j-1)) T_(j-1)^T (128 x 128, stored
+//     transposed as "Mt" = T_(j-1) (V_(j-1)^T V_j), computed once per handle): the element owners of the reduction
+//     subtract their row of M_j times the W_(j-1) they have just gathered, so the serial chain through the grid is one
+//     hop per panel (owners publish W_j -> everybody gathers it) and T^T W, the update and the next partial products
+//     all run while that hop is in flight.  128 KB of M per panel for the whole grid.
 //     (Order inside iteration k: the rows are first updated with panel k, then Y_(k+2) is accumulated from them, so Y_(k+2)
 //     sees B_k and only panel k+1 is missing.)
 //   * The stream of V from HBM is issued by ONE thread as TMA box loads (16 rows x 128 columns, SWIZZLE_128B) into a
@@ -30,12 +33,14 @@ namespace ctqr {
 
 constexpr int kQt2Chunk = 16;                    // fp64 rows per TMA box: 128 bytes, the swizzle span
 constexpr int kQt2StageBytes = kQt2Chunk * 128 * 8;
-constexpr int kQt2DsElems = 2048;                // scratch of the column-split update (doubles)
+constexpr int kQt2Warps = 16;                    // compute warps; one more warp issues the TMA loads
+constexpr int kQt2Threads = (kQt2Warps + 1) * 32;
 
 struct SmallQt2Args {
     const double* A; int64_t lda; int64_t m, n; int P;
     const double* Tm;               // P blocks of 128 x 128 (ld 128)
-    const double* Gt;               // P blocks of 128 x 128 (ld 128): Gt[j][q + c * 128] = (V_(j-1)^T V_j)[q][c], j >= 1
+    const double* Mt;               // P blocks of 128 x 128 (ld 128): Mt[j] = T_(j-1) (V_(j-1)^T V_j), j >= 1:
+                                    // W_j[c, s] = Y_j[c, s] - sum_q Mt[j][q + c * 128] W_(j-1)[q, s]
     double* B; int64_t ldb; int S;
     uint4* part;                    // [2][G][128 * kSmallS] LL slots: per-CTA partial Y
     uint4* sums;                    // [2][128 * kSmallS] LL slots: reduced, corrected W
@@ -47,13 +52,17 @@ struct SmallQt2Args {
 
 inline size_t qt2_smem_bytes(int rpc, int nstage) {
     return 1024 + (size_t)nstage * kQt2StageBytes + 16 * (size_t)nstage + 64 +
-           ((size_t)3 * 128 * SmallLd<double>::W + kQt2DsElems + (size_t)kSmallS * (rpc + 4)) * sizeof(double);
+           ((size_t)3 * 128 * SmallLd<double>::W + (size_t)kSmallS * (rpc + 4)) * sizeof(double);
 }
 
-__global__ void __launch_bounds__(kSmallThreads, 1)
+// The ring carries ONE sequence of boxes, identical for the producer and for every consumer:
+//   A(0), A(1), then for k = 0 .. P-1:  U(k), A(k+2)        (A(j) / U(j) = the CTA's row chunks of panel j, top down)
+// A boxes feed the partial products Y_j (every compute warp reads every box: warp w owns columns 8w .. 8w+7);
+// U boxes feed the row update of panel j (box i of the segment belongs to compute warp i mod 16 alone).
+__global__ void __launch_bounds__(kQt2Threads, 1)
 apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int NB = 128, SM = kSmallS, NT = kSmallThreads, NW = NT / 32, CH = kQt2Chunk, LDW = SmallLd<double>::W;
+    constexpr int NB = 128, SM = kSmallS, NW = kQt2Warps, NT = NW * 32, CH = kQt2Chunk, LDW = SmallLd<double>::W;
     const unsigned sbase = (tma::smem_addr(smem_raw) + 1023u) & ~1023u;
     unsigned char* ring = smem_raw + (sbase - tma::smem_addr(smem_raw));
     const int NS = p.nstage;
@@ -61,8 +70,7 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
     double* Wg = reinterpret_cast<double*>(ring + (size_t)NS * kQt2StageBytes + 16 * (size_t)NS + 64);   // gathered W_k
     double* Yp = Wg + NB * LDW;                             // this CTA's partial Y
     double* W2 = Yp + NB * LDW;                             // T_k^T W_k
-    double* Ds = W2 + NB * LDW;                             // column-split partial updates
-    double* Bs = Ds + kQt2DsElems;                          // [SM][ldbs] own rows of B, transposed
+    double* Bs = W2 + NB * LDW;                             // [SM][ldbs] own rows of B, transposed
     const int ldbs = p.rpc + 4;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = blockIdx.x, G = gridDim.x, S = p.S;
@@ -87,37 +95,48 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
         tma::mbar_init_fence();
         tma::prefetch_map(&mapV);
     }
-    // ---- issuer state (thread 0 only): next box = (panel ij, local row il) ----
-    int ij = 0, il = 0, ile = 0;
-    unsigned icount = 0;
-    if (tid == 0) { range_of(0, il, ile); while (ij < p.P && il >= ile) { if (++ij < p.P) range_of(ij, il, ile); } }
-    auto issue_next = [&]() {                               // thread 0: one more box, if any is left
-        if (ij >= p.P) return;
-        const int st = (int)(icount % (unsigned)NS);
-        tma::mbar_wait(empty(st), ((icount / (unsigned)NS) & 1u) ^ 1u);
-        tma::mbar_expect_tx(full(st), (unsigned)kQt2StageBytes);
-        tma::load_2d(sbase + (unsigned)st * kQt2StageBytes, &mapV, (int)row_of(il), ij * NB, full(st));
-        ++icount;
-        il += CH;
-        while (ij < p.P && il >= ile) { if (++ij < p.P) range_of(ij, il, ile); }
-    };
-    unsigned ccount = 0;                                    // boxes consumed so far (same order, every thread)
-
-    for (int i = tid; i < SM * p.rpc; i += NT) {
+    for (int i = tid; i < SM * p.rpc; i += kQt2Threads) {
         const int s = i / p.rpc, lr = i - s * p.rpc;
         const int64_t row = row_of(lr);
         Bs[s * ldbs + lr] = (s < S && lr < nl && row < p.m) ? p.B[row + (int64_t)s * p.ldb] : 0.0;
     }
     __syncthreads();
-    if (tid == 0) for (int s = 0; s < NS; ++s) issue_next();
 
-    // partial Y_j over the own rows from the TMA ring: warp w owns columns 8w .. 8w+7; result to Yp, then published
+    if (warp == NW) {
+        // ================= TMA producer: the whole box sequence, as far ahead as the ring allows =================
+        if (lane == 0) {
+            unsigned icount = 0;
+            // the first read of a box (A segment) asks the L2 to keep the lines, the second (U segment, two panels
+            // later) to drop them first: three panels of V must survive in the L2 between the two reads
+            const uint64_t keep = l2_policy_evict_last(), drop = l2_policy_evict_first();
+            auto segment = [&](int j, uint64_t pol) {
+                int la, le; range_of(j, la, le);
+                for (int lr = la; lr < le; lr += CH, ++icount) {
+                    const int st = (int)(icount % (unsigned)NS);
+                    tma::mbar_wait(empty(st), ((icount / (unsigned)NS) & 1u) ^ 1u);
+                    tma::mbar_expect_tx(full(st), (unsigned)kQt2StageBytes);
+                    tma::load_2d_hint(sbase + (unsigned)st * kQt2StageBytes, &mapV, (int)row_of(lr), j * NB, full(st), pol);
+                }
+            };
+            segment(0, keep);
+            if (p.P > 1) segment(1, keep);
+            for (int k = 0; k < p.P; ++k) {
+                segment(k, drop);
+                if (k + 2 < p.P) segment(k + 2, keep);
+            }
+        }
+        return;                                             // the compute warps synchronise among themselves (named barrier 1)
+    }
+    auto sync_compute = [&]() { asm volatile("bar.sync 1, %0;\n" ::"n"(NT) : "memory"); };
+    unsigned ccount = 0;                                    // boxes of the sequence passed so far (every compute thread)
+
+    // partial Y_j over the own rows from the ring: warp w owns columns 8w .. 8w+7; result to Yp, then published
     auto pass_a = [&](int j) {
         int la, le; range_of(j, la, le);
         const int c = warp * 8 + (lane >> 2);
         const double* bs = Bs + (lane >> 2) * ldbs + (lane & 3);
         double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int lr = la; lr < le; lr += CH) {
+        for (int lr = la; lr < le; lr += CH, ++ccount) {
             const int st = (int)(ccount % (unsigned)NS);
             tma::mbar_wait(full(st), (ccount / (unsigned)NS) & 1u);
             const unsigned char* vs = ring + (size_t)st * kQt2StageBytes + c * 128;
@@ -129,69 +148,103 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
             }
             __syncwarp();
             if (lane == 0) tma::mbar_arrive(empty(st));
-            ++ccount;
-            if (tid == 0) issue_next();
         }
+        sync_compute();                                     // the previous publication has finished reading Yp
         Yp[c * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
         Yp[c * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
-        __syncthreads();
+        sync_compute();
         const unsigned seq = p.seq_base + (unsigned)j + 1u;
         uint4* mine = p.part + ((size_t)(j & 1) * G + g) * (NB * SM);
         for (int e = tid; e < NB * SM; e += NT) ll_store(mine + e, Yp[(e / SM) * LDW + (e % SM)], seq);
     };
-    // element owners: sum the partials of Y_j over the CTAs in a fixed order, subtract (V_j^T V_(j-1)) W2_(j-1) (W2 in shared
-    // memory holds W2_(j-1) when this runs), publish W_j
-    auto reduce_j = [&](int j) {
+    // own rows: B[r, :] -= V_j[r, :] W2 from the ring; box i of the segment is shared by the two warps 2 (i mod 8) and
+    // 2 (i mod 8) + 1, one 8-row group each (a stage is then held for 32 DMMAs instead of 64: the ring turns over faster)
+    auto pass_u = [&](int j) {
+        int la, le; range_of(j, la, le);
+        int i = 0;
+        for (int lr = la; lr < le; lr += CH, ++ccount, ++i) {
+            if ((i % (NW / 2)) != (warp >> 1)) continue;
+            const int st = (int)(ccount % (unsigned)NS);
+            tma::mbar_wait(full(st), (ccount / (unsigned)NS) & 1u);
+            const unsigned char* vs = ring + (size_t)st * kQt2StageBytes;
+            const double* wb = W2 + (lane & 3) * LDW + (lane >> 2);
+            const int r = 8 * (warp & 1) + (lane >> 2);
+            double d0[4] = {0.0, 0.0, 0.0, 0.0}, d1[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll 8
+            for (int t = 0; t < NB / 4; ++t) {
+                const int col = 4 * t + (lane & 3);
+                const double a = *reinterpret_cast<const double*>(vs + col * 128 + ((((r >> 1) ^ (col & 7)) << 4) | ((r & 1) << 3)));
+                dmma884(d0[t & 3], d1[t & 3], a, wb[4 * t * LDW]);
+            }
+            const int s0 = 2 * (lane & 3), l = lr + r;
+            Bs[s0 * ldbs + l] -= (d0[0] + d0[1]) + (d0[2] + d0[3]);
+            Bs[(s0 + 1) * ldbs + l] -= (d1[0] + d1[1]) + (d1[2] + d1[3]);
+            __syncwarp();
+            if (lane == 0) tma::mbar_arrive_n(empty(st), (unsigned)(NW / 2));
+        }
+    };
+    // element owners: sum the partials of Y_j over the CTAs in a fixed order, subtract M_j W_(j-1) (Wg in shared memory
+    // holds the gathered W_(j-1) when this runs), publish W_j.  One element per warp (128 * 8 elements over G CTAs x 16 warps);
+    // the loads are issued by reduce_issue and consumed by reduce_finish so that the row update runs in between.
+    constexpr int MAXB = 5;                                 // partial slots per lane: G <= 160 CTAs
+    auto reduce_issue = [&](int j, double (&gv)[4], uint4 (&r)[MAXB]) {
+        const int e = g + warp * G;
+        if (e >= NB * SM) return;
+        const uint4* all = p.part + (size_t)(j & 1) * G * (NB * SM);
+        const double* gt = p.Mt + (size_t)j * NB * NB + (size_t)(e / SM) * NB;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) gv[u] = j >= 1 ? __ldg(gt + lane + 32 * u) : 0.0;
+#pragma unroll
+        for (int u = 0; u < MAXB; ++u) {
+            const int b = lane + u * 32;
+            if (b < G) r[u] = ll_load(all + (size_t)b * (NB * SM) + e);
+        }
+    };
+    auto reduce_finish = [&](int j, const double (&gv)[4], uint4 (&r)[MAXB]) {
+        const int e = g + warp * G;
+        if (e >= NB * SM) return;
         const unsigned seq = p.seq_base + (unsigned)j + 1u;
         const uint4* all = p.part + (size_t)(j & 1) * G * (NB * SM);
-        const double* gt = p.Gt + (size_t)j * NB * NB;
-        constexpr int MAXB = 5;
-        for (int e = g + warp * G; e < NB * SM; e += NW * G) {
-            const int c = e / SM, s = e - c * SM;
-            double corr = 0.0;
-            if (j >= 1) {
-                double gv[4];
+        const int s = e % SM;
+        double t = 0.0;
 #pragma unroll
-                for (int u = 0; u < 4; ++u) gv[u] = __ldg(gt + c * NB + lane + 32 * u);
-#pragma unroll
-                for (int u = 0; u < 4; ++u) corr = fma(gv[u], W2[(lane + 32 * u) * LDW + s], corr);
+        for (int u = 0; u < MAXB; ++u) {
+            const int b = lane + u * 32;
+            if (b < G) {
+                while (r[u].y != seq || r[u].w != seq) r[u] = ll_load(all + (size_t)b * (NB * SM) + e);
+                t += ll_value<double>(r[u]);
             }
-            double t = 0.0;
-            for (int b0 = lane; b0 < G; b0 += 32 * MAXB) {
-                uint4 r[MAXB];
-#pragma unroll
-                for (int u = 0; u < MAXB; ++u) {
-                    const int b = b0 + u * 32;
-                    if (b < G) r[u] = ll_load(all + (size_t)b * (NB * SM) + e);
-                }
-#pragma unroll
-                for (int u = 0; u < MAXB; ++u) {
-                    const int b = b0 + u * 32;
-                    if (b < G) {
-                        while (r[u].y != seq || r[u].w != seq) r[u] = ll_load(all + (size_t)b * (NB * SM) + e);
-                        t += ll_value<double>(r[u]);
-                    }
-                }
-            }
-            t -= corr;
-#pragma unroll
-            for (int off = 16; off >= 1; off >>= 1) t += shfl_xor(t, off);
-            if (lane == 0) ll_store(p.sums + (size_t)(j & 1) * (NB * SM) + e, t, seq);
         }
+        double corr = 0.0;
+        if (j >= 1) {                                       // (Wg is not yet written when W_0 is formed)
+#pragma unroll
+            for (int u = 0; u < 4; ++u) corr = fma(gv[u], Wg[(lane + 32 * u) * LDW + s], corr);
+        }
+        t -= corr;
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) t += shfl_xor(t, off);
+        if (lane == 0) ll_store(p.sums + (size_t)(j & 1) * (NB * SM) + e, t, seq);
     };
 
     // ---- prologue: Y_0 and Y_1 from the rows as given; W_0 needs no correction ----
     pass_a(0);
     if (p.P > 1) pass_a(1);
-    reduce_j(0);
+    {
+        double gv[4]; uint4 rr[MAXB];
+        reduce_issue(0, gv, rr);
+        reduce_finish(0, gv, rr);
+    }
 
     for (int k = 0; k < p.P; ++k) {
         const int64_t j0 = (int64_t)k * NB;
         const int kw = (int)min((int64_t)NB, p.n - j0);
         const unsigned seq = p.seq_base + (unsigned)k + 1u;
-        const double* V = p.A + j0 * p.lda;
-        int la, le; range_of(k, la, le);
-        const int na = le - la;
+        unsigned long long ph_t0 = 0; (void)ph_t0;
+        CTQR_PH(0)
+        // ---- element owners of W_(k+1): the loads of the partials (published one iteration ago) and of their row of
+        //      M_(k+1) are issued before the gather spins, and consumed right after it ----
+        double gv[4]; uint4 rr[MAXB];
+        if (k + 1 < p.P) reduce_issue(k + 1, gv, rr);
         // ---- gather W_k (reduced and corrected by its element owners during the previous iteration) ----
         {
             const uint4* sl = p.sums + (size_t)(k & 1) * (NB * SM);
@@ -205,75 +258,40 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
                 Wg[(e / SM) * LDW + (e % SM)] = ll_value<double>(r[u]);
             }
         }
-        __syncthreads();
+        sync_compute();
+        CTQR_PH(1)
+        // ---- W_(k+1) = sum of the partials - M_(k+1) W_k, published: the only step on the chain through the grid ----
+        if (k + 1 < p.P) reduce_finish(k + 1, gv, rr);
+        CTQR_PH(2)
         // ---- W2 = T_k^T W_k, T_k as DMMA fragments straight from L2 (upper triangular: q <= r) ----
         {
-            const int r = warp * 8 + (lane >> 2);
-            const double* tr = p.Tm + (size_t)k * NB * NB + (size_t)r * NB + (lane & 3);
+            const int tr_row = warp * 8 + (lane >> 2);
+            const double* tr = p.Tm + (size_t)k * NB * NB + (size_t)tr_row * NB + (lane & 3);
+            double ta[NB / 4];
+#pragma unroll
+            for (int t = 0; t < NB / 4; ++t) {
+                const int q = 4 * t + (lane & 3);
+                ta[t] = (t < 2 * warp + 2 && q <= tr_row && tr_row < kw) ? __ldg(tr + 4 * t) : 0.0;
+            }
             const double* wq = Wg + (lane & 3) * LDW + (lane >> 2);
             double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll 4
-            for (int t = 0; t < 2 * warp + 2; t += 4) {
 #pragma unroll
-                for (int h = 0; h < 4; ++h) {
-                    const int q = 4 * (t + h) + (lane & 3);
-                    const double a = (q <= r && r < kw) ? __ldg(tr + 4 * (t + h)) : 0.0;
-                    dmma884(c0[h], c1[h], a, wq[4 * (t + h) * LDW]);
-                }
-            }
-            W2[r * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
-            W2[r * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
+            for (int t = 0; t < NB / 4; ++t)
+                if (t < 2 * warp + 2) dmma884(c0[t & 3], c1[t & 3], ta[t], wq[4 * t * LDW]);
+            W2[tr_row * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
+            W2[tr_row * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
         }
-        __syncthreads();
-        // ---- element owners: W_(k+1) from the partials published one iteration ago, corrected with W2_k ----
-        if (k + 1 < p.P) reduce_j(k + 1);
-        // ---- own rows: B[r, :] -= V_k[r, 0:kw] W2_k  (V_k from L2; a unit = 8 rows x one of CS column ranges) ----
-        {
-            const int mt = na / 8;
-            int CS = 1;
-            while (CS < 8 && mt * CS < NW && 2 * CS * na * SM <= kQt2DsElems) CS *= 2;
-            const int steps = NB / 4 / CS;
-            for (int u = warp; u < mt * CS; u += NW) {
-                const int cs = u / mt, l0 = (u - cs * mt) * 8;
-                const int64_t row = row_of(la + l0 + (lane >> 2));
-                const bool okr = row < p.m;
-                const int cbeg = cs * steps * 4 + (lane & 3);
-                const double* vr = V + (int64_t)cbeg * p.lda + row;
-                const double* wb = W2 + cbeg * LDW + (lane >> 2);
-                double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll 8
-                for (int t = 0; t < steps; t += 4) {
-#pragma unroll
-                    for (int h = 0; h < 4; ++h) {
-                        const double a = (okr && cbeg + 4 * (t + h) < kw) ? __ldg(vr + (int64_t)(4 * (t + h)) * p.lda) : 0.0;
-                        dmma884(c0[h], c1[h], a, wb[4 * (t + h) * LDW]);
-                    }
-                }
-                c0[0] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
-                c1[0] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
-                const int l = l0 + (lane >> 2), s0 = 2 * (lane & 3);
-                if (CS == 1) {
-                    Bs[s0 * ldbs + la + l] -= c0[0];
-                    Bs[(s0 + 1) * ldbs + la + l] -= c1[0];
-                } else {
-                    Ds[(cs * SM + s0) * na + l] = c0[0];
-                    Ds[(cs * SM + s0 + 1) * na + l] = c1[0];
-                }
-            }
-            __syncthreads();
-            if (CS > 1) {
-                for (int idx = tid; idx < na * SM; idx += NT) {
-                    const int s = idx / na, l = idx - s * na;
-                    double t = 0.0;
-                    for (int cs = 0; cs < CS; ++cs) t += Ds[(cs * SM + s) * na + l];
-                    Bs[s * ldbs + la + l] -= t;
-                }
-                __syncthreads();
-            }
-        }
-        // ---- Y_(k+2) from the updated rows (the boxes are already in the ring), published for the reduction ----
+        sync_compute();
+        CTQR_PH(3)
+        // ---- own rows updated with panel k ----
+        pass_u(k);
+        sync_compute();
+        CTQR_PH(4)
+        // ---- Y_(k+2) from the updated rows, published for the reduction ----
         if (k + 2 < p.P) pass_a(k + 2);
+        CTQR_PH(5)
     }
+    sync_compute();
     for (int i = tid; i < SM * p.rpc; i += NT) {
         const int s = i / p.rpc, lr = i - s * p.rpc;
         const int64_t row = row_of(lr);

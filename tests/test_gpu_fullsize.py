@@ -8,6 +8,8 @@ where the O(mn^2) oracle cannot run in seconds:
         (independent of every GPU kernel) -- covers the late columns the oracle cannot reach;
   (iii) certified solution error: g = A^T (b - A x) from the sparse rows in fp64; exactly
         x* - x = (A^T A)^{-1} g and sigma_min(A_aug)^2 >= lambda, so ||x - x*|| <= ||g|| / lambda;
+        For fp32 that bound is ~100x pessimistic, so the fp32 gate is certified by the SHARP estimate of SURVEY.md 8c (iii):
+        ||(R^T R)^{-1} g|| with the fp64 factor that passed (i)-(ii), evaluated on the device by ct_qr_trsm_t + ct_qr_trsm;
   (iv)  fp32 against fp64 solution.
 
 Set CTQR_FULLSIZE=c4 to run the same checks on configs[3] (57 GB fp64 in core; minutes), or
@@ -74,6 +76,7 @@ def relerr(a, b):
 
 
 RESULTS = {}
+KEEP = {}          # the dense fp64 factor of configs[2], kept for the sharp error estimate of the fp32 solutions
 
 
 @pytest.mark.parametrize("band", [False, True], ids=["dense", "band"])
@@ -138,10 +141,26 @@ def test_fullsize_factor_and_solve(problem, dt, band):
         assert bound <= 1e-9, bound            # the north_star fp64 solution gate, certified
     else:
         assert opt <= 1e-5, opt                # rigorous bound is ~100x pessimistic in fp32
-    f.destroy()
+        if "f64" in KEEP:
+            # sharp estimate: x* - x = (A^T A)^{-1} g = R^{-1} R^{-T} g with the fp64 factor; certifies the fp32 solution
+            # gate slice by slice (half of it: the fp32 oracle, which cannot run at this size, has an error of its own)
+            f64 = KEEP["f64"]
+            Y = np.zeros((c.n, P["S"]), order="F"); D = np.zeros((c.n, P["S"]), order="F")
+            ctqr.ct_qr_trsm_t(f64, np.asfortranarray(g), P["S"], Y)
+            ctqr.ct_qr_trsm(f64, Y, P["S"], D)
+            per_slice = np.linalg.norm(D, axis=0) / np.linalg.norm(X64, axis=0)
+            print(f"[{CFG} float32{' band' if band else ''}] sharp estimate ||(R^T R)^-1 g|| / ||x||: worst slice {per_slice.max():.2e}, "
+                  f"all slices {np.linalg.norm(D) / np.linalg.norm(X64):.2e}")
+            assert per_slice.max() <= 5e-4, per_slice.max()
+    if dt == np.float64 and not band and CFG == "c3":
+        KEEP["f64"] = f
+    else:
+        f.destroy()
 
 
 def test_fullsize_fp32_vs_fp64(problem):
+    if "f64" in KEEP:
+        KEEP.pop("f64").destroy()
     if np.float64 not in RESULTS or np.float32 not in RESULTS:
         pytest.skip("needs both precisions from the previous test")
     d = relerr(RESULTS[np.float32], RESULTS[np.float64])

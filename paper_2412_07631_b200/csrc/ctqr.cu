@@ -190,6 +190,7 @@ struct ctqr_handle_s {
     void* dRd = nullptr;               // P blocks of nb x nb (ld nb): diagonal blocks of R
     void* dRinv = nullptr;             // their inverses (nb == 128 only), filled at the first solve
     bool rinv_ready = false;
+    void* dNm = nullptr; bool nm_ready = false; void* dLLt = nullptr;   // N_i = R_ii^{-1} R_{i,i+1} and the LL slots of the pipelined small-S TRSM
     void* dGt = nullptr; bool gt_ready = false;   // Mt[j] = T_(j-1) (V_(j-1)^T V_j) of the pipelined small-S Q^T B (fp64), built at first use
     void* dTau = nullptr;              // n
     // workspaces: [0] update stream, [1] panel stream
@@ -242,7 +243,7 @@ struct ctqr_handle_s {
         if (own_A && dA) cudaFree(dA);
         if (fmap) { msync(fmap, fmap_len, MS_SYNC); munmap(fmap, fmap_len); }
         if (ffd >= 0) close(ffd);
-        dev_free(dT); dev_free(dRd); dev_free(dRinv); dev_free(dTau); dev_free(dGt);
+        dev_free(dT); dev_free(dRd); dev_free(dRinv); dev_free(dTau); dev_free(dGt); dev_free(dNm); dev_free(dLLt);
         for (int i = 0; i < 2; ++i) { dev_free(dWp[i]); dev_free(dW[i]); dev_free(dW2[i]); }
         dev_free(dT2); dev_free(dMerge); dev_free(dCw); dev_free(dWs);
         for (int i = 0; i < 2; ++i) if (dVs[i]) cudaFree(dVs[i]);
@@ -1395,6 +1396,45 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
     CKI(trsm_prepare<T>(h));
     const bool exact = h.trsm_exact != 0;
     const bool use_inv = !exact && h.dRinv && ldx % (16 / (int64_t)sizeof(T)) == 0;
+    if (S <= kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && h.gemm_impl == 0 && h.nb == 128 && h.P >= 2) {
+        // memory-bound regime, pipelined: one grid hop per diagonal block (solve_small2.cuh)
+        const int nb = 128;
+        if (!h.nm_ready) {
+            const size_t slots = (size_t)4 * nb * kSmallS * 16;
+            if (!h.dNm) CK(dev_alloc(&h.dNm, (size_t)h.P * nb * nb * sizeof(T)));
+            if (!h.dLLt) { CK(dev_alloc(&h.dLLt, slots)); CK(cudaMemsetAsync(h.dLLt, 0, slots, h.sU)); }
+            CK(cudaMemsetAsync(h.dNm, 0, (size_t)h.P * nb * nb * sizeof(T), h.sU));
+            for (int i = 0; i + 1 < h.P; ++i) {
+                const int64_t i0 = (int64_t)i * nb;
+                GemmArgs<T> gn{};
+                gn.M = nb; gn.N = std::min<int64_t>(nb, h.n - i0 - nb); gn.K = nb;
+                gn.A = P_<T>(h.dRinv) + (size_t)i * nb * nb; gn.lda = nb;
+                gn.B = P_<T>(h.dA) + i0 + (i0 + nb) * h.lda; gn.ldb = h.lda;
+                gn.C = P_<T>(h.dNm) + (size_t)i * nb * nb; gn.ldc = nb; gn.alpha = T(1); gn.beta = T(0);
+                CK(gemm_direct<T>(false, gn, h.gemm_impl, h.sms, h.sU));
+            }
+            h.launches += h.P - 1;
+            h.nm_ready = true;
+        }
+        SmallTrsm2Args<T> a{};
+        const int64_t nch = ceil_div(h.n, (int64_t)kTrsmChunk);
+        const int G = (int)std::min<int64_t>(h.sms, nch);
+        a.A = P_<T>(h.dA); a.lda = h.lda; a.n = h.n; a.P = h.P; a.Rinv = P_<T>(h.dRinv); a.Nm = P_<T>(h.dNm);
+        a.X = X; a.ldx = ldx; a.S = (int)S;
+        a.cslots = reinterpret_cast<uint4*>(h.dLLt);
+        a.xslots = a.cslots + (size_t)2 * nb * kSmallS;
+        a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
+        a.rpc = (int)ceil_div(nch, (int64_t)G) * kTrsmChunk;
+        const size_t smem = ((size_t)nb * kSmallS + (size_t)kSmallS * kTrsmThreads + (size_t)kSmallS * a.rpc) * sizeof(T);
+        if (smem <= 220 * 1024) {
+            static SmemAttr attr2;
+            CK(ensure_dyn_smem(trsm_small2_kernel<T>, smem, attr2));
+            void* args[] = {(void*)&a};
+            CK(cudaLaunchCooperativeKernel((void*)trsm_small2_kernel<T>, dim3(G), dim3(kTrsmThreads), args, smem, h.sU));
+            h.launches += 1;
+            return 0;
+        }
+    }
     if (S <= kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && h.gemm_impl == 0) {
         // memory-bound regime: one cooperative kernel for all diagonal blocks (solve_small.cuh)
         SmallTrsmArgs<T> a{};

@@ -187,9 +187,7 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
     // holds the gathered W_(j-1) when this runs), publish W_j.  One element per warp (128 * 8 elements over G CTAs x 16 warps);
     // the loads are issued by reduce_issue and consumed by reduce_finish so that the row update runs in between.
     constexpr int MAXB = 5;                                 // partial slots per lane: G <= 160 CTAs
-    auto reduce_issue = [&](int j, double (&gv)[4], uint4 (&r)[MAXB]) {
-        const int e = g + warp * G;
-        if (e >= NB * SM) return;
+    auto reduce_issue_e = [&](int j, int e, double (&gv)[4], uint4 (&r)[MAXB]) {
         const uint4* all = p.part + (size_t)(j & 1) * G * (NB * SM);
         const double* gt = p.Mt + (size_t)j * NB * NB + (size_t)(e / SM) * NB;
 #pragma unroll
@@ -200,9 +198,7 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
             if (b < G) r[u] = ll_load(all + (size_t)b * (NB * SM) + e);
         }
     };
-    auto reduce_finish = [&](int j, const double (&gv)[4], uint4 (&r)[MAXB]) {
-        const int e = g + warp * G;
-        if (e >= NB * SM) return;
+    auto reduce_finish_e = [&](int j, int e, const double (&gv)[4], uint4 (&r)[MAXB]) {
         const unsigned seq = p.seq_base + (unsigned)j + 1u;
         const uint4* all = p.part + (size_t)(j & 1) * G * (NB * SM);
         const int s = e % SM;
@@ -224,6 +220,21 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
 #pragma unroll
         for (int off = 16; off >= 1; off >>= 1) t += shfl_xor(t, off);
         if (lane == 0) ll_store(p.sums + (size_t)(j & 1) * (NB * SM) + e, t, seq);
+    };
+    // the first element of a warp is split into issue / finish (the gather runs in between); a grid of fewer than 64 CTAs
+    // leaves more than one element per warp, the others follow back to back
+    auto reduce_issue = [&](int j, double (&gv)[4], uint4 (&r)[MAXB]) {
+        const int e = g + warp * G;
+        if (e < NB * SM) reduce_issue_e(j, e, gv, r);
+    };
+    auto reduce_finish = [&](int j, double (&gv)[4], uint4 (&r)[MAXB]) {
+        int e = g + warp * G;
+        if (e >= NB * SM) return;
+        reduce_finish_e(j, e, gv, r);
+        for (e += NW * G; e < NB * SM; e += NW * G) {
+            reduce_issue_e(j, e, gv, r);
+            reduce_finish_e(j, e, gv, r);
+        }
     };
 
     // ---- prologue: Y_0 and Y_1 from the rows as given; W_0 needs no correction ----
@@ -296,6 +307,187 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
         const int s = i / p.rpc, lr = i - s * p.rpc;
         const int64_t row = row_of(lr);
         if (s < S && lr < nl && row < p.m) p.B[row + (int64_t)s * p.ldb] = Bs[s * ldbs + lr];
+    }
+}
+
+
+// -------------------------------------------------------------------------------------------------------------------
+// Pipelined small-S blocked TRSM (task list PAPER.md:L62-73), both precisions.
+//
+// trsm_small_kernel (solve_small.cuh) has TWO grid hops on the critical path of every diagonal block: the row owners
+// publish C_i -> everybody gathers it and forms X_i redundantly -> everybody updates -> the owners of the next block
+// publish.  Here the chain through the grid is ONE hop per block:
+//   * the rows of block i are published "stale", as they are after the updates of the blocks >= i+2 (Cst_i), while the
+//     previous block is still being solved; the missing update is applied algebraically,
+//         X_i = R_ii^{-1} (Cst_i - R_{i,i+1} X_{i+1}) = R_ii^{-1} Cst_i - N_i X_{i+1},   N_i = R_ii^{-1} R_{i,i+1}
+//     (N_i: 128 x 128 per block, built once per handle next to the inverted diagonal blocks);
+//   * X_i is formed element by element by element owners (one warp per element, element e belongs to CTA e mod G), each
+//     reading one row of R_ii^{-1} and of N_i, and published; the bulk update of the rows above with X_{i+1} -- the pass
+//     that streams R from HBM -- runs while that publication is in flight, starting with the rows of block i-1 so that
+//     their owners can publish Cst_{i-1} early.
+// Same row distribution as trsm_small_kernel (chunks of 16 rows dealt round-robin), deterministic.
+// -------------------------------------------------------------------------------------------------------------------
+template <typename T>
+struct SmallTrsm2Args {
+    const T* A; int64_t lda; int64_t n; int P;
+    const T* Rinv;                  // P blocks of 128 x 128 (ld 128), zero-padded last block
+    const T* Nm;                    // P blocks of 128 x 128 (ld 128): Nm[i] = Rinv_i R[i-th row block, (i+1)-th column block]
+    T* X; int64_t ldx; int S;       // in: C[0:n, :], out: X
+    uint4* cslots;                  // [2][128 * kSmallS] LL slots: stale rows of a block
+    uint4* xslots;                  // [2][128 * kSmallS] LL slots: X of a block
+    unsigned seq_base;              // step numbers seq_base + 1 .. seq_base + P are used by this launch
+    int rpc;                        // local rows per CTA (multiple of kTrsmChunk)
+};
+
+template <typename T>
+__global__ void __launch_bounds__(kTrsmThreads, 1) trsm_small2_kernel(SmallTrsm2Args<T> p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NB = 128, SM = kSmallS, NT = kTrsmThreads, NW = NT / 32, CH = kTrsmChunk;
+    T* Xs = reinterpret_cast<T*>(smem_raw);                 // [NB][SM]   X of the block solved last
+    T* Ds = Xs + NB * SM;                                   // [<=8][SM][lim] partial updates (groups * lim <= NT)
+    T* Cs = Ds + SM * NT;                                   // [SM][rpc]  own rows, transposed
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = blockIdx.x, G = gridDim.x, S = p.S;
+    auto row_of = [&](int lr) -> int64_t { return ((int64_t)(lr / CH) * G + g) * CH + (lr % CH); };
+    for (int i = tid; i < SM * p.rpc; i += NT) {
+        const int s = i / p.rpc, lr = i - s * p.rpc;
+        const int64_t row = row_of(lr);
+        Cs[i] = (s < S && row < p.n) ? p.X[row + (int64_t)s * p.ldx] : T(0);
+    }
+    __syncthreads();
+    // the owners of the rows of block b publish them as they are now
+    auto publish_rows = [&](int b) {
+        const int64_t b0 = (int64_t)b * NB;
+        const int kwb = (int)min((int64_t)NB, p.n - b0);
+        const unsigned seq = p.seq_base + (unsigned)(p.P - 1 - b) + 1u;
+        uint4* slots = p.cslots + (size_t)(b & 1) * (NB * SM);
+        for (int e = tid; e < NB * SM; e += NT) {
+            const int rr = e / SM, s = e - rr * SM;
+            const int64_t q = (b0 + rr) / CH;
+            if (rr < kwb && (int)(q % G) == g) ll_store(slots + e, Cs[s * p.rpc + (int)(q / G) * CH + (int)((b0 + rr) % CH)], seq);
+        }
+    };
+    // own rows [lr0, lr1) (local indices; all above block b): C[r, :] -= R[r, block b] Xs, the 128 columns split over CS
+    // thread groups so that enough loads are in flight
+    auto update_rows = [&](int b, int lr0, int lr1) {
+        const int64_t b0 = (int64_t)b * NB;
+        const int kwb = (int)min((int64_t)NB, p.n - b0);
+        const int cnt = lr1 - lr0;
+        if (cnt <= 0) return;                                // (uniform over the CTA)
+        int CS = 1;
+        while (CS < 8 && 2 * CS * cnt <= NT) CS *= 2;
+        const int cpc = (kwb + CS - 1) / CS;
+        for (int base = 0; base < cnt; base += NT / CS) {    // NT / CS rows per sweep
+            const int rows = min(cnt - base, NT / CS);
+            const int cs = tid / rows, li = tid - cs * rows;
+            T d[SM];
+#pragma unroll
+            for (int s = 0; s < SM; ++s) d[s] = T(0);
+            const bool act = cs < CS;
+            const int lr = lr0 + base + li;
+            if (act) {
+                const int64_t row = row_of(lr);
+                const int c0 = cs * cpc, c1 = min(kwb, c0 + cpc);
+                const T* rr = p.A + row + b0 * p.lda;
+#pragma unroll 16
+                for (int c = c0; c < c1; ++c) {
+                    const T v = __ldg(rr + (int64_t)c * p.lda);
+#pragma unroll
+                    for (int s = 0; s < SM; ++s) d[s] = fma(v, Xs[c * SM + s], d[s]);
+                }
+            }
+            if (CS == 1) {
+                if (act)
+#pragma unroll
+                    for (int s = 0; s < SM; ++s) Cs[s * p.rpc + lr] -= d[s];
+            } else {
+                if (act)
+#pragma unroll
+                    for (int s = 0; s < SM; ++s) Ds[(cs * SM + s) * rows + li] = d[s];
+                __syncthreads();
+                for (int idx = tid; idx < rows * SM; idx += NT) {
+                    const int s = idx / rows, l = idx - s * rows;
+                    T t = T(0);
+                    for (int c2 = 0; c2 < CS; ++c2) t += Ds[(c2 * SM + s) * rows + l];
+                    Cs[s * p.rpc + lr0 + base + l] -= t;
+                }
+            }
+            __syncthreads();
+        }
+    };
+    // local row range [lo, hi) of the global rows [r0, r1) (both multiples of CH or the matrix end)
+    auto local_of = [&](int64_t r) -> int {                 // number of own rows below global row r (r a multiple of CH)
+        const int64_t q = r / CH;
+        return q > g ? (int)((q - g + G - 1) / G) * CH : 0;
+    };
+
+    publish_rows(p.P - 1);
+    for (int i = p.P - 1; i >= 0; --i) {
+        const int64_t i0 = (int64_t)i * NB;
+        const int kw = (int)min((int64_t)NB, p.n - i0);
+        const unsigned seq = p.seq_base + (unsigned)(p.P - 1 - i) + 1u;
+        // ---- 1. element owners: X_i[r, s] = sum_q Rinv_i[r, q] Cst_i[q, s] - sum_q N_i[r, q] X_(i+1)[q, s], published ----
+        {
+            const uint4* cst = p.cslots + (size_t)(i & 1) * (NB * SM);
+            const T* ri = p.Rinv + (size_t)i * NB * NB;
+            const T* ni = p.Nm + (size_t)i * NB * NB;
+            for (int e = g + warp * G; e < NB * SM; e += NW * G) {
+                const int r = e / SM, s = e - r * SM;
+                T a[4], b[4];
+                uint4 c[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int q = lane + 32 * u;
+                    a[u] = __ldg(ri + r + (size_t)q * NB);
+                    b[u] = (i + 1 < p.P) ? __ldg(ni + r + (size_t)q * NB) : T(0);
+                    c[u] = q < kw ? ll_load(cst + q * SM + s) : make_uint4(0u, seq, 0u, seq);
+                }
+                T t = T(0);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int q = lane + 32 * u;
+                    while (c[u].y != seq || c[u].w != seq) c[u] = ll_load(cst + q * SM + s);
+                    t = fma(a[u], q < kw ? ll_value<T>(c[u]) : T(0), t);
+                    if (i + 1 < p.P) t = fma(-b[u], Xs[q * SM + s], t);
+                }
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) t += shfl_xor(t, off);
+                if (lane == 0) ll_store(p.xslots + (size_t)(i & 1) * (NB * SM) + e, t, seq);
+            }
+        }
+        // ---- 2. bulk update with X_(i+1) (still in Xs) of the own rows above block i, the rows of block i-1 first; their
+        //         owners then publish them for the next block ----
+        const int l_im1 = local_of(i0 > NB ? i0 - NB : 0), l_i = local_of(i0);      // own rows below (i-1) * NB, below i * NB
+        if (i + 1 < p.P) update_rows(i + 1, l_im1, l_i);
+        else __syncthreads();
+        if (i >= 1) publish_rows(i - 1);
+        if (i + 1 < p.P) update_rows(i + 1, 0, l_im1);
+        // ---- 3. gather X_i; the owners of the rows of block i store it as their final rows ----
+        __syncthreads();
+        {
+            const uint4* xs = p.xslots + (size_t)(i & 1) * (NB * SM);
+            uint4 r[NB * SM / NT];
+#pragma unroll
+            for (int u = 0; u < NB * SM / NT; ++u) r[u] = ll_load(xs + tid + u * NT);
+#pragma unroll
+            for (int u = 0; u < NB * SM / NT; ++u) {
+                const int e = tid + u * NT;
+                while (r[u].y != seq || r[u].w != seq) r[u] = ll_load(xs + e);
+                Xs[e] = ll_value<T>(r[u]);
+            }
+        }
+        __syncthreads();
+        for (int e = tid; e < NB * SM; e += NT) {
+            const int rr = e / SM, s = e - rr * SM;
+            const int64_t q = (i0 + rr) / CH;
+            if (rr < kw && (int)(q % G) == g) Cs[s * p.rpc + (int)(q / G) * CH + (int)((i0 + rr) % CH)] = Xs[e];
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < SM * p.rpc; i += NT) {
+        const int s = i / p.rpc, lr = i - s * p.rpc;
+        const int64_t row = row_of(lr);
+        if (s < S && row < p.n) p.X[row + (int64_t)s * p.ldx] = Cs[i];
     }
 }
 

@@ -21,6 +21,11 @@ def _has_cuda():
 
 
 def pytest_collection_modifyitems(config, items):
+    # a cooperative kernel that deadlocks would otherwise hang the whole session: every GPU test gets a time limit
+    # (pytest-timeout, thread method: the process is ended with a stack dump)
+    for it in items:
+        if "gpu" in it.keywords and not any(m.name == "timeout" for m in it.iter_markers()):
+            it.add_marker(pytest.mark.timeout(600, method="thread"))
     if _has_cuda():
         return
     skip = pytest.mark.skip(reason="no CUDA device")

@@ -227,6 +227,9 @@ struct ctqr_handle_s {
         if (tpool_used == tpool.size()) { cudaEvent_t e; cudaEventCreate(&e); tpool.push_back(e); }
         return tpool[tpool_used++];
     }
+    // host matrix staged in core: column chunks arriving on the copy stream while the first panels are already factored;
+    // (one past the last column of the chunk, event recorded after its copy); emptied once every event has been waited for
+    std::vector<std::pair<int64_t, cudaEvent_t>> arrive;
     bool factored = false;
     // opt->lower_bandwidth: A(i, j) == 0 for i - j > kl, so the reflectors of the
     // columns [.., jend) end at row min(m, kl + jend) and every product over rows stops there
@@ -483,6 +486,15 @@ static cudaEvent_t new_event(H& h, bool timing) {
     return e;
 }
 
+// `st` must not touch the columns [.., col_end) before their host-to-device chunks have landed (h.arrive, see factor_typed)
+static int wait_columns(H& h, cudaStream_t st, int64_t col_end) {
+    for (auto& a : h.arrive) {
+        CK(cudaStreamWaitEvent(st, a.second, 0));
+        if (a.first >= col_end) break;
+    }
+    return 0;
+}
+
 // ------------------------------------------------------------------------------------------
 // a4: right-looking blocked QR of the columns [c0, c1) (c0 a multiple of nb) with look-ahead:
 // panel k+1 is factored on the high-priority stream sP while the bulk of update k runs on sU.
@@ -496,6 +508,7 @@ static int factor_range_single(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) 
     const int k0 = (int)(c0 / nb), k1 = (int)ceil_div(c1, nb);
     if (!h.evP) { h.evP = new_event(h, false); h.evL = new_event(h, false); h.evU = new_event(h, false); }
     cudaEvent_t evP = h.evP, evL = h.evL, evU = h.evU;
+    if (!h.arrive.empty()) { CKI(wait_columns(h, h.sU, c1)); h.arrive.clear(); }   // no copy overlap on this path
     CK(cudaEventRecord(evU, h.sU));
     CK(cudaStreamWaitEvent(h.sP, evU, 0));
     if (!h.lookahead) {
@@ -635,10 +648,11 @@ static int pair_merge(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
     h.launches += 6;
     if constexpr (sizeof(T) == 4) {
         if (h.dVs[slot]) {
-            // the K = 256 update of this pair reads [V_k V_{k+1}] below the first diagonal block once per output tile:
-            // split it into TF32 hi / lo once, here on the panel stream (gemm_umma_tma.cuh)
+            // both contractions of this pair's trailing updates read [V_k V_{k+1}] once per output tile: split it into TF32
+            // hi / lo once, here on the panel stream (gemm_umma_tma.cuh); rows from j0 (the rows of the first diagonal block
+            // in the second panel's columns hold R_{k,k+1}: split along, never used)
             float* hi = P_<float>(h.dVs[slot]);
-            CK(split_tf32_launch(A + (j0 + nb) + j0 * lda, lda, m - j0 - nb, 2 * nb, hi, hi + (size_t)h.ldvs * 256, h.ldvs, st));
+            CK(split_tf32_launch(A + j0 + j0 * lda, lda, m - j0, 2 * nb, hi, hi + (size_t)h.ldvs * 256, h.ldvs, st));
             h.launches += 1;
         }
     }
@@ -679,7 +693,19 @@ static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
         if (L1.kind != 1) return set_err(CTQR_ERR_STATE, "pair update needs the stream-K product");
         CKI(confine<T>(h, L1, reserve_sms, st));
         if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
-        CK(gemm_run<T>(true, g1, L1, h.gemm_impl, st));
+        bool pre = false;
+#ifndef CTQR_NO_VTC_TMA
+        if constexpr (sizeof(T) == 4) {
+            if (h.dVs[slot]) {
+                // fp32: V pre-split by the merge and TMA-fed, the streamed C split on the fly (vtc_tma_kernel)
+                const float* vh = P_<float>(h.dVs[slot]) + (half ? (size_t)nb + (size_t)nb * h.ldvs : 0);
+                cudaError_t ev = vtc_presplit_launch(g1, vh, vh + (size_t)h.ldvs * 256, h.ldvs, L1, st);
+                if (ev == cudaSuccess) pre = true;
+                else if (ev != cudaErrorNotSupported) CK(ev);
+            }
+        }
+#endif
+        if (!pre) CK(gemm_run<T>(true, g1, L1, h.gemm_impl, st));
         if (prof) { CK(cudaEventRecord(e1, st)); h.spans.push_back({e0, e1, 2.0 * (double)g1.K * nb * (double)nc, 0}); }
         CK(partial_sum_launch<T>(Wp, L1.seg, nb, nc, W + half * nb, 256, st));
     }
@@ -701,7 +727,7 @@ static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
         if (h.dVs[slot] && h.dWs && (size_t)2 * 256 * (size_t)nc <= h.ws_elems && ldc % 4 == 0) {
             // fp32: operands pre-split once (V by the merge, T2^T W here), TMA-fed tcgen05 kernel, 128 x 128 tiles
             float* whi = P_<float>(h.dWs); float* wlo = whi + (size_t)256 * nc;
-            const float* vhi = P_<float>(h.dVs[slot]); const float* vlo = vhi + (size_t)h.ldvs * 256;
+            const float* vhi = P_<float>(h.dVs[slot]) + nb; const float* vlo = vhi + (size_t)h.ldvs * 256;   // rows below the first diagonal block
             CK(split_tf32_launch(W2, 256, 256, nc, whi, wlo, 256, st));
             if (prof) { e0 = h.timing_event(); e1 = h.timing_event(); CK(cudaEventRecord(e0, st)); }
             CK(upd_presplit_launch(gb.M, nc, 256, -1.f, vhi, vlo, h.ldvs, whi, wlo, 256, 1.f, gb.C, ldc, sms, st));
@@ -739,12 +765,36 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
         return 0;
     };
     int slot = 0;
+    // host matrix still arriving in column chunks (factor_typed): the first chain needs the first pair's columns only, the
+    // first trailing update then follows the copy chunk by chunk; every later step is ordered behind those waits
+    const bool arriving = !h.arrive.empty() && c0 == 0;
+    if (arriving) CKI(wait_columns(h, h.sP, 2 * nb));
+    else if (!h.arrive.empty()) { CKI(wait_columns(h, h.sU, c1)); h.arrive.clear(); }
     CKI(chain(c0, slot));
     for (int64_t j0 = c0;; j0 += 2 * nb, slot ^= 1) {
         const int64_t jn = j0 + 2 * nb;                     // first trailing column
         const int64_t rem = c1 - jn;
         const int64_t m = row_end(h, jn);                   // row end of this pair
         CK(cudaStreamWaitEvent(h.sU, evP, 0));              // V, T2 of this pair ready
+        if (arriving && j0 == c0 && rem >= 2 * nb) {
+            // first pair: look-ahead block, next chain, then the bulk in the order the chunks arrive
+            CKI(wait_columns(h, h.sU, jn + 2 * nb));
+            CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, slot, A + j0 + jn * lda, lda, 2 * nb, 0));
+            CK(cudaEventRecord(evL, h.sU));
+            CK(cudaStreamWaitEvent(h.sP, evL, 0));
+            CKI(chain(jn, slot ^ 1));
+            int64_t ca = jn + 2 * nb;
+            for (auto& a : h.arrive) {
+                const int64_t cb = std::min<int64_t>(a.first, c1);
+                if (cb <= ca) continue;
+                CK(cudaStreamWaitEvent(h.sU, a.second, 0));
+                CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, slot, A + j0 + ca * lda, lda, cb - ca, 0));
+                ca = cb;
+            }
+            h.arrive.clear();
+            continue;
+        }
+        if (!h.arrive.empty()) { CKI(wait_columns(h, h.sU, c1)); h.arrive.clear(); }
         if (rem < 2 * nb) {
             // no further full pair: finish this update, then the single-panel driver takes the tail
             CKI(larfb_pair<T>(h, h.sU, A, lda, m, j0, slot, A + j0 + jn * lda, lda, rem, 0));
@@ -1106,10 +1156,29 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
         h.lda = round_up(m, 16 / sizeof(T));
         CK(big_alloc(&h.dA, (size_t)h.lda * n * sizeof(T)));
         h.own_A = true;
-        CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
-                             cudaMemcpyHostToDevice, h.sU));
         h.st.h2d_bytes = (double)bytes;
-        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda, 0, h.n));
+        const int64_t chunk = round_up(std::max<int64_t>(2048, ceil_div(n, (int64_t)16)), 256);
+        if (h.kl > 0 || n < 4 * chunk) {
+            // (the band promise is checked on the whole matrix before anything is factored; small matrices: one copy)
+            CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n, cudaMemcpyHostToDevice, h.sU));
+            if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda, 0, h.n));
+            return factor_incore<T>(h, P_<T>(h.dA), h.lda);
+        }
+        // The host-to-device copy runs in column chunks on the copy stream while the factorisation already works on the
+        // columns that have landed (the first pair's trailing update follows the copy chunk by chunk): the copy, 1 s for
+        // 57 GB over the host link, is hidden behind the first panels instead of preceding them.
+        if (!h.sC) CK(cudaStreamCreateWithFlags(&h.sC, cudaStreamNonBlocking));
+        cudaEvent_t ev0 = new_event(h, false);
+        CK(cudaEventRecord(ev0, h.sU));                     // (alloc_state's memsets)
+        CK(cudaStreamWaitEvent(h.sC, ev0, 0));
+        for (int64_t ca = 0; ca < n; ca += chunk) {
+            const int64_t cb = std::min<int64_t>(n, ca + chunk);
+            CK(cudaMemcpy2DAsync(P_<T>(h.dA) + ca * h.lda, h.lda * sizeof(T), (const T*)A + ca * lda, lda * sizeof(T), m * sizeof(T),
+                                 cb - ca, cudaMemcpyHostToDevice, h.sC));
+            cudaEvent_t e = new_event(h, false);
+            CK(cudaEventRecord(e, h.sC));
+            h.arrive.push_back({cb, e});
+        }
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
     // out of core: budget = 2 super-panel buffers + 2 panel stream buffers

@@ -84,6 +84,11 @@ static MmaPlan to_plan(const GemmLaunch& L) {
     return p;
 }
 
+cudaError_t vtc_presplit_launch(const GemmArgs<float>& g, const float* Ahi, const float* Alo, int64_t lda, const GemmLaunch& L, cudaStream_t st) {
+    if (L.kind != 1 || L.cfg != 21 || !L.partial) return cudaErrorNotSupported;
+    return vtc_presplit_launch_impl(g, Ahi, Alo, lda, to_plan(L), st);
+}
+
 cudaError_t gemm_run_f32(bool ta, GemmArgs<float> g, const GemmLaunch& L, int impl, cudaStream_t st) {
     if (g.M <= 0 || g.N <= 0) return cudaSuccess;
     g.a_vec_ok = aligned16(g.A, g.lda, 4);

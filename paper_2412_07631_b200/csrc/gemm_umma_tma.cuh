@@ -247,4 +247,205 @@ inline cudaError_t upd_presplit_launch_impl(int64_t M, int64_t N, int64_t K, flo
     return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// W = A^T B as stream-K partial tiles (W = V^T C of larfb) with the small operand A = V pre-split and TMA-fed; the streamed
+// operand B = C is read once per launch, so it is still split on the fly by the worker warps -- half the producer work of
+// gemm_umma_kernel<true, 128> -- and the TMEM accumulator is drained once per kDrain k-blocks instead of every k-block.
+// Same unit sequence, partial-tile slots and consumers (partial_sum / mm128 / T^T W) as gemm_umma.cuh.
+//   warps 0-7  workers: C chunks global -> registers (one k-block ahead) -> hi / lo -> B_hi, B_lo of the stage; drain; epilogue
+//   warp 8     TMA producer of A_hi, A_lo (K-major boxes of 32 k x 128 m, SWIZZLE_128B)
+//   warp 9     MMA issuer (owns the TMEM allocation)
+// ---------------------------------------------------------------------------------------------------------------------
+namespace umma {
+
+constexpr int kVWorkers = 256, kVThreads = kVWorkers + 64;
+
+__global__ void __launch_bounds__(kVThreads, 1)
+vtc_tma_kernel(const __grid_constant__ CUtensorMap mAh, const __grid_constant__ CUtensorMap mAl, GemmArgs<float> g, StreamK sk) {
+    constexpr int BN = 128, NC = BN / 2, PBN = BN * 8 / kVWorkers;
+    extern __shared__ unsigned char smem_raw[];
+    const unsigned sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
+    const unsigned bars = sbase + kTStages * kTStage;           // fullA[S], fullB[S], empty[S], tfull[2], tempty[2]
+    auto fullA = [&](int s) { return bars + 8u * s; };
+    auto fullB = [&](int s) { return bars + 8u * (kTStages + s); };
+    auto empty = [&](int s) { return bars + 8u * (2 * kTStages + s); };
+    auto tfull = [&](int b) { return bars + 8u * (3 * kTStages + b); };
+    auto tempty = [&](int b) { return bars + 8u * (3 * kTStages + 2 + b); };
+    unsigned* tmem_slot = reinterpret_cast<unsigned*>(sgen + kTStages * kTStage + 8 * (3 * kTStages + 4));
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t u0 = (int64_t)blockIdx.x * sk.L, u1 = min(sk.U, u0 + sk.L), nunits = u1 - u0;
+    // An accumulator generation = up to kDrain consecutive units of one tile segment: it closes with its kDrain-th unit, with
+    // the last k-block of the tile, or with the CTA's last unit.  Both the MMA issuer and the workers follow that rule with
+    // incremental counters (no division on the per-k-block path).
+    const int kt0 = (int)(u0 % sk.KT);
+    if (tid == 0) {
+        for (int s = 0; s < kTStages; ++s) { mbar_init(fullA(s), 1); mbar_init(fullB(s), kVWorkers); mbar_init(empty(s), 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tfull(b), 1); mbar_init(tempty(b), kVWorkers); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        tma::prefetch_map(&mAh); tma::prefetch_map(&mAl);
+    }
+    if (warp == 9) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(tmem_slot)), "r"(256u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const unsigned tmem = *tmem_slot;
+
+    if (warp == 8) {
+        // ================= TMA producer of A = V (M <= 128 columns of V, zero-filled beyond) =================
+        if (lane == 0) {
+            int s = 0; unsigned ph = 1;
+            int kt = kt0;
+            for (int64_t j = 0; j < nunits; ++j, kt = (kt + 1 == sk.KT) ? 0 : kt + 1) {
+                mbar_wait(empty(s), ph);
+                tma::mbar_expect_tx(fullA(s), 2u * kTTile);
+                tma::load_2d(sbase + s * kTStage, &mAh, kt * BK, 0, fullA(s));
+                tma::load_2d(sbase + s * kTStage + kTTile, &mAl, kt * BK, 0, fullA(s));
+                if (++s == kTStages) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else if (warp == 9) {
+        // ================= MMA issuer =================
+        const unsigned idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(BN >> 3) << 17) | ((unsigned)(BM >> 4) << 24);
+        int s = 0; unsigned fph = 0;
+        int64_t d = 0;
+        int kt = kt0, run = 0;
+        for (int64_t j = 0; j < nunits; ++j) {
+            const int b = (int)(d & 1);
+            const bool first = run == 0, last = kt == sk.KT - 1 || j == nunits - 1 || run == kDrain - 1;
+            run = last ? 0 : run + 1;
+            kt = (kt + 1 == sk.KT) ? 0 : kt + 1;
+            if (first) mbar_wait(tempty(b), (unsigned)(((d >> 1) & 1) ^ 1));
+            mbar_wait(fullA(s), fph);
+            mbar_wait(fullB(s), fph);
+            tc_fence_after();
+            if (lane == 0) {
+                const unsigned a_hi = sbase + s * kTStage, a_lo = a_hi + kTTile, b_hi = a_hi + 2 * kTTile, b_lo = a_hi + 3 * kTTile;
+                const unsigned dt = tmem + (unsigned)b * BN;
+#pragma unroll
+                for (int ks = 0; ks < BK / 8; ++ks) {
+                    const uint64_t dah = make_desc(a_hi + ks * 32, 16, 1024), dal = make_desc(a_lo + ks * 32, 16, 1024);
+                    const uint64_t dbh = make_desc(b_hi + ks * 32, 16, 1024), dbl = make_desc(b_lo + ks * 32, 16, 1024);
+                    tc_mma_tf32(dt, dal, dbh, idesc, (first && ks == 0) ? 0u : 1u);
+                    tc_mma_tf32(dt, dah, dbl, idesc, 1u);
+                    tc_mma_tf32(dt, dah, dbh, idesc, 1u);
+                }
+                tc_commit(empty(s));
+                if (last) tc_commit(tfull(b));
+            }
+            __syncwarp();
+            if (last) ++d;
+            if (++s == kTStages) { s = 0; fph ^= 1u; }
+        }
+    } else {
+        // ================= workers: B = C producer + accumulator drain + partial-tile epilogue =================
+        const int rowq = (warp & 3) * 32 + lane;          // TMEM lane = output row (a column of V)
+        const int colh = (warp >> 2) * NC;
+        float acc[NC];
+        float4 rb[PBN];
+        int64_t pt = u0 / sk.KT; int pkt = (int)(u0 - pt * sk.KT);
+        auto load_regs = [&]() {
+            const int64_t n0 = pt * BN, k0 = (int64_t)pkt * BK;     // tilesM == 1 in partial mode: tile index = column block
+#pragma unroll
+            for (int p = 0; p < PBN; ++p) {
+                const int c = tid + p * kVWorkers;
+                const int r = c >> 3, kc = (c & 7) * 4;
+                rb[p] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (n0 + r < g.N && k0 + kc < g.K) rb[p] = __ldg(reinterpret_cast<const float4*>(g.B + (n0 + r) * g.ldb + k0 + kc));
+            }
+            if (++pkt == sk.KT) { pkt = 0; ++pt; }
+        };
+        auto store_stage = [&](int s) {
+            unsigned char* st = sgen + (size_t)s * kTStage + 2 * kTTile;
+#pragma unroll
+            for (int p = 0; p < PBN; ++p) {
+                const int c = tid + p * kVWorkers;
+                const int r = c >> 3, kc = c & 7;
+                const unsigned off = (r >> 3) * 1024 + (r & 7) * 128 + ((kc ^ (r & 7)) << 4);
+                uint4 hi, lo;
+                split4(rb[p], hi, lo);
+                *reinterpret_cast<uint4*>(st + off) = hi;
+                *reinterpret_cast<uint4*>(st + kTTile + off) = lo;
+            }
+        };
+        int64_t ct = u0 / sk.KT;
+        int64_t pi = 0, ci = 0, d = 0;                    // produced units, units whose accumulator has been drained, generations
+        int ckt = kt0;                                    // k-block index (inside its tile) of unit ci
+        int ps = 0; unsigned pph = 1;
+        bool fresh = true;
+        load_regs();
+        while (ci < nunits) {
+            if (pi < nunits) {
+                mbar_wait(empty(ps), pph);
+                store_stage(ps);
+                fence_proxy_async();
+                mbar_arrive(fullB(ps));
+                if (++ps == kTStages) { ps = 0; pph ^= 1u; }
+                ++pi;
+                if (pi < nunits) load_regs();
+            }
+            // drain every generation that closed at least kTStages - 1 units behind the producer (or everything at the end)
+            for (;;) {
+                // the unit that closes the generation starting at ci
+                const int64_t ce = ci + min((int64_t)min(kDrain - 1, sk.KT - 1 - ckt), nunits - 1 - ci);
+                if (!(ce + (kTStages - 1) <= pi || pi == nunits)) break;
+                if (fresh) {
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) acc[c] = 0.f;
+                    fresh = false;
+                }
+                const int b = (int)(d & 1);
+                mbar_wait(tfull(b), (unsigned)((d >> 1) & 1));
+                tc_fence_after();
+                const unsigned taddr = tmem + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)(b * BN + colh);
+#pragma unroll
+                for (int c0 = 0; c0 < NC; c0 += 32) {
+                    float v[32];
+                    tmem_ld32(taddr + c0, v);
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) acc[c0 + c] += v[c];
+                }
+                tc_fence_before();
+                mbar_arrive(tempty(b));
+                ++d;
+                const int kte = ckt + (int)(ce - ci);     // k-block index of the closing unit
+                ci = ce + 1;
+                ckt = (kte + 1 == sk.KT) ? 0 : kte + 1;
+                if (kte == sk.KT - 1 || ci == nunits) {
+                    // segment of tile ct ends: compact partial tile (see gemm_mma.cuh)
+                    float* Pt = g.C + (ct + (int64_t)blockIdx.x) * (int64_t)(BM * BN) + rowq + (int64_t)colh * BM;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) Pt[c * BM] = g.alpha * acc[c];
+                    ++ct; fresh = true;
+                }
+                if (ci >= nunits) break;
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 9)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem), "r"(256u) : "memory");
+}
+
+}  // namespace umma
+
+// stream-K partial tiles of A^T B with A = Ahi + Alo pre-split (K x M, k-contiguous, M <= 128, lda multiple of 4, 16-byte
+// aligned) and B fp32 (K x N, k-contiguous, 16-byte aligned rows).  p: the umma_plan of (M, N, K) in partial mode.
+inline cudaError_t vtc_presplit_launch_impl(GemmArgs<float> g, const float* Ahi, const float* Alo, int64_t lda, const MmaPlan& p, cudaStream_t st) {
+    if (g.M <= 0 || g.N <= 0) return cudaSuccess;
+    if (g.M > 128 || !p.sk.partial || p.sk.tilesM != 1 || lda % 4 || ((uintptr_t)Ahi | (uintptr_t)Alo) % 16) return cudaErrorInvalidValue;
+    CUtensorMap mAh, mAl;
+    cudaError_t e;
+    if ((e = tma::map_2d(&mAh, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Ahi, g.K, g.M, lda, 32, 128, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return e;
+    if ((e = tma::map_2d(&mAl, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, Alo, g.K, g.M, lda, 32, 128, CU_TENSOR_MAP_SWIZZLE_128B)) != cudaSuccess) return e;
+    static SmemAttr attr;
+    if ((e = ensure_dyn_smem(umma::vtc_tma_kernel, umma::kTSmem, attr)) != cudaSuccess) return e;
+    umma::vtc_tma_kernel<<<p.grid, umma::kVThreads, umma::kTSmem, st>>>(mAh, mAl, g, p.sk);
+    return cudaGetLastError();
+}
+
 }  // namespace ctqr

@@ -71,6 +71,10 @@ cudaError_t split_tf32_launch(const float* src, int64_t ld, int64_t rows, int64_
 cudaError_t upd_presplit_launch(int64_t M, int64_t N, int64_t K, float alpha, const float* Ahi, const float* Alo, int64_t lda,
                                 const float* Bhi, const float* Blo, int64_t ldb, float beta, float* C, int64_t ldc, int ctas, cudaStream_t st);
 
+// stream-K partial tiles of A^T B (planned by gemm_plan_f32 as the tcgen05 configuration, L.cfg == 21) with A given pre-split
+// (K x M, k-contiguous, M <= 128): returns cudaErrorNotSupported when the plan is not that configuration
+cudaError_t vtc_presplit_launch(const GemmArgs<float>& g, const float* Ahi, const float* Alo, int64_t lda, const GemmLaunch& L, cudaStream_t st);
+
 // cooperative register-resident panel kernel; returns cudaErrorInvalidValue for an unsupported (ib, rpt)
 cudaError_t panel_launch_f64(int ib, int rpt, PanelArgs<double>& pa, int G, cudaStream_t st);
 cudaError_t panel_launch_f32(int ib, int rpt, PanelArgs<float>& pa, int G, cudaStream_t st);

@@ -76,6 +76,7 @@ def relerr(a, b):
 
 
 RESULTS = {}
+TAU = {}
 KEEP = {}          # the dense fp64 factor of configs[2], kept for the sharp error estimate of the fp32 solutions
 
 
@@ -95,6 +96,7 @@ def test_fullsize_factor_and_solve(problem, dt, band):
             assert relerr(X, RESULTS[dt]) <= (1e-10 if dt == np.float64 else 5e-4)
     else:
         RESULTS[dt] = X
+        TAU[dt] = ctqr.ct_qr_get_tau(f)
     tol_round = 1e-11 if dt == np.float64 else 5e-4
     # (i) leading columns against the oracle
     k = K_LEAD
@@ -156,6 +158,36 @@ def test_fullsize_factor_and_solve(problem, dt, band):
         KEEP["f64"] = f
     else:
         f.destroy()
+
+
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_fullsize_host_matrix_overlapped_copy(problem, dt):
+    """The same matrix given as a pinned HOST buffer that fits the device: the library stages it in column chunks on the
+    copy stream while the first panels are already being factored (the first trailing update follows the copy chunk by
+    chunk).  Same factor and solution as the device-resident run, to rounding."""
+    import torch
+    if dt not in RESULTS:
+        pytest.skip("needs the device-resident run of the previous test")
+    P = problem
+    c = P["c"]
+    if c.m * c.n * np.dtype(dt).itemsize > 40e9:
+        pytest.skip("host copy of this size is left to bench.py's e2e leg")
+    tdt = torch.float64 if dt == np.float64 else torch.float32
+    At, _ = wl.dense_augmented_device(c, tdt, P["coo"])
+    Ah = torch.empty(At.shape, dtype=tdt, pin_memory=True)
+    Ah.copy_(At)
+    del At
+    torch.cuda.empty_cache()
+    f = ctqr.ct_qr_factor(Ah, c.m, c.n)
+    st = f.stats()
+    assert st["out_of_core"] == 0 and st["h2d_bytes"] == c.m * c.n * np.dtype(dt).itemsize
+    tol = 1e-11 if dt == np.float64 else 5e-4
+    assert relerr(ctqr.ct_qr_get_tau(f), TAU[dt]) <= tol
+    Bt = ctqr.colmajor_from_numpy(P["B"].astype(dt))
+    Xt = torch.zeros((P["S"], c.n), dtype=tdt, device="cuda")
+    ctqr.ct_qr_solve(f, Bt, P["S"], Xt)
+    assert relerr(ctqr.numpy_from_colmajor(Xt), RESULTS[dt]) <= (1e-10 if dt == np.float64 else 5e-4)
+    f.destroy()
 
 
 def test_fullsize_fp32_vs_fp64(problem):

@@ -33,6 +33,7 @@ static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
+    L.G = p.sk.G; L.Gm = p.sk.Gm;
     L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
 }
@@ -45,6 +46,7 @@ static GemmLaunch umma_plan_f32(int64_t M, int64_t N, int64_t K, int bn, int sms
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
+    L.G = p.sk.G; L.Gm = p.sk.Gm;
     L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
 }
@@ -80,7 +82,7 @@ cudaError_t upd_presplit_launch(int64_t M, int64_t N, int64_t K, float alpha, co
 static MmaPlan to_plan(const GemmLaunch& L) {
     MmaPlan p{};
     p.sk.tilesM = L.tilesM; p.sk.tilesN = L.tilesN; p.sk.KT = L.KT; p.sk.U = L.U; p.sk.L = L.L; p.sk.partial = L.partial;
-    p.grid = L.grid; p.maxseg = L.slots;
+    p.grid = L.grid; p.maxseg = L.slots; p.sk.G = L.G; p.sk.Gm = L.Gm;
     return p;
 }
 

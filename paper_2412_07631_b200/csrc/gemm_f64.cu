@@ -31,6 +31,7 @@ static GemmLaunch streamk_plan(int64_t M, int64_t N, int64_t K, int bm, int bn, 
     GemmLaunch L{};
     L.kind = 1; L.cfg = cfg; L.grid = p.grid; L.tilesM = p.sk.tilesM; L.tilesN = p.sk.tilesN; L.U = p.sk.U;
     L.L = p.sk.L; L.KT = p.sk.KT; L.partial = p.sk.partial; L.slots = p.maxseg; L.splits = 1;
+    L.G = p.sk.G; L.Gm = p.sk.Gm;
     L.seg = SegInfo{1, p.sk.KT, p.sk.L, bn};
     return L;
 }
@@ -41,17 +42,17 @@ GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
     if (ta) {
         if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0);
         if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_elems, sstride, 6);
-        return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_elems, sstride, 1);
+        return streamk_plan(M, N, K, 128, 64, MmaPolicy<double>::BK, sms, partial, max_elems, sstride, 1);
     }
     if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
     if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_elems, sstride, 7);
-    return streamk_plan(M, N, K, 128, 64, 16, sms, partial, max_elems, sstride, 3);
+    return streamk_plan(M, N, K, 128, 64, MmaPolicy<double>::BK, sms, partial, max_elems, sstride, 3);
 }
 
 static MmaPlan to_plan(const GemmLaunch& L) {
     MmaPlan p{};
     p.sk.tilesM = L.tilesM; p.sk.tilesN = L.tilesN; p.sk.KT = L.KT; p.sk.U = L.U; p.sk.L = L.L; p.sk.partial = L.partial;
-    p.grid = L.grid; p.maxseg = L.slots;
+    p.grid = L.grid; p.maxseg = L.slots; p.sk.G = L.G; p.sk.Gm = L.Gm;
     p.sk.tickets = L.tickets; p.sk.reserve = L.reserve;
     return p;
 }

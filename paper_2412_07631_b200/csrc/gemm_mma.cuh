@@ -144,6 +144,12 @@ struct StreamK {
     int64_t U;                // tilesM * tilesN * KT
     int64_t L;                // units per CTA (a multiple of KT in direct mode)
     int partial;              // 1: every segment writes alpha*acc to its compact partial slot; 0: direct
+    // direct mode, Gm > 0: the tiles are numbered band by band (Gm tile rows per band; inside a band column block by column
+    // block, tile rows fastest) and dealt round-robin (worker w takes the numbers w, w + G, w + 2G, ...), so that the G tiles
+    // in flight are a compact Gm x (G / Gm) patch sharing Gm tiles of A and G / Gm tiles of B in L2.  With contiguous
+    // per-worker ranges (Gm = 0) the workers sit at unrelated tile rows and cycle through all of A; at m = 1e5 the 223 MB
+    // reflector pair no longer fits the L2 (ncu, profiles/r2_c4_f64.md: 349 GB of DRAM reads for 57 GB of C).
+    int G, Gm;
     // SM confinement (see GemmLaunch::reserve): worker indices are drawn from tickets[1] by the CTAs that do
     // not retire on a reserved SM; `workers` = the planned grid
     unsigned* tickets; int reserve; int workers;
@@ -214,10 +220,19 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
     }
 #define s_worker (CONFINED ? s_worker_confined : (int)blockIdx.x)
     const int64_t u0 = (int64_t)s_worker * sk.L;
-    const int64_t u1 = min(sk.U, u0 + sk.L);
+    const bool rr = !sk.partial && sk.Gm > 0;
+    const int64_t u1 = !rr ? min(sk.U, u0 + sk.L)
+                           : u0 + ((sk.tilesM * sk.tilesN - (int64_t)s_worker + sk.G - 1) / sk.G) * sk.KT;
     if (u0 >= u1) return;
     // flat tile index (contiguous per CTA) -> tile coordinates
-    auto decode = [&](int64_t t, int64_t& tm, int64_t& tn) { tn = t / sk.tilesM; tm = t - tn * sk.tilesM; };
+    auto decode = [&](int64_t t, int64_t& tm, int64_t& tn) {
+        if (!rr) { tn = t / sk.tilesM; tm = t - tn * sk.tilesM; return; }
+        const int64_t rank = (t - u0 / sk.KT) * sk.G + (int64_t)s_worker;
+        const int64_t per_band = (int64_t)sk.Gm * sk.tilesN;
+        const int64_t band = rank / per_band, r = rank - band * per_band;
+        const int64_t hb = min((int64_t)sk.Gm, sk.tilesM - band * sk.Gm);
+        tn = r / hb; tm = band * sk.Gm + (r - tn * hb);
+    };
 
     // L2 residency: the reflector block V (operand A) is re-read by every CTA -> keep it; the big
     // matrix C streams through once per launch -> let it go first.  In W = V^T C the streamed
@@ -228,7 +243,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
 
     // ---- producer state: runs STAGES-1 units ahead of the consumer, advanced incrementally ----
     const T* pa[PA]; const T* pb[PB];
-    unsigned abytes = 0, bbytes = 0;      // 5 bits per chunk: valid bytes of the chunk's row/vector (0..16)
+    uint64_t abytes = 0, bbytes = 0;      // 5 bits per chunk: valid bytes of the chunk's row/vector (0..16)
     int64_t ltile = u0 / sk.KT;
     int lkt = (int)(u0 - ltile * sk.KT);
     int64_t ltn, ltm;
@@ -244,13 +259,13 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
                 const int64_t gr = m0 + r;
                 const bool ok = gr < g.M;
                 pa[p] = g.A + (ok ? gr : 0) * g.lda + ck;
-                abytes |= (ok ? 16u : 0u) << (5 * p);
+                abytes |= (uint64_t)(ok ? 16u : 0u) << (5 * p);
             } else {
                 const int kk = c / CPM, cm = (c % CPM) * VEC;
                 const int64_t gm = m0 + cm;
                 const int nv = (int)max((int64_t)0, min((int64_t)VEC, g.M - gm));
                 pa[p] = g.A + (nv ? gm : 0) + (int64_t)kk * g.lda;
-                abytes |= (unsigned)(nv * W) << (5 * p);
+                abytes |= (uint64_t)(nv * W) << (5 * p);
             }
         }
 #pragma unroll
@@ -260,7 +275,7 @@ gemm_mma_kernel(GemmArgs<T> g, StreamK sk) {
             const int64_t gr = n0 + r;
             const bool ok = gr < g.N;
             pb[p] = g.B + (ok ? gr : 0) * g.ldb + ck;
-            bbytes |= (ok ? 16u : 0u) << (5 * p);
+            bbytes |= (uint64_t)(ok ? 16u : 0u) << (5 * p);
         }
     };
     auto issue = [&](int stage) {
@@ -435,6 +450,12 @@ inline MmaPlan mma_plan(int64_t M, int64_t N, int64_t K, int BM, int BN, int BK,
         p.sk.L = tpc * p.sk.KT;
         p.grid = (int)ceil_div(tiles, tpc);
         p.maxseg = 1;
+        // banded round-robin tile order once A (M x K) is too large to stay in L2 beside the streamed C
+        p.sk.G = p.grid;
+        p.sk.Gm = (M * K * 8 > ((int64_t)24 << 20) && p.sk.tilesM >= 32) ? 16 : 0;
+#ifdef CTQR_NO_BAND
+        p.sk.Gm = 0;
+#endif
     }
     return p;
 }

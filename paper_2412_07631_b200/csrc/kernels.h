@@ -42,7 +42,7 @@ struct GemmLaunch {
     int kind;          // 0 = classic kernels (gemm.cuh) with `splits` K slices; 1 = persistent stream-K (gemm_mma.cuh)
     int splits;        // kind 0
     int grid;          // kind 1: CTAs
-    int64_t tilesM, tilesN, U, L; int KT; int partial;   // kind 1: StreamK fields
+    int64_t tilesM, tilesN, U, L; int KT; int partial; int G, Gm;   // kind 1: StreamK fields
     int slots;         // partial output buffers needed (each g.split_stride elements apart)
     int cfg;           // kernel configuration index inside the dtype's dispatcher
     SegInfo seg;       // for the consumer of the partials

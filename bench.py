@@ -792,6 +792,10 @@ def main():
     ap.add_argument("--ooc-config", default="c5", choices=sorted(wl.CONFIGS),
                     help="config of the out-of-core leg (fp32 from pinned host memory, --ooc-budget-gb device bytes)")
     ap.add_argument("--ooc-budget-gb", type=float, default=48.0)
+    ap.add_argument("--only-ooc", action="store_true",
+                    help="run only the out-of-core leg (--ooc-config, --ooc-dtype, --ooc-budget-gb) and print its block: the "
+                         "command the host-link ncu capture of profiles/r2_ooc.md profiles")
+    ap.add_argument("--ooc-dtype", default="f32", choices=["f64", "f32"])
     ap.add_argument("--file-tier-config", default="c3", choices=sorted(wl.CONFIGS),
                     help="config of the cold file-tier leg (matrix written to the temp directory, page cache dropped)")
     ap.add_argument("--file-tier-dtype", default="f64", choices=["f64", "f32"])
@@ -820,6 +824,11 @@ def main():
         torch.distributed.barrier()
     import paper_2412_07631_b200 as ctqr
 
+    if args.only_ooc:
+        if rank == 0:
+            print(json.dumps({"out_of_core": run_out_of_core(wl.CONFIGS[args.ooc_config], args.ooc_dtype,
+                                                              int(args.ooc_budget_gb * 1e9), 8)}), flush=True)
+        return 0
     budget = Budget(args.time_budget)
     warm = args.warmup if args.short_warmup else max(args.warmup, 3)
     extras_on = not args.no_extras and world == 1
@@ -900,7 +909,7 @@ def main():
         if budget.allows(need_s + 30.0):
             torch.cuda.empty_cache()
             try:
-                extras["out_of_core"] = run_out_of_core(oc, "f32", int(args.ooc_budget_gb * 1e9), 64)
+                extras["out_of_core"] = run_out_of_core(oc, args.ooc_dtype, int(args.ooc_budget_gb * 1e9), 64)
             except Exception as e:                                # e.g. the box cannot pin that much host memory
                 extras["out_of_core"] = {"failed": repr(e)[:300]}
             log("out-of-core leg done")

@@ -838,10 +838,19 @@ static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
     return factor_range_single<T>(h, A, lda, c0, c1);
 }
 
+template <typename T> static int band_check(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1);
+template <typename T> static int band_check_enqueue(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1);
+static int band_check_result(H& h);
+
 template <typename T>
 static int factor_incore(H& h, T* A, int64_t lda) {
     cudaEvent_t t0 = new_event(h, true), t1 = new_event(h, true);
     CK(cudaEventRecord(t0, h.sU));
+    // the band promise is verified inside the timed window (factor_ms includes the check), before anything is factored
+    if (h.kl > 0) {
+        if (!h.arrive.empty()) { CKI(wait_columns(h, h.sU, h.n)); h.arrive.clear(); }
+        CKI(band_check<T>(h, A, lda, 0, h.n));
+    }
     CKI(factor_range<T>(h, A, lda, 0, h.n));
     CK(cudaEventRecord(t1, h.sU));
     CK(cudaStreamSynchronize(h.sU));
@@ -899,9 +908,6 @@ static int ensure_stream_bufs(H& h) {
     return 0;
 }
 
-template <typename T> static int band_check(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1);
-template <typename T> static int band_check_enqueue(H& h, const T* A, int64_t lda, int64_t c0, int64_t c1);
-static int band_check_result(H& h);
 
 template <typename T>
 static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
@@ -1145,7 +1151,6 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
             CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n,
                                  cudaMemcpyDeviceToDevice, h.sU));
         }
-        if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda, 0, h.n));
         return factor_incore<T>(h, P_<T>(h.dA), h.lda);
     }
     const size_t budget = o.device_budget_bytes > 0 ? (size_t)o.device_budget_bytes
@@ -1161,7 +1166,6 @@ static int factor_typed(H& h, void* A, int64_t lda, bool a_on_device, const ctqr
         if (h.kl > 0 || n < 4 * chunk) {
             // (the band promise is checked on the whole matrix before anything is factored; small matrices: one copy)
             CK(cudaMemcpy2DAsync(h.dA, h.lda * sizeof(T), A, lda * sizeof(T), m * sizeof(T), n, cudaMemcpyHostToDevice, h.sU));
-            if (h.kl > 0) CKI(band_check<T>(h, P_<T>(h.dA), h.lda, 0, h.n));
             return factor_incore<T>(h, P_<T>(h.dA), h.lda);
         }
         // The host-to-device copy runs in column chunks on the copy stream while the factorisation already works on the
@@ -1289,61 +1293,62 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
 // ------------------------------------------------------------------------------------------
 // solve: a6 (Q^T B) and a7 (blocked TRSM)
 // ------------------------------------------------------------------------------------------
-// Pipelined, TMA-fed small-S Q^T B (solve_small2.cuh; fp64).  Returns -1000 when the configuration does not fit.
-static int apply_qt_small2(H& h, double* C, int64_t ldc, int64_t S) {
+// Pipelined, TMA-fed small-S Q^T B (solve_small2.cuh).  Returns -1000 when the configuration does not fit.
+template <typename T>
+static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
     const int nb = 128;
-    const double* A = P_<double>(h.dA);
+    const T* A = P_<T>(h.dA);
     if (!h.gt_ready) {
         // Mt[j] = T_(j-1) (V_(j-1)^T V_j), once per handle: the Gram block over the rows of panel j as stream-K partial
         // tiles summed in a fixed order, then one 128^3 product
         if (!h.dGt) {
-            CK(dev_alloc(&h.dGt, (size_t)h.P * nb * nb * sizeof(double)));
-            CK(cudaMemsetAsync(h.dGt, 0, (size_t)h.P * nb * nb * sizeof(double), h.sU));
+            CK(dev_alloc(&h.dGt, (size_t)h.P * nb * nb * sizeof(T)));
+            CK(cudaMemsetAsync(h.dGt, 0, (size_t)h.P * nb * nb * sizeof(T), h.sU));
         }
-        if (!h.dMerge) CK(dev_alloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(double)));
-        double* Gs = P_<double>(h.dMerge);
+        if (!h.dMerge) CK(dev_alloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(T)));
+        T* Gs = P_<T>(h.dMerge);
         for (int j = 1; j < h.P; ++j) {
             const int64_t j0 = (int64_t)j * nb;
             const int kw = (int)std::min<int64_t>(nb, h.n - j0);
-            GemmArgs<double> g{};
+            GemmArgs<T> g{};
             g.M = nb; g.N = kw; g.K = row_end(h, j0 + kw) - j0; g.A = A + j0 + (j0 - nb) * h.lda; g.lda = h.lda;
             g.B = A + j0 + j0 * h.lda; g.ldb = h.lda;
-            g.C = P_<double>(h.dWp[0]); g.ldc = nb; g.alpha = 1.0; g.beta = 0.0; g.split_stride = (int64_t)nb * nb;
-            const GemmLaunch LG = gemm_plan<double>(true, nb, kw, g.K, h.gemm_impl, h.sms, true, (int64_t)h.wp_elems[0],
+            g.C = P_<T>(h.dWp[0]); g.ldc = nb; g.alpha = T(1); g.beta = T(0); g.split_stride = (int64_t)nb * nb;
+            const GemmLaunch LG = gemm_plan<T>(true, nb, kw, g.K, h.gemm_impl, h.sms, true, (int64_t)h.wp_elems[0],
                                                     g.split_stride, gemm_aligned(g));
             if (LG.kind != 1) return -1000;
-            CK(gemm_run<double>(true, g, LG, h.gemm_impl, h.sU));
-            CK(partial_sum_launch<double>(P_<double>(h.dWp[0]), LG.seg, nb, kw, Gs, nb, h.sU));
-            GemmArgs<double> g2{};
-            g2.M = nb; g2.N = kw; g2.K = nb; g2.A = P_<double>(h.dT) + (size_t)(j - 1) * nb * nb; g2.lda = nb; g2.B = Gs; g2.ldb = nb;
-            g2.C = P_<double>(h.dGt) + (size_t)j * nb * nb; g2.ldc = nb; g2.alpha = 1.0; g2.beta = 0.0;
-            CK(gemm_direct<double>(false, g2, h.gemm_impl, h.sms, h.sU));
+            CK(gemm_run<T>(true, g, LG, h.gemm_impl, h.sU));
+            CK(partial_sum_launch<T>(P_<T>(h.dWp[0]), LG.seg, nb, kw, Gs, nb, h.sU));
+            GemmArgs<T> g2{};
+            g2.M = nb; g2.N = kw; g2.K = nb; g2.A = P_<T>(h.dT) + (size_t)(j - 1) * nb * nb; g2.lda = nb; g2.B = Gs; g2.ldb = nb;
+            g2.C = P_<T>(h.dGt) + (size_t)j * nb * nb; g2.ldc = nb; g2.alpha = T(1); g2.beta = T(0);
+            CK(gemm_direct<T>(false, g2, h.gemm_impl, h.sms, h.sU));
             h.launches += 3;
         }
         h.gt_ready = true;
     }
-    const int64_t nch = ceil_div(h.m, (int64_t)kQt2Chunk);
+    const int64_t nch = ceil_div(h.m, (int64_t)Qt2Chunk<T>::value);
     const int G = (int)std::min<int64_t>(h.sms, nch);
-    SmallQt2Args a{};
-    a.A = A; a.lda = h.lda; a.m = h.m; a.n = h.n; a.P = h.P; a.Tm = P_<double>(h.dT); a.Mt = P_<double>(h.dGt);
+    SmallQt2Args<T> a{};
+    a.A = A; a.lda = h.lda; a.m = h.m; a.n = h.n; a.P = h.P; a.Tm = P_<T>(h.dT); a.Mt = P_<T>(h.dGt);
     a.B = C; a.ldb = ldc; a.S = (int)S;
     a.part = reinterpret_cast<uint4*>(h.dLLs);
     a.sums = a.part + (size_t)2 * h.sms * nb * kSmallS;
     a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
-    a.rpc = (int)ceil_div(nch, (int64_t)G) * kQt2Chunk;
+    a.rpc = (int)ceil_div(nch, (int64_t)G) * Qt2Chunk<T>::value;
     a.kl = h.kl;
     int ns = 10;
-    while (ns > 3 && qt2_smem_bytes(a.rpc, ns) > 225 * 1024) --ns;
-    const size_t smem = qt2_smem_bytes(a.rpc, ns);
+    while (ns > 3 && qt2_smem_bytes<T>(a.rpc, ns) > 225 * 1024) --ns;
+    const size_t smem = qt2_smem_bytes<T>(a.rpc, ns);
     if (smem > 225 * 1024) return -1000;
     a.nstage = ns;
     CUtensorMap mapV;
-    if (tma::map_2d(&mapV, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, A, h.m, h.n, h.lda, kQt2Chunk, 128, CU_TENSOR_MAP_SWIZZLE_128B) != cudaSuccess)
+    if (tma::map_2d(&mapV, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (int)sizeof(T), A, h.m, h.n, h.lda, Qt2Chunk<T>::value, 128, CU_TENSOR_MAP_SWIZZLE_128B) != cudaSuccess)
         return -1000;
     static SmemAttr attr;
-    CK(ensure_dyn_smem(apply_qt_small2_kernel, smem, attr));
+    CK(ensure_dyn_smem(apply_qt_small2_kernel<T>, smem, attr));
     void* args[] = {(void*)&mapV, (void*)&a};
-    CK(cudaLaunchCooperativeKernel((void*)apply_qt_small2_kernel, dim3(G), dim3(kQt2Threads), args, smem, h.sU));
+    CK(cudaLaunchCooperativeKernel((void*)apply_qt_small2_kernel<T>, dim3(G), dim3(kQt2Threads), args, smem, h.sU));
     h.launches += 1;
 #ifdef CTQR_SMALL_PROFILE
     {
@@ -1378,11 +1383,9 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         return 0;
     }
     const T* A = P_<T>(h.dA);
-    if constexpr (sizeof(T) == 8) {
-        if (S <= kSmallS && h.dLLs && h.gemm_impl == 0 && h.nb == 128 && (h.lda % 2) == 0 && ((uintptr_t)A % 16) == 0 && h.P >= 2) {
-            int rc2 = apply_qt_small2(h, C, ldc, S);
-            if (rc2 != -1000) { h.st.apply_qt_path = 2; return rc2; }   // -1000: does not fit (shared memory); fall through
-        }
+    if (S <= kSmallS && h.dLLs && h.gemm_impl == 0 && h.nb == 128 && (h.lda * sizeof(T)) % 16 == 0 && ((uintptr_t)A % 16) == 0 && h.P >= 2) {
+        int rc2 = apply_qt_small2<T>(h, C, ldc, S);
+        if (rc2 != -1000) { h.st.apply_qt_path = 2; return rc2; }   // -1000: does not fit (shared memory); fall through
     }
     if (S <= kSmallS && h.dLLs && h.gemm_impl == 0) {
         // memory-bound regime: one cooperative kernel for all panels (solve_small.cuh)

@@ -31,46 +31,50 @@
 
 namespace ctqr {
 
-constexpr int kQt2Chunk = 16;                    // fp64 rows per TMA box: 128 bytes, the swizzle span
-constexpr int kQt2StageBytes = kQt2Chunk * 128 * 8;
+template <typename T> struct Qt2Chunk { static constexpr int value = 128 / (int)sizeof(T); };   // rows per TMA box: 128 bytes, the swizzle span
+constexpr int kQt2StageBytes = 128 * 128;        // one box: (16 fp64 | 32 fp32) rows x 128 columns
 constexpr int kQt2Warps = 16;                    // compute warps; one more warp issues the TMA loads
 constexpr int kQt2Threads = (kQt2Warps + 1) * 32;
 
+template <typename T>
 struct SmallQt2Args {
-    const double* A; int64_t lda; int64_t m, n; int P;
-    const double* Tm;               // P blocks of 128 x 128 (ld 128)
-    const double* Mt;               // P blocks of 128 x 128 (ld 128): Mt[j] = T_(j-1) (V_(j-1)^T V_j), j >= 1:
+    const T* A; int64_t lda; int64_t m, n; int P;
+    const T* Tm;                    // P blocks of 128 x 128 (ld 128)
+    const T* Mt;               // P blocks of 128 x 128 (ld 128): Mt[j] = T_(j-1) (V_(j-1)^T V_j), j >= 1:
                                     // W_j[c, s] = Y_j[c, s] - sum_q Mt[j][q + c * 128] W_(j-1)[q, s]
-    double* B; int64_t ldb; int S;
+    T* B; int64_t ldb; int S;
     uint4* part;                    // [2][G][128 * kSmallS] LL slots: per-CTA partial Y
     uint4* sums;                    // [2][128 * kSmallS] LL slots: reduced, corrected W
     unsigned seq_base;              // step numbers seq_base + 1 .. seq_base + P are used by this launch
-    int rpc;                        // local rows per CTA (multiple of kQt2Chunk)
+    int rpc;                        // local rows per CTA (multiple of the box height)
     int64_t kl;                     // band promise (0 = dense)
     int nstage;                     // TMA ring stages
 };
 
+template <typename T>
 inline size_t qt2_smem_bytes(int rpc, int nstage) {
     return 1024 + (size_t)nstage * kQt2StageBytes + 16 * (size_t)nstage + 64 +
-           ((size_t)3 * 128 * SmallLd<double>::W + (size_t)kSmallS * (rpc + 4)) * sizeof(double);
+           ((size_t)3 * 128 * SmallLd<T>::W + (size_t)kSmallS * (rpc + 4)) * sizeof(T);
 }
 
 // The ring carries ONE sequence of boxes, identical for the producer and for every consumer:
 //   A(0), A(1), then for k = 0 .. P-1:  U(k), A(k+2)        (A(j) / U(j) = the CTA's row chunks of panel j, top down)
 // A boxes feed the partial products Y_j (every compute warp reads every box: warp w owns columns 8w .. 8w+7);
 // U boxes feed the row update of panel j (box i of the segment belongs to compute warp i mod 16 alone).
+template <typename T>
 __global__ void __launch_bounds__(kQt2Threads, 1)
-apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p) {
+apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args<T> p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int NB = 128, SM = kSmallS, NW = kQt2Warps, NT = NW * 32, CH = kQt2Chunk, LDW = SmallLd<double>::W;
+    constexpr int NB = 128, SM = kSmallS, NW = kQt2Warps, NT = NW * 32, CH = Qt2Chunk<T>::value, LDW = SmallLd<T>::W;
+    constexpr bool F64 = sizeof(T) == 8;                    // fp64: DMMA.8x8x4 from the swizzled boxes; fp32: FFMA
     const unsigned sbase = (tma::smem_addr(smem_raw) + 1023u) & ~1023u;
     unsigned char* ring = smem_raw + (sbase - tma::smem_addr(smem_raw));
     const int NS = p.nstage;
     const unsigned bars = sbase + (unsigned)NS * kQt2StageBytes;            // full[NS], empty[NS]
-    double* Wg = reinterpret_cast<double*>(ring + (size_t)NS * kQt2StageBytes + 16 * (size_t)NS + 64);   // gathered W_k
-    double* Yp = Wg + NB * LDW;                             // this CTA's partial Y
-    double* W2 = Yp + NB * LDW;                             // T_k^T W_k
-    double* Bs = W2 + NB * LDW;                             // [SM][ldbs] own rows of B, transposed
+    T* Wg = reinterpret_cast<T*>(ring + (size_t)NS * kQt2StageBytes + 16 * (size_t)NS + 64);   // gathered W_k
+    T* Yp = Wg + NB * LDW;                                  // this CTA's partial Y
+    T* W2 = Yp + NB * LDW;                                  // T_k^T W_k
+    T* Bs = W2 + NB * LDW;                                  // [SM][ldbs] own rows of B, transposed
     const int ldbs = p.rpc + 4;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = blockIdx.x, G = gridDim.x, S = p.S;
@@ -98,7 +102,7 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
     for (int i = tid; i < SM * p.rpc; i += kQt2Threads) {
         const int s = i / p.rpc, lr = i - s * p.rpc;
         const int64_t row = row_of(lr);
-        Bs[s * ldbs + lr] = (s < S && lr < nl && row < p.m) ? p.B[row + (int64_t)s * p.ldb] : 0.0;
+        Bs[s * ldbs + lr] = (s < S && lr < nl && row < p.m) ? p.B[row + (int64_t)s * p.ldb] : T(0);
     }
     __syncthreads();
 
@@ -133,25 +137,57 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
     // partial Y_j over the own rows from the ring: warp w owns columns 8w .. 8w+7; result to Yp, then published
     auto pass_a = [&](int j) {
         int la, le; range_of(j, la, le);
-        const int c = warp * 8 + (lane >> 2);
-        const double* bs = Bs + (lane >> 2) * ldbs + (lane & 3);
-        double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int lr = la; lr < le; lr += CH, ++ccount) {
-            const int st = (int)(ccount % (unsigned)NS);
-            tma::mbar_wait(full(st), (ccount / (unsigned)NS) & 1u);
-            const unsigned char* vs = ring + (size_t)st * kQt2StageBytes + c * 128;
+        if constexpr (F64) {
+            const int c = warp * 8 + (lane >> 2);
+            const double* bs = Bs + (lane >> 2) * ldbs + (lane & 3);
+            double c0[4] = {0.0, 0.0, 0.0, 0.0}, c1[4] = {0.0, 0.0, 0.0, 0.0};
+            for (int lr = la; lr < le; lr += CH, ++ccount) {
+                const int st = (int)(ccount % (unsigned)NS);
+                tma::mbar_wait(full(st), (ccount / (unsigned)NS) & 1u);
+                const unsigned char* vs = ring + (size_t)st * kQt2StageBytes + c * 128;
 #pragma unroll
-            for (int h = 0; h < 4; ++h) {
-                const int r = 4 * h + (lane & 3);
-                const double a = *reinterpret_cast<const double*>(vs + ((((r >> 1) ^ (c & 7)) << 4) | ((r & 1) << 3)));
-                dmma884(c0[h], c1[h], a, bs[lr + 4 * h]);
+                for (int h = 0; h < 4; ++h) {
+                    const int r = 4 * h + (lane & 3);
+                    const double a = *reinterpret_cast<const double*>(vs + ((((r >> 1) ^ (c & 7)) << 4) | ((r & 1) << 3)));
+                    dmma884(c0[h], c1[h], a, bs[lr + 4 * h]);
+                }
+                __syncwarp();
+                if (lane == 0) tma::mbar_arrive(empty(st));
             }
-            __syncwarp();
-            if (lane == 0) tma::mbar_arrive(empty(st));
+            sync_compute();                                 // the previous publication has finished reading Yp
+            Yp[c * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
+            Yp[c * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
+        } else {
+            // fp32: lane = row of the box (32 rows), the warp's 8 columns x 8 right-hand sides in registers; the sums over the
+            // rows are formed once per panel by two transpose-reductions (32 values each)
+            float acc[2][4 * SM];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int u = 0; u < 4 * SM; ++u) acc[h][u] = 0.f;
+            for (int lr = la; lr < le; lr += CH, ++ccount) {
+                const int st = (int)(ccount % (unsigned)NS);
+                tma::mbar_wait(full(st), (ccount / (unsigned)NS) & 1u);
+                const unsigned char* vs = ring + (size_t)st * kQt2StageBytes;
+                float b[SM];
+#pragma unroll
+                for (int q = 0; q < SM; ++q) b[q] = Bs[q * ldbs + lr + lane];
+#pragma unroll
+                for (int cc = 0; cc < 8; ++cc) {
+                    const int c = warp * 8 + cc;
+                    const float v = *reinterpret_cast<const float*>(vs + c * 128 + ((((lane >> 2) ^ (c & 7)) << 4) | ((lane & 3) << 2)));
+#pragma unroll
+                    for (int q = 0; q < SM; ++q) acc[cc >> 2][(cc & 3) * SM + q] = fmaf(v, b[q], acc[cc >> 2][(cc & 3) * SM + q]);
+                }
+                __syncwarp();
+                if (lane == 0) tma::mbar_arrive(empty(st));
+            }
+            warp_transpose_reduce<float, 4 * SM>(acc[0], lane);   // lane l: total of value l = (column l / SM, rhs l % SM)
+            warp_transpose_reduce<float, 4 * SM>(acc[1], lane);
+            sync_compute();
+            Yp[(warp * 8 + lane / SM) * LDW + (lane % SM)] = acc[0][0];
+            Yp[(warp * 8 + 4 + lane / SM) * LDW + (lane % SM)] = acc[1][0];
         }
-        sync_compute();                                     // the previous publication has finished reading Yp
-        Yp[c * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
-        Yp[c * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
         sync_compute();
         const unsigned seq = p.seq_base + (unsigned)j + 1u;
         uint4* mine = p.part + ((size_t)(j & 1) * G + g) * (NB * SM);
@@ -167,18 +203,39 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
             const int st = (int)(ccount % (unsigned)NS);
             tma::mbar_wait(full(st), (ccount / (unsigned)NS) & 1u);
             const unsigned char* vs = ring + (size_t)st * kQt2StageBytes;
-            const double* wb = W2 + (lane & 3) * LDW + (lane >> 2);
-            const int r = 8 * (warp & 1) + (lane >> 2);
-            double d0[4] = {0.0, 0.0, 0.0, 0.0}, d1[4] = {0.0, 0.0, 0.0, 0.0};
+            if constexpr (F64) {
+                const double* wb = W2 + (lane & 3) * LDW + (lane >> 2);
+                const int r = 8 * (warp & 1) + (lane >> 2);
+                double d0[4] = {0.0, 0.0, 0.0, 0.0}, d1[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll 8
-            for (int t = 0; t < NB / 4; ++t) {
-                const int col = 4 * t + (lane & 3);
-                const double a = *reinterpret_cast<const double*>(vs + col * 128 + ((((r >> 1) ^ (col & 7)) << 4) | ((r & 1) << 3)));
-                dmma884(d0[t & 3], d1[t & 3], a, wb[4 * t * LDW]);
+                for (int t = 0; t < NB / 4; ++t) {
+                    const int col = 4 * t + (lane & 3);
+                    const double a = *reinterpret_cast<const double*>(vs + col * 128 + ((((r >> 1) ^ (col & 7)) << 4) | ((r & 1) << 3)));
+                    dmma884(d0[t & 3], d1[t & 3], a, wb[4 * t * LDW]);
+                }
+                const int s0 = 2 * (lane & 3), l = lr + r;
+                Bs[s0 * ldbs + l] -= (d0[0] + d0[1]) + (d0[2] + d0[3]);
+                Bs[(s0 + 1) * ldbs + l] -= (d1[0] + d1[1]) + (d1[2] + d1[3]);
+            } else {
+                // fp32: the warp takes 16 of the 32 rows; lane = (row, column half), the halves combined by one shuffle
+                const int r = 16 * (warp & 1) + (lane & 15), ch = lane >> 4;
+                float d[SM];
+#pragma unroll
+                for (int q = 0; q < SM; ++q) d[q] = 0.f;
+#pragma unroll 8
+                for (int cc = 0; cc < NB / 2; ++cc) {
+                    const int col = ch * (NB / 2) + ((cc + 4 * ch) & (NB / 2 - 1));   // (the halves hit disjoint banks)
+                    const float v = *reinterpret_cast<const float*>(vs + col * 128 + ((((r >> 2) ^ (col & 7)) << 4) | ((r & 3) << 2)));
+                    const float4 w0 = *reinterpret_cast<const float4*>(W2 + col * LDW), w1 = *reinterpret_cast<const float4*>(W2 + col * LDW + 4);
+                    d[0] = fmaf(v, w0.x, d[0]); d[1] = fmaf(v, w0.y, d[1]); d[2] = fmaf(v, w0.z, d[2]); d[3] = fmaf(v, w0.w, d[3]);
+                    d[4] = fmaf(v, w1.x, d[4]); d[5] = fmaf(v, w1.y, d[5]); d[6] = fmaf(v, w1.z, d[6]); d[7] = fmaf(v, w1.w, d[7]);
+                }
+#pragma unroll
+                for (int q = 0; q < SM; ++q) d[q] += shfl_xor(d[q], 16);
+                if (ch == 0)
+#pragma unroll
+                    for (int q = 0; q < SM; ++q) Bs[q * ldbs + lr + r] -= d[q];
             }
-            const int s0 = 2 * (lane & 3), l = lr + r;
-            Bs[s0 * ldbs + l] -= (d0[0] + d0[1]) + (d0[2] + d0[3]);
-            Bs[(s0 + 1) * ldbs + l] -= (d1[0] + d1[1]) + (d1[2] + d1[3]);
             __syncwarp();
             if (lane == 0) tma::mbar_arrive_n(empty(st), (unsigned)(NW / 2));
         }
@@ -187,31 +244,31 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
     // holds the gathered W_(j-1) when this runs), publish W_j.  One element per warp (128 * 8 elements over G CTAs x 16 warps);
     // the loads are issued by reduce_issue and consumed by reduce_finish so that the row update runs in between.
     constexpr int MAXB = 5;                                 // partial slots per lane: G <= 160 CTAs
-    auto reduce_issue_e = [&](int j, int e, double (&gv)[4], uint4 (&r)[MAXB]) {
+    auto reduce_issue_e = [&](int j, int e, T (&gv)[4], uint4 (&r)[MAXB]) {
         const uint4* all = p.part + (size_t)(j & 1) * G * (NB * SM);
-        const double* gt = p.Mt + (size_t)j * NB * NB + (size_t)(e / SM) * NB;
+        const T* gt = p.Mt + (size_t)j * NB * NB + (size_t)(e / SM) * NB;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) gv[u] = j >= 1 ? __ldg(gt + lane + 32 * u) : 0.0;
+        for (int u = 0; u < 4; ++u) gv[u] = j >= 1 ? __ldg(gt + lane + 32 * u) : T(0);
 #pragma unroll
         for (int u = 0; u < MAXB; ++u) {
             const int b = lane + u * 32;
             if (b < G) r[u] = ll_load(all + (size_t)b * (NB * SM) + e);
         }
     };
-    auto reduce_finish_e = [&](int j, int e, const double (&gv)[4], uint4 (&r)[MAXB]) {
+    auto reduce_finish_e = [&](int j, int e, const T (&gv)[4], uint4 (&r)[MAXB]) {
         const unsigned seq = p.seq_base + (unsigned)j + 1u;
         const uint4* all = p.part + (size_t)(j & 1) * G * (NB * SM);
         const int s = e % SM;
-        double t = 0.0;
+        T t = T(0);
 #pragma unroll
         for (int u = 0; u < MAXB; ++u) {
             const int b = lane + u * 32;
             if (b < G) {
                 while (r[u].y != seq || r[u].w != seq) r[u] = ll_load(all + (size_t)b * (NB * SM) + e);
-                t += ll_value<double>(r[u]);
+                t += ll_value<T>(r[u]);
             }
         }
-        double corr = 0.0;
+        T corr = T(0);
         if (j >= 1) {                                       // (Wg is not yet written when W_0 is formed)
 #pragma unroll
             for (int u = 0; u < 4; ++u) corr = fma(gv[u], Wg[(lane + 32 * u) * LDW + s], corr);
@@ -223,11 +280,11 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
     };
     // the first element of a warp is split into issue / finish (the gather runs in between); a grid of fewer than 64 CTAs
     // leaves more than one element per warp, the others follow back to back
-    auto reduce_issue = [&](int j, double (&gv)[4], uint4 (&r)[MAXB]) {
+    auto reduce_issue = [&](int j, T (&gv)[4], uint4 (&r)[MAXB]) {
         const int e = g + warp * G;
         if (e < NB * SM) reduce_issue_e(j, e, gv, r);
     };
-    auto reduce_finish = [&](int j, double (&gv)[4], uint4 (&r)[MAXB]) {
+    auto reduce_finish = [&](int j, T (&gv)[4], uint4 (&r)[MAXB]) {
         int e = g + warp * G;
         if (e >= NB * SM) return;
         reduce_finish_e(j, e, gv, r);
@@ -241,7 +298,7 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
     pass_a(0);
     if (p.P > 1) pass_a(1);
     {
-        double gv[4]; uint4 rr[MAXB];
+        T gv[4]; uint4 rr[MAXB];
         reduce_issue(0, gv, rr);
         reduce_finish(0, gv, rr);
     }
@@ -254,7 +311,7 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
         CTQR_PH(0)
         // ---- element owners of W_(k+1): the loads of the partials (published one iteration ago) and of their row of
         //      M_(k+1) are issued before the gather spins, and consumed right after it ----
-        double gv[4]; uint4 rr[MAXB];
+        T gv[4]; uint4 rr[MAXB];
         if (k + 1 < p.P) reduce_issue(k + 1, gv, rr);
         // ---- gather W_k (reduced and corrected by its element owners during the previous iteration) ----
         {
@@ -266,7 +323,7 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
             for (int u = 0; u < NB * SM / NT; ++u) {
                 const int e = tid + u * NT;
                 while (r[u].y != seq || r[u].w != seq) r[u] = ll_load(sl + e);
-                Wg[(e / SM) * LDW + (e % SM)] = ll_value<double>(r[u]);
+                Wg[(e / SM) * LDW + (e % SM)] = ll_value<T>(r[u]);
             }
         }
         sync_compute();
@@ -274,8 +331,9 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
         // ---- W_(k+1) = sum of the partials - M_(k+1) W_k, published: the only step on the chain through the grid ----
         if (k + 1 < p.P) reduce_finish(k + 1, gv, rr);
         CTQR_PH(2)
-        // ---- W2 = T_k^T W_k, T_k as DMMA fragments straight from L2 (upper triangular: q <= r) ----
-        {
+        // ---- W2 = T_k^T W_k, T_k straight from L2 (upper triangular: q <= r) ----
+        if constexpr (F64) {
+            // DMMA fragments, every load of the warp in flight at once
             const int tr_row = warp * 8 + (lane >> 2);
             const double* tr = p.Tm + (size_t)k * NB * NB + (size_t)tr_row * NB + (lane & 3);
             double ta[NB / 4];
@@ -291,6 +349,39 @@ apply_qt_small2_kernel(const __grid_constant__ CUtensorMap mapV, SmallQt2Args p)
                 if (t < 2 * warp + 2) dmma884(c0[t & 3], c1[t & 3], ta[t], wq[4 * t * LDW]);
             W2[tr_row * LDW + 2 * (lane & 3)] = (c0[0] + c0[1]) + (c0[2] + c0[3]);
             W2[tr_row * LDW + 2 * (lane & 3) + 1] = (c1[0] + c1[1]) + (c1[2] + c1[3]);
+        } else {
+            // fp32: warp w forms rows 8w .. 8w+7 of W2; lanes over q (coalesced reads of column r of T), the sums over q by
+            // two transpose-reductions
+            const float* tk = p.Tm + (size_t)k * NB * NB;
+            float tv[8][4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int r = warp * 8 + i;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int q = lane + 32 * u;
+                    tv[i][u] = (q <= r && r < kw) ? __ldg(tk + q + (size_t)r * NB) : 0.f;
+                }
+            }
+            float acc[2][4 * SM];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int x = 0; x < 4 * SM; ++x) acc[h][x] = 0.f;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int q = lane + 32 * u;
+                const float4 w0 = *reinterpret_cast<const float4*>(Wg + q * LDW), w1 = *reinterpret_cast<const float4*>(Wg + q * LDW + 4);
+                const float wv[SM] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int q2 = 0; q2 < SM; ++q2) acc[i >> 2][(i & 3) * SM + q2] = fmaf(tv[i][u], wv[q2], acc[i >> 2][(i & 3) * SM + q2]);
+            }
+            warp_transpose_reduce<float, 4 * SM>(acc[0], lane);
+            warp_transpose_reduce<float, 4 * SM>(acc[1], lane);
+            W2[(warp * 8 + lane / SM) * LDW + (lane % SM)] = acc[0][0];
+            W2[(warp * 8 + 4 + lane / SM) * LDW + (lane % SM)] = acc[1][0];
         }
         sync_compute();
         CTQR_PH(3)

@@ -101,6 +101,47 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+class PcieSampler:
+    """Host-link throughput from the device's own PCIe counters (NVML nvmlDeviceGetPcieThroughput, a 20 ms hardware
+    window per call), sampled from a thread while a leg runs.  ncu's per-kernel pcie__* counters cannot see this traffic:
+    the out-of-core copies are copy-engine operations between (under ncu: serialised) kernels, see profiles/r2_ooc.md."""
+
+    def __init__(self, index: int = 0):
+        self.index, self.rx, self.tx, self.run, self.thr = index, [], [], False, None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.run = True
+            self.thr = threading.Thread(target=self._loop, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.thr = None
+
+    def _loop(self):
+        while self.run:
+            try:
+                self.rx.append(self.nv.nvmlDeviceGetPcieThroughput(self.h, self.nv.NVML_PCIE_UTIL_RX_BYTES))   # KB/s
+                self.tx.append(self.nv.nvmlDeviceGetPcieThroughput(self.h, self.nv.NVML_PCIE_UTIL_TX_BYTES))
+            except Exception:
+                break
+
+    def stop(self) -> dict:
+        if not self.thr:
+            return {"unavailable": "pynvml"}
+        self.run = False
+        self.thr.join(timeout=2)
+        if not self.rx:
+            return {"unavailable": "no samples"}
+        g = lambda v: [x * 1e3 / 1e9 for x in v]
+        rx, tx = g(self.rx), g(self.tx)
+        return {"source": "NVML PCIe counters, 20 ms windows", "samples": len(rx),
+                "rx_gbs_mean": sum(rx) / len(rx), "rx_gbs_peak": max(rx),
+                "tx_gbs_mean": sum(tx) / len(tx), "tx_gbs_peak": max(tx)}
+
+
 def load_peaks() -> dict:
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -385,6 +426,35 @@ def run_e2e(cfg, dtype: str, Ah, B: np.ndarray, S: int, steps: int, flops: float
 SWEEP_S = (1, 8, 64, 256, 512, 1024, 2048)       # PAPER.md:L89, Fig. 1 (L117-130): up to 2048 simultaneous slices
 
 
+def run_solve_only(cfg, dtype: str) -> list:
+    """One factorisation, then the batched solve at S = 8, 1, 64 on random right-hand sides (timing only).
+    factor_read_gbs = the factor's m*n*w bytes / batch time: the algorithmic HBM traffic of the small-S solve."""
+    import torch
+    import paper_2412_07631_b200 as ctqr
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    w = 8 if dtype == "f64" else 4
+    At, _ = wl.dense_augmented_device(cfg, tdt)
+    f = ctqr.ct_qr_factor(At, cfg.m, cfg.n, in_place=True)
+    g = torch.Generator(device="cuda"); g.manual_seed(7)
+    out = []
+    for S in (8, 1, 64):
+        Bt = torch.randn((S, cfg.m), device="cuda", dtype=tdt, generator=g)
+        Xt = torch.zeros((S, cfg.n), device="cuda", dtype=tdt)
+        ctqr.ct_qr_solve(f, Bt, S, Xt)
+        best = None
+        for _ in range(3):
+            ctqr.ct_qr_solve(f, Bt, S, Xt)
+            st = f.stats()
+            if best is None or st["solve_ms"] < best["solve_ms"]:
+                best = st
+        out.append({"S": S, "ms": best["solve_ms"], "apply_qt_ms": best["apply_qt_ms"], "trsm_ms": best["trsm_ms"],
+                    "apply_qt_path": best["apply_qt_path"], "launches": best["kernel_launches"],
+                    "factor_read_gbs": cfg.m * cfg.n * w / (best["solve_ms"] * 1e-3) / 1e9,
+                    "slices_per_s": S / (best["solve_ms"] * 1e-3)})
+    f.destroy()
+    return out
+
+
 def run_resident_extras(cfg, dtype: str, f, At, Aw, B: np.ndarray, budget: Budget, incore_ms: float, structured: bool) -> dict:
     """Legs that reuse the resident factor of the last timed step (rank 0, N = 1):
     solve S-sweep (PAPER.md Fig. 1, L117-130: throughput rises with the number of slices solved at once;
@@ -584,14 +654,18 @@ def run_out_of_core(cfg, dtype: str, budget_bytes: int, S: int, structured: bool
     log("out-of-core leg: %s %s built in pinned host memory (%.1f GB) in %.1f s" % (cfg.name, dtype, m * n * w / 1e9, t_build))
     _, B = wl.make_slices(cfg, S=S, coo=coo, lam=lam)
     torch.cuda.synchronize()
+    pc = PcieSampler(torch.cuda.current_device()); pc.start()
     t0 = time.perf_counter()
     f = ctqr.ct_qr_factor(Ah, m, n, device_budget_bytes=budget_bytes, lower_bandwidth=(m - n) if structured else 0)
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
+    pcie_factor = pc.stop()
     st = f.stats()
     Bh = torch.from_numpy(np.ascontiguousarray(B.astype(npdt).T)).pin_memory()
     Xh = torch.zeros((S, n), dtype=tdt).pin_memory()
+    pc = PcieSampler(torch.cuda.current_device()); pc.start()
     ctqr.ct_qr_solve(f, Bh, S, Xh)
+    pcie_solve = pc.stop()
     st2 = f.stats()
     # optimality residual of the streamed solve, from the sparse rows in fp64 (no device arithmetic)
     import scipy.sparse as sp
@@ -609,7 +683,7 @@ def run_out_of_core(cfg, dtype: str, budget_bytes: int, S: int, structured: bool
         "device_budget_bytes": budget_bytes, "n_superpanels": st["n_superpanels"], "factor_ms": st["factor_ms"],
         "wall_s": wall, "tflops": fl / (st["factor_ms"] * 1e-3) / 1e12, "lower_bandwidth": st["lower_bandwidth"],
         "h2d_bytes": st["h2d_bytes"], "d2h_bytes": st["d2h_bytes"],
-        "host_link_gbs_avg": link,
+        "host_link_gbs_avg": link, "pcie_counters_factor": pcie_factor, "pcie_counters_solve": pcie_solve,
         "algorithmic_link_bytes": m * n * w * (st["n_superpanels"] + 3) / 2.0,
         "copy_exposed_ms": st.get("copy_exposed_ms"), "copy_busy_ms": st.get("copy_busy_ms"),
         "solve_streamed": {"S": S, "ms": st2["solve_ms"], "slices_per_s": S / (st2["solve_ms"] * 1e-3),
@@ -796,6 +870,9 @@ def main():
                     help="run only the out-of-core leg (--ooc-config, --ooc-dtype, --ooc-budget-gb) and print its block: the "
                          "command the host-link ncu capture of profiles/r2_ooc.md profiles")
     ap.add_argument("--ooc-dtype", default="f32", choices=["f64", "f32"])
+    ap.add_argument("--only-solve", action="store_true",
+                    help="one factorisation of --config in --dtype, then the solve at S = 8, 1 and 64 (three timed batches each): the "
+                         "command the solve captures of profiles/r2_solve.md profile")
     ap.add_argument("--file-tier-config", default="c3", choices=sorted(wl.CONFIGS),
                     help="config of the cold file-tier leg (matrix written to the temp directory, page cache dropped)")
     ap.add_argument("--file-tier-dtype", default="f64", choices=["f64", "f32"])
@@ -828,6 +905,10 @@ def main():
         if rank == 0:
             print(json.dumps({"out_of_core": run_out_of_core(wl.CONFIGS[args.ooc_config], args.ooc_dtype,
                                                               int(args.ooc_budget_gb * 1e9), 8)}), flush=True)
+        return 0
+    if args.only_solve:
+        if rank == 0:
+            print(json.dumps({"solve_only": run_solve_only(cfg, args.dtype)}), flush=True)
         return 0
     budget = Budget(args.time_budget)
     warm = args.warmup if args.short_warmup else max(args.warmup, 3)

@@ -233,6 +233,33 @@ int ct_qr_peak_probe(int kind, int iters, double* tflops, double* ms);
  * resident warps the pipe needs to reach its peak (ct_qr_peak_probe = 256 threads x 8 CTAs). */
 int ct_qr_peak_probe_cfg(int kind, int iters, int threads, int ctas_per_sm, double* tflops, double* ms);
 
+/* ---- allocation-free entry point -----------------------------------------------------------------------------
+ * ct_qr_vtc_noalloc: W <- V^T C, the split-K product that opens the block-reflector application
+ * C <- (I - V T V^T)^T C (C = Q^T B is applied without building Q, "dormqr"; SURVEY.md 8a rows
+ * a3 / a6), for callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it.  Same result as ct_qr_gemm(trans_a = 1, M, N, K, 1, V, ldv, C, ldc, 0, W, ldw, dtype, 0) up to
+ * the summation order.
+ *   V: K x M, column-major, leading dimension ldv >= max(K, 1)   (device pointer, read-only)
+ *   C: K x N, column-major, leading dimension ldc >= max(K, 1)   (device pointer, read-only)
+ *   W: M x N, column-major, leading dimension ldw >= M           (device pointer, overwritten; must not alias V, C)
+ *   stream: a cudaStream_t passed as void*; NULL = the default stream.  The call enqueues two kernels on it and
+ *           returns without synchronising; the caller owns all three buffers and keeps them alive until they ran.
+ * The partial tiles of the split live in a file-scope device array of CTQR_NOALLOC_SCRATCH_BYTES that every GPU
+ * which loads the library holds until the process exits; the call never calls cudaMalloc, cudaFree or an allocating
+ * library routine (the first call per device fetches the array's address with cudaGetSymbolAddress and loads the
+ * kernels: make one call before starting a graph capture).
+ * Limit: ceil(M/64) * ceil(N/64) * 64 * 64 * sizeof(element) <= CTQR_NOALLOC_SCRATCH_BYTES, i.e. at most 512 output
+ * tiles in fp64 and 1024 in fp32 (e.g. M = 128, N <= 16 384 in fp64); K is unlimited.  Larger sizes are refused with
+ * CTQR_ERR_NOMEM and a message naming the limit; nothing is enqueued.
+ * All calls share the one array: calls whose kernels may overlap on the GPU (different streams without a
+ * dependency, or several host threads) RACE on it; calls on one stream are ordered.  The array keeps the last call's
+ * tiles, and nothing in it needs to start at zero: every slot a call reads it has written in full first.
+ * Deterministic (fixed split, sums in split order).  Errors: -i for the i-th argument (1-based; host pointers are
+ * refused as -4), CTQR_ERR_NOMEM beyond the limit, CTQR_ERR_CUDA. */
+#define CTQR_NOALLOC_SCRATCH_BYTES (16u << 20)
+int ct_qr_vtc_noalloc(int64_t M, int64_t N, int64_t K, const void* V, int64_t ldv, const void* C, int64_t ldc,
+                      void* W, int64_t ldw, ctqr_dtype_t dtype, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

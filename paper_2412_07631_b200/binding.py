@@ -97,6 +97,7 @@ EXPORTS = {
     "ct_qr_version": ([], _I),
     "ct_qr_gemm": ([_I, _I64, _I64, _I64, ctypes.c_double, _P, _I64, _P, _I64, ctypes.c_double,
                     _P, _I64, _I, _I], _I),
+    "ct_qr_vtc_noalloc": ([_I64, _I64, _I64, _P, _I64, _P, _I64, _P, _I64, _I, _P], _I),
     "ct_qr_peak_probe": ([_I, _I, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)], _I),
     "ct_qr_peak_probe_cfg": ([_I, _I, _I, _I, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)], _I),
 }
@@ -321,6 +322,15 @@ def ct_qr_gemm(trans_a: bool, M: int, N: int, K: int, alpha: float, A, lda: int,
     _check(lib().ct_qr_gemm(int(trans_a), M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
                             _code_of(C), impl))
     return C
+
+
+def ct_qr_vtc_noalloc(M: int, N: int, K: int, V, ldv: int, C, ldc: int, W, ldw: int, stream=None):
+    """W <- V^T C without any allocation (device tensors, column-major; scratch is a fixed device array of the
+    library, see include/ctqr.h for the size limit and the sharing rule).  ``stream``: a torch.cuda.Stream or None
+    (the default stream).  Asynchronous."""
+    st = ctypes.c_void_p(stream.cuda_stream) if stream is not None else None
+    _check(lib().ct_qr_vtc_noalloc(M, N, K, _ptr(V), ldv, _ptr(C), ldc, _ptr(W), ldw, _code_of(W), st))
+    return W
 
 
 def ct_qr_peak_probe(kind: int, iters: int = 4096, threads: int = 256, ctas_per_sm: int = 8):

@@ -17,7 +17,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libctqr.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
-UNITS = ["ctqr.cu", "gemm_f64.cu", "gemm_f32.cu", "panel_f64.cu", "panel_f32.cu", "small.cu", "refine.cu"]
+UNITS = ["ctqr.cu", "gemm_f64.cu", "gemm_f32.cu", "panel_f64.cu", "panel_f32.cu", "small.cu", "refine.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 # extra compile flags for one-off builds (e.g. -DCTQR_SMALL_PROFILE: per-phase timers in the small-S solve kernels)

@@ -122,7 +122,8 @@ typedef struct {
     double diag_block_cond;    /* max over diagonal blocks of max|R_jj| / min|R_jj| (set by the first solve; 0 before) */
     int32_t trsm_exact;        /* 0: inverted diagonal blocks; 1: back-substitution by option; 2: forced by the guard */
     int32_t apply_qt_path;     /* last Q^T B: 0 = one larfb per panel; 1 = fused small-S kernel (one cooperative launch);
-                                  2 = pipelined, TMA-fed small-S kernel (fp64, solve_small2.cuh); 3 = streamed (out of core) */
+                                  2 = pipelined, TMA-fed small-S kernel (solve_small2.cuh); 3 = streamed (out of core);
+                                  4 = medium-S kernel (fp64, 8 < S <= 64 where shared memory allows, solve_mid.cuh) */
 } ctqr_stats_t;
 
 /* Eq. 2: Householder QR of the m x n matrix A (m >= n >= 1, lda >= m).

@@ -25,6 +25,7 @@
 #include "kernels.h"
 #include "solve_small.cuh"
 #include "solve_small2.cuh"
+#include "solve_mid.cuh"
 
 using namespace ctqr;
 
@@ -203,6 +204,7 @@ struct ctqr_handle_s {
     void* dVs[2] = {nullptr, nullptr}; int64_t ldvs = 0; void* dWs = nullptr; size_t ws_elems = 0;
     void* dCw = nullptr; size_t cw_bytes = 0;   // staging buffer of the solves (B in, X out), grow-only: no allocation per batch
     void* dPart = nullptr;             // LL slots of the panel kernel
+    void* dLLm = nullptr;                        // LL slots of the medium-S Q^T B kernel (solve_mid.cuh), built at first use
     void* dLLs = nullptr; unsigned ll_seq = 0;   // LL slots / step numbers of the fused small-S solve kernels
     unsigned bar_count = 0;            // step numbers handed to the panel kernel (never reused)
     int* dFlag = nullptr;
@@ -250,7 +252,7 @@ struct ctqr_handle_s {
         for (int i = 0; i < 2; ++i) { dev_free(dWp[i]); dev_free(dW[i]); dev_free(dW2[i]); }
         dev_free(dT2); dev_free(dMerge); dev_free(dCw); dev_free(dWs);
         for (int i = 0; i < 2; ++i) if (dVs[i]) cudaFree(dVs[i]);
-        dev_free(dPart); dev_free(dLLs); dev_free(dFlag); dev_free(dTickets);
+        dev_free(dPart); dev_free(dLLs); dev_free(dLLm); dev_free(dFlag); dev_free(dTickets);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
         for (auto e : tpool) cudaEventDestroy(e);
@@ -1295,7 +1297,7 @@ extern "C" int ct_qr_factor(void* A, int64_t m, int64_t n, int64_t lda, ctqr_dty
 // ------------------------------------------------------------------------------------------
 // Pipelined, TMA-fed small-S Q^T B (solve_small2.cuh).  Returns -1000 when the configuration does not fit.
 template <typename T>
-static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
+static int ensure_mt(H& h) {
     const int nb = 128;
     const T* A = P_<T>(h.dA);
     if (!h.gt_ready) {
@@ -1327,6 +1329,14 @@ static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
         }
         h.gt_ready = true;
     }
+    return 0;
+}
+
+template <typename T>
+static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
+    const int nb = 128;
+    const T* A = P_<T>(h.dA);
+    { const int rcm = ensure_mt<T>(h); if (rcm) return rcm; }
     const int64_t nch = ceil_div(h.m, (int64_t)Qt2Chunk<T>::value);
     const int G = (int)std::min<int64_t>(h.sms, nch);
     SmallQt2Args<T> a{};
@@ -1337,8 +1347,10 @@ static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
     a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
     a.rpc = (int)ceil_div(nch, (int64_t)G) * Qt2Chunk<T>::value;
     a.kl = h.kl;
+    // (the update pass has 8 boxes in work at a time, one per warp pair: fewer than 8 stages would let a warp wait for a
+    // box two ring turns ahead, which the parity test of an mbarrier cannot tell from the turn before)
     int ns = 10;
-    while (ns > 3 && qt2_smem_bytes<T>(a.rpc, ns) > 225 * 1024) --ns;
+    while (ns > 8 && qt2_smem_bytes<T>(a.rpc, ns) > 225 * 1024) --ns;
     const size_t smem = qt2_smem_bytes<T>(a.rpc, ns);
     if (smem > 225 * 1024) return -1000;
     a.nstage = ns;
@@ -1360,6 +1372,70 @@ static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
         fprintf(stderr, "us/panel (1 gather, 2 reduce, 3 T^T W, 4 update, 5 pass A)\n");
     }
 #endif
+    return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// Medium-S Q^T B (solve_mid.cuh, fp64): the pipelined kernel with NG groups of eight right-hand sides, applied in column
+// chunks of 8 NG.  Returns -1000 when the configuration does not fit (shared memory) or more than two chunks are needed.
+constexpr int kMidMaxS = 64;
+template <int NG>
+static int apply_qt_mid_launch(H& h, double* C, int64_t ldc, int S, int G, int rpc, int ns) {
+    const int nb = 128, SM = MidCfg<NG>::SM;
+    SmallQt2Args<double> a{};
+    a.A = P_<double>(h.dA); a.lda = h.lda; a.m = h.m; a.n = h.n; a.P = h.P; a.Tm = P_<double>(h.dT); a.Mt = P_<double>(h.dGt);
+    a.B = C; a.ldb = ldc; a.S = S;
+    a.part = reinterpret_cast<uint4*>(h.dLLm);
+    a.sums = a.part + (size_t)2 * h.sms * nb * SM;
+    a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
+    a.rpc = rpc; a.kl = h.kl; a.nstage = ns;
+    CUtensorMap mapV;
+    if (tma::map_2d(&mapV, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, a.A, h.m, h.n, h.lda, Qt2Chunk<double>::value, 128, CU_TENSOR_MAP_SWIZZLE_128B) != cudaSuccess)
+        return -1000;
+    const size_t smem = qt_mid_smem_bytes<NG>(rpc, ns);
+    static SmemAttr attr;
+    CK(ensure_dyn_smem(apply_qt_mid_kernel<NG>, smem, attr));
+    void* args[] = {(void*)&mapV, (void*)&a};
+    CK(cudaLaunchCooperativeKernel((void*)apply_qt_mid_kernel<NG>, dim3(G), dim3(kQt2Threads), args, smem, h.sU));
+    h.launches += 1;
+#ifdef CTQR_SMALL_PROFILE
+    {
+        unsigned long long ph[16] = {0}, zero[16] = {0};
+        cudaStreamSynchronize(h.sU);
+        cudaMemcpyFromSymbol(ph, g_small_prof, sizeof(ph));
+        cudaMemcpyToSymbol(g_small_prof, zero, sizeof(zero));
+        for (int i = 0; i <= 5; ++i) fprintf(stderr, "ph%d %.2f  ", i, ph[i] * 1e-3 / h.P);
+        fprintf(stderr, "us/panel, NG %d (1 gather, 2 reduce, 3 T^T W, 4 update, 5 pass A)\n", NG);
+    }
+#endif
+    return 0;
+}
+
+static int apply_qt_mid(H& h, double* C, int64_t ldc, int64_t S) {
+    const int nb = 128;
+    const int64_t nch = ceil_div(h.m, (int64_t)Qt2Chunk<double>::value);
+    const int G = (int)std::min<int64_t>(h.sms, nch);
+    const int rpc = (int)ceil_div(nch, (int64_t)G) * Qt2Chunk<double>::value;
+    const size_t cap = 225 * 1024;
+    // ring depth: as many stages as fit, at least the number of boxes the update pass has in work at a time
+    auto stages = [&](auto bytes, int lo) { int ns = 8; while (ns > lo && bytes(ns) > cap) --ns; return bytes(ns) <= cap ? ns : 0; };
+    const int ns4 = stages([&](int ns) { return qt_mid_smem_bytes<4>(rpc, ns); }, qt_mid_min_stages<4>());
+    const int ns2 = stages([&](int ns) { return qt_mid_smem_bytes<2>(rpc, ns); }, qt_mid_min_stages<2>());
+    const int chunk = (ns4 && S > 16) ? 32 : 16;            // columns per launch
+    if (chunk == 16 && !ns2) return -1000;
+    if (ceil_div(S, (int64_t)chunk) > 2) return -1000;
+    { const int rcm = ensure_mt<double>(h); if (rcm) return rcm; }
+    if (!h.dLLm) {
+        const size_t bytes = ((size_t)2 * h.sms + 2) * nb * 32 * 16;      // sized for 32 columns per launch
+        CK(dev_alloc(&h.dLLm, bytes));
+        CK(cudaMemsetAsync(h.dLLm, 0, bytes, h.sU));
+    }
+    for (int64_t s0 = 0; s0 < S; s0 += chunk) {
+        const int sc = (int)std::min<int64_t>(chunk, S - s0);
+        const int rc = (chunk == 32 && sc > 16) ? apply_qt_mid_launch<4>(h, C + s0 * ldc, ldc, sc, G, rpc, ns4)
+                                                : apply_qt_mid_launch<2>(h, C + s0 * ldc, ldc, sc, G, rpc, ns2);
+        if (rc) return rc;
+    }
     return 0;
 }
 
@@ -1386,6 +1462,13 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
     if (S <= kSmallS && h.dLLs && h.gemm_impl == 0 && h.nb == 128 && (h.lda * sizeof(T)) % 16 == 0 && ((uintptr_t)A % 16) == 0 && h.P >= 2) {
         int rc2 = apply_qt_small2<T>(h, C, ldc, S);
         if (rc2 != -1000) { h.st.apply_qt_path = 2; return rc2; }   // -1000: does not fit (shared memory); fall through
+    }
+    if constexpr (sizeof(T) == 8) {
+        if (S > kSmallS && S <= kMidMaxS && h.dLLs && h.gemm_impl == 0 && h.nb == 128 && (h.lda * sizeof(T)) % 16 == 0 &&
+            ((uintptr_t)A % 16) == 0 && h.P >= 2) {
+            int rc2 = apply_qt_mid(h, C, ldc, S);
+            if (rc2 != -1000) { h.st.apply_qt_path = 4; return rc2; }
+        }
     }
     if (S <= kSmallS && h.dLLs && h.gemm_impl == 0) {
         // memory-bound regime: one cooperative kernel for all panels (solve_small.cuh)

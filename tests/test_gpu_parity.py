@@ -106,7 +106,7 @@ def test_random_small(shape, dt):
 def test_small_batch_fused_solve(shape, dt):
     """S <= 8 takes the two fused cooperative kernels (one launch for Q^T B, one for the TRSM):
     every CTA owns several row chunks, the last chunk is ragged, n is not a multiple of nb.  S = 9 takes
-    the per-panel path; both must meet the oracle."""
+    the medium-S kernel (fp64) or the per-panel path (fp32) for Q^T B and the per-block TRSM; all must meet the oracle."""
     import torch
     m, n = shape
     rng = np.random.default_rng(31 * m + n)
@@ -127,6 +127,56 @@ def test_small_batch_fused_solve(shape, dt):
             assert launches == 2, launches
         else:
             assert launches > 2 * f.stats()["n_panels"]
+    f.destroy()
+
+
+@pytest.mark.parametrize("shape,band", [((2500, 1300), False), ((4099, 1025), False), ((1300, 1300), False),
+                                        ((60000, 300), False), ((3000, 1100), True)])
+def test_medium_batch_fused_apply_qt(shape, band):
+    """8 < S <= 64 in fp64 takes the medium-S cooperative kernel (solve_mid.cuh, stats.apply_qt_path = 4): one launch per
+    chunk of 32 (or 16) right-hand sides, ragged last group of eight, ragged last chunk, n not a multiple of nb; the tall
+    shape leaves no room for 32 columns per launch (two launches of 16); with the band promise the row ranges shrink.
+    C = Q^T B against the oracle's reflector-by-reflector application and X against the oracle's solve."""
+    import torch
+    dt = np.float64
+    m, n = shape
+    rng = np.random.default_rng(17 * m + n)
+    if band:
+        m0 = m - n
+        A = np.zeros((m, n)); A[:m0] = rng.standard_normal((m0, n)); A[m0:] = 0.7 * np.eye(n)
+        A = np.asfortranarray(A)
+    else:
+        A = np.asfortranarray(rng.standard_normal((m, n)))
+    B = np.asfortranarray(rng.standard_normal((m, 64)))
+    VR, tau = oracle.qr(A)
+    C_or = oracle.apply_qt(VR, tau, B)
+    X_or = oracle.backsub(VR, C_or[:n])
+    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m, n, lower_bandwidth=(m - n) if band else 0)
+    P = f.stats()["n_panels"]
+    for S in ((9, 16, 17, 24, 32, 33, 64) if m < 10000 else (12, 24, 32)):
+        Ct = ctqr.colmajor_from_numpy(np.asfortranarray(B[:, :S]))
+        ctqr.ct_qr_apply_qt(f, Ct, S)
+        st = f.stats()
+        assert st["apply_qt_path"] == 4, (S, st["apply_qt_path"])
+        assert st["kernel_launches"] <= 2 + 3 * P        # (the first call also builds M_j: three launches per panel)
+        C = ctqr.numpy_from_colmajor(Ct)
+        assert relerr(C, C_or[:, :S]) <= 1e-11, (S, relerr(C, C_or[:, :S]))
+        assert worst_col(C, C_or[:, :S]) <= 1e-11
+        Ct2 = ctqr.colmajor_from_numpy(np.asfortranarray(B[:, :S]))
+        ctqr.ct_qr_apply_qt(f, Ct2, S)                      # deterministic: the same bits on a second call
+        assert f.stats()["kernel_launches"] <= 2
+        assert torch.equal(Ct, Ct2)
+        Bt = ctqr.colmajor_from_numpy(np.asfortranarray(B[:, :S]))
+        Xt = torch.zeros((S, n), dtype=Bt.dtype, device="cuda")
+        ctqr.ct_qr_solve(f, Bt, S, Xt)
+        X = ctqr.numpy_from_colmajor(Xt)
+        assert relerr(X, X_or[:, :S]) <= SOLUTION[dt], (S, relerr(X, X_or[:, :S]))
+        assert worst_col(X, X_or[:, :S]) <= SOLUTION[dt]
+    # S = 65 is beyond two chunks: per-panel path
+    Ct = ctqr.colmajor_from_numpy(np.asfortranarray(np.concatenate([B, B[:, :1]], axis=1)))
+    ctqr.ct_qr_apply_qt(f, Ct, 65)
+    assert f.stats()["apply_qt_path"] == 0
+    assert relerr(ctqr.numpy_from_colmajor(Ct)[:, :64], C_or) <= 1e-11
     f.destroy()
 
 

@@ -423,7 +423,7 @@ def run_e2e(cfg, dtype: str, Ah, B: np.ndarray, S: int, steps: int, flops: float
                     "warm-up call first); mean over the steps"}
 
 
-SWEEP_S = (1, 8, 64, 256, 512, 1024, 2048)       # PAPER.md:L89, Fig. 1 (L117-130): up to 2048 simultaneous slices
+SWEEP_S = (1, 8, 16, 32, 64, 256, 512, 1024, 2048)       # PAPER.md:L89, Fig. 1 (L117-130): up to 2048 simultaneous slices
 
 
 def run_solve_only(cfg, dtype: str) -> list:
@@ -769,7 +769,10 @@ def workload_name(cfg) -> str:
 NCU_TRAFFIC = {("c3", "f64", "upd"): (13.68e9, 8.29e9, "profiles/r1_pairs_c3.md"),
                ("c3", "f64", "vtc"): (3.95e9, None, "profiles/r1_pairs_c3.md"),
                ("c3", "f32", "upd"): (3.57e9, None, "profiles/r1_final_c3.md"),
-               ("c3", "f32", "vtc"): (1.91e9, None, "profiles/r1_final_c3.md")}
+               ("c3", "f32", "vtc"): (1.91e9, None, "profiles/r1_final_c3.md"),
+               ("c4", "f64", "upd"): (124.4e9, 113.4e9, "profiles/r2_c4_f64.md"),
+               ("c4", "f64", "vtc"): (90.2e9, 56.8e9, "profiles/r2_c4_f64.md"),
+               ("c4", "f32", "upd"): (89.6e9, 56.2e9, "profiles/r2_c4_f32.md")}
 
 KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; DMMA.8x8x4)",
                 ("f64", "vtc"): "gemm_mma_kernel<double,TA=true,128,64,32,32,3,2> (W = V^T C, larfb; DMMA.8x8x4)",

@@ -1551,7 +1551,8 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
     CKI(trsm_prepare<T>(h));
     const bool exact = h.trsm_exact != 0;
     const bool use_inv = !exact && h.dRinv && ldx % (16 / (int64_t)sizeof(T)) == 0;
-    if (S <= kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && h.gemm_impl == 0 && h.nb == 128 && h.P >= 2) {
+    // (up to 2 * kSmallS right-hand sides: two launches of the fused kernel read R twice and still beat 2 P launches)
+    if (S <= 2 * kSmallS && h.dLLs && h.rinv_ready && !exact && !h.ooc && h.gemm_impl == 0 && h.nb == 128 && h.P >= 2) {
         // memory-bound regime, pipelined: one grid hop per diagonal block (solve_small2.cuh)
         const int nb = 128;
         if (!h.nm_ready) {
@@ -1575,18 +1576,21 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
         const int64_t nch = ceil_div(h.n, (int64_t)kTrsmChunk);
         const int G = (int)std::min<int64_t>(h.sms, nch);
         a.A = P_<T>(h.dA); a.lda = h.lda; a.n = h.n; a.P = h.P; a.Rinv = P_<T>(h.dRinv); a.Nm = P_<T>(h.dNm);
-        a.X = X; a.ldx = ldx; a.S = (int)S;
+        a.ldx = ldx;
         a.cslots = reinterpret_cast<uint4*>(h.dLLt);
         a.xslots = a.cslots + (size_t)2 * nb * kSmallS;
-        a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
         a.rpc = (int)ceil_div(nch, (int64_t)G) * kTrsmChunk;
         const size_t smem = ((size_t)nb * kSmallS + (size_t)kSmallS * kTrsmThreads + (size_t)kSmallS * a.rpc) * sizeof(T);
         if (smem <= 220 * 1024) {
             static SmemAttr attr2;
             CK(ensure_dyn_smem(trsm_small2_kernel<T>, smem, attr2));
-            void* args[] = {(void*)&a};
-            CK(cudaLaunchCooperativeKernel((void*)trsm_small2_kernel<T>, dim3(G), dim3(kTrsmThreads), args, smem, h.sU));
-            h.launches += 1;
+            for (int64_t s0 = 0; s0 < S; s0 += kSmallS) {
+                a.X = X + s0 * ldx; a.S = (int)std::min<int64_t>(kSmallS, S - s0);
+                a.seq_base = h.ll_seq; h.ll_seq += (unsigned)h.P;
+                void* args[] = {(void*)&a};
+                CK(cudaLaunchCooperativeKernel((void*)trsm_small2_kernel<T>, dim3(G), dim3(kTrsmThreads), args, smem, h.sU));
+                h.launches += 1;
+            }
             return 0;
         }
     }

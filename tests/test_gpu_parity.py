@@ -125,6 +125,8 @@ def test_small_batch_fused_solve(shape, dt):
         launches = f.stats()["kernel_launches"]
         if S <= 8:
             assert launches == 2, launches
+        elif dt == np.float64:
+            assert launches == 3, launches          # medium-S Q^T B kernel + the fused TRSM in two chunks of <= 8 columns
         else:
             assert launches > 2 * f.stats()["n_panels"]
     f.destroy()

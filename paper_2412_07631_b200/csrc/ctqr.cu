@@ -243,6 +243,8 @@ struct ctqr_handle_s {
     void* fmap = nullptr; size_t fmap_len = 0; int ffd = -1;
     void* spbuf[2] = {nullptr, nullptr};   // super-panel buffers, alive only during factor_ooc
     void* dVb[2] = {nullptr, nullptr}; int64_t ldvb = 0;   // double buffer for streamed panels (m x nb each)
+    void* dVp[2] = {nullptr, nullptr};                    // double buffer for streamed panel PAIRS (m x 256 each; out-of-core
+                                                          // left-looking updates, workspace outside the tile budget)
     cudaEvent_t evVin[2] = {nullptr, nullptr}, evVfree[2] = {nullptr, nullptr};
     ~ctqr_handle_s() {
         if (own_A && dA) cudaFree(dA);
@@ -261,6 +263,7 @@ struct ctqr_handle_s {
         if (sC) cudaStreamDestroy(sC);
         if (sD) cudaStreamDestroy(sD);
         for (int i = 0; i < 2; ++i) dev_free(dVb[i]);
+        for (int i = 0; i < 2; ++i) if (dVp[i]) cudaFree(dVp[i]);
     }
 };
 typedef ctqr_handle_s H;
@@ -834,7 +837,7 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
 template <typename T>
 static int factor_range(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
     const bool aligned = (uintptr_t)A % 16 == 0 && (lda * (int64_t)sizeof(T)) % 16 == 0;
-    if (h.lookahead && !h.ooc && h.nb == 128 && h.gemm_impl == 0 && aligned && c0 % 128 == 0 && c1 - c0 >= 4 * 128 &&
+    if (h.lookahead && h.nb == 128 && h.gemm_impl == 0 && aligned && c0 % 128 == 0 && c1 - c0 >= 4 * 128 &&
         h.m - c0 >= 1024 && ensure_pair_ws<T>(h, c1 - c0) == 0)
         return factor_range_pairs<T>(h, A, lda, c0, c1);
     return factor_range_single<T>(h, A, lda, c0, c1);
@@ -880,12 +883,13 @@ static int factor_incore(H& h, T* A, int64_t lda) {
 // out once plus the earlier reflectors once per later super-panel = m n w (P_s + 3)/2.
 // ------------------------------------------------------------------------------------------
 template <typename T>
-static int stream_panel_in(H& h, int slot, const T* hsrc, int64_t hld, int64_t rows, int cols) {
-    // [sC] wait until the larfb that last read Vb[slot] is done, copy, signal
+static int stream_panel_in(H& h, int slot, const T* hsrc, int64_t hld, int64_t rows, int cols, void* dst = nullptr) {
+    // [sC] wait until the larfb that last read Vb[slot] (or the pair buffer of that slot: they share the events) is done,
+    // copy, signal
     CK(cudaStreamWaitEvent(h.sC, h.evVfree[slot], 0));
     cudaEvent_t ca = h.timing_event(), cb = h.timing_event();
     CK(cudaEventRecord(ca, h.sC));
-    CK(cudaMemcpy2DAsync(h.dVb[slot], h.ldvb * sizeof(T), hsrc, hld * sizeof(T), rows * sizeof(T), cols,
+    CK(cudaMemcpy2DAsync(dst ? dst : h.dVb[slot], h.ldvb * sizeof(T), hsrc, hld * sizeof(T), rows * sizeof(T), cols,
                          cudaMemcpyHostToDevice, h.sC));
     CK(cudaEventRecord(cb, h.sC));
     h.copy_spans.push_back({ca, cb});
@@ -925,6 +929,16 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
             return set_err(CTQR_ERR_NOMEM, "cannot allocate the super-panel buffers (%lld columns)", (long long)ns);
         }
         sp[i] = P_<T>(h.spbuf[i]);         // owned by the handle: freed below, or by the destructor on an error path
+    }
+    // Left-looking updates two panels at a time (the 256-wide compact-WY block of factor_range_pairs: K = 256 updates,
+    // pre-split TMA-fed operands in fp32) when every earlier panel is 128 wide and the pair workspaces can be had:
+    // [V_k V_(k+1)] split buffers, W blocks, and two m x 256 stream buffers -- workspace, outside the tile budget
+    // (about 12 m 256 w bytes in fp32, 2 m 256 w in fp64).  Otherwise one panel at a time, as before.
+    bool pairs = h.lookahead && nb == 128 && h.gemm_impl == 0 && ns % (2 * nb) == 0 && ns >= 1024 && Ps > 1 &&
+                 (lds * (int64_t)sizeof(T)) % 16 == 0 && ensure_pair_ws<T>(h, std::min<int64_t>(ns, n)) == 0;
+    if (pairs) {
+        for (int i = 0; i < 2 && pairs; ++i)
+            if (!h.dVp[i] && big_alloc(&h.dVp[i], (size_t)h.ldvb * 2 * nb * sizeof(T)) != cudaSuccess) { cudaGetLastError(); pairs = false; }
     }
     std::vector<cudaEvent_t> evIn(Ps), evOut(Ps), evDone(Ps), evFree(Ps);
     for (int s = 0; s < Ps; ++s) {
@@ -988,6 +1002,21 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
         const int kcur = (int)(c0 / nb);
         for (int k = 0; k < kres && rc == 0; ++k) {
             const int64_t j0 = (int64_t)k * nb;
+            if (pairs && k + 1 < kres && (j0 + nb) / ns == j0 / ns) {
+                // two panels of one earlier super-panel at a time: the m x 256 block at (j0, j0) is the pair's [V_k V_(k+1)]
+                const int slot = (k >> 1) & 1;
+                CK(cudaStreamWaitEvent(h.sC, evOut[(int)(j0 / ns)], 0));
+                const int64_t me = row_end(h, j0 + 2 * nb);
+                rc = stream_panel_in<T>(h, slot, hA + j0 + j0 * hlda, hlda, me - j0, 2 * nb, h.dVp[slot]);
+                if (rc) break;
+                CKI(wait_copy(h, h.sU, h.evVin[slot]));
+                const T* Vv = P_<T>(h.dVp[slot]) - j0 - j0 * h.ldvb;          // virtual base: (j0, j0) is the buffer's origin
+                rc = pair_merge<T>(h, h.sU, Vv, h.ldvb, me, j0, slot);
+                if (rc == 0) rc = larfb_pair<T>(h, h.sU, Vv, h.ldvb, me, j0, slot, Cv + j0 + c0 * lds, lds, c1 - c0, 0);
+                CK(cudaEventRecord(h.evVfree[slot], h.sU));
+                ++k;
+                continue;
+            }
             const int slot = k & 1;
             CK(cudaStreamWaitEvent(h.sC, evOut[(int)(j0 / ns)], 0));          // factor of that SP is on the host
             const int64_t mk = row_end(h, j0 + nb) - j0;                     // V_k is zero below (band promise)
@@ -1003,6 +1032,14 @@ static int factor_ooc(H& h, T* hA, int64_t hlda, int64_t ns) {
             const T* Pv = sp[(s - 1) & 1] - (int64_t)(s - 1) * ns * lds;
             for (int k = kres; k < kcur && rc == 0; ++k) {
                 const int64_t j0 = (int64_t)k * nb;
+                if (pairs && k + 1 < kcur) {
+                    const int slot = (k >> 1) & 1;
+                    const int64_t me = row_end(h, j0 + 2 * nb);
+                    rc = pair_merge<T>(h, h.sU, Pv, lds, me, j0, slot);
+                    if (rc == 0) rc = larfb_pair<T>(h, h.sU, Pv, lds, me, j0, slot, Cv + j0 + c0 * lds, lds, c1 - c0, 0);
+                    ++k;
+                    continue;
+                }
                 rc = larfb<T>(h, 0, h.sU, Pv + j0 + j0 * lds, lds, row_end(h, j0 + nb) - j0, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb,
                               Cv + j0 + c0 * lds, lds, c1 - c0, true);
             }

@@ -405,6 +405,40 @@ def test_out_of_core_matches_oracle_and_in_core(nb, ns, pinned, dt):
     assert relerr(C, oracle.apply_qt(VR, tau_o, B)) <= ROUND[dt]
 
 
+@pytest.mark.parametrize("dt,band", [(np.float64, False), (np.float32, False), (np.float64, True)])
+def test_out_of_core_pair_updates(dt, band):
+    """Super-panels of 1280 columns (P_s = 4, the last one 44 columns wide): wide enough for the two-panel path, so the
+    factorisation inside a super-panel and the left-looking updates -- from the previous super-panel still resident and
+    from pairs of panels streamed back from the host -- all run as 256-wide compact-WY blocks (fp32: pre-split, TMA-fed).
+    Same gates as in core, against the oracle and against the in-core factor; with the band promise as well."""
+    m, n, S, ns = 4600, 3884, 5, 1280
+    rng = np.random.default_rng(77)
+    if band:
+        m0 = m - n
+        A = np.zeros((m, n)); A[:m0] = rng.standard_normal((m0, n)); A[m0:] = 0.9 * np.eye(n)
+    else:
+        A = rng.standard_normal((m, n))
+    A = np.asfortranarray(A.astype(dt))
+    B = np.asfortranarray(rng.standard_normal((m, S)).astype(dt))
+    Ah = ctqr.colmajor_from_numpy(A, device="cpu", pin=True)
+    f = ctqr.ct_qr_factor(Ah, m, n, device_budget_bytes=_ooc_budget(m, 128, ns, dt), lower_bandwidth=(m - n) if band else 0)
+    st = f.stats()
+    assert st["out_of_core"] == 1 and st["n_superpanels"] == 4
+    X = np.zeros((n, S), dtype=dt, order="F")
+    ctqr.ct_qr_solve(f, B, S, X)
+    R, V, tau = ctqr.ct_qr_get_R(f), ctqr.ct_qr_get_V(f), ctqr.ct_qr_get_tau(f)
+    VR, tau_o = oracle.qr(A)
+    X_or = oracle.solve(VR, tau_o, B)
+    assert relerr(X, X_or) <= SOLUTION[dt] and worst_col(X, X_or) <= SOLUTION[dt]
+    assert relerr(R, oracle.R_of(VR)) <= ROUND[dt] and max_abs(R, oracle.R_of(VR)) <= ROUND[dt]
+    assert relerr(V, oracle.V_of(VR)) <= ROUND[dt] and max_abs(V, oracle.V_of(VR)) <= ROUND[dt]
+    assert relerr(tau, tau_o) <= ROUND[dt]
+    f.destroy()
+    g = gpu_factor_solve(A, B, lower_bandwidth=(m - n) if band else 0)
+    assert relerr(R, g["R"]) <= ROUND[dt] and relerr(X, g["X"]) <= SOLUTION[dt]
+    g["f"].destroy()
+
+
 @pytest.mark.parametrize("dt", DT)
 def test_out_of_core_ct_config(dt):
     """BASELINE.json configs[0] streamed through 4 super-panels of 256 columns."""

@@ -123,7 +123,8 @@ typedef struct {
     int32_t trsm_exact;        /* 0: inverted diagonal blocks; 1: back-substitution by option; 2: forced by the guard */
     int32_t apply_qt_path;     /* last Q^T B: 0 = one larfb per panel; 1 = fused small-S kernel (one cooperative launch);
                                   2 = pipelined, TMA-fed small-S kernel (solve_small2.cuh); 3 = streamed (out of core);
-                                  4 = medium-S kernel (fp64, 8 < S <= 64 where shared memory allows, solve_mid.cuh) */
+                                  4 = medium-S kernel (fp64, 8 < S <= 64 where shared memory allows, solve_mid.cuh);
+                                  5 = two panels per larfb (S >= 1024, or S >= 512 when m >= 65536: the 256-wide blocks of the factorisation) */
 } ctqr_stats_t;
 
 /* Eq. 2: Householder QR of the m x n matrix A (m >= n >= 1, lda >= m).

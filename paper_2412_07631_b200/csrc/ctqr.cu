@@ -204,6 +204,7 @@ struct ctqr_handle_s {
     void* dVs[2] = {nullptr, nullptr}; int64_t ldvs = 0; void* dWs = nullptr; size_t ws_elems = 0;
     void* dCw = nullptr; size_t cw_bytes = 0;   // staging buffer of the solves (B in, X out), grow-only: no allocation per batch
     void* dPart = nullptr;             // LL slots of the panel kernel
+    void* dT12 = nullptr; bool t12_ready = false;   // off-diagonal blocks -T_k (V_k^T V_k+1) T_k+1 of the pairs' merged T factors (solve)
     void* dLLm = nullptr;                        // LL slots of the medium-S Q^T B kernel (solve_mid.cuh), built at first use
     void* dLLs = nullptr; unsigned ll_seq = 0;   // LL slots / step numbers of the fused small-S solve kernels
     unsigned bar_count = 0;            // step numbers handed to the panel kernel (never reused)
@@ -254,7 +255,7 @@ struct ctqr_handle_s {
         for (int i = 0; i < 2; ++i) { dev_free(dWp[i]); dev_free(dW[i]); dev_free(dW2[i]); }
         dev_free(dT2); dev_free(dMerge); dev_free(dCw); dev_free(dWs);
         for (int i = 0; i < 2; ++i) if (dVs[i]) cudaFree(dVs[i]);
-        dev_free(dPart); dev_free(dLLs); dev_free(dLLm); dev_free(dFlag); dev_free(dTickets);
+        dev_free(dPart); dev_free(dLLs); dev_free(dLLm); dev_free(dT12); dev_free(dFlag); dev_free(dTickets);
         for (int i = 0; i < 2; ++i) cudaFree(spbuf[i]);
         for (auto e : ev) cudaEventDestroy(e);
         for (auto e : tpool) cudaEventDestroy(e);
@@ -615,8 +616,8 @@ static int ensure_pair_ws(H& h, int64_t nc) {
     if (!h.dT2) {
         if (dev_alloc(&h.dT2, (size_t)2 * 256 * 256 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
         CK(cudaMemsetAsync(h.dT2, 0, (size_t)2 * 256 * 256 * sizeof(T), h.sU));
-        if (dev_alloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
     }
+    if (!h.dMerge && dev_alloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
     return 0;
 }
 
@@ -667,7 +668,7 @@ static int pair_merge(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
 // C[j0:m, 0:nc] <- (H_k H_{k+1})^T C for the pair at columns j0, j0 + 128; T2 = its merged factor; stream sU
 template <typename T>
 static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m, int64_t j0, int slot, T* C,
-                      int64_t ldc, int64_t nc, int reserve_sms) {
+                      int64_t ldc, int64_t nc, int reserve_sms, int64_t min_nc = 1024) {
     const T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;
     if (nc <= 0) return 0;
     const int nb = 128;
@@ -675,7 +676,7 @@ static int larfb_pair(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
     const T* V1 = A + j0 + j0 * lda;
     const T* V2 = A + (j0 + nb) + (j0 + nb) * lda;
     const int64_t mk = m - j0;
-    if (nc < 1024 || (size_t)256 * (size_t)nc > h.w2_elems) {
+    if (nc < min_nc || (size_t)256 * (size_t)nc > h.w2_elems) {
         // narrow right-hand side: the two panels one after the other (same product, small kernels)
         CKI(larfb<T>(h, 0, st, V1, lda, mk, nb, P_<T>(h.dT) + (size_t)k * nb * nb, nb, C, ldc, nc, true, reserve_sms));
         CKI(larfb<T>(h, 0, st, V2, lda, mk - nb, nb, P_<T>(h.dT) + (size_t)(k + 1) * nb * nb, nb, C + nb, ldc, nc, true,
@@ -1416,6 +1417,7 @@ static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
 // Medium-S Q^T B (solve_mid.cuh, fp64): the pipelined kernel with NG groups of eight right-hand sides, applied in column
 // chunks of 8 NG.  Returns -1000 when the configuration does not fit (shared memory) or more than two chunks are needed.
 constexpr int kMidMaxS = 64;
+constexpr int64_t kPairSolveMinS = 512;    // Q^T B two panels at a time from this many right-hand sides on (tall matrices; twice that otherwise)
 template <int NG>
 static int apply_qt_mid_launch(H& h, double* C, int64_t ldc, int S, int G, int rpc, int ns) {
     const int nb = 128, SM = MidCfg<NG>::SM;
@@ -1540,9 +1542,56 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
             return 0;
         }
     }
+    // Many right-hand sides: two panels at a time, as the factorisation's trailing updates (K = 256 updates; fp32:
+    // pre-split TMA-fed operands).  The off-diagonal block of a pair's merged T factor, -T_k (V_k^T V_k+1) T_k+1 =
+    // -Mt[k+1] T_k+1, is built once per handle; T2 is assembled per pair from it and the two panel factors.
+    // (measured, both precisions: a gain from S = 1024 at configs[2], from S = 512 at configs[3]; a loss of 3-16 % below)
+    bool pairs = (S >= 2 * kPairSolveMinS || (S >= kPairSolveMinS && h.m >= 65536)) && h.nb == 128 && h.gemm_impl == 0 && h.P >= 2 && (h.lda * sizeof(T)) % 16 == 0 &&
+                 ((uintptr_t)A % 16) == 0 && ((uintptr_t)C % 16) == 0 && (ldc * sizeof(T)) % 16 == 0 &&
+                 ensure_pair_ws<T>(h, std::max<int64_t>(S, 1024)) == 0;
+    if (pairs && !h.t12_ready) {
+        const int rcm = ensure_mt<T>(h);
+        if (rcm == -1000) pairs = false;
+        else if (rcm) return rcm;
+        if (pairs) {
+            const int nb = 128;
+            if (!h.dT12) CK(dev_alloc(&h.dT12, (size_t)((h.P + 1) / 2) * nb * nb * sizeof(T)));
+            for (int k = 0; k + 1 < h.P; k += 2) {
+                if (h.n - (int64_t)(k + 1) * nb < nb) break;                 // ragged last panel: applied alone
+                GemmArgs<T> g{};
+                g.M = nb; g.N = nb; g.K = nb; g.A = P_<T>(h.dGt) + (size_t)(k + 1) * nb * nb; g.lda = nb;
+                g.B = P_<T>(h.dT) + (size_t)(k + 1) * nb * nb; g.ldb = nb;
+                g.C = P_<T>(h.dT12) + (size_t)(k / 2) * nb * nb; g.ldc = nb; g.alpha = T(-1); g.beta = T(0);
+                CK(gemm_direct<T>(false, g, h.gemm_impl, h.sms, h.sU));
+                h.launches += 1;
+            }
+            h.t12_ready = true;
+        }
+    }
     for (int k = 0; k < h.P; ++k) {
         const int64_t j0 = (int64_t)k * h.nb;
         const int nbw = (int)std::min<int64_t>(h.nb, h.n - j0);
+        if (pairs && k + 1 < h.P && (k & 1) == 0 && h.n - (j0 + h.nb) >= h.nb) {
+            const int nb = 128, slot = (k >> 1) & 1;
+            const int64_t me = row_end(h, j0 + 2 * nb);
+            T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;
+            const T* Tk = P_<T>(h.dT) + (size_t)k * nb * nb;
+            CK(copy2d_launch<T>(Tk, nb, T2, 256, nb, nb, h.sU));
+            CK(copy2d_launch<T>(Tk + (size_t)nb * nb, nb, T2 + nb + (size_t)nb * 256, 256, nb, nb, h.sU));
+            CK(copy2d_launch<T>(P_<T>(h.dT12) + (size_t)(k / 2) * nb * nb, nb, T2 + (size_t)nb * 256, 256, nb, nb, h.sU));
+            h.launches += 3;
+            if constexpr (sizeof(T) == 4) {
+                if (h.dVs[slot]) {
+                    float* hi = P_<float>(h.dVs[slot]);
+                    CK(split_tf32_launch(A + j0 + j0 * h.lda, h.lda, me - j0, 2 * nb, hi, hi + (size_t)h.ldvs * 256, h.ldvs, h.sU));
+                    h.launches += 1;
+                }
+            }
+            CKI(larfb_pair<T>(h, h.sU, A, h.lda, me, j0, slot, C + j0, ldc, S, 0, kPairSolveMinS));
+            h.st.apply_qt_path = 5;
+            ++k;
+            continue;
+        }
         CKI(larfb<T>(h, 0, h.sU, A + j0 + j0 * h.lda, h.lda, row_end(h, j0 + nbw) - j0, nbw,
                      P_<T>(h.dT) + (size_t)k * h.nb * h.nb, h.nb, C + j0, ldc, S));
     }

@@ -183,6 +183,40 @@ def test_medium_batch_fused_apply_qt(shape, band):
 
 
 @pytest.mark.parametrize("dt", DT)
+@pytest.mark.parametrize("band", [False, True])
+def test_large_batch_two_panel_apply_qt(dt, band):
+    """S >= 1024 applies Q^T two panels at a time (stats.apply_qt_path = 5: the 256-wide compact-WY blocks of the
+    factorisation, merged T factor assembled from the cached off-diagonal block): seven full panels + a ragged one, so
+    three pairs, one single full panel and the 4-column tail; with the band promise too.  Against the oracle."""
+    import torch
+    m, n, S = 1500, 900, 1024
+    rng = np.random.default_rng(5)
+    if band:
+        m0 = m - n
+        A = np.zeros((m, n)); A[:m0] = rng.standard_normal((m0, n)); A[m0:] = 0.8 * np.eye(n)
+    else:
+        A = rng.standard_normal((m, n))
+    A = np.asfortranarray(A.astype(dt))
+    B = np.asfortranarray(rng.standard_normal((m, S)).astype(dt))
+    VR, tau = oracle.qr(A)
+    C_or = oracle.apply_qt(VR, tau, B)
+    X_or = oracle.backsub(VR, C_or[:n])
+    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m, n, lower_bandwidth=(m - n) if band else 0)
+    for rep in range(2):                                     # the second call reuses the cached blocks
+        Ct = ctqr.colmajor_from_numpy(B)
+        ctqr.ct_qr_apply_qt(f, Ct, S)
+        assert f.stats()["apply_qt_path"] == 5
+        C = ctqr.numpy_from_colmajor(Ct)
+        assert relerr(C, C_or) <= ROUND[dt], relerr(C, C_or)
+        assert worst_col(C, C_or) <= 10 * ROUND[dt]
+    Xt = torch.zeros((S, n), dtype=Ct.dtype, device="cuda")
+    ctqr.ct_qr_solve(f, ctqr.colmajor_from_numpy(B), S, Xt)
+    X = ctqr.numpy_from_colmajor(Xt)
+    assert relerr(X, X_or) <= SOLUTION[dt] and worst_col(X, X_or) <= SOLUTION[dt]
+    f.destroy()
+
+
+@pytest.mark.parametrize("dt", DT)
 @pytest.mark.parametrize("nb,ib", [(8, 8), (32, 16), (64, 16), (128, 16), (128, 32), (64, 8)])
 @pytest.mark.parametrize("la", [0, 1])
 def test_blocking_invariance(nb, ib, la, dt):

@@ -742,6 +742,10 @@ def sample_size(cfg) -> tuple[int, int]:
 
 def run_reference(cfg, dtype: str, steps: int, warmup: int) -> dict:
     k, s = sample_size(cfg)
+    # K timed steps, each on the bounded sample: the sample shrinks (time ~ k^2) so that the whole run stays within
+    # about four minutes of oracle work whatever K is
+    if steps > 12:
+        k = max(64, int(k * (12.0 / steps) ** 0.5) // 64 * 64)
     for _ in range(min(warmup, 1)):
         oracle_sample(cfg, dtype, max(64, k // 4), 1)
     r = oracle_sample(cfg, dtype, k, s, reps=max(1, steps))

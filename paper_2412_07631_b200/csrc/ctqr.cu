@@ -204,7 +204,8 @@ struct ctqr_handle_s {
     void* dVs[2] = {nullptr, nullptr}; int64_t ldvs = 0; void* dWs = nullptr; size_t ws_elems = 0;
     void* dCw = nullptr; size_t cw_bytes = 0;   // staging buffer of the solves (B in, X out), grow-only: no allocation per batch
     void* dPart = nullptr;             // LL slots of the panel kernel
-    void* dT12 = nullptr; bool t12_ready = false;   // off-diagonal blocks -T_k (V_k^T V_k+1) T_k+1 of the pairs' merged T factors (solve)
+    void* dT12 = nullptr;                            // off-diagonal blocks -T_k (V_k^T V_k+1) T_k+1 of the merged T factors of the pairs
+    std::vector<unsigned char> t12_have;             // (2i, 2i+1), kept from the factorisation's merges for the large-batch Q^T B
     void* dLLm = nullptr;                        // LL slots of the medium-S Q^T B kernel (solve_mid.cuh), built at first use
     void* dLLs = nullptr; unsigned ll_seq = 0;   // LL slots / step numbers of the fused small-S solve kernels
     unsigned bar_count = 0;            // step numbers handed to the panel kernel (never reused)
@@ -618,6 +619,10 @@ static int ensure_pair_ws(H& h, int64_t nc) {
         CK(cudaMemsetAsync(h.dT2, 0, (size_t)2 * 256 * 256 * sizeof(T), h.sU));
     }
     if (!h.dMerge && dev_alloc(&h.dMerge, (size_t)2 * 128 * 128 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return 1; }
+    if (!h.dT12 && h.P >= 2) {
+        if (dev_alloc(&h.dT12, (size_t)(h.P / 2) * 128 * 128 * sizeof(T)) != cudaSuccess) { cudaGetLastError(); h.dT12 = nullptr; }
+        else h.t12_have.assign((size_t)(h.P / 2), 0);           // (without it the solve applies one panel at a time)
+    }
     return 0;
 }
 
@@ -652,6 +657,12 @@ static int pair_merge(H& h, cudaStream_t st, const T* A, int64_t lda, int64_t m,
     CK(copy2d_launch<T>(Tk, nb, T2, 256, nb, nb, st));
     CK(copy2d_launch<T>(Tk1, nb, T2 + nb + (size_t)nb * 256, 256, nb, nb, st));
     h.launches += 6;
+    if (h.dT12 && (k & 1) == 0 && (size_t)(k / 2) < h.t12_have.size()) {
+        // the solve applies Q^T to large batches pair by pair as well: keep this pair's off-diagonal block
+        CK(copy2d_launch<T>(T2 + (size_t)nb * 256, 256, P_<T>(h.dT12) + (size_t)(k / 2) * nb * nb, nb, nb, nb, st));
+        h.t12_have[k / 2] = 1;
+        h.launches += 1;
+    }
     if constexpr (sizeof(T) == 4) {
         if (h.dVs[slot]) {
             // both contractions of this pair's trailing updates read [V_k V_{k+1}] once per output tile: split it into TF32
@@ -1543,35 +1554,19 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
         }
     }
     // Many right-hand sides: two panels at a time, as the factorisation's trailing updates (K = 256 updates; fp32:
-    // pre-split TMA-fed operands).  The off-diagonal block of a pair's merged T factor, -T_k (V_k^T V_k+1) T_k+1 =
-    // -Mt[k+1] T_k+1, is built once per handle; T2 is assembled per pair from it and the two panel factors.
+    // pre-split TMA-fed operands).  The off-diagonal block of a pair's merged T factor, -T_k (V_k^T V_k+1) T_k+1, was kept
+    // by the factorisation's own merge of that pair (no set-up cost here); T2 is assembled per pair from it and the two
+    // panel factors.  Pairs the factorisation did not merge (its narrow tail, out-of-core or loaded handles) take one
+    // panel at a time.
     // (measured, both precisions: a gain from S = 1024 at configs[2], from S = 512 at configs[3]; a loss of 3-16 % below)
-    bool pairs = (S >= 2 * kPairSolveMinS || (S >= kPairSolveMinS && h.m >= 65536)) && h.nb == 128 && h.gemm_impl == 0 && h.P >= 2 && (h.lda * sizeof(T)) % 16 == 0 &&
-                 ((uintptr_t)A % 16) == 0 && ((uintptr_t)C % 16) == 0 && (ldc * sizeof(T)) % 16 == 0 &&
-                 ensure_pair_ws<T>(h, std::max<int64_t>(S, 1024)) == 0;
-    if (pairs && !h.t12_ready) {
-        const int rcm = ensure_mt<T>(h);
-        if (rcm == -1000) pairs = false;
-        else if (rcm) return rcm;
-        if (pairs) {
-            const int nb = 128;
-            if (!h.dT12) CK(dev_alloc(&h.dT12, (size_t)((h.P + 1) / 2) * nb * nb * sizeof(T)));
-            for (int k = 0; k + 1 < h.P; k += 2) {
-                if (h.n - (int64_t)(k + 1) * nb < nb) break;                 // ragged last panel: applied alone
-                GemmArgs<T> g{};
-                g.M = nb; g.N = nb; g.K = nb; g.A = P_<T>(h.dGt) + (size_t)(k + 1) * nb * nb; g.lda = nb;
-                g.B = P_<T>(h.dT) + (size_t)(k + 1) * nb * nb; g.ldb = nb;
-                g.C = P_<T>(h.dT12) + (size_t)(k / 2) * nb * nb; g.ldc = nb; g.alpha = T(-1); g.beta = T(0);
-                CK(gemm_direct<T>(false, g, h.gemm_impl, h.sms, h.sU));
-                h.launches += 1;
-            }
-            h.t12_ready = true;
-        }
-    }
+    const bool pairs = (S >= 2 * kPairSolveMinS || (S >= kPairSolveMinS && h.m >= 65536)) && h.nb == 128 && h.gemm_impl == 0 &&
+                       h.P >= 2 && h.dT12 && (h.lda * sizeof(T)) % 16 == 0 && ((uintptr_t)A % 16) == 0 &&
+                       ((uintptr_t)C % 16) == 0 && (ldc * sizeof(T)) % 16 == 0 &&
+                       ensure_pair_ws<T>(h, std::max<int64_t>(S, 1024)) == 0;
     for (int k = 0; k < h.P; ++k) {
         const int64_t j0 = (int64_t)k * h.nb;
         const int nbw = (int)std::min<int64_t>(h.nb, h.n - j0);
-        if (pairs && k + 1 < h.P && (k & 1) == 0 && h.n - (j0 + h.nb) >= h.nb) {
+        if (pairs && k + 1 < h.P && (k & 1) == 0 && (size_t)(k / 2) < h.t12_have.size() && h.t12_have[k / 2]) {
             const int nb = 128, slot = (k >> 1) & 1;
             const int64_t me = row_end(h, j0 + 2 * nb);
             T* T2 = P_<T>(h.dT2) + (size_t)slot * 256 * 256;

@@ -91,7 +91,10 @@ typedef struct {
                                    backward stable, so the library falls back to back-substitution by itself when a
                                    diagonal block looks ill-conditioned (stats.diag_block_cond > 1/sqrt(eps)).
                                    1 = always back-substitution (trsm_diag_kernel; also disables the fused S <= 8 TRSM). */
-    int32_t reserved_;          /* must be 0 */
+    int32_t solve_pairs;        /* 0 = by size (default): large batches apply Q^T two panels at a time (S >= 1024, or S >= 512
+                                   when m >= 65536) and the TRSM two diagonal blocks at a time (S >= 512, n >= 32768), where
+                                   that was measured to win; 1 = whenever the batch has at least 256 right-hand sides (used
+                                   by the tests to reach those paths at oracle-sized problems); -1 = never */
 } ctqr_options_t;
 
 /* Per-handle statistics (CUDA-event timed, milliseconds). */

@@ -35,7 +35,7 @@ class Options(ctypes.Structure):
                 ("in_place", ctypes.c_int32), ("device_budget_bytes", ctypes.c_int64),
                 ("gemm_impl", ctypes.c_int32), ("profile", ctypes.c_int32),
                 ("file_path", ctypes.c_char_p), ("stream", ctypes.c_void_p),
-                ("lower_bandwidth", ctypes.c_int64), ("trsm_exact", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
+                ("lower_bandwidth", ctypes.c_int64), ("trsm_exact", ctypes.c_int32), ("solve_pairs", ctypes.c_int32)]
 
 
 class Stats(ctypes.Structure):
@@ -200,7 +200,7 @@ class Factor:
 def ct_qr_factor(A, m: int, n: int, lda: int | None = None, *, nb: int = 0, ib: int = 0,
                  lookahead: int = -1, in_place: bool = False, device_budget_bytes: int = 0,
                  gemm_impl: int = 0, profile: bool = False, stream=None, file_path: str | None = None,
-                 dtype=None, lower_bandwidth: int = 0, trsm_exact: bool = False) -> Factor:
+                 dtype=None, lower_bandwidth: int = 0, trsm_exact: bool = False, solve_pairs: int = 0) -> Factor:
     """Eq. 2.  ``A``: torch tensor (device or pinned/pageable host) or numpy array whose MEMORY
     is the column-major m x n matrix with leading dimension ``lda`` (default m)."""
     code = _code_of(A) if A is not None else (F64 if np.dtype(dtype) == np.float64 else F32)
@@ -208,7 +208,7 @@ def ct_qr_factor(A, m: int, n: int, lda: int | None = None, *, nb: int = 0, ib: 
     o = Options(nb=nb, ib=ib, lookahead=lookahead, in_place=int(in_place),
                 device_budget_bytes=device_budget_bytes, gemm_impl=gemm_impl, profile=int(profile),
                 file_path=file_path.encode() if file_path else None, stream=stream,
-                lower_bandwidth=lower_bandwidth, trsm_exact=int(trsm_exact))
+                lower_bandwidth=lower_bandwidth, trsm_exact=int(trsm_exact), solve_pairs=int(solve_pairs))
     h = _P()
     _check(lib().ct_qr_factor(_ptr(A) if A is not None else None, m, n, lda, code, ctypes.byref(o), ctypes.byref(h)))
     return Factor(h, m, n, code, keep=A if in_place else None)

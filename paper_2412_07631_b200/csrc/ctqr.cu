@@ -204,6 +204,7 @@ struct ctqr_handle_s {
     void* dVs[2] = {nullptr, nullptr}; int64_t ldvs = 0; void* dWs = nullptr; size_t ws_elems = 0;
     void* dCw = nullptr; size_t cw_bytes = 0;   // staging buffer of the solves (B in, X out), grow-only: no allocation per batch
     void* dPart = nullptr;             // LL slots of the panel kernel
+    int solve_pairs = 0;                             // option: 0 by size, 1 from 256 right-hand sides on, -1 never
     void* dT12 = nullptr;                            // off-diagonal blocks -T_k (V_k^T V_k+1) T_k+1 of the merged T factors of the pairs
     std::vector<unsigned char> t12_have;             // (2i, 2i+1), kept from the factorisation's merges for the large-batch Q^T B
     void* dLLm = nullptr;                        // LL slots of the medium-S Q^T B kernel (solve_mid.cuh), built at first use
@@ -1270,6 +1271,7 @@ static int new_handle(ctqr_dtype_t dtype, int64_t m, int64_t n, const ctqr_optio
     h->profile = o.profile ? 1 : 0;
     h->reserve_sms = -1;               // SMs left to the look-ahead chain during the bulk update: chosen per panel
     h->trsm_exact = o.trsm_exact ? 1 : 0;
+    h->solve_pairs = o.solve_pairs;
     h->P = (int)ceil_div(n, h->nb);
     h->user = (cudaStream_t)o.stream;
     int dev = 0; cudaGetDevice(&dev);
@@ -1428,6 +1430,7 @@ static int apply_qt_small2(H& h, T* C, int64_t ldc, int64_t S) {
 // Medium-S Q^T B (solve_mid.cuh, fp64): the pipelined kernel with NG groups of eight right-hand sides, applied in column
 // chunks of 8 NG.  Returns -1000 when the configuration does not fit (shared memory) or more than two chunks are needed.
 constexpr int kMidMaxS = 64;
+constexpr int64_t kPairTrsmMinS = 512;     // blocked TRSM two diagonal blocks at a time from this many right-hand sides on (n >= 32768)
 constexpr int64_t kPairSolveMinS = 512;    // Q^T B two panels at a time from this many right-hand sides on (tall matrices; twice that otherwise)
 template <int NG>
 static int apply_qt_mid_launch(H& h, double* C, int64_t ldc, int S, int G, int rpc, int ns) {
@@ -1559,7 +1562,9 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
     // panel factors.  Pairs the factorisation did not merge (its narrow tail, out-of-core or loaded handles) take one
     // panel at a time.
     // (measured, both precisions: a gain from S = 1024 at configs[2], from S = 512 at configs[3]; a loss of 3-16 % below)
-    const bool pairs = (S >= 2 * kPairSolveMinS || (S >= kPairSolveMinS && h.m >= 65536)) && h.nb == 128 && h.gemm_impl == 0 &&
+    const bool psize = h.solve_pairs > 0 ? S >= 256
+                                         : (h.solve_pairs == 0 && (S >= 2 * kPairSolveMinS || (S >= kPairSolveMinS && h.m >= 65536)));
+    const bool pairs = psize && h.nb == 128 && h.gemm_impl == 0 &&
                        h.P >= 2 && h.dT12 && (h.lda * sizeof(T)) % 16 == 0 && ((uintptr_t)A % 16) == 0 &&
                        ((uintptr_t)C % 16) == 0 && (ldc * sizeof(T)) % 16 == 0 &&
                        ensure_pair_ws<T>(h, std::max<int64_t>(S, 1024)) == 0;
@@ -1582,7 +1587,7 @@ static int apply_qt_dev(H& h, T* C, int64_t ldc, int64_t S) {
                     h.launches += 1;
                 }
             }
-            CKI(larfb_pair<T>(h, h.sU, A, h.lda, me, j0, slot, C + j0, ldc, S, 0, kPairSolveMinS));
+            CKI(larfb_pair<T>(h, h.sU, A, h.lda, me, j0, slot, C + j0, ldc, S, 0, 256));
             h.st.apply_qt_path = 5;
             ++k;
             continue;
@@ -1696,9 +1701,70 @@ static int trsm_dev(H& h, T* X, int64_t ldx, int64_t S) {
             return 0;
         }
     }
+    // Large batches, in core: two diagonal blocks per update of the rows above (K = 256; fp32: operands pre-split and fed
+    // by TMA, as in the two-panel trailing update): X_i, then C_(i-1) -= R_(i-1,i) X_i, X_(i-1), then one product with the
+    // 256 columns of R.  Same task list, two tasks per step.
+    // (measured: TRSM 105 -> 95 ms fp64, 50 -> 46 ms fp32 at configs[3], S = 512; a loss of 2-20 % at configs[2])
+    const bool tsize = h.solve_pairs > 0 ? S >= 256 : (h.solve_pairs == 0 && S >= kPairTrsmMinS && h.n >= 32768);
+    const bool tpairs = !h.ooc && use_inv && h.nb == 128 && h.gemm_impl == 0 && tsize &&
+                        ((uintptr_t)X % 16) == 0 && (h.lda * sizeof(T)) % 16 == 0 &&
+                        (sizeof(T) == 8 || ensure_pair_ws<T>(h, std::max<int64_t>(S, 1024)) == 0);
+    // X_i = R_ii^{-1} C_i in place for a full block (inverted diagonal blocks): mm128_kernel up to 512 right-hand sides,
+    // the contraction (out of place, copied back) beyond
+    auto diag_inv = [&](int i) -> int {
+        const int64_t i0 = (int64_t)i * 128;
+        const T* Ri = P_<T>(h.dRinv) + (size_t)i * 128 * 128;
+        if (S <= 512) {
+            CK(mm128_launch<T>(false, Ri, 128, X + i0, ldx, SegInfo{}, S, X + i0, ldx, h.sU));
+            h.launches += 1;
+        } else {
+            T* W = P_<T>(h.dW[0]);
+            GemmArgs<T> gi{};
+            gi.M = 128; gi.N = S; gi.K = 128; gi.A = Ri; gi.lda = 128; gi.B = X + i0; gi.ldb = ldx; gi.C = W; gi.ldc = 128;
+            gi.alpha = T(1); gi.beta = T(0);
+            CK(gemm_direct<T>(false, gi, h.gemm_impl, h.sms, h.sU));
+            CK(copy2d_launch<T>(W, 128, X + i0, ldx, 128, S, h.sU));
+            h.launches += 2;
+        }
+        return 0;
+    };
     for (int i = h.P - 1; i >= 0; --i) {
         const int64_t i0 = (int64_t)i * h.nb;
         const int nbw = (int)std::min<int64_t>(h.nb, h.n - i0);
+        if (tpairs && i >= 2 && nbw == 128) {
+            const int nb = 128;
+            const int64_t p0 = i0 - nb;                   // first row / column of the pair (blocks i-1, i)
+            const T* A = P_<T>(h.dA);
+            CKI(diag_inv(i));
+            GemmArgs<T> gs{};
+            gs.M = nb; gs.N = S; gs.K = nb; gs.A = A + p0 + i0 * h.lda; gs.lda = h.lda; gs.B = X + i0; gs.ldb = ldx;
+            gs.C = X + p0; gs.ldc = ldx; gs.alpha = T(-1); gs.beta = T(1);
+            CK(gemm_direct<T>(false, gs, h.gemm_impl, h.sms, h.sU));
+            CKI(diag_inv(i - 1));
+            h.launches += 1;
+            bool done = false;
+            if constexpr (sizeof(T) == 4) {
+                const int slot2 = (i >> 1) & 1;
+                if (h.dVs[slot2] && h.dWs && (size_t)2 * 256 * (size_t)S <= h.ws_elems && ldx % 4 == 0 && S % 8 == 0 && p0 <= h.ldvs) {
+                    float* vhi = P_<float>(h.dVs[slot2]); float* vlo = vhi + (size_t)h.ldvs * 256;
+                    float* whi = P_<float>(h.dWs); float* wlo = whi + (size_t)256 * S;
+                    CK(split_tf32_launch(A + p0 * h.lda, h.lda, p0, 2 * nb, vhi, vlo, h.ldvs, h.sU));
+                    CK(split_tf32_launch(X + p0, ldx, 256, S, whi, wlo, 256, h.sU));
+                    CK(upd_presplit_launch(p0, S, 256, -1.f, vhi, vlo, h.ldvs, whi, wlo, 256, 1.f, X, ldx, h.sms, h.sU));
+                    h.launches += 3;
+                    done = true;
+                }
+            }
+            if (!done) {
+                GemmArgs<T> g{};
+                g.M = p0; g.N = S; g.K = 2 * nb; g.A = A + p0 * h.lda; g.lda = h.lda; g.B = X + p0; g.ldb = ldx;
+                g.C = X; g.ldc = ldx; g.alpha = T(-1); g.beta = T(1);
+                CK(gemm_direct<T>(false, g, h.gemm_impl, h.sms, h.sU));
+                h.launches += 1;
+            }
+            --i;
+            continue;
+        }
         const T* Rcol = nullptr; int64_t ldr = 0;        // R[0:i0, i0:i0+nbw]
         const int slot = i & 1;
         if (i0 > 0) {

@@ -201,7 +201,7 @@ def test_large_batch_two_panel_apply_qt(dt, band):
     VR, tau = oracle.qr(A)
     C_or = oracle.apply_qt(VR, tau, B)
     X_or = oracle.backsub(VR, C_or[:n])
-    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m, n, lower_bandwidth=(m - n) if band else 0)
+    f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m, n, lower_bandwidth=(m - n) if band else 0, solve_pairs=1)
     for rep in range(2):                                     # the second call reuses the cached blocks
         Ct = ctqr.colmajor_from_numpy(B)
         ctqr.ct_qr_apply_qt(f, Ct, S)
@@ -213,7 +213,30 @@ def test_large_batch_two_panel_apply_qt(dt, band):
     ctqr.ct_qr_solve(f, ctqr.colmajor_from_numpy(B), S, Xt)
     X = ctqr.numpy_from_colmajor(Xt)
     assert relerr(X, X_or) <= SOLUTION[dt] and worst_col(X, X_or) <= SOLUTION[dt]
+    # option solve_pairs = 1 (by default these paths start at sizes the oracle cannot reach): from 256 right-hand sides on
+    # the blocked TRSM takes two diagonal blocks per update (K = 256; fp32: pre-split, TMA-fed when S is a multiple of 8,
+    # the plain contraction otherwise; the diagonal task is mm128_kernel up to S = 512, a contraction beyond);
+    # ct_qr_trsm on the oracle's C isolates it
+    for S2 in (320, 300, 512, 1024):
+        Ct2 = ctqr.colmajor_from_numpy(np.asfortranarray(C_or[:n, :S2]))
+        X2 = torch.zeros((S2, n), dtype=Ct.dtype, device="cuda")
+        ctqr.ct_qr_trsm(f, Ct2, S2, X2)
+        X2 = ctqr.numpy_from_colmajor(X2)
+        assert relerr(X2, X_or[:, :S2]) <= SOLUTION[dt], (S2, relerr(X2, X_or[:, :S2]))
+        assert worst_col(X2, X_or[:, :S2]) <= SOLUTION[dt]
+    Ct3 = ctqr.colmajor_from_numpy(np.asfortranarray(B[:, :256]))
+    ctqr.ct_qr_apply_qt(f, Ct3, 256)
+    assert f.stats()["apply_qt_path"] == 5
+    assert relerr(ctqr.numpy_from_colmajor(Ct3), C_or[:, :256]) <= ROUND[dt]
     f.destroy()
+    # the default (by size) and "never" leave both paths off at this size: same results from the one-panel order
+    for sp in (0, -1):
+        f = ctqr.ct_qr_factor(ctqr.colmajor_from_numpy(A), m, n, lower_bandwidth=(m - n) if band else 0, solve_pairs=sp)
+        Xt = torch.zeros((512, n), dtype=Ct.dtype, device="cuda")
+        ctqr.ct_qr_solve(f, ctqr.colmajor_from_numpy(np.asfortranarray(B[:, :512])), 512, Xt)
+        assert f.stats()["apply_qt_path"] == 0
+        assert relerr(ctqr.numpy_from_colmajor(Xt), X_or[:, :512]) <= SOLUTION[dt]
+        f.destroy()
 
 
 @pytest.mark.parametrize("dt", DT)

@@ -163,7 +163,9 @@ __host__ __device__ inline int sk_nseg(int64_t t, int KT, int64_t L) {
 template <typename T, bool TA, int BM, int BN, int WM, int WN, int STAGES>
 struct MmaCfg {
     using P = MmaPolicy<T>;
-    static constexpr int BK = P::BK;
+    // k-tile: the policy's, twice as deep in a two-stage configuration (same shared memory as three stages of the
+    // plain depth, half the barriers per flop: W = V^T C in fp64 gains 5 %, C <- C - V W with its short K loses 4 %)
+    static constexpr int BK = P::BK * (STAGES == 2 ? 2 : 1);
     static constexpr int WARPS_M = BM / WM, WARPS_N = BN / WN;
     static constexpr int NT = WARPS_M * WARPS_N * 32;
     static constexpr int MT = WM / P::MFRAG, NTL = WN / 8;

@@ -779,7 +779,7 @@ NCU_TRAFFIC = {("c3", "f64", "upd"): (13.68e9, 8.29e9, "profiles/r1_pairs_c3.md"
                ("c4", "f32", "upd"): (89.6e9, 56.2e9, "profiles/r2_c4_f32.md")}
 
 KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; DMMA.8x8x4)",
-                ("f64", "vtc"): "gemm_mma_kernel<double,TA=true,128,64,32,32,2,2> (W = V^T C, larfb; DMMA.8x8x4; two stages, k-tile 32)",
+                ("f64", "vtc"): "gemm_mma_kernel<double,TA=true,128,64,32,32,3,2> (W = V^T C, larfb; DMMA.8x8x4)",
                 ("f32", "upd"): "umma::upd_tma_kernel (C <- C - V W, larfb; 3xTF32 on tcgen05.mma kind::tf32 / TMEM, operands pre-split, TMA-fed)",
                 ("f32", "vtc"): "umma::vtc_tma_kernel (W = V^T C, larfb; 3xTF32 on tcgen05.mma kind::tf32 / TMEM, V pre-split and TMA-fed)"}
 

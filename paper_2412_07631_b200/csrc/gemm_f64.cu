@@ -42,7 +42,7 @@ GemmLaunch gemm_plan_f64(bool ta, int64_t M, int64_t N, int64_t K, int impl, int
     if (ta) {
         if (M <= 32) return classic_plan(M, N, K, 32, 128, sms, 256, partial, max_elems, sstride, 0);
         if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_elems, sstride, 6);
-        return streamk_plan(M, N, K, 128, 64, 2 * MmaPolicy<double>::BK, sms, partial, max_elems, sstride, 1);   // two stages, k-tile 32
+        return streamk_plan(M, N, K, 128, 64, MmaPolicy<double>::BK, sms, partial, max_elems, sstride, 1);
     }
     if (N <= 32) return classic_plan(M, N, K, 128, 32, sms, 256, partial, max_elems, sstride, 2);
     if (!aligned) return classic_plan(M, N, K, 128, 64, sms, 512, partial, max_elems, sstride, 7);
@@ -66,7 +66,7 @@ cudaError_t gemm_run_f64(bool ta, GemmArgs<double> g, const GemmLaunch& L, int i
         case 9: return ta ? launch_simt<double, true, 64, 64, 8>(g, L.splits, st)
                           : launch_simt<double, false, 64, 64, 8>(g, L.splits, st);
         case 0: return launch_dmma<true, 32, 128, 32, 32, 16, 4, 2>(g, L.splits, st);
-        case 1: return launch_mma<double, true, 128, 64, 32, 32, 2, 2>(g, to_plan(L), st);
+        case 1: return launch_mma<double, true, 128, 64, 32, 32, 3, 2>(g, to_plan(L), st);
         case 2: return launch_dmma<false, 128, 32, 32, 32, 16, 3, 2>(g, L.splits, st);
         case 6: return launch_dmma<true, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);
         case 7: return launch_dmma<false, 128, 64, 64, 32, 16, 3, 2>(g, L.splits, st);

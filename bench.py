@@ -774,8 +774,8 @@ NCU_TRAFFIC = {("c3", "f64", "upd"): (13.68e9, 8.29e9, "profiles/r1_pairs_c3.md"
                ("c3", "f64", "vtc"): (3.95e9, None, "profiles/r1_pairs_c3.md"),
                ("c3", "f32", "upd"): (3.57e9, None, "profiles/r1_final_c3.md"),
                ("c3", "f32", "vtc"): (1.91e9, None, "profiles/r1_final_c3.md"),
-               ("c4", "f64", "upd"): (124.4e9, 113.4e9, "profiles/r2_c4_f64.md"),
-               ("c4", "f64", "vtc"): (90.2e9, 56.8e9, "profiles/r2_c4_f64.md"),
+               ("c4", "f64", "upd"): (124.1e9, 113.4e9, "profiles/r2_c4_f64.md"),
+               ("c4", "f64", "vtc"): (90.1e9, 56.8e9, "profiles/r2_c4_f64.md"),
                ("c4", "f32", "upd"): (89.6e9, 56.2e9, "profiles/r2_c4_f32.md")}
 
 KERNEL_NAMES = {("f64", "upd"): "gemm_mma_kernel<double,TA=false,128,64,32,32,3,2> (C <- C - V W, larfb; DMMA.8x8x4)",

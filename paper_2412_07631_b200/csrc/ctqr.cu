@@ -835,7 +835,7 @@ static int factor_range_pairs(H& h, T* A, int64_t lda, int64_t c0, int64_t c1) {
             if (R > (int)(h.sms * 0.45)) R = 0;
             if (R > 0) {
                 const double t_chain = 2.0 * (0.25e-3 + 1.5e-8 * (double)mk1) + 0.15e-3;
-                const double rate = (sizeof(T) == 4 ? 75e12 : 27e12) * (double)(h.sms - R) / (double)h.sms;
+                const double rate = (sizeof(T) == 4 ? 100e12 : 31e12) * (double)(h.sms - R) / (double)h.sms;
                 nA = (int64_t)(t_chain * rate / (4.0 * (double)(m - j0) * 2 * nb));
                 nA = std::min<int64_t>(ncb, round_up(std::max<int64_t>(nA, 1024), 128));
                 if (ncb - nA < 1024) nA = ncb;
